@@ -1,0 +1,160 @@
+"""CPU oracle for the FEW interpolated mode summation -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Thin numpy/ctypes front end of `few_oracle.c` (plain C, gcc).  Only `tests/`, `__graft_entry__.smoke()` and
+`bench.py`'s `cpu_baseline` / `--impl reference` legs may import this package.  It imports nothing from
+`paper_2104_04582_b200` and shares no code with the CUDA path.
+
+Functions (each follows the passage cited in few_oracle.c):
+  spline_fit(t, y)            O1, FP64
+  spline_fit_ext(t, y)        O1, x87 extended    PAPER.md:153 + DESIGN.md R13
+  ylm(l, m, theta, phi)       O2
+  select_modes(...)           O3
+  sum_waveform(...)           O4                  PAPER.md:155-159, Eq. (9), Eq. (10)
+  waveform(workload)          chain O2 -> O3 -> O1 -> O4 in the paper's pipeline order
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "few_oracle.c")
+_SO = os.path.join(_HERE, "libfew_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile few_oracle.c with gcc (-ffp-contract=off: every FP64 product and sum is rounded separately)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-std=c11",
+                               _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+
+
+def _ptr(a, typ=_dp):
+    return None if a is None else a.ctypes.data_as(typ)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.oracle_spline_fit.argtypes = [_dp, _dp, C.c_int, C.c_int, _dp]
+        L.oracle_spline_fit_ext.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_void_p]
+        L.oracle_ylm.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _dp]
+        L.oracle_swsh.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp]
+        L.oracle_select_modes.argtypes = [_dp, _ip, _dp, _dp, C.c_double, C.c_int, C.c_int, _ip, _ip, _dp]
+        L.oracle_sum_waveform.argtypes = [_dp, _dp, C.c_void_p, _ip, _ip, _ip, _ip, C.c_int, _dp, _dp, C.c_double,
+                                          C.c_int, C.c_double, C.c_double, C.c_longlong, C.c_longlong, C.c_int,
+                                          C.c_int, _dp]
+        L.oracle_num_threads.restype = C.c_int
+        L.oracle_set_threads.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(int(n))
+
+
+_ERR = {-1: "n_t < 4", -2: "t not strictly increasing"}
+
+
+def spline_fit(t, y):
+    """O1 in FP64.  t [n_t], y [n_t, n_sys] -> coef [n_t-1, 4, n_sys] (c0, c1, c2, c3)."""
+    t = np.ascontiguousarray(t, np.float64); y = np.ascontiguousarray(y, np.float64)
+    n_t, n_sys = y.shape
+    coef = np.empty((max(n_t - 1, 0), 4, n_sys), np.float64)
+    rc = lib().oracle_spline_fit(_ptr(t), _ptr(y), n_t, n_sys, _ptr(coef))
+    if rc: raise ValueError(_ERR[rc])
+    return coef
+
+
+def spline_fit_ext(t, y):
+    """O1 in x87 extended precision -> np.longdouble coef [n_t-1, 4, n_sys]."""
+    assert np.finfo(np.longdouble).nmant == 63, "oracle needs x87 80-bit long double"
+    t = np.ascontiguousarray(t, np.float64); y = np.ascontiguousarray(y, np.float64)
+    n_t, n_sys = y.shape
+    coef = np.empty((max(n_t - 1, 0), 4, n_sys), np.longdouble)
+    rc = lib().oracle_spline_fit_ext(_ptr(t), _ptr(y), n_t, n_sys, coef.ctypes.data)
+    if rc: raise ValueError(_ERR[rc])
+    return coef
+
+
+def ylm(l: int, m: int, theta: float, phi: float, s: int = -2) -> complex:
+    out = np.empty(2)
+    rc = lib().oracle_swsh(int(s), int(l), int(m), float(theta), float(phi), _ptr(out))
+    if rc: raise ValueError("need l >= |s| and |m| <= l")
+    return complex(out[0], out[1])
+
+
+def ylm_modes(l, m, theta: float, phi: float):
+    """Y+_j = -2Y_{l_j, m_j}, Y-_j = -2Y_{l_j, -m_j} for a mode list -> two complex128 [n_modes]."""
+    yp = np.array([ylm(a, b, theta, phi) for a, b in zip(l, m)], np.complex128)
+    ym = np.array([ylm(a, -b, theta, phi) for a, b in zip(l, m)], np.complex128)
+    return yp, ym
+
+
+def _c2d(z):
+    return None if z is None else np.ascontiguousarray(z, np.complex128).view(np.float64)
+
+
+def select_modes(amp, m, ylm_plus, ylm_minus, eps: float):
+    """O3.  amp [n_t, n_modes] complex -> (keep_idx ascending int32 [n_keep], margin float64 [n_modes])."""
+    a = _c2d(amp); n_t, n_modes = amp.shape
+    m = np.ascontiguousarray(m, np.int32)
+    yp, ym = _c2d(ylm_plus), _c2d(ylm_minus)
+    keep = np.empty(n_modes, np.int32); nk = C.c_int(0); margin = np.empty(n_modes)
+    lib().oracle_select_modes(_ptr(a), _ptr(m, _ip), _ptr(yp), _ptr(ym), float(eps), n_t, n_modes, _ptr(keep, _ip),
+                              C.byref(nk), _ptr(margin))
+    return keep[: nk.value].copy(), margin
+
+
+def sum_waveform(t, coef_amp, coef_phase_ext, l, m, n, keep_idx, ylm_plus, ylm_minus, t0, dt, n_samples,
+                 scale: float = 1.0, fold: bool = True, i0: int = 0):
+    """O4.  coef_amp [n_t-1, 4, 2*n_modes] float64, coef_phase_ext [n_t-1, 4, 2] longdouble -> h complex128 [n_samples]."""
+    t = np.ascontiguousarray(t, np.float64)
+    ca = np.ascontiguousarray(coef_amp, np.float64)
+    cp = np.ascontiguousarray(coef_phase_ext, np.longdouble)
+    l, m, n = (np.ascontiguousarray(x, np.int32) for x in (l, m, n))
+    n_t, n_modes = t.shape[0], l.shape[0]
+    assert ca.shape == (n_t - 1, 4, 2 * n_modes) and cp.shape == (n_t - 1, 4, 2)
+    k = None if keep_idx is None else np.ascontiguousarray(keep_idx, np.int32)
+    yp = _c2d(ylm_plus)
+    ym = _c2d(ylm_minus if ylm_minus is not None else np.zeros(n_modes, np.complex128))
+    h = np.empty((int(n_samples), 2), np.float64)
+    rc = lib().oracle_sum_waveform(_ptr(t), _ptr(ca), cp.ctypes.data, _ptr(l, _ip), _ptr(m, _ip), _ptr(n, _ip),
+                                   _ptr(k, _ip), 0 if k is None else len(k), _ptr(yp), _ptr(ym), float(scale),
+                                   int(bool(fold)), float(t0), float(dt), int(i0), int(n_samples), n_t, n_modes, _ptr(h))
+    if rc: raise ValueError(_ERR[rc])
+    return h.view(np.complex128)[:, 0]
+
+
+def waveform(w, *, windows=None, return_parts: bool = False):
+    """Whole path for a synth.Workload, in the paper's order: harmonics, mode selection, spline
+    fits, interpolated summation.  `windows` = list of (i0, n) sample ranges (default: the whole grid).
+    Returns h [n_src][len(windows)] arrays (or a single [n_src, n_samples] array), plus parts on request."""
+    hs, parts = [], []
+    for s in range(w.n_src):
+        yp, ym = ylm_modes(w.l, w.m, float(w.theta[s]), float(w.phi[s]))
+        keep, margin = select_modes(w.amp[s], w.m, yp, ym, w.eps)
+        ca = spline_fit(w.t[s], _c2d(w.amp[s]))
+        cp = spline_fit_ext(w.t[s], w.phase[s])
+        wins = windows if windows is not None else [(0, w.n_samples)]
+        hw = [sum_waveform(w.t[s], ca, cp, w.l, w.m, w.n, keep, yp, ym, w.t0, w.dt, nn, i0=i0) for (i0, nn) in wins]
+        hs.append(hw if windows is not None else hw[0])
+        parts.append(dict(ylm_plus=yp, ylm_minus=ym, keep_idx=keep, margin=margin, coef_amp=ca, coef_phase=cp))
+    out = hs if windows is not None else np.stack(hs)
+    return (out, parts) if return_parts else out
