@@ -1,0 +1,153 @@
+/* few.h -- C ABI of libfew_b200: the interpolated harmonic-mode summation of FastEMRIWaveforms
+ * (Katz, Chua, Speri, Warburton, Hughes, arXiv:2104.04582; cited below as PAPER.md:<line>) as hand-written
+ * CUDA for NVIDIA B200 (sm_100a), FP64, one GPU per process.
+ *
+ * The hot path:
+ *   S0  few_ylm_modes      per-source harmonic constants  -2Y_{l,+-m}(theta, phi)
+ *   S1  few_spline_fit     batched not-a-knot cubic splines of A_lmn(t_k)
+ *       few_spline_fit_dd  the same for the two phases, solved and stored in double-double (R13)
+ *   S2  few_select_modes   power sort + cumulative sum + eps threshold per sparse step, union over steps
+ *                                                                                        PAPER.md:167
+ *   S3  few_sum_waveform   h_+ - i h_x = sum_kept A_lmn(t) Y_lm exp(-i(m Phi_phi + n Phi_r)), m<0 folded in by
+ *                          A_{l,-m,-n} = (-1)^l conj(A_lmn)                              PAPER.md:155-159, Eq.(9), Eq.(10)
+ *   few_waveform / few_waveform_host  chain S0->S2->S1->S3 in the paper's pipeline order
+ *
+ * Conventions
+ *   - Every function returns an int status: FEW_OK (0) or a negative FEW_ERR_*.  No exception crosses the ABI.
+ *     few_strerror(code) names a code; few_last_error() returns the calling thread's last detailed message.
+ *   - Pointers are DEVICE pointers (on the context's device) unless the name or comment says "host".
+ *   - Ownership: the caller owns every input, output and workspace buffer.  The library keeps only a few KB of
+ *     state in few_ctx.  Workspace sizes come from the *_workspace() queries; workspaces need 256-byte alignment.
+ *   - All work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as void*; NULL = legacy
+ *     default stream).  No device-pointer call synchronises; n_keep stays on the device so S2 -> S1 -> S3 chain
+ *     without a host round trip.  Only few_waveform_host and few_device_status synchronise.
+ *   - Shapes are validated on the host (FEW_ERR_INVALID_ARG, FEW_ERR_TOO_FEW_POINTS, FEW_ERR_LIMIT).  Data that
+ *     lives on the device (t increasing, (l,m,n) validity) is checked by the kernels, which OR a FEW_DEV_* bit into a
+ *     device status word read back by few_device_status().  Outputs are unspecified when a bit is set.
+ *   - Layouts are C-contiguous with the LAST index fastest.  Complex numbers are (re, im) pairs of doubles.
+ *   - n_t, n_samples, t0, dt are uniform across a batch (true for every workload of the paper); sources differ in
+ *     t, amplitudes, phases, angles and kept modes.
+ *   - There is no CPU fallback: without a CUDA device few_create fails with FEW_ERR_CUDA.
+ */
+#ifndef FEW_H
+#define FEW_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FEW_VERSION 100 /* 0.1.0 */
+
+enum {
+    FEW_OK = 0,
+    FEW_ERR_INVALID_ARG = -1,     /* NULL pointer, non-positive size, bad flag */
+    FEW_ERR_TOO_FEW_POINTS = -2,  /* n_t < 4: a not-a-knot cubic spline needs 4 knots */
+    FEW_ERR_NOT_INCREASING = -3,  /* t not strictly increasing (reported by few_device_status) */
+    FEW_ERR_BAD_MODE = -4,        /* l < 2, |m| > l, m < 0, |n| > FEW_MAX_ABS_N, l > FEW_MAX_L (few_device_status / few_ylm) */
+    FEW_ERR_WORKSPACE = -5,       /* workspace NULL, misaligned or smaller than the query says */
+    FEW_ERR_CUDA = -6,            /* a CUDA runtime call failed; few_last_error() has the text */
+    FEW_ERR_LIMIT = -7            /* size beyond a documented limit (FEW_MAX_*) */
+};
+
+/* bits of the device status word */
+enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_TOO_MANY_L = 4 };
+
+#define FEW_MAX_L 63            /* l <= 63 (factorials in FP64, 64-bit l masks) */
+#define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
+#define FEW_MAX_L_PER_M 9       /* at most 9 distinct l per m among the kept modes (l in [2,10]) */
+#define FEW_MAX_NT_SPLINE 896   /* n_t limit of few_spline_fit (one shared-memory column per system) */
+#define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
+
+typedef struct few_ctx few_ctx;
+
+/* Context: binds a CUDA device, holds the device status word.  `device` = CUDA ordinal. */
+int few_create(few_ctx** out, int device);
+int few_destroy(few_ctx* ctx);
+const char* few_strerror(int code);
+const char* few_last_error(void);
+int few_version(void);
+
+/* Synchronises `stream`, returns FEW_OK or the FEW_ERR_* of the lowest FEW_DEV_* bit set by kernels since the last
+ * call, and clears the word.  Optional `bits_out` (host) receives the raw bits. */
+int few_device_status(few_ctx* ctx, int* bits_out, void* stream);
+
+/* ---- S0: spin-weighted spherical harmonics, s = -2 (Goldberg et al. convention, R11).
+ * few_ylm is a HOST helper: out (host) = {Re, Im} of -2Y_lm(theta, phi).  FEW_ERR_BAD_MODE if l < 2, |m| > l, l > FEW_MAX_L.
+ * few_ylm_modes: theta, phi [n_src]; l, m [n_modes] int32 (m >= 0) -> ylm_plus[n_src][n_modes][2] = -2Y_{l,m},
+ * ylm_minus[n_src][n_modes][2] = -2Y_{l,-m}. */
+int few_ylm(int l, int m, double theta, double phi, double* out_host);
+int few_ylm_modes(few_ctx* ctx, const double* theta, const double* phi, const int* l, const int* m,
+                  int n_src, int n_modes, double* ylm_plus, double* ylm_minus, void* stream);
+
+/* ---- S1: batched not-a-knot cubic spline fit on a per-source shared grid.
+ * t[n_src][n_t] strictly increasing; y[n_src][n_t][n_sys] (systems fastest: the amplitude module's [n_t, n_modes]
+ * complex array viewed as doubles has n_sys = 2 n_modes).
+ * coef[n_src][n_t-1][4][n_sys]: on segment k, S(t) = c0 + c1 dx + c2 dx^2 + c3 dx^3 with dx = t - t_k; c0 = y_k bitwise.
+ * Limits: 4 <= n_t <= FEW_MAX_NT_SPLINE. */
+int few_spline_fit(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
+                   double* coef, void* stream);
+
+/* Same spline, solved and stored in double-double (unevaluated sum hi + lo, |lo| <= ulp(hi)/2) for the orbital phases,
+ * whose 1e5..1e6 rad magnitude needs more than 53 bits to reach 1e-10 on the waveform (R13).
+ * y[n_src][n_t][n_sys] (FP64 knot values) -> coef_dd[n_src][n_t-1][4][n_sys][2] (hi, lo).  n_sys is small (2: Phi_phi, Phi_r). */
+int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
+                      double* coef_dd, void* stream);
+
+/* ---- S2: Mode Selector.  Per source and sparse step k: entries = every mode j (power
+ * |A_j(t_k)|^2 |Y+_j|^2) plus, for m_j > 0, its mirror (l,-m,-n) (power |A_j(t_k)|^2 |Y-_j|^2, owner j); sort by power
+ * descending (ties: lower entry index first); inclusive cumulative sum C; entry of rank r is kept iff r == 0 or
+ * C_{r-1} < (1 - eps) C_last.  Kept set = union over k of the owners.  eps <= 0 keeps every mode.
+ * ylm_plus == NULL (then ylm_minus is ignored): power = |A|^2, no mirror entries.
+ * amp[n_src][n_t][n_modes][2]; m[n_modes]; ylm_*[n_src][n_modes][2];
+ * keep_idx[n_src][n_modes] int32 ascending, padded with -1; n_keep[n_src] int32.
+ * Limit: n_modes + #(m>0) <= FEW_MAX_SELECT_ENTRIES. */
+size_t few_select_modes_workspace(int n_src, int n_t, int n_modes);
+int few_select_modes(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
+                     double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,
+                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- S3: interpolated summation (Eq.(9), Eq.(10)).  For i in [0, n_samples): t_i = t0 + i*dt
+ * (product and sum rounded separately); outside [t_0, t_{n_t-1}] h = 0; otherwise with k = max{k: t_k <= t_i} (clamped
+ * to n_t-2), dx = t_i - t_k:
+ *   h_i = scale * sum_{j kept} [ Y+_j W_j + (m_j > 0) (-1)^{l_j} Y-_j conj(W_j) ],  W_j = A_j(t_i) exp(-i(m_j Phi_phi + n_j Phi_r)).
+ * coef_amp[n_src][n_t-1][4][2 n_modes] from few_spline_fit; coef_phase_dd[n_src][n_t-1][4][2][2] from few_spline_fit_dd
+ * (system 0 = Phi_phi, 1 = Phi_r); l, m, n [n_modes] int32 shared by the sources, m >= 0;
+ * keep_idx[n_src][n_modes] / n_keep[n_src] from few_select_modes, or both NULL = all modes;
+ * scale[n_src] or NULL (= 1) is the mu/d_L prefactor of Eq.(10);
+ * h[n_src][n_samples][2] = (h_+, -h_x). */
+size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples);
+int few_sum_waveform(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
+                     const int* l, const int* m, const int* n, const int* keep_idx, const int* n_keep,
+                     const double* ylm_plus, const double* ylm_minus, const double* scale,
+                     double t0, double dt, long long n_samples, double* h,
+                     int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- Whole path on device buffers: S0 -> S2 -> S1 -> S3, no host synchronisation.
+ * t[n_src][n_t], phase[n_src][n_t][2] (Phi_phi, Phi_r), amp[n_src][n_t][n_modes][2], theta/phi[n_src], l/m/n[n_modes].
+ * Outputs: h[n_src][n_samples][2]; optional keep_idx[n_src][n_modes], n_keep[n_src] (NULL: kept inside the workspace). */
+size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples);
+int few_waveform(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                 const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
+                 double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                 double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): allocates device
+ * buffers, copies inputs host->device, runs few_waveform, copies h (and keep_idx/n_keep if not NULL) device->host,
+ * synchronises, frees.  `scale_host` may be NULL.  Returns the device status as well. */
+int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
+                      const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
+                      const double* phi_host, const double* scale_host, double eps, double t0, double dt,
+                      long long n_samples, int n_src, int n_t, int n_modes,
+                      double* h_host, int* keep_idx_host, int* n_keep_host);
+
+/* ---- Measurement aid: register-resident DFMA chains on every SM (the FP64 roofline denominator).
+ * Launches `blocks` x `threads` threads, each doing `iters` x 16 dependent-chain-free DFMAs; writes one double per thread
+ * to sink[blocks*threads].  FLOPs = 2 * 16 * iters * blocks * threads. */
+int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double* sink, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FEW_H */

@@ -1,0 +1,225 @@
+"""Thin Python binding of libfew_b200 (include/few.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch supplies device buffers and the current stream.
+Function names and argument meaning mirror include/few.h.  There is no CPU fallback: importing this module fails
+loudly when libfew_b200.so is missing and cannot be built, and `context()` fails when no CUDA device is present.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_PKG, "libfew_b200.so")
+
+FEW_OK = 0
+SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_version", "few_device_status", "few_ylm",
+           "few_ylm_modes", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
+           "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
+           "few_fp64_peak_probe"]
+
+
+class FewError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = _lib.few_strerror(code).decode()
+        detail = _lib.few_last_error().decode()
+        super().__init__(f"{where}: {msg}" + (f" ({detail})" if detail else ""))
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(_SO):
+        _build.build()          # raises if nvcc is missing: no fallback
+    lib = C.CDLL(_SO)
+    vp, i, d, ll, sz = C.c_void_p, C.c_int, C.c_double, C.c_longlong, C.c_size_t
+    sig = {
+        "few_create": (i, [C.POINTER(vp), i]),
+        "few_destroy": (i, [vp]),
+        "few_strerror": (C.c_char_p, [i]),
+        "few_last_error": (C.c_char_p, []),
+        "few_version": (i, []),
+        "few_device_status": (i, [vp, C.POINTER(i), vp]),
+        "few_ylm": (i, [i, i, d, d, C.POINTER(d)]),
+        "few_ylm_modes": (i, [vp, vp, vp, vp, vp, i, i, vp, vp, vp]),
+        "few_spline_fit": (i, [vp, vp, vp, i, i, i, vp, vp]),
+        "few_spline_fit_dd": (i, [vp, vp, vp, i, i, i, vp, vp]),
+        "few_select_modes_workspace": (sz, [i, i, i]),
+        "few_select_modes": (i, [vp, vp, vp, vp, vp, d, i, i, i, vp, vp, vp, sz, vp]),
+        "few_sum_waveform_workspace": (sz, [i, i, i, ll]),
+        "few_sum_waveform": (i, [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, d, d, ll, vp, i, i, i, vp, sz, vp]),
+        "few_waveform_workspace": (sz, [i, i, i, ll]),
+        "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
+        "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
+        "few_fp64_peak_probe": (i, [vp, i, i, i, vp, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+_lib = _load()
+_ctx: dict[int, C.c_void_p] = {}
+
+
+def context(device: int | None = None) -> C.c_void_p:
+    """few_ctx of a CUDA device (created once per device)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("libfew_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+    dev = torch.cuda.current_device() if device is None else int(device)
+    if dev not in _ctx:
+        h = C.c_void_p()
+        rc = _lib.few_create(C.byref(h), dev)
+        if rc != FEW_OK:
+            raise FewError(rc, "few_create")
+        _ctx[dev] = h
+    return _ctx[dev]
+
+
+def _chk(rc: int, where: str):
+    if rc != FEW_OK:
+        raise FewError(rc, where)
+
+
+def _p(x: torch.Tensor | None, dtype=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if x is None:
+        return None
+    if not (x.is_cuda and x.is_contiguous()):
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and x.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {x.dtype}")
+    return C.c_void_p(x.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ws(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)   # torch CUDA allocations are 512-B aligned
+
+
+def few_version() -> int:
+    return int(_lib.few_version())
+
+
+def few_device_status(raise_on_error: bool = True) -> int:
+    bits = C.c_int(0)
+    rc = _lib.few_device_status(context(), C.byref(bits), _stream())
+    if rc != FEW_OK and raise_on_error:
+        raise FewError(rc, "few_device_status")
+    return rc
+
+
+def few_ylm(l: int, m: int, theta: float, phi: float) -> complex:
+    out = (C.c_double * 2)()
+    _chk(_lib.few_ylm(int(l), int(m), float(theta), float(phi), out), "few_ylm")
+    return complex(out[0], out[1])
+
+
+def few_ylm_modes(theta, phi, l, m):
+    """theta, phi [n_src] f64; l, m [n_modes] i32 -> (ylm_plus, ylm_minus) complex128 [n_src, n_modes]."""
+    n_src, n_modes = theta.shape[0], l.shape[0]
+    yp = torch.empty((n_src, n_modes), dtype=torch.complex128, device=theta.device)
+    ym = torch.empty_like(yp)
+    _chk(_lib.few_ylm_modes(context(), _p(theta, torch.float64), _p(phi, torch.float64), _p(l, torch.int32), _p(m, torch.int32),
+                            n_src, n_modes, _p(yp), _p(ym), _stream()), "few_ylm_modes")
+    return yp, ym
+
+
+def few_spline_fit(t, y, out=None):
+    """t [n_src, n_t] f64; y [n_src, n_t, n_sys] f64 (or complex128 [n_src, n_t, n_modes], viewed as 2 n_modes systems)
+    -> coef [n_src, n_t-1, 4, n_sys]."""
+    if y.dtype == torch.complex128:
+        y = torch.view_as_real(y).reshape(y.shape[0], y.shape[1], -1)
+    n_src, n_t, n_sys = y.shape
+    coef = out if out is not None else torch.empty((n_src, max(n_t - 1, 0), 4, n_sys), dtype=torch.float64, device=y.device)
+    _chk(_lib.few_spline_fit(context(), _p(t, torch.float64), _p(y, torch.float64), n_src, n_t, n_sys, _p(coef, torch.float64),
+                             _stream()), "few_spline_fit")
+    return coef
+
+
+def few_spline_fit_dd(t, y, out=None):
+    """y [n_src, n_t, n_sys] f64 -> coef_dd [n_src, n_t-1, 4, n_sys, 2] (hi, lo)."""
+    n_src, n_t, n_sys = y.shape
+    coef = out if out is not None else torch.empty((n_src, max(n_t - 1, 0), 4, n_sys, 2), dtype=torch.float64, device=y.device)
+    _chk(_lib.few_spline_fit_dd(context(), _p(t, torch.float64), _p(y, torch.float64), n_src, n_t, n_sys, _p(coef, torch.float64),
+                                _stream()), "few_spline_fit_dd")
+    return coef
+
+
+def few_select_modes(amp, m, ylm_plus, ylm_minus, eps: float, workspace=None):
+    """amp [n_src, n_t, n_modes] c128 -> (keep_idx [n_src, n_modes] i32 ascending, padded -1; n_keep [n_src] i32)."""
+    n_src, n_t, n_modes = amp.shape
+    keep = torch.empty((n_src, n_modes), dtype=torch.int32, device=amp.device)
+    nk = torch.empty((n_src,), dtype=torch.int32, device=amp.device)
+    need = _lib.few_select_modes_workspace(n_src, n_t, n_modes)
+    ws = workspace if workspace is not None else _ws(need, amp.device)
+    _chk(_lib.few_select_modes(context(), _p(amp, torch.complex128), _p(m, torch.int32), _p(ylm_plus), _p(ylm_minus), float(eps),
+                               n_src, n_t, n_modes, _p(keep), _p(nk), _p(ws), ws.numel(), _stream()), "few_select_modes")
+    return keep, nk
+
+
+def few_sum_waveform(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, ylm_plus, ylm_minus, t0: float, dt: float,
+                     n_samples: int, scale=None, out=None, workspace=None):
+    """-> h [n_src, n_samples] complex128 = h_+ - i h_x."""
+    n_src, n_t = t.shape
+    n_modes = l.shape[0]
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    ws = workspace if workspace is not None else _ws(need, t.device)
+    _chk(_lib.few_sum_waveform(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
+                               _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32), _p(keep_idx), _p(n_keep),
+                               _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale), float(t0), float(dt),
+                               int(n_samples), _p(h), n_src, n_t, n_modes, _p(ws), ws.numel(), _stream()), "few_sum_waveform")
+    return h
+
+
+def few_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int) -> int:
+    return int(_lib.few_waveform_workspace(n_src, n_t, n_modes, int(n_samples)))
+
+
+def few_waveform(t, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int, scale=None,
+                 out=None, keep_idx=None, n_keep=None, workspace=None):
+    """Whole path on device tensors.  -> h [n_src, n_samples] complex128 (keep_idx / n_keep are filled if given)."""
+    n_src, n_t, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    ws = workspace if workspace is not None else _ws(few_waveform_workspace(n_src, n_t, n_modes, n_samples), t.device)
+    _chk(_lib.few_waveform(context(), _p(t, torch.float64), _p(phase, torch.float64), _p(amp, torch.complex128), _p(l, torch.int32),
+                           _p(m, torch.int32), _p(n, torch.int32), _p(theta, torch.float64), _p(phi, torch.float64), _p(scale),
+                           float(eps), float(t0), float(dt), int(n_samples), n_src, n_t, n_modes, _p(h), _p(keep_idx), _p(n_keep),
+                           _p(ws), ws.numel(), _stream()), "few_waveform")
+    return h
+
+
+def _hp(x, dtype):
+    """Host pointer of a contiguous CPU tensor."""
+    if x is None:
+        return None
+    if x.is_cuda or not x.is_contiguous() or x.dtype != dtype:
+        raise ValueError(f"expected a contiguous CPU tensor of dtype {dtype}")
+    return C.c_void_p(x.data_ptr())
+
+
+def few_waveform_host(t, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int, scale=None,
+                      out=None, keep_idx=None, n_keep=None, device: int | None = None):
+    """Whole path on HOST tensors (pinned recommended): H2D, kernels, D2H inside the library.  -> h (CPU) [n_src, n_samples]."""
+    n_src, n_t, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, pin_memory=True)
+    _chk(_lib.few_waveform_host(context(device), _hp(t, torch.float64), _hp(phase, torch.float64), _hp(amp, torch.complex128),
+                                _hp(l, torch.int32), _hp(m, torch.int32), _hp(n, torch.int32), _hp(theta, torch.float64),
+                                _hp(phi, torch.float64), _hp(scale, torch.float64), float(eps), float(t0), float(dt), int(n_samples),
+                                n_src, n_t, n_modes, _hp(h, torch.complex128), _hp(keep_idx, torch.int32), _hp(n_keep, torch.int32)),
+         "few_waveform_host")
+    return h
+
+
+def few_fp64_peak_probe(blocks: int, threads: int, iters: int, sink=None):
+    sink = sink if sink is not None else torch.empty(blocks * threads, dtype=torch.float64, device="cuda")
+    _chk(_lib.few_fp64_peak_probe(context(), blocks, threads, iters, _p(sink), _stream()), "few_fp64_peak_probe")
+    return 2.0 * 16 * iters * blocks * threads   # FLOPs launched

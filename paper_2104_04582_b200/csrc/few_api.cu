@@ -1,0 +1,227 @@
+// few_api.cu -- context, error reporting, the chained whole-path entry points and the FP64 peak probe.
+#include <stdarg.h>
+#include <string.h>
+#include <new>
+#include "few_common.cuh"
+
+static thread_local char g_last_error[512] = "";
+
+void few_set_error(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_last_error, sizeof(g_last_error), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char* few_last_error(void) { return g_last_error; }
+extern "C" int few_version(void) { return FEW_VERSION; }
+
+extern "C" const char* few_strerror(int code)
+{
+    switch (code) {
+        case FEW_OK: return "FEW_OK";
+        case FEW_ERR_INVALID_ARG: return "FEW_ERR_INVALID_ARG: NULL pointer, non-positive size or bad flag";
+        case FEW_ERR_TOO_FEW_POINTS: return "FEW_ERR_TOO_FEW_POINTS: a not-a-knot cubic spline needs n_t >= 4";
+        case FEW_ERR_NOT_INCREASING: return "FEW_ERR_NOT_INCREASING: sparse times are not strictly increasing";
+        case FEW_ERR_BAD_MODE: return "FEW_ERR_BAD_MODE: need 2 <= l <= FEW_MAX_L, 0 <= m <= l, |n| <= FEW_MAX_ABS_N, <= 9 distinct l per m";
+        case FEW_ERR_WORKSPACE: return "FEW_ERR_WORKSPACE: workspace NULL, misaligned or too small";
+        case FEW_ERR_CUDA: return "FEW_ERR_CUDA: CUDA runtime error";
+        case FEW_ERR_LIMIT: return "FEW_ERR_LIMIT: size beyond a documented FEW_MAX_* limit";
+        default: return "unknown FEW status code";
+    }
+}
+
+extern "C" int few_create(few_ctx** out, int device)
+{
+    FEW_REQUIRE(out != nullptr, FEW_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int count = 0;
+    FEW_CUDA_CHECK(cudaGetDeviceCount(&count));
+    FEW_REQUIRE(device >= 0 && device < count, FEW_ERR_INVALID_ARG, "no such CUDA device");
+    FEW_CUDA_CHECK(cudaSetDevice(device));
+    few_ctx* c = new (std::nothrow) few_ctx();
+    FEW_REQUIRE(c != nullptr, FEW_ERR_INVALID_ARG, "out of host memory");
+    c->device = device;
+    cudaError_t e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_status, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, sizeof(int));
+    if (e != cudaSuccess) {
+        few_set_error("few_create: %s", cudaGetErrorString(e));
+        delete c;
+        return FEW_ERR_CUDA;
+    }
+    *out = c;
+    return FEW_OK;
+}
+
+extern "C" int few_destroy(few_ctx* ctx)
+{
+    if (!ctx) return FEW_OK;
+    cudaFree(ctx->d_status);
+    delete ctx;
+    return FEW_OK;
+}
+
+extern "C" int few_device_status(few_ctx* ctx, int* bits_out, void* stream)
+{
+    FEW_REQUIRE(ctx != nullptr, FEW_ERR_INVALID_ARG, "ctx is NULL");
+    int bits = 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    FEW_CUDA_CHECK(cudaMemcpyAsync(&bits, ctx->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+    FEW_CUDA_CHECK(cudaMemsetAsync(ctx->d_status, 0, sizeof(int), st));
+    FEW_CUDA_CHECK(cudaStreamSynchronize(st));
+    if (bits_out) *bits_out = bits;
+    if (bits & FEW_DEV_NOT_INCREASING) { few_set_error("device check: sparse times not strictly increasing"); return FEW_ERR_NOT_INCREASING; }
+    if (bits & (FEW_DEV_BAD_MODE | FEW_DEV_TOO_MANY_L)) { few_set_error("device check: invalid (l, m, n) or more than 9 distinct l for one m"); return FEW_ERR_BAD_MODE; }
+    return FEW_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Whole path: S0 -> S2 -> S1 -> S3 ("combined with the spin-weighted spherical harmonics and then put through
+// mode selection ... Following mode selection, the waveform is built using the interpolated summation").
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+struct wf_layout {
+    double *ylm_plus, *ylm_minus, *coef_amp, *coef_phase;
+    int *keep_idx, *n_keep;
+    void *sel_ws, *sum_ws;
+    size_t sel_bytes, sum_bytes;
+};
+
+wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, size_t* bytes)
+{
+    few_carver c(ws);
+    wf_layout L;
+    L.ylm_plus = c.take<double>((size_t)n_src * n_modes * 2);
+    L.ylm_minus = c.take<double>((size_t)n_src * n_modes * 2);
+    L.coef_amp = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 2 * n_modes);
+    L.coef_phase = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 2 * 2);
+    L.keep_idx = c.take<int>((size_t)n_src * n_modes);
+    L.n_keep = c.take<int>(n_src);
+    L.sel_bytes = few_select_modes_workspace(n_src, n_t, n_modes);
+    L.sum_bytes = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples);
+    L.sel_ws = c.take<char>(L.sel_bytes);
+    L.sum_ws = c.take<char>(L.sum_bytes);
+    if (bytes) *bytes = c.off;
+    return L;
+}
+}  // namespace
+
+extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
+{
+    if (n_src <= 0 || n_t < 4 || n_modes <= 0) return 0;
+    size_t bytes = 0;
+    wf_carve(nullptr, n_src, n_t, n_modes, n_samples, &bytes);
+    return bytes;
+}
+
+extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                            const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
+                            double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                            double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(ctx && t && phase && amp && l && m && n && theta && phi, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
+    FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
+    FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
+                    workspace_bytes >= few_waveform_workspace(n_src, n_t, n_modes, n_samples),
+                FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
+    wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, nullptr);
+    int* kidx = keep_idx ? keep_idx : L.keep_idx;
+    int* nk = n_keep ? n_keep : L.n_keep;
+    int rc;
+    if ((rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream))) return rc;
+    if ((rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream))) return rc;
+    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, stream))) return rc;
+    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, stream))) return rc;
+    return few_sum_waveform(ctx, t, L.coef_amp, L.coef_phase, l, m, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, t0, dt, n_samples, h,
+                            n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
+}
+
+extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
+                                 const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
+                                 const double* phi_host, const double* scale_host, double eps, double t0, double dt,
+                                 long long n_samples, int n_src, int n_t, int n_modes,
+                                 double* h_host, int* keep_idx_host, int* n_keep_host)
+{
+    FEW_REQUIRE(ctx && t_host && phase_host && amp_host && l_host && m_host && n_host && theta_host && phi_host,
+                FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
+    FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
+    FEW_REQUIRE(n_samples == 0 || h_host, FEW_ERR_INVALID_ARG, "h_host is NULL");
+    FEW_CUDA_CHECK(cudaSetDevice(ctx->device));
+    const size_t b_t = (size_t)n_src * n_t * 8, b_ph = b_t * 2, b_amp = (size_t)n_src * n_t * n_modes * 16;
+    const size_t b_lmn = (size_t)n_modes * 4, b_ang = (size_t)n_src * 8, b_h = (size_t)n_src * n_samples * 16;
+    const size_t b_keep = (size_t)n_src * n_modes * 4, b_nk = (size_t)n_src * 4;
+    const size_t ws_bytes = few_waveform_workspace(n_src, n_t, n_modes, n_samples);
+    // one device allocation, carved
+    size_t total = 0;
+    few_carver sz(nullptr);
+    sz.take<char>(b_t); sz.take<char>(b_ph); sz.take<char>(b_amp); sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_lmn);
+    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_h); sz.take<char>(b_keep); sz.take<char>(b_nk);
+    sz.take<char>(ws_bytes);
+    total = sz.off;
+    void* dev = nullptr;
+    cudaStream_t st = nullptr;
+    FEW_CUDA_CHECK(cudaMalloc(&dev, total));
+    int rc = FEW_OK;
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { few_set_error("cudaStreamCreate: %s", cudaGetErrorString(e)); cudaFree(dev); return FEW_ERR_CUDA; }
+    few_carver c(dev);
+    double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph); double* d_amp = (double*)c.take<char>(b_amp);
+    int* d_l = (int*)c.take<char>(b_lmn); int* d_m = (int*)c.take<char>(b_lmn); int* d_n = (int*)c.take<char>(b_lmn);
+    double* d_th = (double*)c.take<char>(b_ang); double* d_phi = (double*)c.take<char>(b_ang); double* d_sc = (double*)c.take<char>(b_ang);
+    double* d_h = (double*)c.take<char>(b_h); int* d_keep = (int*)c.take<char>(b_keep); int* d_nk = (int*)c.take<char>(b_nk);
+    void* d_ws = c.take<char>(ws_bytes);
+#define FEW_H2D(dst, src, bytes) if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st)
+    FEW_H2D(d_t, t_host, b_t); FEW_H2D(d_ph, phase_host, b_ph); FEW_H2D(d_amp, amp_host, b_amp);
+    FEW_H2D(d_l, l_host, b_lmn); FEW_H2D(d_m, m_host, b_lmn); FEW_H2D(d_n, n_host, b_lmn);
+    FEW_H2D(d_th, theta_host, b_ang); FEW_H2D(d_phi, phi_host, b_ang);
+    if (scale_host) FEW_H2D(d_sc, scale_host, b_ang);
+#undef FEW_H2D
+    if (e == cudaSuccess) {
+        rc = few_waveform(ctx, d_t, d_ph, d_amp, d_l, d_m, d_n, d_th, d_phi, scale_host ? d_sc : nullptr, eps, t0, dt, n_samples,
+                          n_src, n_t, n_modes, d_h, d_keep, d_nk, d_ws, ws_bytes, st);
+        if (rc == FEW_OK) {
+            if (n_samples) e = cudaMemcpyAsync(h_host, d_h, b_h, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess && keep_idx_host) e = cudaMemcpyAsync(keep_idx_host, d_keep, b_keep, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess && n_keep_host) e = cudaMemcpyAsync(n_keep_host, d_nk, b_nk, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) rc = few_device_status(ctx, nullptr, st);   // synchronises
+        }
+    }
+    if (e != cudaSuccess) { few_set_error("few_waveform_host: %s", cudaGetErrorString(e)); rc = FEW_ERR_CUDA; }
+    cudaStreamSynchronize(st);
+    cudaStreamDestroy(st);
+    cudaFree(dev);
+    return rc;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// FP64 peak probe: 16 independent DFMA chains per thread, all in registers.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void few_fp64_peak_kernel(int iters, double* sink)
+{
+    double a[16];
+    const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-12 * (blockIdx.x + 1);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = 1.0 + i * 1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fma(a[i], x, y);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double* sink, void* stream)
+{
+    FEW_REQUIRE(ctx && sink, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(blocks > 0 && threads > 0 && threads <= 1024 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
+    few_fp64_peak_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    return FEW_OK;
+}

@@ -1,0 +1,84 @@
+// few_ylm.cu -- S0: spin-weight -2 spherical harmonics as per-source constants (Eq. (10):
+// "the regular -2 spin-weighted spherical harmonics ... constant over the whole orbit").
+//
+// Computed from the Wigner small-d function,  sY_lm(theta, phi) = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},
+//   d^l_{a,b}(beta) = sqrt((l+a)!(l-a)!(l+b)!(l-b)!) sum_k (-1)^{a-b+k} cos(beta/2)^{2l+b-a-2k} sin(beta/2)^{a-b+2k}
+//                     / ((l+b-k)! k! (a-b+k)! (l-a-k)!),
+// which agrees with the Goldberg et al. convention (R11).  One thread per (source, mode); the same
+// __host__ __device__ routine backs the host helper few_ylm.
+#include <math.h>
+#include "few_common.cuh"
+
+__host__ __device__ static inline double few_fact(int k)
+{
+    double f = 1.0;
+    for (int i = 2; i <= k; ++i) f *= (double)i;
+    return f;
+}
+
+__host__ __device__ static inline double few_ipow(double x, int e)
+{
+    double r = 1.0;
+    for (int i = 0; i < e; ++i) r *= x;
+    return r;
+}
+
+// -2Y_lm(theta, phi); caller guarantees 2 <= l <= FEW_MAX_L, |m| <= l.
+__host__ __device__ static inline void few_ylm_m2(int l, int m, double theta, double phi, double* re, double* im)
+{
+    const int a = m, b = 2;                    // d^l_{m, -s}, s = -2
+    const double ch = cos(0.5 * theta), sh = sin(0.5 * theta);
+    int k0 = (b - a) > 0 ? (b - a) : 0;        // a - b + k >= 0
+    int k1 = (l + b) < (l - a) ? (l + b) : (l - a);
+    double tot = 0.0;
+    for (int k = k0; k <= k1; ++k) {
+        double term = few_ipow(ch, 2 * l + b - a - 2 * k) * few_ipow(sh, a - b + 2 * k) /
+                      (few_fact(l + b - k) * few_fact(k) * few_fact(a - b + k) * few_fact(l - a - k));
+        tot += ((a - b + k) & 1) ? -term : term;
+    }
+    double d = sqrt(few_fact(l + a) * few_fact(l - a) * few_fact(l + b) * few_fact(l - b)) * tot;
+    double v = sqrt((2.0 * l + 1.0) / (4.0 * 3.14159265358979323846)) * d;   // (-1)^s = +1
+    *re = v * cos(m * phi);
+    *im = v * sin(m * phi);
+}
+
+extern "C" int few_ylm(int l, int m, double theta, double phi, double* out_host)
+{
+    FEW_REQUIRE(out_host != nullptr, FEW_ERR_INVALID_ARG, "out is NULL");
+    FEW_REQUIRE(l >= 2 && l <= FEW_MAX_L && m <= l && m >= -l, FEW_ERR_BAD_MODE, "need 2 <= l <= FEW_MAX_L and |m| <= l");
+    few_ylm_m2(l, m, theta, phi, &out_host[0], &out_host[1]);
+    return FEW_OK;
+}
+
+__global__ void few_ylm_modes_kernel(const double* __restrict__ theta, const double* __restrict__ phi,
+                                     const int* __restrict__ l, const int* __restrict__ m, int n_src, int n_modes,
+                                     double2* __restrict__ ylm_plus, double2* __restrict__ ylm_minus, int* status)
+{
+    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (long long)n_src * n_modes) return;
+    int s = (int)(gid / n_modes), j = (int)(gid % n_modes);
+    int lj = l[j], mj = m[j];
+    double2 yp = make_double2(0.0, 0.0), ym = yp;
+    if (lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj) {
+        atomicOr(status, FEW_DEV_BAD_MODE);
+    } else {
+        few_ylm_m2(lj, mj, theta[s], phi[s], &yp.x, &yp.y);
+        few_ylm_m2(lj, -mj, theta[s], phi[s], &ym.x, &ym.y);
+    }
+    ylm_plus[gid] = yp;
+    ylm_minus[gid] = ym;
+}
+
+extern "C" int few_ylm_modes(few_ctx* ctx, const double* theta, const double* phi, const int* l, const int* m,
+                             int n_src, int n_modes, double* ylm_plus, double* ylm_minus, void* stream)
+{
+    FEW_REQUIRE(ctx && theta && phi && l && m && ylm_plus && ylm_minus, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(n_src > 0 && n_modes > 0, FEW_ERR_INVALID_ARG, "n_src and n_modes must be positive");
+    long long total = (long long)n_src * n_modes;
+    int threads = 128;
+    unsigned blocks = (unsigned)((total + threads - 1) / threads);
+    few_ylm_modes_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(theta, phi, l, m, n_src, n_modes,
+                                                                      (double2*)ylm_plus, (double2*)ylm_minus, ctx->d_status);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    return FEW_OK;
+}
