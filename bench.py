@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the FEW interpolated mode-summation hot path on B200 (one process per GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+
+A step is ONE pass of the whole hot path (S0 harmonics, S2 mode selection, S1 spline fits, S3 summation; DESIGN.md
+section 1) over one synthetic workload: by default BASELINE.json configs[1], the one-year single-source waveform with
+eps = 1e-5 that the metric "ms per 1-yr FP64 waveform; sample*mode evals/s; % of FP64 roofline" is quoted on.
+With N > 1 every rank runs its own copy of the workload (independent waveforms, as in an MCMC: weak scaling, no
+data-path collective); value = total sample*mode evaluations of all ranks / max-over-ranks time.
+
+Prints ONE JSON line (see the keys at the bottom).  `--impl reference` times the CPU oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FLOP_PER_EVAL = 20.0          # algorithmic: complex cubic Horner (6 DFMA) + complex multiply-accumulate (4 DFMA), DESIGN.md section 6
+DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
+GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 + spline_dd 1 + sum 3
+GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.rows, self.stop_evt, self.index = [], threading.Event(), index
+        self.thread = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        try:
+            proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                     "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return
+        try:
+            while not self.stop_evt.is_set():
+                line = proc.stdout.readline()
+                if not line:
+                    break
+                self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
+        finally:
+            proc.terminate()
+
+    def start(self): self.thread.start()
+
+    def stop(self, t_begin: float, t_end: float):
+        self.stop_evt.set(); self.thread.join(timeout=3)
+        rows = [r for (ts, r) in self.rows if t_begin <= ts <= t_end + 0.15] or [r for (_, r) in self.rows[-3:]]
+        sm = [float(r[0]) for r in rows if r and r[0].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in rows for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        mx = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "reasons": reasons, "samples": len(rows)}
+
+
+def oracle_sample(w, target_s: float):
+    """Times the CPU oracle, as it stands, on a bounded contiguous slice of the workload (whole path: harmonics,
+    selection, spline fits, summation).  Returns (evals/s, description, cores, seconds)."""
+    import oracle
+    from paper_2104_04582_b200 import synth
+    oracle.build()
+    cores = oracle.num_threads()
+    mid = (w.n_samples // 2) // 256 * 256
+
+    def run(n):
+        ws = synth.Workload(w.name, w.t[:1], w.phase[:1], w.amp[:1], w.l, w.m, w.n, w.theta[:1], w.phi[:1],
+                            w.t0 + mid * w.dt, w.dt, n, w.eps)
+        t0 = time.perf_counter()
+        _, parts = oracle.waveform(ws, return_parts=True)
+        return time.perf_counter() - t0, len(parts[0]["keep_idx"])
+
+    t_cal, K = run(4096)
+    rate = 4096 * K / t_cal
+    n = int(min(max(target_s * rate / K, 4096), w.n_samples - mid, 1 << 22))
+    t_run, K = run(n)
+    return n * K / t_run, f"{n} contiguous samples of source 0 from sample {mid}, whole path, K={K}", cores, t_run, n, K
+
+
+def reference_arm(args):
+    """--impl reference: the CPU oracle on the host cores, each step a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2104_04582_b200 import synth
+    w = synth.make_config(args.config)
+    per_step = max(6.0, min(30.0, 120.0 / max(args.steps + args.warmup, 1)))
+    vals, times = [], []
+    desc = cores = None
+    for i in range(args.warmup + args.steps):
+        v, desc, cores, t_run, n, K = oracle_sample(w, per_step if i >= args.warmup else 2.0)
+        if i >= args.warmup:
+            vals.append(v); times.append(t_run)
+    value = float(np.mean(vals))
+    out = {"impl": "reference", "metric": "sample*mode evaluations per second (1-yr FP64 waveform, whole hot path)", "value": value,
+           "unit": "evals/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "n_samples_full": w.n_samples, "eps": w.eps,
+                                                            "n_modes": w.n_modes, "n_t": w.n_t},
+           "cpu_baseline": {"value": value, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc},
+           "e2e": {"value": value, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = headline; 2, 3, 4 for profiling)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--eps", type=float, default=None)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return reference_arm(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2104_04582_b200 import api, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    w = synth.make_config(args.config, eps=args.eps)
+    host = dict(t=w.t, phase=w.phase, amp=w.amp, l=w.l, m=w.m, n=w.n, theta=w.theta, phi=w.phi)
+    pinned = {k: torch.as_tensor(np.ascontiguousarray(v)).pin_memory() for k, v in host.items()}
+    g = {k: v.to(dev) for k, v in pinned.items()}
+    h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
+    keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device=dev)
+    nk = torch.empty((w.n_src,), dtype=torch.int32, device=dev)
+    ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)            # > 126 MB L2
+    api.few_profile_enable(True)
+
+    def step():
+        api.few_waveform(g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
+                         w.n_samples, out=h, keep_idx=keep, n_keep=nk, workspace=ws)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1); step()
+    api.few_device_status()
+    K_kept = int(nk.sum().item())            # kept modes summed over sources
+    evals_per_step = float(w.n_samples) * K_kept
+
+    # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
+    sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
+    api.few_fp64_peak_probe(148 * 8, 256, 2000, sink)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(); e0.record()
+    probe_flops = api.few_fp64_peak_probe(148 * 8, 256, 20000, sink)
+    e1.record(); torch.cuda.synchronize()
+    fp64_measured_tflops = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start(); time.sleep(0.3)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sum_ms = []
+    barrier()
+    t_begin = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                      # L2 flush between timed iterations (outside the event pair)
+        a.record(); step(); b.record()
+        sum_ms.append(api.few_profile_sum_ms())     # waits for this step's hot kernel: its own CUDA events on the launch stream
+    barrier()
+    t_end = time.perf_counter()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+        ev_all = torch.tensor([evals_per_step], dtype=torch.float64, device=dev)
+        dist.all_reduce(ev_all, op=dist.ReduceOp.SUM)
+        evals_all = float(ev_all.item())
+    else:
+        evals_all = evals_per_step
+    clocks = sampler.stop(t_begin, t_end) if sampler else None
+    ms_per_step = float(total_ms.item()) / args.steps
+    value = evals_all / (ms_per_step * 1e-3)
+
+    # e2e: the same metric through the C-ABI call with HOST buffers (H2D of the inputs and D2H of h inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        h_host = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128).pin_memory()
+        p = pinned
+        call = lambda: api.few_waveform_host(p["t"], p["phase"], p["amp"], p["l"], p["m"], p["n"], p["theta"], p["phi"], w.eps, w.t0,
+                                             w.dt, w.n_samples, out=h_host, device=local)
+        call()
+        n_e2e = max(3, min(args.steps, 10))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            call()                           # synchronous: returns after the D2H copy completed
+        t_e2e = torch.tensor([(time.perf_counter() - t0) / n_e2e], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        h2d = sum(v.numel() * v.element_size() for v in pinned.values())
+        e2e = {"value": evals_all / float(t_e2e.item()), "unit": "evals/s", "ms_per_step": 1e3 * float(t_e2e.item()),
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h_host.numel() * 16),
+               "note": "few_waveform_host: cudaMalloc + H2D + 9 kernels + D2H + free, pinned host buffers"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
+    sum_ms_avg = float(np.mean(sum_ms))
+    peak_tflops = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    achieved_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "few_sum_kernel", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved_tflops / peak_tflops, "traffic": None,
+                "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
+                "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
+                "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
+                "algorithmic": f"{FLOP_PER_EVAL:.0f} flop per sample*mode evaluation x {evals_per_step:.4g} evaluations per launch"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, desc, cores, t_run, n, K = oracle_sample(w, 12.0)
+        cpu = {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": t_run}
+    out = {"metric": "sample*mode evaluations per second (1-yr FP64 waveform, whole hot path)", "value": value, "unit": "evals/s",
+           "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": w.name, "n_src": w.n_src, "n_t": w.n_t, "n_modes": w.n_modes, "n_samples": w.n_samples, "dt": w.dt,
+                      "eps": w.eps, "kept_modes": K_kept, "l2": "flushed between timed steps (256 MiB write)",
+                      "parallelism": f"{world} independent replicas" if world > 1 else "single GPU"},
+           "ms_per_waveform": ms_per_step / w.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+           "gpu_launches": (GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) * args.steps, "clocks": clocks,
+           "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

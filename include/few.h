@@ -57,7 +57,7 @@ enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_TOO_MANY_L = 4 
 #define FEW_MAX_L 63            /* l <= 63 (factorials in FP64, 64-bit l masks) */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
 #define FEW_MAX_L_PER_M 9       /* at most 9 distinct l per m among the kept modes (l in [2,10]) */
-#define FEW_MAX_NT_SPLINE 896   /* n_t limit of few_spline_fit (one shared-memory column per system) */
+#define FEW_MAX_NT_SPLINE 760   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
 
 typedef struct few_ctx few_ctx;
@@ -146,6 +146,13 @@ int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_ho
  * Launches `blocks` x `threads` threads, each doing `iters` x 16 dependent-chain-free DFMAs; writes one double per thread
  * to sink[blocks*threads].  FLOPs = 2 * 16 * iters * blocks * threads. */
 int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double* sink, void* stream);
+
+/* ---- Measurement aid: with profiling on, few_sum_waveform (also inside few_waveform) brackets its hot kernel
+ * (few_sum_kernel, the dominant launch of the path) with two CUDA events on the caller's stream.  few_profile_sum_ms
+ * waits for the closing event of the most recent launch and writes its duration in milliseconds to ms_host.
+ * FEW_ERR_INVALID_ARG if profiling is off or nothing was launched since it was switched on. */
+int few_profile_enable(few_ctx* ctx, int on);
+int few_profile_sum_ms(few_ctx* ctx, float* ms_host);
 
 #ifdef __cplusplus
 }

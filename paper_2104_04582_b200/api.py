@@ -20,7 +20,7 @@ FEW_OK = 0
 SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_version", "few_device_status", "few_ylm",
            "few_ylm_modes", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
-           "few_fp64_peak_probe"]
+           "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms"]
 
 
 class FewError(RuntimeError):
@@ -55,6 +55,8 @@ def _load() -> C.CDLL:
         "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
         "few_fp64_peak_probe": (i, [vp, i, i, i, vp, vp]),
+        "few_profile_enable": (i, [vp, i]),
+        "few_profile_sum_ms": (i, [vp, C.POINTER(C.c_float)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -223,3 +225,14 @@ def few_fp64_peak_probe(blocks: int, threads: int, iters: int, sink=None):
     sink = sink if sink is not None else torch.empty(blocks * threads, dtype=torch.float64, device="cuda")
     _chk(_lib.few_fp64_peak_probe(context(), blocks, threads, iters, _p(sink), _stream()), "few_fp64_peak_probe")
     return 2.0 * 16 * iters * blocks * threads   # FLOPs launched
+
+
+def few_profile_enable(on: bool = True) -> None:
+    _chk(_lib.few_profile_enable(context(), int(bool(on))), "few_profile_enable")
+
+
+def few_profile_sum_ms() -> float:
+    """Duration (ms) of the most recent few_sum_kernel launch, from the library's own CUDA events on the launch stream."""
+    ms = C.c_float(0.0)
+    _chk(_lib.few_profile_sum_ms(context(), C.byref(ms)), "few_profile_sum_ms")
+    return float(ms.value)

@@ -47,6 +47,8 @@ extern "C" int few_create(few_ctx** out, int device)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_status, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev_sum[0]);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev_sum[1]);
     if (e != cudaSuccess) {
         few_set_error("few_create: %s", cudaGetErrorString(e));
         delete c;
@@ -60,7 +62,26 @@ extern "C" int few_destroy(few_ctx* ctx)
 {
     if (!ctx) return FEW_OK;
     cudaFree(ctx->d_status);
+    if (ctx->ev_sum[0]) cudaEventDestroy(ctx->ev_sum[0]);
+    if (ctx->ev_sum[1]) cudaEventDestroy(ctx->ev_sum[1]);
     delete ctx;
+    return FEW_OK;
+}
+
+extern "C" int few_profile_enable(few_ctx* ctx, int on)
+{
+    FEW_REQUIRE(ctx != nullptr, FEW_ERR_INVALID_ARG, "ctx is NULL");
+    ctx->profile = on ? 1 : 0;
+    ctx->profile_valid = 0;
+    return FEW_OK;
+}
+
+extern "C" int few_profile_sum_ms(few_ctx* ctx, float* ms_host)
+{
+    FEW_REQUIRE(ctx && ms_host, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(ctx->profile && ctx->profile_valid, FEW_ERR_INVALID_ARG, "profiling is off or no summation was launched");
+    FEW_CUDA_CHECK(cudaEventSynchronize(ctx->ev_sum[1]));
+    FEW_CUDA_CHECK(cudaEventElapsedTime(ms_host, ctx->ev_sum[0], ctx->ev_sum[1]));
     return FEW_OK;
 }
 

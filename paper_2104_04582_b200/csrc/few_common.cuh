@@ -10,6 +10,9 @@ struct few_ctx {
     int sm_count;
     int smem_optin;      // max dynamic shared memory per block (bytes)
     int* d_status;       // device status word (FEW_DEV_* bits)
+    int profile;         // few_profile_enable
+    int profile_valid;   // a sum kernel was bracketed since profiling was switched on
+    cudaEvent_t ev_sum[2];
 };
 
 void few_set_error(const char* fmt, ...);

@@ -116,7 +116,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     int* sj = uj + n_modes;                                       // [n_modes]
     unsigned short* gid = reinterpret_cast<unsigned short*>(sj + n_modes);   // [n_modes]
     unsigned short* rid = gid + n_modes;                          // [n_modes]
-    int* gmask = reinterpret_cast<int*>(rid + n_modes + (n_modes & 1));      // [n_modes]
+    int* gmask = reinterpret_cast<int*>(rid + n_modes);                      // [n_modes] (gid + rid = 4 n_modes bytes: aligned)
     __shared__ unsigned long long run_l[kMaxRuns];
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
@@ -440,8 +440,10 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
     FEW_CUDA_CHECK(cudaGetLastError());
     few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_keep, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
+    if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     few_sum_kernel<kSumR><<<dim3((unsigned)max_tiles, n_src), kSumThreads, 0, st>>>(t, (const dd*)coef_phase_dd, t0, dt, n_samples,
                                                                                    n_t, n_modes, L, (double2*)h);
     FEW_CUDA_CHECK(cudaGetLastError());
+    if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     return FEW_OK;
 }

@@ -66,7 +66,7 @@ def test_ylm_modes_vs_oracle(api):
 
 # ------------------------------------------------------------------------------------------- S1
 @pytest.mark.parametrize("n_t,n_sys,uniform", [(4, 1, True), (5, 33, False), (20, 18, True), (100, 257, False), (100, 7688, False),
-                                              (300, 129, False), (896, 40, False)])
+                                              (300, 129, False), (760, 40, False)])
 def test_spline_fit_vs_oracle(api, n_t, n_sys, uniform):
     rng = np.random.default_rng(n_t * 1000 + n_sys)
     n_src = 2
@@ -285,8 +285,15 @@ def test_bad_modes_reported(api):
     bad_m = w.m.copy(); bad_m[2] = w.l[2] + 1
     api.few_ylm_modes(g["theta"], g["phi"], g["l"], dev(bad_m))
     assert api.few_device_status(raise_on_error=False) == -4             # FEW_ERR_BAD_MODE
-    with pytest.raises(api.FewError):
-        api.few_sum_waveform(g["t"], g["t"], g["t"], g["l"], g["m"], g["n"], None, None, g["t"], g["t"], 0.0, -1.0, 10)
+    yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
+    with pytest.raises(api.FewError) as e:                               # dt <= 0 is rejected on the host
+        api.few_sum_waveform(g["t"], g["t"], g["t"], g["l"], g["m"], g["n"], None, None, yp, ym, 0.0, -1.0, 10)
+    assert e.value.code == -1
+    # a kept list with more than 9 distinct l for one m is reported by the plan kernel
+    l = np.arange(2, 13, dtype=np.int32); m = np.zeros_like(l); n = np.zeros_like(l)
+    t = dev(np.linspace(0, 10, 6)[None]); amp = dev(np.ones((1, 6, len(l)), np.complex128)); ph = dev(np.zeros((1, 6, 2)))
+    api.few_waveform(t, ph, amp, dev(l), dev(m), dev(n), dev(np.array([0.7])), dev(np.array([1.1])), 0.0, 0.0, 0.1, 16)
+    assert api.few_device_status(raise_on_error=False) == -4
 
 
 def test_whole_path_host_buffers(api):
