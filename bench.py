@@ -28,7 +28,8 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-FLOP_PER_EVAL = 20.0          # algorithmic: complex cubic Horner (6 DFMA) + complex multiply-accumulate (4 DFMA), DESIGN.md section 6
+FLOP_PER_EVAL = 20.0          # nominal per-mode figure of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA)
+FLOP_PER_PAIR = 38.0          # executed algorithm: per sample and (m,n) pair 18 DFMA + 2 DMUL = 20 FP64 slots
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
 GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 + spline_dd 1 + sum 3
 GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
@@ -183,6 +184,10 @@ def main():
     api.few_device_status()
     K_kept = int(nk.sum().item())            # kept modes summed over sources
     evals_per_step = float(w.n_samples) * K_kept
+    # (m, n) pairs among the kept modes (bookkeeping for the roofline: the kernel sums all l of a pair into one spline pair)
+    keep_h, nk_h = keep.cpu().numpy(), nk.cpu().numpy()
+    pairs = sum(len({(int(w.m[j]), int(w.n[j])) for j in keep_h[s, : nk_h[s]]}) for s in range(w.n_src))
+    pair_evals_per_step = float(w.n_samples) * pairs
 
     # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
     sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
@@ -248,13 +253,18 @@ def main():
     hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
     sum_ms_avg = float(np.mean(sum_ms))
     peak_tflops = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    achieved_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
+    achieved_tflops = pair_evals_per_step * FLOP_PER_PAIR / (sum_ms_avg * 1e-3) / 1e12
+    nominal_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "few_sum_kernel", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops, "traffic": None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
-                "algorithmic": f"{FLOP_PER_EVAL:.0f} flop per sample*mode evaluation x {evals_per_step:.4g} evaluations per launch"}
+                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {pair_evals_per_step:.4g} "
+                               f"pair evaluations per launch ({pairs} pairs from {K_kept} kept modes)",
+                "nominal_per_mode": {"achieved": nominal_tflops, "frac": nominal_tflops / peak_tflops,
+                                     "note": "20 flop per sample*mode evaluation (per-mode formulation); exceeds the executed "
+                                             "figure because all l of an (m,n) pair are summed into one spline before the sample loop"}}
     cpu = None
     if not args.no_cpu_baseline:
         v, desc, cores, t_run, n, K = oracle_sample(w, 12.0)
@@ -263,7 +273,7 @@ def main():
            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": w.name, "n_src": w.n_src, "n_t": w.n_t, "n_modes": w.n_modes, "n_samples": w.n_samples, "dt": w.dt,
-                      "eps": w.eps, "kept_modes": K_kept, "l2": "flushed between timed steps (256 MiB write)",
+                      "eps": w.eps, "kept_modes": K_kept, "mn_pairs": pairs, "l2": "flushed between timed steps (256 MiB write)",
                       "parallelism": f"{world} independent replicas" if world > 1 else "single GPU"},
            "ms_per_waveform": ms_per_step / w.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
            "gpu_launches": (GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) * args.steps, "clocks": clocks,

@@ -52,11 +52,10 @@ enum {
 };
 
 /* bits of the device status word */
-enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_TOO_MANY_L = 4 };
+enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
 
 #define FEW_MAX_L 63            /* l <= 63 (factorials in FP64, 64-bit l masks) */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
-#define FEW_MAX_L_PER_M 9       /* at most 9 distinct l per m among the kept modes (l in [2,10]) */
 #define FEW_MAX_NT_SPLINE 760   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
 

@@ -24,7 +24,7 @@ extern "C" const char* few_strerror(int code)
         case FEW_ERR_INVALID_ARG: return "FEW_ERR_INVALID_ARG: NULL pointer, non-positive size or bad flag";
         case FEW_ERR_TOO_FEW_POINTS: return "FEW_ERR_TOO_FEW_POINTS: a not-a-knot cubic spline needs n_t >= 4";
         case FEW_ERR_NOT_INCREASING: return "FEW_ERR_NOT_INCREASING: sparse times are not strictly increasing";
-        case FEW_ERR_BAD_MODE: return "FEW_ERR_BAD_MODE: need 2 <= l <= FEW_MAX_L, 0 <= m <= l, |n| <= FEW_MAX_ABS_N, <= 9 distinct l per m";
+        case FEW_ERR_BAD_MODE: return "FEW_ERR_BAD_MODE: need 2 <= l <= FEW_MAX_L, 0 <= m <= l, |n| <= FEW_MAX_ABS_N";
         case FEW_ERR_WORKSPACE: return "FEW_ERR_WORKSPACE: workspace NULL, misaligned or too small";
         case FEW_ERR_CUDA: return "FEW_ERR_CUDA: CUDA runtime error";
         case FEW_ERR_LIMIT: return "FEW_ERR_LIMIT: size beyond a documented FEW_MAX_* limit";
@@ -95,7 +95,7 @@ extern "C" int few_device_status(few_ctx* ctx, int* bits_out, void* stream)
     FEW_CUDA_CHECK(cudaStreamSynchronize(st));
     if (bits_out) *bits_out = bits;
     if (bits & FEW_DEV_NOT_INCREASING) { few_set_error("device check: sparse times not strictly increasing"); return FEW_ERR_NOT_INCREASING; }
-    if (bits & (FEW_DEV_BAD_MODE | FEW_DEV_TOO_MANY_L)) { few_set_error("device check: invalid (l, m, n) or more than 9 distinct l for one m"); return FEW_ERR_BAD_MODE; }
+    if (bits & FEW_DEV_BAD_MODE) { few_set_error("device check: invalid (l, m, n) or kept-mode index"); return FEW_ERR_BAD_MODE; }
     return FEW_OK;
 }
 

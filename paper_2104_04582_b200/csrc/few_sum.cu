@@ -4,59 +4,71 @@
 //    ... only compute modes for m >= 0 ... the modes in a single time step are combined."
 //   h(t_i) = scale * sum_{j kept} [ Y+_j W_j + (m_j>0) (-1)^{l_j} Y-_j conj(W_j) ],  W_j = A_j(t_i) exp(-i(m_j Phi_phi + n_j Phi_r)).
 //
+// Algebra used (exact): with E = exp(-i theta) = e_r + i e_i and Ybar = (-1)^l Y- (0 for m = 0),
+//   Y+ A E + Ybar conj(A) conj(E) = e_r U + e_i V,   U = Y+ A + Ybar conj(A),   V = i (Y+ A - Ybar conj(A)).
+// U and V are linear in A's spline coefficients, and E depends on (m, n) only, so all kept l of one (m, n) PAIR are summed
+// into one pair of complex cubics (U_mn, V_mn) per sparse segment BEFORE the sample loop.  The hot loop then costs, per
+// sample and pair, 12 DFMA (two complex cubic Horners) + 4 DFMA (h += e_r U + e_i V) + 4 (E *= Z_r), with no per-l state.
+//
 // Three launches per call, all on the caller's stream, nothing read back to the host:
-//   1. few_sum_plan_kernel  (one block per source)
-//        - clips the dense sample grid to the sparse segments (first sample of every knot) and prefix-sums the
-//          per-segment tile counts, so that every block of the sum kernel works inside ONE segment (uniform coefficients);
-//        - orders the kept modes by (m, sign n, |n|, l) and describes them as "groups" (one (m, n) pair with a bit mask
-//          of the l present) inside "runs" (one m): E_mn = Z_phi^m Z_r^n is then built by ONE complex multiply per
-//          group (walking n upward from 0 with Z_r, downward with conj Z_r), shared by all l of the group;
-//        - folds Y+, (-1)^l Y- and scale into 4 real constants per (m, l).
-//   2. few_sum_pack_kernel  gathers the kept modes' spline coefficients into plan order, 64 contiguous bytes per mode
-//        and segment (c0..c3 x re,im), so the hot loop streams them with 128-bit uniform loads.
-//   3. few_sum_kernel       the hot loop.  Per thread R samples in registers; per sample the two phases are evaluated
-//        ONCE in double-double (Horner on the dd coefficients, reduction by 2 pi in dd, one sincos each) giving
-//        Z_phi = exp(-i Phi_phi), Z_r = exp(-i Phi_r); per mode 6 DFMA (complex cubic Horner) + 4 DFMA (S_l += A E);
-//        per group 4 DFMA (E *= Z_r); per (m, l) 4 DFMA (fold into h).  Output: coalesced 16-byte stores.
-// FP64 pipe only: the path is elementwise work with a reduction over modes, not a dense contraction.
+//   1. few_sum_plan_kernel  (one block per source): clips the dense sample grid to the sparse segments and prefix-sums
+//        the per-segment tile counts (every block of the sum kernel works inside ONE segment, so its coefficients are
+//        block-uniform); orders the kept modes by (m, sign n, |n|, l), finds the pairs and describes how E_mn = Z_phi^m Z_r^n
+//        is reached from the previous pair (walking n upward from 0 with Z_r, then downward with conj Z_r).
+//   2. few_sum_pack_kernel  (one block per source and segment): forms (U_mn, V_mn) from the kept modes' spline coefficients
+//        and Y+, Ybar, scale, and writes them as a stream of 4 KB stages (30 pairs x 128 B + 30 descriptors).
+//   3. few_sum_kernel       the hot loop.  Stages arrive in shared memory through a ring of TMA bulk copies
+//        (cp.async.bulk + mbarrier) and are read with 128-bit broadcast loads.  Each thread owns R samples in registers;
+//        per sample the two phases are evaluated ONCE in double-double (Horner, reduction by 2 pi, one sincos each).
+//        Output: coalesced 16-byte streaming stores.
+// FP64 pipe only: per-sample elementwise work with a reduction over modes, not a dense contraction.
 #include "few_common.cuh"
 
 namespace {
 
-constexpr int kNSlot = FEW_MAX_L_PER_M;      // accumulators S_l per m-run
-constexpr int kMaxRuns = FEW_MAX_L + 1;      // distinct m values
 constexpr int kPlanThreads = 1024;
 constexpr int kSumThreads = 128;
-constexpr int kSumR = 2;                     // samples per thread
-constexpr int kTile = kSumThreads * kSumR;   // samples per block
+constexpr int kSumR = 4;                      // samples per thread
+constexpr int kTile = kSumThreads * kSumR;    // samples per block
+constexpr int kStagePairs = 30;               // pairs per stage
+constexpr int kStageBytes = 4096;             // 30 * 128 B of coefficients + 64 ints of header
+constexpr int kStageD2 = kStageBytes / 16;    // stage size in double2
+constexpr int kRing = 4;                      // stages in flight per block
 
-// group descriptor bits
-constexpr int kMaskBits = 9, kAdvShift = 9, kAdvBits = 12;
-constexpr int kNewSub = 1 << 21, kDirNeg = 1 << 22, kDmShift = 23, kNewRun = 1 << 30;
+// pair descriptor: bit 0 = special (anything but "advance E by one step"); then
+constexpr int kAdvShift = 1, kAdvBits = 12;   // number of E steps before this pair
+constexpr int kNewSub = 1 << 13;              // restart E from Z_phi^m (n changes sign or m changes)
+constexpr int kDirNeg = 1 << 14;              // walk with conj(Z_r)
+constexpr int kDmShift = 15, kDmBits = 7;     // m increment of a new run
+constexpr int kNewRun = 1 << 22;
 
 struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
     int* tile_start;     // [n_src][n_t + 2]   exclusive prefix of tiles per pseudo-segment; last = total
-    int* n_groups;       // [n_src]
-    int* grp;            // [n_src][n_modes]
-    int* order_j;        // [n_src][n_modes]   mode index of packed slot r
-    int* run_mask;       // [n_src][kMaxRuns]  slot mask of each run
-    double* yc;          // [n_src][kMaxRuns][kNSlot][4]
-    double* pack;        // [n_src][n_t - 1][n_modes][8]
+    int* n_groups;       // [n_src]            number of (m, n) pairs
+    int* desc;           // [n_src][n_modes]   pair descriptors
+    int* g_first;        // [n_src][n_modes+1] first sorted mode of each pair
+    int* order_j;        // [n_src][n_modes]   mode index of sorted position r
+    double* yfold;       // [n_src][n_modes][4] scale * (Y+ re, Y+ im, Ybar re, Ybar im) of sorted position r
+    double* pack;        // [n_src][n_t - 1][max_stages][kStageBytes / 8]
+    int max_stages;
 };
+
+__host__ __device__ inline int stages_for(int n_pairs) { return (n_pairs + kStagePairs - 1) / kStagePairs; }
 
 sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, size_t* bytes = nullptr)
 {
     few_carver c(ws);
     sum_layout L;
+    L.max_stages = stages_for(n_modes);
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
     L.n_groups = c.take<int>(n_src);
-    L.grp = c.take<int>((size_t)n_src * n_modes);
+    L.desc = c.take<int>((size_t)n_src * n_modes);
+    L.g_first = c.take<int>((size_t)n_src * (n_modes + 1));
     L.order_j = c.take<int>((size_t)n_src * n_modes);
-    L.run_mask = c.take<int>((size_t)n_src * kMaxRuns);
-    L.yc = c.take<double>((size_t)n_src * kMaxRuns * kNSlot * 4);
-    L.pack = c.take<double>((size_t)n_src * (n_t - 1) * n_modes * 8);
+    L.yfold = c.take<double>((size_t)n_src * n_modes * 4);
+    L.pack = c.take<double>((size_t)n_src * (n_t - 1) * L.max_stages * (kStageBytes / 8));
     if (bytes) *bytes = c.off;
     return L;
 }
@@ -97,6 +109,7 @@ __device__ __forceinline__ int plan_block_scan(int v, int* warp_sums, int* total
     return res;
 }
 
+// sort key: m | sign(n) | |n| | l  (ascending): runs of equal m, inside them n = 0, 1, 2, ... then -1, -2, ...
 __device__ __forceinline__ int key_m(unsigned k) { return (int)(k >> 21); }
 __device__ __forceinline__ int key_dir(unsigned k) { return (int)(k >> 20) & 1; }
 __device__ __forceinline__ int key_absn(unsigned k) { return (int)(k >> 8) & 0xfff; }
@@ -114,10 +127,6 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     unsigned* skey = ukey + n_modes;                              // [n_modes] sorted keys
     int* uj = reinterpret_cast<int*>(skey + n_modes);             // [n_modes]
     int* sj = uj + n_modes;                                       // [n_modes]
-    unsigned short* gid = reinterpret_cast<unsigned short*>(sj + n_modes);   // [n_modes]
-    unsigned short* rid = gid + n_modes;                          // [n_modes]
-    int* gmask = reinterpret_cast<int*>(rid + n_modes);                      // [n_modes] (gid + rid = 4 n_modes bytes: aligned)
-    __shared__ unsigned long long run_l[kMaxRuns];
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
 
@@ -149,7 +158,6 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
 
     // ---- (b) kept modes -> keys
     const int K = n_keep ? min(max(n_keep[src], 0), n_modes) : n_modes;
-    for (int r = tid; r < kMaxRuns; r += kPlanThreads) run_l[r] = 0ull;
     for (int q = tid; q < K; q += kPlanThreads) {
         int j = keep_idx ? keep_idx[(size_t)src * n_modes + q] : q;
         bool ok = j >= 0 && j < n_modes;
@@ -171,89 +179,89 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         skey[rank] = key; sj[rank] = uj[q];
     }
     __syncthreads();
-    // ---- (d) group / run ids by a chunked scan of boundary flags (group count low 16 bits, run count high 16 bits)
+    // ---- (d) pairs: chunked scan of "new (m, n)" flags; descriptors; per-mode fold constants
     if (tid == 0) carry_s = 0;
     __syncthreads();
+    int* desc = L.desc + (size_t)src * n_modes;
+    int* gfirst = L.g_first + (size_t)src * (n_modes + 1);
+    int* oj = L.order_j + (size_t)src * n_modes;
+    double* yf = L.yfold + (size_t)src * n_modes * 4;
+    const double sc = scale ? scale[src] : 1.0;
     for (int base = 0; base < K; base += kPlanThreads) {
-        int r = base + tid, flag = 0;
+        int r = base + tid;
+        bool new_run = false, new_sub = false, new_grp = false;
+        unsigned key = 0, prev = 0;
         if (r < K) {
-            unsigned key = skey[r], prev = r ? skey[r - 1] : 0u;
-            bool new_run = r == 0 || key_m(key) != key_m(prev);
-            bool new_grp = new_run || (key >> 8) != (prev >> 8);
-            flag = (new_grp ? 1 : 0) | (new_run ? 1 << 16 : 0);
+            key = skey[r]; prev = r ? skey[r - 1] : 0u;
+            new_run = r == 0 || key_m(key) != key_m(prev);
+            new_sub = new_run || key_dir(key) != key_dir(prev);
+            new_grp = new_sub || key_absn(key) != key_absn(prev);
         }
-        int total, incl = plan_block_scan(flag, warp_sums, &total);
+        int total, incl = plan_block_scan(new_grp ? 1 : 0, warp_sums, &total);
         int carry = carry_s;
         if (r < K) {
-            int v = carry + incl;
-            gid[r] = (unsigned short)((v & 0xffff) - 1);
-            int ru = (v >> 16) - 1;
-            rid[r] = (unsigned short)ru;
-            atomicOr(&run_l[ru], 1ull << key_l(skey[r]));
-            gmask[r] = 0;
+            int j = sj[r];
+            oj[r] = j;
+            if (new_grp) {
+                int g = carry + incl - 1;
+                int nadv = new_sub ? key_absn(key) : key_absn(key) - key_absn(prev);
+                int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
+                int d = (nadv << kAdvShift) | (new_sub ? kNewSub : 0) | (key_dir(key) ? kDirNeg : 0) | (dm << kDmShift) |
+                        (new_run ? kNewRun : 0);
+                if (new_sub || nadv != 1) d |= 1;
+                desc[g] = d;
+                gfirst[g] = r;
+            }
+            double2 yp = ylm_plus[(size_t)src * n_modes + j], yb = make_double2(0.0, 0.0);
+            if (key_m(key) > 0) {                       // Eq. (9): the (l,-m,-n) mirror, Ybar = (-1)^l Y_{l,-m}
+                double2 ym = ylm_minus[(size_t)src * n_modes + j];
+                double sg = (key_l(key) & 1) ? -1.0 : 1.0;
+                yb = make_double2(sg * ym.x, sg * ym.y);
+            }
+            yf[4 * r] = sc * yp.x; yf[4 * r + 1] = sc * yp.y; yf[4 * r + 2] = sc * yb.x; yf[4 * r + 3] = sc * yb.y;
         }
         __syncthreads();
         if (tid == 0) carry_s = carry + total;
         __syncthreads();
     }
-    const int G = carry_s & 0xffff, n_runs = carry_s >> 16;
-    // ---- (e) slots, group masks
-    for (int r = tid; r < K; r += kPlanThreads) {
-        unsigned long long rl = run_l[rid[r]];
-        int slot = __popcll(rl & ((1ull << key_l(skey[r])) - 1ull));
-        if (__popcll(rl) > kNSlot) { atomicOr(status, FEW_DEV_TOO_MANY_L); slot = slot % kNSlot; }
-        atomicOr(&gmask[gid[r]], 1 << slot);
-    }
-    __syncthreads();
-    // ---- (f) emit descriptors, fold constants, packed order
-    int* grp = L.grp + (size_t)src * n_modes;
-    int* oj = L.order_j + (size_t)src * n_modes;
-    double* yc = L.yc + (size_t)src * kMaxRuns * kNSlot * 4;
-    const double sc = scale ? scale[src] : 1.0;
-    for (int r = tid; r < K; r += kPlanThreads) {
-        unsigned key = skey[r], prev = r ? skey[r - 1] : 0u;
-        int j = sj[r];
-        oj[r] = j;
-        bool new_run = r == 0 || key_m(key) != key_m(prev);
-        bool new_sub = new_run || key_dir(key) != key_dir(prev);
-        bool new_grp = new_sub || key_absn(key) != key_absn(prev);
-        if (new_grp) {
-            int nadv = new_sub ? key_absn(key) : key_absn(key) - key_absn(prev);
-            int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
-            grp[gid[r]] = gmask[gid[r]] | (nadv << kAdvShift) | (new_sub ? kNewSub : 0) | (key_dir(key) ? kDirNeg : 0) |
-                          (dm << kDmShift) | (new_run ? kNewRun : 0);
-        }
-        // 4 real constants of the (m, l) fold:  h += Y+ S + Ybar conj(S),  Ybar = (-1)^l Y- for m > 0, else 0
-        unsigned long long rl = run_l[rid[r]];
-        int lj = key_l(key), slot = __popcll(rl & ((1ull << lj) - 1ull)) % kNSlot;
-        double2 yp = ylm_plus[(size_t)src * n_modes + j], yb = make_double2(0.0, 0.0);
-        if (key_m(key) > 0) {
-            double2 ym = ylm_minus[(size_t)src * n_modes + j];
-            double sg = (lj & 1) ? -1.0 : 1.0;
-            yb = make_double2(sg * ym.x, sg * ym.y);
-        }
-        double* c = yc + ((size_t)rid[r] * kNSlot + slot) * 4;
-        c[0] = sc * (yp.x + yb.x); c[1] = sc * (-yp.y + yb.y); c[2] = sc * (yp.y + yb.y); c[3] = sc * (yp.x - yb.x);
-    }
-    for (int r = tid; r < n_runs; r += kPlanThreads) {
-        int cnt = __popcll(run_l[r]); if (cnt > kNSlot) cnt = kNSlot;
-        L.run_mask[(size_t)src * kMaxRuns + r] = (1 << cnt) - 1;
-    }
-    if (tid == 0) L.n_groups[src] = G;
+    if (tid == 0) { L.n_groups[src] = carry_s; gfirst[carry_s] = K; }
 }
 
-// coef_amp[src][k][p][2 n_modes] -> pack[src][k][r][p][re,im] for the kept modes in plan order.
-__global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, const int* __restrict__ n_keep, int n_t, int n_modes,
-                                    sum_layout L)
+// (U_mn, V_mn) per pair and segment, written as the stage stream the sum kernel consumes.
+__global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_t, int n_modes, sum_layout L)
 {
     const int k = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
-    const int K = n_keep ? min(max(n_keep[src], 0), n_modes) : n_modes;
+    const int G = L.n_groups[src];
+    const int* gfirst = L.g_first + (size_t)src * (n_modes + 1);
     const int* oj = L.order_j + (size_t)src * n_modes;
+    const int* desc = L.desc + (size_t)src * n_modes;
+    const double4* yf = reinterpret_cast<const double4*>(L.yfold) + (size_t)src * n_modes;
     const double2* in = coef_amp + ((size_t)src * n_seg + k) * 4 * n_modes;
-    double2* out = reinterpret_cast<double2*>(L.pack) + ((size_t)src * n_seg + k) * n_modes * 4;
-    for (int idx = threadIdx.x; idx < 4 * K; idx += blockDim.x) {
-        int r = idx >> 2, p = idx & 3;
-        out[idx] = in[(size_t)p * n_modes + oj[r]];
+    double2* out = reinterpret_cast<double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
+    for (int idx = threadIdx.x; idx < 4 * G; idx += blockDim.x) {
+        const int g = idx >> 2, p = idx & 3;
+        double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
+        for (int r = gfirst[g]; r < gfirst[g + 1]; ++r) {
+            const double2 c = in[(size_t)p * n_modes + oj[r]];
+            const double4 y = yf[r];
+            const double ar = y.x * c.x - y.y * c.y, ai = y.x * c.y + y.y * c.x;      // Y+ c
+            const double br = y.z * c.x + y.w * c.y, bi = y.w * c.x - y.z * c.y;      // Ybar conj(c)
+            ur += ar + br; ui += ai + bi;                                             // U  = a + b
+            vr -= ai - bi; vi += ar - br;                                             // V  = i (a - b)
+        }
+        double2* slot = out + (size_t)(g / kStagePairs) * kStageD2 + (g % kStagePairs) * 8;
+        slot[p] = make_double2(ur, ui);
+        slot[4 + p] = make_double2(vr, vi);
+    }
+    const int n_stages = stages_for(G);
+    for (int idx = threadIdx.x; idx < n_stages * 64; idx += blockDim.x) {     // header: [0] count, [1] special mask, [2+q] descriptor q
+        const int s = idx >> 6, q = idx & 63;
+        int v = 0;
+        const int cnt = min(kStagePairs, G - s * kStagePairs);
+        if (q == 0) v = cnt;
+        else if (q == 1) { for (int i = 0; i < cnt; ++i) v |= (desc[s * kStagePairs + i] & 1) << i; }
+        else if (q - 2 < cnt) v = desc[s * kStagePairs + q - 2];
+        reinterpret_cast<int*>(out + (size_t)s * kStageD2 + kStagePairs * 8)[q] = v;
     }
 }
 
@@ -274,11 +282,42 @@ __device__ __forceinline__ void phase_factor(const dd* __restrict__ c, int strid
     *zi = -fma(q.lo, co, s);          // -sin(hi + lo)
 }
 
-template <int R>
-__global__ void __launch_bounds__(kSumThreads)
-few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
-               int n_t, int n_modes, sum_layout L, double2* __restrict__ h_all)
+// ---- mbarrier / TMA bulk copy (1-D cp.async.bulk global -> shared, completion counted in bytes on an mbarrier)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
 {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+
+template <int R>
+__global__ void __launch_bounds__(kSumThreads, 4)
+few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
+               int n_t, sum_layout L, double2* __restrict__ h_all)
+{
+    __shared__ __align__(128) double2 ring[kRing][kStageD2];
+    __shared__ __align__(8) unsigned long long full[kRing];
+    __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
+
     const int src = blockIdx.y, tid = threadIdx.x, n_seg = n_t - 1;
     const int* TS = L.tile_start + (size_t)src * (n_t + 2);
     const int tile = blockIdx.x;
@@ -297,9 +336,24 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         return;
     }
     const int k = p - 1;
+    const int n_stages = stages_for(L.n_groups[src]);
+    const double2* gsrc = reinterpret_cast<const double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
+
+    // ---- producer prologue: thread 0 arms the ring with the first kRing - 1 stages
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kRing; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (int s = 0; s < kRing - 1 && s < n_stages; ++s) {
+            mbar_expect_tx(&full[s], kStageBytes);
+            bulk_g2s(&ring[s][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[s]);
+        }
+    }
+
+    // ---- per-sample setup (overlaps the first copies): dx and the two phase factors
     const double tk = t_all[(size_t)src * n_t + k];
     const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 8;     // [4][2] dd
-
     double dx[R], zpr[R], zpi[R], zrr[R], zri[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -309,85 +363,96 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         phase_factor(cph + 0, 2, dx[r], &zpr[r], &zpi[r]);
         phase_factor(cph + 1, 2, dx[r], &zrr[r], &zri[r]);
     }
+    // Z_phi and the run's Z_phi^m are needed only when m or the sign of n changes: parked in shared memory, not registers
+#pragma unroll
+    for (int r = 0; r < R; ++r) { stash_zp[r][tid] = make_double2(zpr[r], zpi[r]); stash_pm[r][tid] = make_double2(1.0, 0.0); }
+    double hre[R], him[R], er[R], ei[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { hre[r] = him[r] = 0.0; er[r] = 1.0; ei[r] = 0.0; }
+    bool neg = false;                                               // zri currently holds -Im Z_r (walking n downward)
 
-    double hre[R], him[R], pmr[R], pmi[R], er[R], ei[R], sti[R];
-    double sre[kNSlot][R], sim[kNSlot][R];
+    for (int st = 0; st < n_stages; ++st) {
+        __syncthreads();                                            // stage st-1 fully consumed (and barriers initialised)
+        if (tid == 0 && st + kRing - 1 < n_stages) {
+            const int s = st + kRing - 1, b = s % kRing;
+            mbar_expect_tx(&full[b], kStageBytes);
+            bulk_g2s(&ring[b][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[b]);
+        }
+        const int b = st % kRing;
+        mbar_wait(&full[b], (unsigned)(st / kRing) & 1u);
+        const double2* cp = &ring[b][0];
+        const int* hdr = reinterpret_cast<const int*>(cp + kStagePairs * 8);
+        const int ng = hdr[0];
+        unsigned spec = (unsigned)hdr[1];
+        for (int gi = 0; gi < ng; ++gi, cp += 8, spec >>= 1) {
+            if (spec & 1u) {                                        // rare: new m, sign change of n, or a gap in n
+                const int d = hdr[2 + gi];
+                if (d & kNewRun) {
+                    const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
 #pragma unroll
-    for (int r = 0; r < R; ++r) { hre[r] = him[r] = 0.0; pmr[r] = 1.0; pmi[r] = 0.0; er[r] = 1.0; ei[r] = 0.0; sti[r] = zri[r]; }
+                    for (int r = 0; r < R; ++r) {
+                        double2 pm = stash_pm[r][tid];
+                        const double2 zp = stash_zp[r][tid];
+                        for (int q = 0; q < dm; ++q) {
+                            double a = pm.x * zp.x - pm.y * zp.y;
+                            pm.y = pm.x * zp.y + pm.y * zp.x;
+                            pm.x = a;
+                        }
+                        stash_pm[r][tid] = pm;
+                    }
+                }
+                if (d & kNewSub) {
+                    const bool want_neg = (d & kDirNeg) != 0;
 #pragma unroll
-    for (int s = 0; s < kNSlot; ++s)
+                    for (int r = 0; r < R; ++r) {
+                        const double2 pm = stash_pm[r][tid];
+                        er[r] = pm.x; ei[r] = pm.y;
+                        if (want_neg != neg) zri[r] = -zri[r];
+                    }
+                    neg = want_neg;
+                }
+                const int nadv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
+                for (int q = 0; q < nadv; ++q) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) sre[s][r] = sim[s][r] = 0.0;
-
-    const int G = L.n_groups[src];
-    const int* grp = L.grp + (size_t)src * n_modes;
-    const int* run_mask = L.run_mask + (size_t)src * kMaxRuns;
-    const double* yc = L.yc + (size_t)src * kMaxRuns * kNSlot * 4;
-    const double2* cp = reinterpret_cast<const double2*>(L.pack) + ((size_t)src * n_seg + k) * n_modes * 4;
-
-    auto fold = [&](int run) {
-        const int rm = run_mask[run];
-        const double* c = yc + (size_t)run * kNSlot * 4;
-#pragma unroll
-        for (int s = 0; s < kNSlot; ++s) {
-            if (rm & (1 << s)) {
-                const double a = c[4 * s], b = c[4 * s + 1], cc = c[4 * s + 2], d = c[4 * s + 3];
+                    for (int r = 0; r < R; ++r) {
+                        double a = er[r] * zrr[r] - ei[r] * zri[r];
+                        ei[r] = er[r] * zri[r] + ei[r] * zrr[r];
+                        er[r] = a;
+                    }
+                }
+            } else {                                                // common: next n of the same run, E *= Z_r
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    hre[r] = fma(a, sre[s][r], hre[r]); hre[r] = fma(b, sim[s][r], hre[r]);
-                    him[r] = fma(cc, sre[s][r], him[r]); him[r] = fma(d, sim[s][r], him[r]);
-                    sre[s][r] = 0.0; sim[s][r] = 0.0;
+                    double a = er[r] * zrr[r] - ei[r] * zri[r];
+                    ei[r] = er[r] * zri[r] + ei[r] * zrr[r];
+                    er[r] = a;
                 }
             }
-        }
-    };
-
-    int run = -1;
-    for (int g = 0; g < G; ++g) {
-        const int d = grp[g];
-        if (d & kNewRun) {
-            if (run >= 0) fold(run);
-            ++run;
-            const int dm = (d >> kDmShift) & 0x7f;
-            for (int q = 0; q < dm; ++q) {
+            double ar[R], ai[R];
+            {
+                const double2 u3 = cp[3], u2 = cp[2], u1 = cp[1], u0 = cp[0];
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    double a = pmr[r] * zpr[r] - pmi[r] * zpi[r];
-                    pmi[r] = pmr[r] * zpi[r] + pmi[r] * zpr[r];
-                    pmr[r] = a;
-                }
+                for (int r = 0; r < R; ++r) { ar[r] = fma(u3.x, dx[r], u2.x); ai[r] = fma(u3.y, dx[r], u2.y); }
+#pragma unroll
+                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], u1.x); ai[r] = fma(ai[r], dx[r], u1.y); }
+#pragma unroll
+                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], u0.x); ai[r] = fma(ai[r], dx[r], u0.y); }
+#pragma unroll
+                for (int r = 0; r < R; ++r) { hre[r] = fma(er[r], ar[r], hre[r]); him[r] = fma(er[r], ai[r], him[r]); }
             }
-        }
-        if (d & kNewSub) {
-            const double sg = (d & kDirNeg) ? -1.0 : 1.0;
+            {
+                const double2 v3 = cp[7], v2 = cp[6], v1 = cp[5], v0 = cp[4];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { er[r] = pmr[r]; ei[r] = pmi[r]; sti[r] = sg * zri[r]; }
-        }
-        const int nadv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
-        for (int q = 0; q < nadv; ++q) {
+                for (int r = 0; r < R; ++r) { ar[r] = fma(v3.x, dx[r], v2.x); ai[r] = fma(v3.y, dx[r], v2.y); }
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                double a = er[r] * zrr[r] - ei[r] * sti[r];
-                ei[r] = er[r] * sti[r] + ei[r] * zrr[r];
-                er[r] = a;
-            }
-        }
+                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], v1.x); ai[r] = fma(ai[r], dx[r], v1.y); }
 #pragma unroll
-        for (int s = 0; s < kNSlot; ++s) {
-            if (d & (1 << s)) {
-                const double2 c0 = __ldg(cp), c1 = __ldg(cp + 1), c2 = __ldg(cp + 2), c3 = __ldg(cp + 3);
-                cp += 4;
+                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], v0.x); ai[r] = fma(ai[r], dx[r], v0.y); }
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    double ar = fma(fma(fma(c3.x, dx[r], c2.x), dx[r], c1.x), dx[r], c0.x);
-                    double ai = fma(fma(fma(c3.y, dx[r], c2.y), dx[r], c1.y), dx[r], c0.y);
-                    sre[s][r] = fma(ar, er[r], sre[s][r]); sre[s][r] = fma(-ai, ei[r], sre[s][r]);
-                    sim[s][r] = fma(ar, ei[r], sim[s][r]); sim[s][r] = fma(ai, er[r], sim[s][r]);
-                }
+                for (int r = 0; r < R; ++r) { hre[r] = fma(ei[r], ar[r], hre[r]); him[r] = fma(ei[r], ai[r], him[r]); }
             }
         }
     }
-    if (run >= 0) fold(run);
 
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -396,7 +461,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     }
 }
 
-size_t plan_smem_bytes(int n_modes) { return (size_t)n_modes * (4 + 4 + 4 + 4 + 2 + 2 + 4) + 16; }
+size_t plan_smem_bytes(int n_modes) { return (size_t)n_modes * 16 + 16; }
 
 }  // namespace
 
@@ -420,7 +485,7 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
     FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
     FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
-    FEW_REQUIRE(n_src <= 65535 && n_modes <= 65535, FEW_ERR_LIMIT, "n_src or n_modes > 65535");
+    FEW_REQUIRE(n_src <= 65535 && n_t <= 65535, FEW_ERR_LIMIT, "n_src or n_t > 65535");
     if (n_samples == 0) return FEW_OK;
     FEW_REQUIRE(h != nullptr, FEW_ERR_INVALID_ARG, "h is NULL");
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
@@ -438,11 +503,11 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
                                                           (const double2*)ylm_minus, scale, t0, dt, n_samples, n_t, n_modes, L,
                                                           ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
-    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_keep, n_t, n_modes, L);
+    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     few_sum_kernel<kSumR><<<dim3((unsigned)max_tiles, n_src), kSumThreads, 0, st>>>(t, (const dd*)coef_phase_dd, t0, dt, n_samples,
-                                                                                   n_t, n_modes, L, (double2*)h);
+                                                                                   n_t, L, (double2*)h);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     return FEW_OK;

@@ -289,11 +289,21 @@ def test_bad_modes_reported(api):
     with pytest.raises(api.FewError) as e:                               # dt <= 0 is rejected on the host
         api.few_sum_waveform(g["t"], g["t"], g["t"], g["l"], g["m"], g["n"], None, None, yp, ym, 0.0, -1.0, 10)
     assert e.value.code == -1
-    # a kept list with more than 9 distinct l for one m is reported by the plan kernel
-    l = np.arange(2, 13, dtype=np.int32); m = np.zeros_like(l); n = np.zeros_like(l)
-    t = dev(np.linspace(0, 10, 6)[None]); amp = dev(np.ones((1, 6, len(l)), np.complex128)); ph = dev(np.zeros((1, 6, 2)))
-    api.few_waveform(t, ph, amp, dev(l), dev(m), dev(n), dev(np.array([0.7])), dev(np.array([1.1])), 0.0, 0.0, 0.1, 16)
-    assert api.few_device_status(raise_on_error=False) == -4
+
+
+def test_many_l_per_pair_and_n_gaps(api):
+    """Mode lists outside the paper's grid: 20 distinct l for one (m, n), gaps in n, a single negative-n run."""
+    rng = np.random.default_rng(7)
+    modes = [(l, 0, 0) for l in range(2, 22)] + [(l, 3, n) for l in (3, 5, 9) for n in (-17, -4, 2, 11)] + [(6, 6, -2), (7, 5, 40)]
+    l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
+    n_t = 9
+    t = np.sort(rng.uniform(0, 500.0, n_t)); t[0] = 0.0
+    amp = rng.normal(size=(1, n_t, len(l))) + 1j * rng.normal(size=(1, n_t, len(l)))
+    phase = np.stack([0.9 * t + 1e-3 * t ** 2, 0.4 * t + 2e-4 * t ** 2], axis=1)[None]
+    w = synth.Workload("many_l", t[None], phase, amp, l, m, n, np.array([1.3]), np.array([0.4]), 3.0, 0.37, 1200, 0.0)
+    h, keep, nk = run_gpu_chain(api, w)
+    ref = oracle.waveform(w)
+    assert nk[0] == len(l) and rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
 
 
 def test_whole_path_host_buffers(api):
