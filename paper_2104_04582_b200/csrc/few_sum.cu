@@ -46,6 +46,7 @@ struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
     int* tile_start;     // [n_src][n_t + 2]   exclusive prefix of tiles per pseudo-segment; last = total
     int* n_groups;       // [n_src]            number of (m, n) pairs
+    int* tile_counter;   // [1]                dynamic tile scheduler of the persistent sum kernel
     int* desc;           // [n_src][n_modes]   pair descriptors
     int* g_first;        // [n_src][n_modes+1] first sorted mode of each pair
     int* order_j;        // [n_src][n_modes]   mode index of sorted position r
@@ -64,6 +65,7 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, size_t* bytes = 
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
     L.n_groups = c.take<int>(n_src);
+    L.tile_counter = c.take<int>(1);
     L.desc = c.take<int>((size_t)n_src * n_modes);
     L.g_first = c.take<int>((size_t)n_src * (n_modes + 1));
     L.order_j = c.take<int>((size_t)n_src * n_modes);
@@ -224,7 +226,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         if (tid == 0) carry_s = carry + total;
         __syncthreads();
     }
-    if (tid == 0) { L.n_groups[src] = carry_s; gfirst[carry_s] = K; }
+    if (tid == 0) { L.n_groups[src] = carry_s; gfirst[carry_s] = K; if (src == 0) *L.tile_counter = 0; }
 }
 
 // (U_mn, V_mn) per pair and segment, written as the stage stream the sum kernel consumes.
@@ -266,20 +268,30 @@ __global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_
 }
 
 // exp(-i Phi) for Phi = c0 + dx (c1 + dx (c2 + dx c3)) with double-double coefficients (R13, R15).
+// c0, c1 dx and c2 dx^2 reach 1e3..1e6 rad and are carried as hi + lo pairs; c3 dx^3 stays below a few rad per segment
+// and enters in FP64.  The sum is reduced by 2 pi with a three-part constant (k 2pi_1 and k 2pi_2 are exact products for
+// k < 2^23) and the reduced argument goes through one sincos; the low word is applied as a first-order correction.
+__device__ __forceinline__ dd dd_add_fast(dd a, dd b)            // error O(eps^2 (|a|+|b|)): enough for 1e-12 rad on 1e6 rad
+{
+    dd s = two_sum(a.hi, b.hi);
+    s.lo = __dadd_rn(s.lo, __dadd_rn(a.lo, b.lo));
+    return quick_two_sum(s.hi, s.lo);
+}
+
 __device__ __forceinline__ void phase_factor(const dd* __restrict__ c, int stride, double dx, double* zr, double* zi)
 {
-    dd r = c[3 * stride];
-    r = dd_add(dd_mul_d(r, dx), c[2 * stride]);
-    r = dd_add(dd_mul_d(r, dx), c[stride]);
-    r = dd_add(dd_mul_d(r, dx), c[0]);
-    const double two_pi_hi = 6.283185307179586232e+00, two_pi_lo = 2.449293598294706414e-16;
-    double kk = rint(r.hi * 1.591549430918953456e-01);
-    dd q = dd_sub(r, two_prod(kk, two_pi_hi));
-    q = dd_sub(q, two_prod(kk, two_pi_lo));
+    dd r = dd_add_d(c[2 * stride], __dmul_rn(c[3 * stride].hi, dx));
+    r = dd_add_fast(dd_mul_d(r, dx), c[stride]);
+    r = dd_add_fast(dd_mul_d(r, dx), c[0]);
+    const double p1 = 0x1.921fb54000000p+2, p2 = 0x1.10b4611800000p-28, p3 = 0x1.313198a2e0370p-59;   // 2 pi = p1 + p2 + p3
+    const double kk = rint(r.hi * 1.591549430918953456e-01);
+    double q = fma(-kk, p1, r.hi);            // exact
+    q = fma(-kk, p2, q);
+    const double ql = fma(-kk, p3, r.lo);
     double s, co;
-    sincos(q.hi, &s, &co);
-    *zr = fma(-q.lo, s, co);          // cos(hi + lo)
-    *zi = -fma(q.lo, co, s);          // -sin(hi + lo)
+    sincos(q, &s, &co);
+    *zr = fma(-ql, s, co);                    // cos(q + ql)
+    *zi = -fma(ql, co, s);                    // -sin(q + ql)
 }
 
 // ---- mbarrier / TMA bulk copy (1-D cp.async.bulk global -> shared, completion counted in bytes on an mbarrier)
@@ -312,16 +324,34 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 template <int R>
 __global__ void __launch_bounds__(kSumThreads, 4)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
-               int n_t, sum_layout L, double2* __restrict__ h_all)
+               int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all)
 {
     __shared__ __align__(128) double2 ring[kRing][kStageD2];
     __shared__ __align__(8) unsigned long long full[kRing];
     __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
+    __shared__ int tile_s;
 
-    const int src = blockIdx.y, tid = threadIdx.x, n_seg = n_t - 1;
+    const int tid = threadIdx.x, n_seg = n_t - 1;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kRing; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    unsigned gst = 0;                       // stages consumed by this block so far: ring slot gst % kRing, parity (gst / kRing) & 1
+
+    // Persistent block: tiles (512 samples of one sparse segment of one source) are handed out by an atomic counter, so
+    // SMs never idle on wave boundaries and the blocks of an SM drift apart (one block's phase setup overlaps the others'
+    // FP64 loops).
+    for (;;) {
+    __syncthreads();
+    if (tid == 0) tile_s = atomicAdd(L.tile_counter, 1);
+    __syncthreads();
+    const int tg = tile_s;
+    if (tg >= n_src * max_tiles) break;
+    const int src = tg / max_tiles, tile = tg - src * max_tiles;
     const int* TS = L.tile_start + (size_t)src * (n_t + 2);
-    const int tile = blockIdx.x;
-    if (tile >= TS[n_t + 1]) return;
+    if (tile >= TS[n_t + 1]) continue;
     // pseudo-segment of this tile: largest p with TS[p] <= tile
     int lo = 0, hi = n_t + 1;
     while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (TS[mid] <= tile) lo = mid; else hi = mid; }
@@ -333,21 +363,18 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (p == 0 || p == n_t) {           // outside [t_0, t_last]: h = 0 (R12)
 #pragma unroll
         for (int r = 0; r < R; ++r) { long long i = i_begin + r * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
-        return;
+        continue;
     }
     const int k = p - 1;
     const int n_stages = stages_for(L.n_groups[src]);
     const double2* gsrc = reinterpret_cast<const double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
 
-    // ---- producer prologue: thread 0 arms the ring with the first kRing - 1 stages
+    // ---- producer prologue: thread 0 arms the ring with the first kRing - 1 stages of this tile
     if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < kRing; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         for (int s = 0; s < kRing - 1 && s < n_stages; ++s) {
-            mbar_expect_tx(&full[s], kStageBytes);
-            bulk_g2s(&ring[s][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[s]);
+            const int b = (gst + s) % kRing;
+            mbar_expect_tx(&full[b], kStageBytes);
+            bulk_g2s(&ring[b][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[b]);
         }
     }
 
@@ -374,12 +401,13 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     for (int st = 0; st < n_stages; ++st) {
         __syncthreads();                                            // stage st-1 fully consumed (and barriers initialised)
         if (tid == 0 && st + kRing - 1 < n_stages) {
-            const int s = st + kRing - 1, b = s % kRing;
+            const int s = st + kRing - 1, b = (gst + kRing - 1) % kRing;
             mbar_expect_tx(&full[b], kStageBytes);
             bulk_g2s(&ring[b][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[b]);
         }
-        const int b = st % kRing;
-        mbar_wait(&full[b], (unsigned)(st / kRing) & 1u);
+        const int b = gst % kRing;
+        mbar_wait(&full[b], (gst / kRing) & 1u);
+        ++gst;
         const double2* cp = &ring[b][0];
         const int* hdr = reinterpret_cast<const int*>(cp + kStagePairs * 8);
         const int ng = hdr[0];
@@ -421,35 +449,48 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                     }
                 }
             } else {                                                // common: next n of the same run, E *= Z_r
+                // operand order chosen for the register-file reuse latches: a DFMA with three fresh
+                // per-thread register operands issues every 3 cycles instead of 2
+                double m1[R], m2[R];
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    double a = er[r] * zrr[r] - ei[r] * zri[r];
-                    ei[r] = er[r] * zri[r] + ei[r] * zrr[r];
-                    er[r] = a;
-                }
+                for (int r = 0; r < R; ++r) { m1[r] = ei[r] * zri[r]; m2[r] = ei[r] * zrr[r]; }
+#pragma unroll
+                for (int r = 0; r < R; ++r) { const double e0 = er[r]; er[r] = fma(e0, zrr[r], -m1[r]); ei[r] = fma(e0, zri[r], m2[r]); }
             }
-            double ar[R], ai[R];
+            double tr[R], ti[R];
             {
                 const double2 u3 = cp[3], u2 = cp[2], u1 = cp[1], u0 = cp[0];
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(u3.x, dx[r], u2.x); ai[r] = fma(u3.y, dx[r], u2.y); }
+                for (int r = 0; r < R; ++r) tr[r] = fma(u3.x, dx[r], u2.x);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], u1.x); ai[r] = fma(ai[r], dx[r], u1.y); }
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(u3.y, dx[r], u2.y);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], u0.x); ai[r] = fma(ai[r], dx[r], u0.y); }
+                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], u1.x);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { hre[r] = fma(er[r], ar[r], hre[r]); him[r] = fma(er[r], ai[r], him[r]); }
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], u1.y);
+#pragma unroll
+                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], u0.x);
+#pragma unroll
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], u0.y);
+#pragma unroll
+                for (int r = 0; r < R; ++r) { hre[r] = fma(tr[r], er[r], hre[r]); him[r] = fma(ti[r], er[r], him[r]); }
             }
             {
                 const double2 v3 = cp[7], v2 = cp[6], v1 = cp[5], v0 = cp[4];
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(v3.x, dx[r], v2.x); ai[r] = fma(v3.y, dx[r], v2.y); }
+                for (int r = 0; r < R; ++r) tr[r] = fma(v3.x, dx[r], v2.x);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], v1.x); ai[r] = fma(ai[r], dx[r], v1.y); }
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(v3.y, dx[r], v2.y);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { ar[r] = fma(ar[r], dx[r], v0.x); ai[r] = fma(ai[r], dx[r], v0.y); }
+                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], v1.x);
 #pragma unroll
-                for (int r = 0; r < R; ++r) { hre[r] = fma(ei[r], ar[r], hre[r]); him[r] = fma(ei[r], ai[r], him[r]); }
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], v1.y);
+#pragma unroll
+                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], v0.x);
+#pragma unroll
+                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], v0.y);
+#pragma unroll
+                for (int r = 0; r < R; ++r) { hre[r] = fma(tr[r], ei[r], hre[r]); him[r] = fma(ti[r], ei[r], him[r]); }
             }
         }
     }
@@ -459,6 +500,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         long long i = i_begin + r * kSumThreads + tid;
         if (i < i_end) __stcs(&h[i], make_double2(hre[r], him[r]));
     }
+    }   // persistent tile loop
 }
 
 size_t plan_smem_bytes(int n_modes) { return (size_t)n_modes * 16 + 16; }
@@ -506,8 +548,10 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
     few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
-    few_sum_kernel<kSumR><<<dim3((unsigned)max_tiles, n_src), kSumThreads, 0, st>>>(t, (const dd*)coef_phase_dd, t0, dt, n_samples,
-                                                                                   n_t, L, (double2*)h);
+    FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
+    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * 4;
+    few_sum_kernel<kSumR><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
+        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     return FEW_OK;
