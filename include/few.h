@@ -56,7 +56,7 @@ enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
 
 #define FEW_MAX_L 63            /* l <= 63 (factorials in FP64, 64-bit l masks) */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
-#define FEW_MAX_NT_SPLINE 760   /* n_t limit of few_spline_fit (one shared-memory column per system) */
+#define FEW_MAX_NT_SPLINE 736   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
 
 typedef struct few_ctx few_ctx;

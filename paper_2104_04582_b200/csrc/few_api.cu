@@ -49,6 +49,11 @@ extern "C" int few_create(few_ctx** out, int device)
     if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev_sum[0]);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev_sum[1]);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         few_set_error("few_create: %s", cudaGetErrorString(e));
         delete c;
@@ -64,6 +69,11 @@ extern "C" int few_destroy(few_ctx* ctx)
     cudaFree(ctx->d_status);
     if (ctx->ev_sum[0]) cudaEventDestroy(ctx->ev_sum[0]);
     if (ctx->ev_sum[1]) cudaEventDestroy(ctx->ev_sum[1]);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     delete ctx;
     return FEW_OK;
 }
@@ -152,11 +162,21 @@ extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, 
     wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, nullptr);
     int* kidx = keep_idx ? keep_idx : L.keep_idx;
     int* nk = n_keep ? n_keep : L.n_keep;
+    // The spline fits depend on the inputs only, so they run on two side streams beside harmonics + mode selection and
+    // join before the summation (fork/join with events: nothing synchronises the host, and the pattern is graph-capturable).
+    cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_fork, st));
+    FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[0], ctx->ev_fork, 0));
+    FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[1], ctx->ev_fork, 0));
+    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, ctx->side[0]))) return rc;
+    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, ctx->side[1]))) return rc;
+    FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[0], ctx->side[0]));
+    FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[1], ctx->side[1]));
     if ((rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream))) return rc;
     if ((rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream))) return rc;
-    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, stream))) return rc;
-    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, stream))) return rc;
+    FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[0], 0));
+    FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[1], 0));
     return few_sum_waveform(ctx, t, L.coef_amp, L.coef_phase, l, m, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, t0, dt, n_samples, h,
                             n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
 }

@@ -13,6 +13,8 @@ struct few_ctx {
     int profile;         // few_profile_enable
     int profile_valid;   // a sum kernel was bracketed since profiling was switched on
     cudaEvent_t ev_sum[2];
+    cudaStream_t side[2];  // few_waveform: the two spline fits run beside harmonics + mode selection
+    cudaEvent_t ev_fork, ev_join[2];
 };
 
 void few_set_error(const char* fmt, ...);

@@ -66,7 +66,7 @@ def test_ylm_modes_vs_oracle(api):
 
 # ------------------------------------------------------------------------------------------- S1
 @pytest.mark.parametrize("n_t,n_sys,uniform", [(4, 1, True), (5, 33, False), (20, 18, True), (100, 257, False), (100, 7688, False),
-                                              (300, 129, False), (760, 40, False)])
+                                              (300, 129, False), (736, 40, False), (430, 70, False)])
 def test_spline_fit_vs_oracle(api, n_t, n_sys, uniform):
     rng = np.random.default_rng(n_t * 1000 + n_sys)
     n_src = 2
