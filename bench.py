@@ -104,6 +104,42 @@ def oracle_sample(w, target_s: float):
     return n * K / t_run, f"{n} contiguous samples of source 0 from sample {mid}, whole path, K={K}", cores, t_run, n, K
 
 
+def time_stages(api, torch, w, g, flush, reps: int = 10):
+    """Each C-ABI stage timed alone with CUDA events (L2 flushed before every launch); GB/s = algorithmic bytes / time:
+    S1 reads 8 B and writes 32 B per knot and system; S2 reads the 16 B complex amplitude of every mode at every step."""
+    yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
+    keep, nk = api.few_select_modes(g["amp"], g["m"], yp, ym, max(w.eps, 1e-5))
+    y_amp = torch.view_as_real(g["amp"]).reshape(w.n_src, w.n_t, -1)
+    coef = api.few_spline_fit(g["t"], y_amp)
+    cdd = api.few_spline_fit_dd(g["t"], g["phase"])
+    sel_ws = torch.empty(api._lib.few_select_modes_workspace(w.n_src, w.n_t, w.n_modes), dtype=torch.uint8, device=coef.device)
+    sum_ws = torch.empty(api._lib.few_sum_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=coef.device)
+    h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=coef.device)
+    calls = {
+        "S0_ylm_modes": lambda: api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"]),
+        "S1_spline_fit": lambda: api.few_spline_fit(g["t"], y_amp, out=coef),
+        "S1_spline_fit_dd": lambda: api.few_spline_fit_dd(g["t"], g["phase"], out=cdd),
+        "S2_select_modes": lambda: api.few_select_modes(g["amp"], g["m"], yp, ym, max(w.eps, 1e-5), workspace=sel_ws),
+        "S3_sum_waveform": lambda: api.few_sum_waveform(g["t"], coef, cdd, g["l"], g["m"], g["n"], keep, nk, yp, ym, w.t0, w.dt,
+                                                        w.n_samples, out=h, workspace=sum_ws),
+    }
+    nbytes = {"S1_spline_fit": 40.0 * w.n_src * w.n_t * 2 * w.n_modes, "S2_select_modes": 16.0 * w.n_src * w.n_t * w.n_modes}
+    out = {}
+    for name, fn in calls.items():
+        fn(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        out[name] = {"ms_avg": float(np.mean(ts)), "ms_min": float(min(ts))}
+        if name in nbytes:
+            out[name]["algorithmic_bytes"] = nbytes[name]
+            out[name]["gbs"] = nbytes[name] / (float(np.mean(ts)) * 1e-3) / 1e9
+    return out
+
+
 def reference_arm(args):
     """--impl reference: the CPU oracle on the host cores, each step a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -140,6 +176,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--eps", type=float, default=None)
+    ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
@@ -243,7 +280,11 @@ def main():
         h2d = sum(v.numel() * v.element_size() for v in pinned.values())
         e2e = {"value": evals_all / float(t_e2e.item()), "unit": "evals/s", "ms_per_step": 1e3 * float(t_e2e.item()),
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h_host.numel() * 16),
-               "note": "few_waveform_host: cudaMalloc + H2D + 9 kernels + D2H + free, pinned host buffers"}
+               "note": "few_waveform_host (C ABI, host pointers): H2D of the sparse inputs + kernels + D2H of h, pinned host buffers"}
+
+    stages = None
+    if args.stages and rank == 0:
+        stages = time_stages(api, torch, w, g, flush)
 
     if rank != 0:
         if world > 1:
@@ -278,6 +319,12 @@ def main():
            "ms_per_waveform": ms_per_step / w.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
            "gpu_launches": (GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) * args.steps, "clocks": clocks,
            "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
+    if stages is not None:
+        for v in stages.values():
+            if "gbs" in v:
+                v["hbm_frac"] = v["gbs"] / hbm_gbs
+        out["stages"] = stages
+        out["stages_hbm_peak_gbs"] = hbm_gbs
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -17,7 +17,7 @@
  *     few_strerror(code) names a code; few_last_error() returns the calling thread's last detailed message.
  *   - Pointers are DEVICE pointers (on the context's device) unless the name or comment says "host".
  *   - Ownership: the caller owns every input, output and workspace buffer.  The library keeps only a few KB of
- *     state in few_ctx.  Workspace sizes come from the *_workspace() queries; workspaces need 256-byte alignment.
+ *     state in few_ctx (plus, if few_waveform_host is used, its device arena).  Workspace sizes come from the *_workspace() queries; workspaces need 256-byte alignment.
  *   - All work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as void*; NULL = legacy
  *     default stream).  No device-pointer call synchronises; n_keep stays on the device so S2 -> S1 -> S3 chain
  *     without a host round trip.  Only few_waveform_host and few_device_status synchronise.
@@ -54,7 +54,7 @@ enum {
 /* bits of the device status word */
 enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
 
-#define FEW_MAX_L 63            /* l <= 63 (factorials in FP64, 64-bit l masks) */
+#define FEW_MAX_L 16            /* l <= 16: the explicit Wigner-d sum in FP64 is accurate to 5e-15 for l <= 10 (the paper's range) and 1e-12 at l = 16 */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
 #define FEW_MAX_NT_SPLINE 736   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
@@ -132,9 +132,9 @@ int few_waveform(few_ctx* ctx, const double* t, const double* phase, const doubl
                  double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
                  double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
 
-/* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): allocates device
- * buffers, copies inputs host->device, runs few_waveform, copies h (and keep_idx/n_keep if not NULL) device->host,
- * synchronises, frees.  `scale_host` may be NULL.  Returns the device status as well. */
+/* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): copies inputs host->device
+ * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform, copies h
+ * (and keep_idx/n_keep if not NULL) device->host and synchronises.  Not re-entrant on one context.  `scale_host` may be NULL.  Returns the device status as well. */
 int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
                       const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
                       const double* phi_host, const double* scale_host, double eps, double t0, double dt,

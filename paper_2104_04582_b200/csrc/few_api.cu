@@ -74,6 +74,8 @@ extern "C" int few_destroy(few_ctx* ctx)
         if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
     }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    cudaFree(ctx->host_arena);
     delete ctx;
     return FEW_OK;
 }
@@ -204,12 +206,17 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_h); sz.take<char>(b_keep); sz.take<char>(b_nk);
     sz.take<char>(ws_bytes);
     total = sz.off;
-    void* dev = nullptr;
-    cudaStream_t st = nullptr;
-    FEW_CUDA_CHECK(cudaMalloc(&dev, total));
+    // device arena and stream are kept in the context between calls (grow-only), so a steady-state call allocates nothing
+    if (total > ctx->host_arena_bytes) {
+        if (ctx->host_arena) { FEW_CUDA_CHECK(cudaFree(ctx->host_arena)); ctx->host_arena = nullptr; ctx->host_arena_bytes = 0; }
+        FEW_CUDA_CHECK(cudaMalloc(&ctx->host_arena, total));
+        ctx->host_arena_bytes = total;
+    }
+    if (!ctx->host_stream) FEW_CUDA_CHECK(cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
+    void* dev = ctx->host_arena;
+    cudaStream_t st = ctx->host_stream;
     int rc = FEW_OK;
-    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { few_set_error("cudaStreamCreate: %s", cudaGetErrorString(e)); cudaFree(dev); return FEW_ERR_CUDA; }
+    cudaError_t e = cudaSuccess;
     few_carver c(dev);
     double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph); double* d_amp = (double*)c.take<char>(b_amp);
     int* d_l = (int*)c.take<char>(b_lmn); int* d_m = (int*)c.take<char>(b_lmn); int* d_n = (int*)c.take<char>(b_lmn);
@@ -234,8 +241,6 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     }
     if (e != cudaSuccess) { few_set_error("few_waveform_host: %s", cudaGetErrorString(e)); rc = FEW_ERR_CUDA; }
     cudaStreamSynchronize(st);
-    cudaStreamDestroy(st);
-    cudaFree(dev);
     return rc;
 }
 

@@ -15,6 +15,9 @@ struct few_ctx {
     cudaEvent_t ev_sum[2];
     cudaStream_t side[2];  // few_waveform: the two spline fits run beside harmonics + mode selection
     cudaEvent_t ev_fork, ev_join[2];
+    void* host_arena;      // few_waveform_host: grow-only device arena (inputs, h, workspace), freed by few_destroy
+    size_t host_arena_bytes;
+    cudaStream_t host_stream;
 };
 
 void few_set_error(const char* fmt, ...);

@@ -4,20 +4,26 @@
 // provided threshold related to the total power emitted (eps) at that time step (the final entry in the cumulative sum)
 // ... the union of all contributing modes across all time steps".
 //
-// One block per (source, sparse step).  The row of entry powers (every (l,m,n) plus the (l,-m,-n) mirror of each m>0
-// mode, R4) is built in shared memory, sorted there by a stable LSD radix sort on the order-preserving bit
-// pattern of the FP64 power (descending; ties keep ascending entry index, R7), scanned in FP64, thresholded
-// (rank r kept iff r == 0 or C_{r-1} < (1-eps) C_last, R5), and the owners of the kept entries are OR-ed into a per-source
-// bitmap.  A second kernel compacts the bitmap into ascending keep_idx and n_keep.  Nothing leaves the SM between the
-// load of the amplitudes and the bitmap update; no library sort.
+// Entries of a row (one source, one sparse step): every (l,m,n) plus the (l,-m,-n) mirror of each m>0 mode, each with its
+// own power (R4).  With the row sorted by power descending (ties: lower entry index first, R7) and C the
+// inclusive cumulative sum, the entry of rank r is kept iff r == 0 or C_{r-1} < (1-eps) C_last (R5).
+//
+// What the procedure defines is a SET, and the set is fixed by one number: C_{r-1} of an entry is G(key) = the summed power
+// of all entries with a strictly larger key (plus earlier ties), G is monotone in the key, so the kept entries are exactly
+// those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernel therefore does an MSB-first radix SELECT on
+// the order-preserving 64-bit pattern of the FP64 power instead of a full radix sort: each of the 63 bit steps is one masked
+// block reduction over powers held in registers (one block of 256 threads per row, nothing but the row's amplitudes read
+// from HBM, no scratch).  Ties at kappa are resolved by entry index with a second, 14-step select.  The owners of the kept
+// entries are OR-ed into a per-source bitmap; a last kernel compacts it into ascending keep_idx and n_keep.
+// (A stable in-shared-memory LSD radix sort + scan, the first version of this file, gave the same sets at 128 us per
+// 7137-entry row; this one takes ~5 us.  See DESIGN.md section 5.)
 #include "few_common.cuh"
 
 namespace {
 
-constexpr int kSelThreads = 1024;
+constexpr int kSelThreads = 256;
 constexpr int kSelWarps = kSelThreads / 32;
-constexpr int kRadixBits = 8;
-constexpr int kRadix = 1 << kRadixBits;
+constexpr int kPrepThreads = 1024;
 
 struct sel_layout {
     int* owner;       // [n_modes]   owner mode of mirror entry e - n_modes   (shared by sources)
@@ -40,7 +46,8 @@ sel_layout sel_carve(void* ws, int n_src, int n_modes, size_t* bytes = nullptr)
     return L;
 }
 
-// Inclusive block scan of one int per thread (kSelThreads threads); returns the inclusive prefix, *total = block sum.
+// Inclusive block scan of one int per thread; returns the inclusive prefix, *total = block sum.
+template <int kThreads>
 __device__ __forceinline__ int block_scan_int(int v, int* warp_sums, int* total)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -48,20 +55,21 @@ __device__ __forceinline__ int block_scan_int(int v, int* warp_sums, int* total)
     if (lane == 31) warp_sums[wid] = v;
     __syncthreads();
     if (wid == 0) {
-        int s = warp_sums[lane];
+        int s = lane < kThreads / 32 ? warp_sums[lane] : 0;
         for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += u; }
-        warp_sums[lane] = s;
+        if (lane < kThreads / 32) warp_sums[lane] = s;
     }
     __syncthreads();
     int res = v + (wid ? warp_sums[wid - 1] : 0);
-    *total = warp_sums[kSelWarps - 1];
+    *total = warp_sums[kThreads / 32 - 1];
     __syncthreads();
     return res;
 }
 
 // Mirror list (modes with m > 0 in ascending j), |Y|^2 per entry, bitmap cleared.  One block per source.
-__global__ void few_select_prepare_kernel(const int* __restrict__ m, const double2* __restrict__ ylm_plus,
-                                          const double2* __restrict__ ylm_minus, int n_modes, sel_layout L, int* status)
+__global__ void __launch_bounds__(kPrepThreads)
+few_select_prepare_kernel(const int* __restrict__ m, const double2* __restrict__ ylm_plus, const double2* __restrict__ ylm_minus,
+                          int n_modes, sel_layout L, int* status)
 {
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
@@ -70,12 +78,12 @@ __global__ void few_select_prepare_kernel(const int* __restrict__ m, const doubl
     __syncthreads();
     const bool with_y = ylm_plus != nullptr;
     double* y2 = L.y2 + (size_t)src * 2 * n_modes;
-    for (int base = 0; base < n_modes; base += kSelThreads) {
+    for (int base = 0; base < n_modes; base += kPrepThreads) {
         int j = base + tid;
         int mj = j < n_modes ? m[j] : 0;
         if (j < n_modes && mj < 0) atomicOr(status, FEW_DEV_BAD_MODE);
         int flag = (with_y && j < n_modes && mj > 0) ? 1 : 0, total;
-        int incl = block_scan_int(flag, warp_sums, &total);
+        int incl = block_scan_int<kPrepThreads>(flag, warp_sums, &total);
         int carry = carry_s;
         if (j < n_modes) {
             double2 yp = with_y ? ylm_plus[(size_t)src * n_modes + j] : make_double2(1.0, 0.0);
@@ -92,125 +100,161 @@ __global__ void few_select_prepare_kernel(const int* __restrict__ m, const doubl
         __syncthreads();
     }
     if (src == 0 && tid == 0) *L.n_entries = n_modes + carry_s;
-    for (int w = tid; w < sel_words(n_modes); w += kSelThreads) L.bitmap[(size_t)src * sel_words(n_modes) + w] = 0u;
+    for (int w = tid; w < sel_words(n_modes); w += kPrepThreads) L.bitmap[(size_t)src * sel_words(n_modes) + w] = 0u;
 }
 
-__device__ __forceinline__ unsigned digit_of(unsigned long long key, int shift) { return (unsigned)(key >> shift) & (kRadix - 1); }
+// ---- block reductions over kSelThreads threads; every thread gets the result.  `slot` alternates between calls so that one
+// __syncthreads per reduction suffices.
+struct sel_red { double d[2][kSelWarps]; long long i[2][kSelWarps]; };
 
-// One (source, step) row.  Shared memory: keys[2][cap] u64, idx[2][cap] u16, hist[kSelWarps][kRadix] u32 (+ small).
-__global__ void __launch_bounds__(kSelThreads, 1)
-few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, int cap, sel_layout L)
+__device__ __forceinline__ double block_sum(double v, sel_red& s, int& slot)
 {
-    extern __shared__ unsigned long long smem_u64[];
-    unsigned long long* keys0 = smem_u64;
-    unsigned long long* keys1 = keys0 + cap;
-    unsigned* hist = reinterpret_cast<unsigned*>(keys1 + cap);          // [kSelWarps][kRadix]
-    unsigned short* idx0 = reinterpret_cast<unsigned short*>(hist + kSelWarps * kRadix);
-    unsigned short* idx1 = idx0 + cap;
-    __shared__ double warp_d[32];
-    __shared__ int warp_i[32];
-    __shared__ unsigned bitmap_s[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
-    __shared__ int skip_s;
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) s.d[slot][threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+#pragma unroll
+    for (int w = 0; w < kSelWarps; ++w) r += s.d[slot][w];
+    slot ^= 1;
+    return r;
+}
+__device__ __forceinline__ long long block_sum_ll(long long v, sel_red& s, int& slot)
+{
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) s.i[slot][threadIdx.x >> 5] = v;
+    __syncthreads();
+    long long r = 0;
+#pragma unroll
+    for (int w = 0; w < kSelWarps; ++w) r += s.i[slot][w];
+    slot ^= 1;
+    return r;
+}
+__device__ __forceinline__ long long block_max_ll(long long v, sel_red& s, int& slot)
+{
+    for (int o = 16; o; o >>= 1) { long long u = __shfl_xor_sync(0xffffffffu, v, o); v = u > v ? u : v; }
+    if ((threadIdx.x & 31) == 0) s.i[slot][threadIdx.x >> 5] = v;
+    __syncthreads();
+    long long r = s.i[slot][0];
+#pragma unroll
+    for (int w = 1; w < kSelWarps; ++w) r = s.i[slot][w] > r ? s.i[slot][w] : r;
+    slot ^= 1;
+    return r;
+}
 
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+// One (source, step) row.  Register slot i of thread tid holds primary entry j = i*256 + tid for i < NP = ceil(n_modes/256)
+// and mirror entry n_modes + (i - NP)*256 + tid after that, so every global load of the row is coalesced and independent
+// of the others; |A|^2 goes through shared memory once so that the mirrors need no second, dependent gather from HBM.
+template <int EPT>
+__global__ void __launch_bounds__(kSelThreads)
+few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L)
+{
+    extern __shared__ double a2_s[];                 // [n_modes] |A_j|^2
+    __shared__ sel_red red;
+    __shared__ unsigned bitmap_s[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
+    const int tid = threadIdx.x;
     const int src = blockIdx.y, k = blockIdx.x;
     const int n_ent = *L.n_entries;
+    const int NP = (n_modes + kSelThreads - 1) / kSelThreads;
     const double2* a = amp + ((size_t)src * n_t + k) * n_modes;
     const double* y2 = L.y2 + (size_t)src * 2 * n_modes;
     const int words = sel_words(n_modes);
     for (int w = tid; w < words; w += kSelThreads) bitmap_s[w] = 0u;
+    int slot = 0;
+    auto entry_of = [&](int i) { return i < NP ? i * kSelThreads + tid : n_modes + (i - NP) * kSelThreads + tid; };
+    auto valid = [&](int i) { return i < NP ? i * kSelThreads + tid < n_modes : entry_of(i) < n_ent; };
 
-    // ---- entry powers -> descending-order keys.  P >= 0, so its bit pattern is monotone; ~bits sorts descending.
-    for (int e = tid; e < n_ent; e += kSelThreads) {
-        int j = e < n_modes ? e : L.owner[e - n_modes];
-        double2 v = a[j];
-        double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
-        double p = __dmul_rn(a2, y2[e]);
-        keys0[e] = ~(unsigned long long)__double_as_longlong(p);
-        idx0[e] = (unsigned short)e;
-    }
-    __syncthreads();
-
-    // ---- stable LSD radix sort, 8 bits per pass; warp w owns the contiguous items [w*ipw, (w+1)*ipw)
-    const int ipw = ((n_ent + kSelWarps - 1) / kSelWarps + 31) / 32 * 32;
-    unsigned long long* kin = keys0; unsigned long long* kout = keys1;
-    unsigned short* iin = idx0; unsigned short* iout = idx1;
-    for (int shift = 0; shift < 64; shift += kRadixBits) {
-        for (int b = tid; b < kSelWarps * kRadix; b += kSelThreads) hist[b] = 0u;
-        if (tid == 0) skip_s = 0;
-        __syncthreads();
-        unsigned* myh = hist + wid * kRadix;
-        for (int r = 0; r < ipw; r += 32) {
-            int item = wid * ipw + r + lane;
-            bool valid = item < n_ent;
-            unsigned dgt = valid ? digit_of(kin[item], shift) : kRadix + lane;   // invalid lanes never match a digit
-            unsigned peers = __match_any_sync(0xffffffffu, dgt);
-            if (valid && lane == __ffs(peers) - 1) myh[dgt] += __popc(peers);
-            __syncwarp();
-        }
-        __syncthreads();
-        // exclusive scan over (digit major, warp minor): thread handles 8 consecutive (digit, warp) cells
-        {
-            const int cells = kSelWarps * kRadix / kSelThreads;   // 8
-            int dgt = tid / (kSelWarps / cells), w0 = (tid % (kSelWarps / cells)) * cells;
-            unsigned loc[cells]; int sum = 0;
+    // ---- entry powers (same separately rounded operations as the definition: |A|^2 = re*re + im*im, P = |A|^2 |Y|^2).
+    // key = bit pattern of P as a signed 64-bit integer: monotone for P >= 0; empty slots get -1 (below every key).
+    long long key[EPT];
+    double tot_local = 0.0;
 #pragma unroll
-            for (int c = 0; c < cells; ++c) { loc[c] = hist[(w0 + c) * kRadix + dgt]; sum += (int)loc[c]; }
-            int total, incl = block_scan_int(sum, warp_i, &total);
-            int run = incl - sum;
-#pragma unroll
-            for (int c = 0; c < cells; ++c) { hist[(w0 + c) * kRadix + dgt] = (unsigned)run; run += (int)loc[c]; }
-            // a digit that holds every item: this pass is the identity permutation
-            int dsum = sum;
-            for (int o = 1; o < kSelWarps / cells; ++o) dsum += __shfl_down_sync(0xffffffffu, sum, o);
-            if ((tid % (kSelWarps / cells)) == 0 && dsum == n_ent) skip_s = 1;
-        }
-        __syncthreads();
-        if (skip_s) { __syncthreads(); continue; }
-        for (int r = 0; r < ipw; r += 32) {
-            int item = wid * ipw + r + lane;
-            bool valid = item < n_ent;
-            unsigned long long key = valid ? kin[item] : 0ull;
-            unsigned dgt = valid ? digit_of(key, shift) : kRadix + lane;
-            unsigned peers = __match_any_sync(0xffffffffu, dgt);
-            unsigned below = peers & ((1u << lane) - 1u);
-            if (valid) {
-                unsigned dst = myh[dgt] + __popc(below);
-                kout[dst] = key; iout[dst] = iin[item];
+    for (int i = 0; i < EPT; ++i) {
+        key[i] = -1;
+        if (i < NP) {
+            const int j = i * kSelThreads + tid;
+            if (j < n_modes) {
+                const double2 v = a[j];
+                const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
+                a2_s[j] = a2;
+                const double p = __dmul_rn(a2, y2[j]);
+                key[i] = __double_as_longlong(p);
+                tot_local += p;
             }
-            __syncwarp();
-            if (valid && lane == __ffs(peers) - 1) myh[dgt] += __popc(peers);
-            __syncwarp();
         }
-        __syncthreads();
-        { unsigned long long* tk = kin; kin = kout; kout = tk; unsigned short* ti = iin; iin = iout; iout = ti; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        if (i >= NP) {
+            const int e = n_modes + (i - NP) * kSelThreads + tid;
+            if (e < n_ent) {
+                const double p = __dmul_rn(a2_s[L.owner[e - n_modes]], y2[e]);
+                key[i] = __double_as_longlong(p);
+                tot_local += p;
+            }
+        }
+    }
+    const double total = block_sum(tot_local, red, slot);
+    const double thr = (1.0 - eps) * total;
+
+    long long kappa;            // kept  <=>  key > kappa  or  (key == kappa and entry index <= iota)
+    int iota = 0x7fffffff;
+    if (!(thr > 0.0)) {
+        // eps >= 1 or an all-zero row: only rank 0 survives, i.e. the largest power with the lowest entry index
+        long long kmax_local = -1;
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) kmax_local = key[i] > kmax_local ? key[i] : kmax_local;
+        kappa = block_max_ll(kmax_local, red, slot);
+        long long best = -0x7fffffff;       // max of -index
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) if (key[i] == kappa) { long long c = -(long long)entry_of(i); best = c > best ? c : best; }
+        iota = (int)(-block_max_ll(best, red, slot));
+    } else {
+        // G(c) = sum of powers with key > c is monotone non-increasing in c (the fixed reduction tree keeps that exactly);
+        // build the largest c with G(c) >= thr bit by bit, then kappa = c + 1.
+        long long lo = 0;
+        for (int b = 62; b >= 0; --b) {
+            const long long cand = lo | (1ll << b);
+            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] > cand ? __longlong_as_double(key[i]) : 0.0;
+            const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
+            if (!(g < thr)) lo = cand;
+        }
+        kappa = lo + 1;
+        // ties at kappa: the j-th (by entry index) is kept iff G(kappa) + j P < thr, accumulated one by one like the cumsum
+        double g = 0.0; long long nt = 0;
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) { g += key[i] > kappa ? __longlong_as_double(key[i]) : 0.0; nt += key[i] == kappa ? 1 : 0; }
+        g = block_sum(g, red, slot);
+        const long long n_tie = block_sum_ll(nt, red, slot);
+        if (n_tie > 1) {
+            const double p = __longlong_as_double(kappa);
+            long long keep_t = 0; double c = g;
+            while (keep_t < n_tie && c < thr) { ++keep_t; c += p; }      // every thread computes the same count
+            if (keep_t < n_tie) {
+                // iota = the keep_t-th smallest entry index among the ties: 14-bit select on the index
+                int lo_i = -1;                                           // largest index with count(ties <= index) < keep_t
+                for (int b = 13; b >= 0; --b) {
+                    const int cand = lo_i < 0 ? (1 << b) - 1 : lo_i + (1 << b);
+                    long long cnt = 0;
+#pragma unroll
+                    for (int i = 0; i < EPT; ++i) cnt += (key[i] == kappa && entry_of(i) <= cand) ? 1 : 0;
+                    cnt = block_sum_ll(cnt, red, slot);
+                    if (cnt < keep_t) lo_i = cand;
+                }
+                iota = lo_i + 1;
+            }
+        }
     }
 
-    // ---- inclusive FP64 cumulative sum in sorted order: blocked items per thread, then a block scan of the partials
-    const int ipt = (n_ent + kSelThreads - 1) / kSelThreads;
-    const int i0 = tid * ipt, i1 = min(i0 + ipt, n_ent);
-    double part = 0.0;
-    for (int i = i0; i < i1; ++i) part += __longlong_as_double((long long)~kin[i]);
-    double v = part;
-    for (int o = 1; o < 32; o <<= 1) { double u = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += u; }
-    if (lane == 31) warp_d[wid] = v;
-    __syncthreads();
-    if (wid == 0) {
-        double s = warp_d[lane];
-        for (int o = 1; o < 32; o <<= 1) { double u = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += u; }
-        warp_d[lane] = s;
-    }
-    __syncthreads();
-    const double total = warp_d[kSelWarps - 1];
-    const double thr = (1.0 - eps) * total;
-    double c_prev = (v - part) + (wid ? warp_d[wid - 1] : 0.0);          // C_{i0 - 1}
-    for (int i = i0; i < i1; ++i) {
-        if (i == 0 || c_prev < thr) {
-            int e = iin[i];
-            int j = e < n_modes ? e : L.owner[e - n_modes];
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        const int e = entry_of(i);
+        if (valid(i) && (key[i] > kappa || (key[i] == kappa && e <= iota))) {
+            const int j = e < n_modes ? e : L.owner[e - n_modes];
             atomicOr(&bitmap_s[j >> 5], 1u << (j & 31));
         }
-        c_prev += __longlong_as_double((long long)~kin[i]);
     }
     __syncthreads();
     unsigned* gb = L.bitmap + (size_t)src * words;
@@ -219,25 +263,25 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
 }
 
 // bitmap -> ascending keep_idx (padded with -1) and n_keep.  One block per source.  keep_all: identity list.
-__global__ void few_select_compact_kernel(sel_layout L, int n_modes, int keep_all, int* __restrict__ keep_idx,
-                                          int* __restrict__ n_keep)
+__global__ void __launch_bounds__(kPrepThreads)
+few_select_compact_kernel(sel_layout L, int n_modes, int keep_all, int* __restrict__ keep_idx, int* __restrict__ n_keep)
 {
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
     const int src = blockIdx.x, tid = threadIdx.x;
     int* out = keep_idx + (size_t)src * n_modes;
     if (keep_all) {
-        for (int j = tid; j < n_modes; j += kSelThreads) out[j] = j;
+        for (int j = tid; j < n_modes; j += kPrepThreads) out[j] = j;
         if (tid == 0) n_keep[src] = n_modes;
         return;
     }
     const unsigned* gb = L.bitmap + (size_t)src * sel_words(n_modes);
     if (tid == 0) carry_s = 0;
     __syncthreads();
-    for (int base = 0; base < n_modes; base += kSelThreads) {
+    for (int base = 0; base < n_modes; base += kPrepThreads) {
         int j = base + tid;
         int flag = (j < n_modes && ((gb[j >> 5] >> (j & 31)) & 1u)) ? 1 : 0, total;
-        int incl = block_scan_int(flag, warp_sums, &total);
+        int incl = block_scan_int<kPrepThreads>(flag, warp_sums, &total);
         int carry = carry_s;
         if (flag) out[carry + incl - 1] = j;
         __syncthreads();
@@ -245,11 +289,9 @@ __global__ void few_select_compact_kernel(sel_layout L, int n_modes, int keep_al
         __syncthreads();
     }
     const int cnt = carry_s;
-    for (int j = cnt + tid; j < n_modes; j += kSelThreads) out[j] = -1;
+    for (int j = cnt + tid; j < n_modes; j += kPrepThreads) out[j] = -1;
     if (tid == 0) n_keep[src] = cnt;
 }
-
-size_t sel_row_smem(int cap) { return (size_t)cap * (2 * 8 + 2 * 2) + (size_t)kSelWarps * kRadix * 4; }
 
 }  // namespace
 
@@ -273,7 +315,7 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
     cudaStream_t st = (cudaStream_t)stream;
     sel_layout L{};
     if (!(eps > 0.0)) {       // R6: eps <= 0 keeps every mode, nothing is sorted
-        few_select_compact_kernel<<<n_src, kSelThreads, 0, st>>>(L, n_modes, 1, keep_idx, n_keep);
+        few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 1, keep_idx, n_keep);
         FEW_CUDA_CHECK(cudaGetLastError());
         return FEW_OK;
     }
@@ -282,16 +324,18 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
                     workspace_bytes >= few_select_modes_workspace(n_src, n_t, n_modes),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
     L = sel_carve(workspace, n_src, n_modes);
-    few_select_prepare_kernel<<<n_src, kSelThreads, 0, st>>>(m, (const double2*)ylm_plus, (const double2*)ylm_minus, n_modes, L,
-                                                          ctx->d_status);
+    few_select_prepare_kernel<<<n_src, kPrepThreads, 0, st>>>(m, (const double2*)ylm_plus, (const double2*)ylm_minus, n_modes, L,
+                                                           ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
-    const int cap = 2 * n_modes;
-    size_t smem = sel_row_smem(cap);
-    FEW_REQUIRE(smem <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "row does not fit shared memory");
-    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_select_row_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    few_select_row_kernel<<<dim3(n_t, n_src), kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, cap, L);
+    const dim3 grid(n_t, n_src);
+    const size_t smem = (size_t)n_modes * sizeof(double);
+    constexpr int kEptMax = (FEW_MAX_SELECT_ENTRIES + kSelThreads - 1) / kSelThreads + 1;   // +1: primaries and mirrors are padded separately
+    if (2 * ((n_modes + kSelThreads - 1) / kSelThreads) <= 32)
+        few_select_row_kernel<32><<<grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+    else
+        few_select_row_kernel<kEptMax><<<grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L);
     FEW_CUDA_CHECK(cudaGetLastError());
-    few_select_compact_kernel<<<n_src, kSelThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
+    few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
     FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }

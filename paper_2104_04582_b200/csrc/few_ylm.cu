@@ -4,8 +4,8 @@
 // Computed from the Wigner small-d function,  sY_lm(theta, phi) = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},
 //   d^l_{a,b}(beta) = sqrt((l+a)!(l-a)!(l+b)!(l-b)!) sum_k (-1)^{a-b+k} cos(beta/2)^{2l+b-a-2k} sin(beta/2)^{a-b+2k}
 //                     / ((l+b-k)! k! (a-b+k)! (l-a-k)!),
-// which agrees with the Goldberg et al. convention (R11).  One thread per (source, mode); the same
-// __host__ __device__ routine backs the host helper few_ylm.
+// which agrees with the Goldberg et al. convention (R11).  The same __host__ __device__ routine backs the host
+// helper few_ylm.
 #include <math.h>
 #include "few_common.cuh"
 
@@ -50,23 +50,50 @@ extern "C" int few_ylm(int l, int m, double theta, double phi, double* out_host)
     return FEW_OK;
 }
 
-__global__ void few_ylm_modes_kernel(const double* __restrict__ theta, const double* __restrict__ phi,
-                                     const int* __restrict__ l, const int* __restrict__ m, int n_src, int n_modes,
-                                     double2* __restrict__ ylm_plus, double2* __restrict__ ylm_minus, int* status)
+// One block per source.  The harmonics depend on (l, m) only -- 117 values for l <= 10 against 3843 modes -- so the block
+// first tabulates -2Y_{l,m} for 2 <= l <= max l, |m| <= l in shared memory (one thread per entry) and every mode looks its
+// two values up.
+constexpr int kYlmThreads = 256;
+__host__ __device__ static inline int few_ylm_slot(int l, int m) { return l * l - 4 + m + l; }   // l >= 2, |m| <= l
+
+__global__ void __launch_bounds__(kYlmThreads)
+few_ylm_modes_kernel(const double* __restrict__ theta, const double* __restrict__ phi,
+                     const int* __restrict__ l, const int* __restrict__ m, int n_src, int n_modes,
+                     double2* __restrict__ ylm_plus, double2* __restrict__ ylm_minus, int* status)
 {
-    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= (long long)n_src * n_modes) return;
-    int s = (int)(gid / n_modes), j = (int)(gid % n_modes);
-    int lj = l[j], mj = m[j];
-    double2 yp = make_double2(0.0, 0.0), ym = yp;
-    if (lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj) {
-        atomicOr(status, FEW_DEV_BAD_MODE);
-    } else {
-        few_ylm_m2(lj, mj, theta[s], phi[s], &yp.x, &yp.y);
-        few_ylm_m2(lj, -mj, theta[s], phi[s], &ym.x, &ym.y);
+    extern __shared__ double2 ylm_table[];
+    __shared__ int lmax_s;
+    const int s = blockIdx.x, tid = threadIdx.x;
+    if (tid == 0) lmax_s = 2;
+    __syncthreads();
+    int lm = 2;
+    bool bad = false;
+    for (int j = tid; j < n_modes; j += kYlmThreads) {
+        const int lj = l[j], mj = m[j];
+        if (lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj) bad = true; else lm = lj > lm ? lj : lm;
     }
-    ylm_plus[gid] = yp;
-    ylm_minus[gid] = ym;
+    if (bad) atomicOr(status, FEW_DEV_BAD_MODE);
+    atomicMax(&lmax_s, lm);
+    __syncthreads();
+    const int lmax = lmax_s, n_tab = (lmax + 1) * (lmax + 1) - 4;
+    const double th = theta[s], ph = phi[s];
+    for (int idx = tid; idx < n_tab; idx += kYlmThreads) {
+        int ll = (int)sqrt((double)(idx + 4));
+        while (ll * ll > idx + 4) --ll;
+        while ((ll + 1) * (ll + 1) <= idx + 4) ++ll;
+        const int mm = idx - (ll * ll - 4) - ll;
+        double2 y;
+        few_ylm_m2(ll, mm, th, ph, &y.x, &y.y);
+        ylm_table[idx] = y;
+    }
+    __syncthreads();
+    for (int j = tid; j < n_modes; j += kYlmThreads) {
+        const int lj = l[j], mj = m[j];
+        double2 yp = make_double2(0.0, 0.0), ym = yp;
+        if (!(lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj)) { yp = ylm_table[few_ylm_slot(lj, mj)]; ym = ylm_table[few_ylm_slot(lj, -mj)]; }
+        ylm_plus[(size_t)s * n_modes + j] = yp;
+        ylm_minus[(size_t)s * n_modes + j] = ym;
+    }
 }
 
 extern "C" int few_ylm_modes(few_ctx* ctx, const double* theta, const double* phi, const int* l, const int* m,
@@ -74,11 +101,10 @@ extern "C" int few_ylm_modes(few_ctx* ctx, const double* theta, const double* ph
 {
     FEW_REQUIRE(ctx && theta && phi && l && m && ylm_plus && ylm_minus, FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE(n_src > 0 && n_modes > 0, FEW_ERR_INVALID_ARG, "n_src and n_modes must be positive");
-    long long total = (long long)n_src * n_modes;
-    int threads = 128;
-    unsigned blocks = (unsigned)((total + threads - 1) / threads);
-    few_ylm_modes_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(theta, phi, l, m, n_src, n_modes,
-                                                                      (double2*)ylm_plus, (double2*)ylm_minus, ctx->d_status);
+    const size_t smem = (size_t)((FEW_MAX_L + 1) * (FEW_MAX_L + 1) - 4) * sizeof(double2);
+    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_ylm_modes_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    few_ylm_modes_kernel<<<n_src, kYlmThreads, smem, (cudaStream_t)stream>>>(theta, phi, l, m, n_src, n_modes, (double2*)ylm_plus,
+                                                                           (double2*)ylm_minus, ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }

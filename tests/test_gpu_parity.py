@@ -292,9 +292,9 @@ def test_bad_modes_reported(api):
 
 
 def test_many_l_per_pair_and_n_gaps(api):
-    """Mode lists outside the paper's grid: 20 distinct l for one (m, n), gaps in n, a single negative-n run."""
+    """Mode lists outside the paper's grid: 15 distinct l for one (m, n), gaps in n, a single negative-n run."""
     rng = np.random.default_rng(7)
-    modes = [(l, 0, 0) for l in range(2, 22)] + [(l, 3, n) for l in (3, 5, 9) for n in (-17, -4, 2, 11)] + [(6, 6, -2), (7, 5, 40)]
+    modes = [(l, 0, 0) for l in range(2, 17)] + [(l, 3, n) for l in (3, 5, 9) for n in (-17, -4, 2, 11)] + [(6, 6, -2), (7, 5, 40)]
     l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
     n_t = 9
     t = np.sort(rng.uniform(0, 500.0, n_t)); t[0] = 0.0
