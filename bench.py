@@ -31,7 +31,7 @@ import numpy as np  # noqa: E402
 FLOP_PER_EVAL = 20.0          # nominal per-mode figure of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA)
 FLOP_PER_PAIR = 38.0          # executed algorithm: per sample and (m,n) pair 18 DFMA + 2 DMUL = 20 FP64 slots
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
-GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 + spline_dd 1 + sum 3
+GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
 GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
 
 
@@ -112,12 +112,13 @@ def time_stages(api, torch, w, g, flush, reps: int = 10):
     y_amp = torch.view_as_real(g["amp"]).reshape(w.n_src, w.n_t, -1)
     coef = api.few_spline_fit(g["t"], y_amp)
     cdd = api.few_spline_fit_dd(g["t"], g["phase"])
+    spl_ws = torch.empty(max(api._lib.few_spline_fit_workspace(w.n_src, w.n_t), 256), dtype=torch.uint8, device=coef.device)
     sel_ws = torch.empty(api._lib.few_select_modes_workspace(w.n_src, w.n_t, w.n_modes), dtype=torch.uint8, device=coef.device)
     sum_ws = torch.empty(api._lib.few_sum_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=coef.device)
     h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=coef.device)
     calls = {
         "S0_ylm_modes": lambda: api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"]),
-        "S1_spline_fit": lambda: api.few_spline_fit(g["t"], y_amp, out=coef),
+        "S1_spline_fit": lambda: api.few_spline_fit(g["t"], y_amp, out=coef, workspace=spl_ws),
         "S1_spline_fit_dd": lambda: api.few_spline_fit_dd(g["t"], g["phase"], out=cdd),
         "S2_select_modes": lambda: api.few_select_modes(g["amp"], g["m"], yp, ym, max(w.eps, 1e-5), workspace=sel_ws),
         "S3_sum_waveform": lambda: api.few_sum_waveform(g["t"], coef, cdd, g["l"], g["m"], g["n"], keep, nk, yp, ym, w.t0, w.dt,
@@ -317,7 +318,8 @@ def main():
                       "eps": w.eps, "kept_modes": K_kept, "mn_pairs": pairs, "l2": "flushed between timed steps (256 MiB write)",
                       "parallelism": f"{world} independent replicas" if world > 1 else "single GPU"},
            "ms_per_waveform": ms_per_step / w.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-           "gpu_launches": (GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) * args.steps, "clocks": clocks,
+           "gpu_launches": ((GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) + (0 if (2 * w.n_modes * w.n_src + 31) // 32 <= 148 * (232448 // (w.n_t * 608)) else 1)) * args.steps,
+           "clocks": clocks,
            "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
     if stages is not None:
         for v in stages.values():

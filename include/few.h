@@ -84,9 +84,12 @@ int few_ylm_modes(few_ctx* ctx, const double* theta, const double* phi, const in
  * t[n_src][n_t] strictly increasing; y[n_src][n_t][n_sys] (systems fastest: the amplitude module's [n_t, n_modes]
  * complex array viewed as doubles has n_sys = 2 n_modes).
  * coef[n_src][n_t-1][4][n_sys]: on segment k, S(t) = c0 + c1 dx + c2 dx^2 + c3 dx^3 with dx = t - t_k; c0 = y_k bitwise.
+ * workspace: few_spline_fit_workspace(n_src, n_t) bytes; receives each source's factorised tridiagonal matrix (the matrix
+ * depends on the grid only, so it is factored once per source, not once per system).
  * Limits: 4 <= n_t <= FEW_MAX_NT_SPLINE. */
+size_t few_spline_fit_workspace(int n_src, int n_t);
 int few_spline_fit(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
-                   double* coef, void* stream);
+                   double* coef, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Same spline, solved and stored in double-double (unevaluated sum hi + lo, |lo| <= ulp(hi)/2) for the orbital phases,
  * whose 1e5..1e6 rad magnitude needs more than 53 bits to reach 1e-10 on the waveform (R13).

@@ -18,7 +18,7 @@ _SO = os.path.join(_PKG, "libfew_b200.so")
 
 FEW_OK = 0
 SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_version", "few_device_status", "few_ylm",
-           "few_ylm_modes", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
+           "few_ylm_modes", "few_spline_fit_workspace", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms"]
 
@@ -45,7 +45,8 @@ def _load() -> C.CDLL:
         "few_device_status": (i, [vp, C.POINTER(i), vp]),
         "few_ylm": (i, [i, i, d, d, C.POINTER(d)]),
         "few_ylm_modes": (i, [vp, vp, vp, vp, vp, i, i, vp, vp, vp]),
-        "few_spline_fit": (i, [vp, vp, vp, i, i, i, vp, vp]),
+        "few_spline_fit_workspace": (sz, [i, i]),
+        "few_spline_fit": (i, [vp, vp, vp, i, i, i, vp, vp, sz, vp]),
         "few_spline_fit_dd": (i, [vp, vp, vp, i, i, i, vp, vp]),
         "few_select_modes_workspace": (sz, [i, i, i]),
         "few_select_modes": (i, [vp, vp, vp, vp, vp, d, i, i, i, vp, vp, vp, sz, vp]),
@@ -134,15 +135,16 @@ def few_ylm_modes(theta, phi, l, m):
     return yp, ym
 
 
-def few_spline_fit(t, y, out=None):
+def few_spline_fit(t, y, out=None, workspace=None):
     """t [n_src, n_t] f64; y [n_src, n_t, n_sys] f64 (or complex128 [n_src, n_t, n_modes], viewed as 2 n_modes systems)
     -> coef [n_src, n_t-1, 4, n_sys]."""
     if y.dtype == torch.complex128:
         y = torch.view_as_real(y).reshape(y.shape[0], y.shape[1], -1)
     n_src, n_t, n_sys = y.shape
     coef = out if out is not None else torch.empty((n_src, max(n_t - 1, 0), 4, n_sys), dtype=torch.float64, device=y.device)
+    ws = workspace if workspace is not None else _ws(_lib.few_spline_fit_workspace(n_src, n_t), y.device)
     _chk(_lib.few_spline_fit(context(), _p(t, torch.float64), _p(y, torch.float64), n_src, n_t, n_sys, _p(coef, torch.float64),
-                             _stream()), "few_spline_fit")
+                             _p(ws), ws.numel(), _stream()), "few_spline_fit")
     return coef
 
 

@@ -119,8 +119,8 @@ namespace {
 struct wf_layout {
     double *ylm_plus, *ylm_minus, *coef_amp, *coef_phase;
     int *keep_idx, *n_keep;
-    void *sel_ws, *sum_ws;
-    size_t sel_bytes, sum_bytes;
+    void *sel_ws, *sum_ws, *spl_ws;
+    size_t sel_bytes, sum_bytes, spl_bytes;
 };
 
 wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, size_t* bytes)
@@ -135,6 +135,8 @@ wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_sample
     L.n_keep = c.take<int>(n_src);
     L.sel_bytes = few_select_modes_workspace(n_src, n_t, n_modes);
     L.sum_bytes = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples);
+    L.spl_bytes = few_spline_fit_workspace(n_src, n_t);
+    L.spl_ws = c.take<char>(L.spl_bytes);
     L.sel_ws = c.take<char>(L.sel_bytes);
     L.sum_ws = c.take<char>(L.sum_bytes);
     if (bytes) *bytes = c.off;
@@ -171,7 +173,7 @@ extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, 
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_fork, st));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[0], ctx->ev_fork, 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[1], ctx->ev_fork, 0));
-    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, ctx->side[0]))) return rc;
+    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]))) return rc;
     if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, ctx->side[1]))) return rc;
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[0], ctx->side[0]));
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[1], ctx->side[1]));

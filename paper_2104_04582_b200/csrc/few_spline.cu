@@ -8,12 +8,13 @@
 //   last row       mirror image at t_{n-2}.
 // The matrix depends on the grid only, which every system of a source shares.
 //
+// few_spline_factor_kernel (one block per source): the matrix depends on the grid only, so its Thomas factorisation (no
+// pivoting) is done ONCE per source into six per-knot arrays in the caller's workspace -- a serial chain of n_t divisions
+// that would otherwise sit on the critical path of every block of the fit kernel (it cost as much as the block's whole
+// HBM time, profiles/r01b_spline_cfg3.md).
 // few_spline_fit_kernel (FP64, thousands of systems): one thread per system, systems fastest in memory so every global
-// access of a warp is a contiguous row.  A block first streams its [n_t x W] tile of y into shared memory with cp.async
-// (all rows in flight at once: the kernel is HBM-bound, 8 B read + 32 B written per knot and system), while thread 0
-// factors the tridiagonal matrix (Thomas, no pivoting) into per-knot multipliers.  The forward and backward substitutions
-// are then single-FMA recurrences out of shared memory, and the four coefficient planes are written as coalesced rows.
-// No cuSPARSE, no global scratch.
+// access of a warp is a contiguous row.  The kernel is HBM-bound (8 B read + 32 B written per knot and system); see the
+// comment at the kernel.  No cuSPARSE.
 //
 // few_spline_fit_dd_kernel (double-double, the two phases): the serial recurrences stay in FP64 and the extra precision
 // comes from iterative refinement: solve in FP64, form the residual of the EXACT system (grid spacings and right-hand
@@ -23,14 +24,6 @@
 
 namespace {
 
-constexpr int kConstArrays = 7;   // inv_h, w, inv_d, u = up*inv_d, rA, rB, (spare for alignment)
-
-__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gmem_src)
-{
-    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // Grid-only part shared by both kernels: 1/h, rhs weights, Thomas factorisation in FP64 (thread 0).
 __device__ void factor_grid(const double* __restrict__ t, int n, double* inv_h, double* wm, double* inv_d, double* um,
@@ -71,75 +64,140 @@ __device__ void factor_grid(const double* __restrict__ t, int n, double* inv_h, 
     }
 }
 
-template <bool kTwoTiles>
-__global__ void few_spline_fit_kernel(const double* __restrict__ t_all, const double* __restrict__ y_all,
-                                      int n_t, int n_sys, double* __restrict__ coef_all, int* status)
+// Factorisation of every source's grid into the workspace: fac[src][6][n_t] = inv_h, w, inv_d, u, rA, rB.
+__global__ void __launch_bounds__(128)
+few_spline_factor_kernel(const double* __restrict__ t_all, int n_t, double* __restrict__ fac_all, int* status)
 {
     extern __shared__ double smem[];
-    const int W = blockDim.x, tid = threadIdx.x, n = n_t;
-    double* inv_h = smem;             // [n]   1/h_i
-    double* wm = inv_h + n;           // [n]   elimination multiplier lo_i / di'_{i-1}
-    double* inv_d = wm + n;           // [n]   1 / di'_i
-    double* um = inv_d + n;           // [n]   up_i / di'_i
-    double* rA = um + n;              // [n]   rhs_i = rA_i * d_{ia} + rB_i * d_{ib}
-    double* rB = rA + n;              // [n]
-    double* Y = rB + 2 * n;           // [n][W] knot values (later overwritten by the forward-swept rhs if !kTwoTiles)
-    double* D = kTwoTiles ? Y + (size_t)n * W : Y;
-
-    const int src = blockIdx.y;
-    const double* t = t_all + (size_t)src * n;
-    const double* y = y_all + (size_t)src * n * n_sys;
-    double* coef = coef_all + (size_t)src * (n - 1) * 4 * n_sys;
-    const int q = blockIdx.x * W + tid;
-    const bool active = q < n_sys;
-
-    // ---- stream the tile in: n rows of W doubles, every row in flight at once
-    if (active) {
-        const double* yq = y + q;
-        for (int i = 0; i < n; ++i) cp_async_8(&Y[i * W + tid], yq + (size_t)i * n_sys);
-    }
-    factor_grid(t, n, inv_h, wm, inv_d, um, rA, rB, status);
-    cp_async_wait_all();
+    const int n = n_t;
+    factor_grid(t_all + (size_t)blockIdx.x * n, n, smem, smem + n, smem + 2 * n, smem + 3 * n, smem + 4 * n, smem + 5 * n, status);
     __syncthreads();
-    if (!active) return;
+    double* fac = fac_all + (size_t)blockIdx.x * 6 * n;
+    for (int i = threadIdx.x; i < 6 * n; i += blockDim.x) fac[i] = smem[i];
+}
 
-    // ---- forward substitution: d'_i = rhs_i - w_i d'_{i-1}  (one dependent FMA per knot)
-    double y_cur = Y[tid], y_nxt = Y[W + tid];
-    double dl_prev = (y_nxt - y_cur) * inv_h[0];                 // d_0
-    y_cur = y_nxt; y_nxt = Y[2 * W + tid];
-    double dl = (y_nxt - y_cur) * inv_h[1];                      // d_1
-    double d = rA[0] * dl_prev + rB[0] * dl;
-    if (!kTwoTiles) coef[q] = Y[tid];                            // c0 of segment 0 leaves before its slot is reused
-    D[tid] = d;
-#pragma unroll 4
-    for (int i = 1; i <= n - 2; ++i) {
-        // here: dl_prev = d_{i-1}, dl = d_i, y_cur = y_i, y_nxt = y_{i+1}
-        d = fma(-wm[i], d, fma(rA[i], dl_prev, rB[i] * dl));
-        if (!kTwoTiles) coef[(size_t)i * 4 * n_sys + q] = y_cur;
-        D[i * W + tid] = d;
-        if (i < n - 2) {
-            y_cur = y_nxt; y_nxt = Y[(i + 2) * W + tid];
-            dl_prev = dl; dl = (y_nxt - y_cur) * inv_h[i + 1];
+// One thread per system.  Shared memory holds the source's factorisation and ONE tile, the forward-swept right-hand
+// side D[n_t][W] (8 B per knot and system: what bounds the systems in flight per SM).  y is streamed straight from global
+// memory in both sweeps through a register ring filled kSplU knots ahead (the second pass re-reads it from L2), so no load
+// sits on the serial recurrences; c0..c3 of a segment are written together in the backward sweep as four coalesced rows.
+constexpr int kSplU = 8;
+
+__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gmem_src)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// kLatency (few blocks per SM, e.g. one source): nothing bounds shared memory, so the block also stages its whole y tile
+// with cp.async (every row in flight at once) and factors the grid itself while the rows arrive -- no pre-kernel, no
+// global load inside the sweeps.  Same arithmetic in both modes.
+template <bool kLatency>
+__global__ void __launch_bounds__(128)
+few_spline_fit_kernel(const double* __restrict__ t_all, const double* __restrict__ fac_all, const double* __restrict__ y_all,
+                      int n_t, int n_sys, double* __restrict__ coef_all, int* status)
+{
+    extern __shared__ double4 smem4[];
+    const int W = blockDim.x, tid = threadIdx.x, n = n_t;
+    double4* F = smem4;                                   // [n] {w_i, rA_i, rB_i, 1/h_i}
+    double2* Bk = reinterpret_cast<double2*>(F + n);      // [n] {u_i, 1/d'_i}
+    double* D = reinterpret_cast<double*>(Bk + n);        // [n][W]
+    double* Y = D + (size_t)n * W;                        // kLatency: [n][W] knot values, then [6][n] raw factorisation
+    const int src = blockIdx.y;
+    const int q = blockIdx.x * W + tid;
+    const double* y = y_all + (size_t)src * n * n_sys + q;
+    if (kLatency) {
+        if (q < n_sys)
+            for (int i = 0; i < n; ++i) cp_async_8(&Y[i * W + tid], y + (size_t)i * n_sys);
+        double* raw = Y + (size_t)n * W;
+        factor_grid(t_all + (size_t)src * n, n, raw, raw + n, raw + 2 * n, raw + 3 * n, raw + 4 * n, raw + 5 * n, status);
+        __syncthreads();
+        for (int i = tid; i < n; i += W) {
+            F[i] = make_double4(raw[n + i], raw[4 * n + i], raw[5 * n + i], raw[i]);
+            Bk[i] = make_double2(raw[3 * n + i], raw[2 * n + i]);
+        }
+        cp_async_wait_all();
+    } else {
+        const double* fac = fac_all + (size_t)src * 6 * n;   // inv_h, w, inv_d, u, rA, rB
+        for (int i = tid; i < n; i += W) {
+            F[i] = make_double4(fac[n + i], fac[4 * n + i], fac[5 * n + i], fac[i]);
+            Bk[i] = make_double2(fac[3 * n + i], fac[2 * n + i]);
         }
     }
-    // now dl = d_{n-2}, dl_prev = d_{n-3} (n >= 4), y_nxt = y_{n-1}
-    d = fma(-wm[n - 1], d, fma(rA[n - 1], dl_prev, rB[n - 1] * dl));
+    __syncthreads();
+    if (q >= n_sys) return;
+    double* coef = coef_all + (size_t)src * (n - 1) * 4 * n_sys + q;
+    auto ld = [&](int i) {
+        if (!(i >= 0 && i < n)) return 0.0;
+        return kLatency ? Y[i * W + tid] : __ldg(y + (size_t)i * n_sys);
+    };
+
+    // ---- forward substitution: D_i = rhs_i - w_i D_{i-1}, rhs_i = rA_i d_{i-1} + rB_i d_i  (one dependent FMA per knot)
+    double ring[kSplU];
+    const double y0 = ld(0), y1 = ld(1), y2 = ld(2);
+#pragma unroll
+    for (int u = 0; u < kSplU; ++u) ring[u] = ld(3 + u);
+    double dl_prev = (y1 - y0) * F[0].w;                  // d_0
+    double dl = (y2 - y1) * F[1].w;                       // d_1
+    double d = F[0].y * dl_prev + F[0].z * dl;            // row 0
+    D[tid] = d;
+    double y_cur = y2;                                    // y_{i+1} at the top of iteration i
+    for (int base = 1; base <= n - 2; base += kSplU) {
+        double nxt[kSplU];
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) nxt[u] = ld(base + kSplU + 2 + u);
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) {
+            const int i = base + u;
+            if (i <= n - 2) {
+                // here: dl_prev = d_{i-1}, dl = d_i, y_cur = y_{i+1}, ring[u] = y_{i+2}
+                const double4 f = F[i];
+                d = fma(-f.x, d, fma(f.y, dl_prev, f.z * dl));
+                D[i * W + tid] = d;
+                if (i < n - 2) {
+                    const double y_nxt = ring[u];
+                    dl_prev = dl; dl = (y_nxt - y_cur) * F[i + 1].w;
+                    y_cur = y_nxt;
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) ring[u] = nxt[u];
+    }
+    // now dl = d_{n-2}, dl_prev = d_{n-3} (n >= 4), y_cur = y_{n-1}
+    {
+        const double4 f = F[n - 1];
+        d = fma(-f.x, d, fma(f.y, dl_prev, f.z * dl));
+    }
 
     // ---- back substitution + coefficients, written segment by segment (coalesced rows of n_sys)
-    double s_nxt = d * inv_d[n - 1];
-    double y_hi = y_nxt;                                         // y_{n-1}
-#pragma unroll 4
-    for (int i = n - 2; i >= 0; --i) {
-        const double s = fma(-um[i], s_nxt, D[i * W + tid] * inv_d[i]);
-        double* c = coef + (size_t)i * 4 * n_sys + q;
-        const double y_lo = kTwoTiles ? Y[i * W + tid] : c[0];   // !kTwoTiles: re-read what this thread wrote (L1/L2 hit)
-        const double ih = inv_h[i];
-        const double dli = (y_hi - y_lo) * ih;
-        if (kTwoTiles) c[0] = y_lo;
-        c[n_sys] = s;
-        c[(size_t)2 * n_sys] = (3.0 * dli - 2.0 * s - s_nxt) * ih;
-        c[(size_t)3 * n_sys] = (s + s_nxt - 2.0 * dli) * (ih * ih);
-        s_nxt = s; y_hi = y_lo;
+    double s_nxt = d * Bk[n - 1].y;
+    double y_hi = y_cur;                                  // y_{i+1}
+#pragma unroll
+    for (int u = 0; u < kSplU; ++u) ring[u] = ld(n - 2 - u);
+    for (int top = n - 2; top >= 0; top -= kSplU) {
+        double nxt[kSplU];
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) nxt[u] = ld(top - kSplU - u);
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) {
+            const int i = top - u;
+            if (i >= 0) {
+                const double2 b = Bk[i];
+                const double ih = F[i].w;
+                const double s = fma(-b.x, s_nxt, D[i * W + tid] * b.y);
+                const double y_lo = ring[u];
+                const double dli = (y_hi - y_lo) * ih;
+                double* c = coef + (size_t)i * 4 * n_sys;
+                c[0] = y_lo;
+                c[n_sys] = s;
+                c[(size_t)2 * n_sys] = (3.0 * dli - 2.0 * s - s_nxt) * ih;
+                c[(size_t)3 * n_sys] = (s + s_nxt - 2.0 * dli) * (ih * ih);
+                s_nxt = s; y_hi = y_lo;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kSplU; ++u) ring[u] = nxt[u];
     }
 }
 
@@ -259,31 +317,45 @@ static int few_spline_check(few_ctx* ctx, const void* t, const void* y, const vo
     return FEW_OK;
 }
 
+extern "C" size_t few_spline_fit_workspace(int n_src, int n_t)
+{
+    if (n_src <= 0 || n_t < 4) return 0;
+    return few_align_up((size_t)n_src * 6 * n_t * sizeof(double));
+}
+
 extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
-                              double* coef, void* stream)
+                              double* coef, void* workspace, size_t workspace_bytes, void* stream)
 {
     int rc = few_spline_check(ctx, t, y, coef, n_src, n_t, n_sys);
     if (rc) return rc;
     FEW_REQUIRE(n_t <= FEW_MAX_NT_SPLINE, FEW_ERR_LIMIT, "n_t > FEW_MAX_NT_SPLINE");
-    // Block width W (systems per block): keep every SM busy (>= 2 blocks per SM when the batch allows) and at least two
-    // blocks resident per SM; prefer two shared-memory tiles (y and the swept rhs), fall back to one.
-    auto bytes = [&](int w, bool two) { return (size_t)(kConstArrays + (two ? 2 : 1) * w) * n_t * sizeof(double); };
+    FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 && workspace_bytes >= few_spline_fit_workspace(n_src, n_t),
+                FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
+    cudaStream_t st = (cudaStream_t)stream;
+    double* fac = static_cast<double*>(workspace);
     const size_t cap = (size_t)ctx->smem_optin, half = cap / 2;
-    int W = 128;
     const long long total = (long long)n_sys * n_src;
-    while (W > 32 && (bytes(W, true) > half || total / W < 2LL * ctx->sm_count)) W >>= 1;
-    bool two = bytes(W, true) <= cap;
-    if (!two) { W = 128; while (W > 32 && bytes(W, false) > half) W >>= 1; }
-    FEW_REQUIRE(bytes(W, two) <= cap, FEW_ERR_LIMIT, "n_t too large for shared memory");
-    dim3 grid((n_sys + W - 1) / W, n_src);
-    const size_t sm = bytes(W, two);
-    if (two) {
-        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-        few_spline_fit_kernel<true><<<grid, W, sm, (cudaStream_t)stream>>>(t, y, n_t, n_sys, coef, ctx->d_status);
-    } else {
-        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-        few_spline_fit_kernel<false><<<grid, W, sm, (cudaStream_t)stream>>>(t, y, n_t, n_sys, coef, ctx->d_status);
+    // Latency regime: so few systems that all 32-wide blocks, each with its two tiles, are resident at once (one wave).
+    auto bytes_lat = [&](int w) { return (size_t)n_t * (48 + 48 + 16 * (size_t)w); };
+    if (bytes_lat(32) <= cap && (total + 31) / 32 <= (long long)ctx->sm_count * (long long)(cap / bytes_lat(32))) {
+        const int W = 32;
+        dim3 grid((n_sys + W - 1) / W, n_src);
+        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes_lat(W)));
+        few_spline_fit_kernel<true><<<grid, W, bytes_lat(W), st>>>(t, nullptr, y, n_t, n_sys, coef, ctx->d_status);
+        FEW_CUDA_CHECK(cudaGetLastError());
+        return FEW_OK;
     }
+    // Throughput regime.  Block width W (systems per block): as wide as possible (longer contiguous rows per store) while at
+    // least two blocks fit an SM and the grid still covers every SM twice.
+    few_spline_factor_kernel<<<n_src, 128, (size_t)6 * n_t * sizeof(double), st>>>(t, n_t, fac, ctx->d_status);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    auto bytes = [&](int w) { return (size_t)n_t * (48 + 8 * (size_t)w); };
+    int W = 128;
+    while (W > 32 && (bytes(W) > half || total / W < 2LL * ctx->sm_count)) W >>= 1;
+    FEW_REQUIRE(bytes(W) <= cap, FEW_ERR_LIMIT, "n_t too large for shared memory");
+    dim3 grid((n_sys + W - 1) / W, n_src);
+    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes(W)));
+    few_spline_fit_kernel<false><<<grid, W, bytes(W), st>>>(t, fac, y, n_t, n_sys, coef, ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }
@@ -293,7 +365,7 @@ extern "C" int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y,
 {
     int rc = few_spline_check(ctx, t, y, coef_dd, n_src, n_t, n_sys);
     if (rc) return rc;
-    const size_t bytes = ((size_t)(kConstArrays + 1) + 2 * 2 + kDdSys * (2 + 2 + 1)) * n_t * sizeof(double);
+    const size_t bytes = ((size_t)8 + 2 * 2 + kDdSys * (2 + 2 + 1)) * n_t * sizeof(double);
     FEW_REQUIRE(bytes <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "n_t too large for shared memory");
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_dd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     dim3 grid((n_sys + kDdSys - 1) / kDdSys, n_src);

@@ -28,7 +28,12 @@ namespace {
 
 constexpr int kPlanThreads = 1024;
 constexpr int kSumThreads = 128;
-constexpr int kSumR = 4;                      // samples per thread
+#ifndef FEW_SUM_R
+#define FEW_SUM_R 4
+#define FEW_SUM_BPS 3
+#endif
+constexpr int kSumR = FEW_SUM_R;              // samples per thread
+constexpr int kSumBlocksPerSm = FEW_SUM_BPS;  // resident blocks per SM (register budget 65536 / (128 * blocks))
 constexpr int kTile = kSumThreads * kSumR;    // samples per block
 constexpr int kStagePairs = 30;               // pairs per stage
 constexpr int kStageBytes = 4096;             // 30 * 128 B of coefficients + 64 ints of header
@@ -321,8 +326,41 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
     } while (!ok);
 }
 
+// E <- E * Z_r for the R samples of a thread (Z_r or conj Z_r, whichever zri currently holds)
 template <int R>
-__global__ void __launch_bounds__(kSumThreads, 4)
+__device__ __forceinline__ void advance_e(double (&er)[R], double (&ei)[R], const double (&zrr)[R], const double (&zri)[R])
+{
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const double m1 = ei[r] * zri[r], m2 = ei[r] * zrr[r], e0 = er[r];
+        er[r] = fma(e0, zrr[r], -m1);
+        ei[r] = fma(e0, zri[r], m2);
+    }
+}
+
+// acc_p += e_r U_p + e_i V_p for the four powers p of dx.  Every DFMA has one block-uniform operand (a coefficient, shared by
+// the R samples of the thread) and two per-thread ones: the form the FP64 pipe sustains at one warp instruction per two
+// cycles (three fresh per-thread register operands cost three).
+template <int R>
+__device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, const double (&er)[R], const double (&ei)[R],
+                                                double (&are)[4][R], double (&aim)[4][R])
+{
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const double2 u = cp[p];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { are[p][r] = fma(er[r], u.x, are[p][r]); aim[p][r] = fma(er[r], u.y, aim[p][r]); }
+    }
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const double2 v = cp[4 + p];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { are[p][r] = fma(ei[r], v.x, are[p][r]); aim[p][r] = fma(ei[r], v.y, aim[p][r]); }
+    }
+}
+
+template <int R, int kBlocksPerSm>
+__global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
                int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all)
 {
@@ -340,7 +378,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     }
     unsigned gst = 0;                       // stages consumed by this block so far: ring slot gst % kRing, parity (gst / kRing) & 1
 
-    // Persistent block: tiles (512 samples of one sparse segment of one source) are handed out by an atomic counter, so
+    // Persistent block: tiles (R*128 samples of one sparse segment of one source) are handed out by an atomic counter, so
     // SMs never idle on wave boundaries and the blocks of an SM drift apart (one block's phase setup overlaps the others'
     // FP64 loops).
     for (;;) {
@@ -381,21 +419,25 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     // ---- per-sample setup (overlaps the first copies): dx and the two phase factors
     const double tk = t_all[(size_t)src * n_t + k];
     const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 8;     // [4][2] dd
-    double dx[R], zpr[R], zpi[R], zrr[R], zri[R];
+    double zrr[R], zri[R], er[R], ei[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         long long i = i_begin + r * kSumThreads + tid;
         if (i >= i_end) i = i_end - 1;                              // tail lanes recompute the last sample, never store
-        dx[r] = __dsub_rn(sample_time(t0, dt, i), tk);
-        phase_factor(cph + 0, 2, dx[r], &zpr[r], &zpi[r]);
-        phase_factor(cph + 1, 2, dx[r], &zrr[r], &zri[r]);
+        const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
+        double zpr, zpi;
+        phase_factor(cph + 0, 2, dx, &zpr, &zpi);
+        phase_factor(cph + 1, 2, dx, &zrr[r], &zri[r]);
+        // Z_phi and the run's Z_phi^m are needed only when m or the sign of n changes: parked in shared memory, not registers
+        stash_zp[r][tid] = make_double2(zpr, zpi);
+        stash_pm[r][tid] = make_double2(1.0, 0.0);
+        er[r] = 1.0; ei[r] = 0.0;
     }
-    // Z_phi and the run's Z_phi^m are needed only when m or the sign of n changes: parked in shared memory, not registers
+    double are[4][R], aim[4][R];                                    // sum over pairs of e_r U_p + e_i V_p, p = power of dx
 #pragma unroll
-    for (int r = 0; r < R; ++r) { stash_zp[r][tid] = make_double2(zpr[r], zpi[r]); stash_pm[r][tid] = make_double2(1.0, 0.0); }
-    double hre[R], him[R], er[R], ei[R];
+    for (int q = 0; q < 4; ++q)
 #pragma unroll
-    for (int r = 0; r < R; ++r) { hre[r] = him[r] = 0.0; er[r] = 1.0; ei[r] = 0.0; }
+        for (int r = 0; r < R; ++r) are[q][r] = aim[q][r] = 0.0;
     bool neg = false;                                               // zri currently holds -Im Z_r (walking n downward)
 
     for (int st = 0; st < n_stages; ++st) {
@@ -412,7 +454,16 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         const int* hdr = reinterpret_cast<const int*>(cp + kStagePairs * 8);
         const int ng = hdr[0];
         unsigned spec = (unsigned)hdr[1];
-        for (int gi = 0; gi < ng; ++gi, cp += 8, spec >>= 1) {
+        int gi = 0;
+        while (gi < ng) {
+            if ((spec & 3u) == 0u && gi + 1 < ng) {                 // common: the next two n of the same run, E *= Z_r each
+                advance_e<R>(er, ei, zrr, zri);
+                accumulate_pair<R>(cp, er, ei, are, aim);
+                advance_e<R>(er, ei, zrr, zri);
+                accumulate_pair<R>(cp + 8, er, ei, are, aim);
+                gi += 2; cp += 16; spec >>= 2;
+                continue;
+            }
             if (spec & 1u) {                                        // rare: new m, sign change of n, or a gap in n
                 const int d = hdr[2 + gi];
                 if (d & kNewRun) {
@@ -440,65 +491,25 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                     neg = want_neg;
                 }
                 const int nadv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
-                for (int q = 0; q < nadv; ++q) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        double a = er[r] * zrr[r] - ei[r] * zri[r];
-                        ei[r] = er[r] * zri[r] + ei[r] * zrr[r];
-                        er[r] = a;
-                    }
-                }
-            } else {                                                // common: next n of the same run, E *= Z_r
-                // operand order chosen for the register-file reuse latches: a DFMA with three fresh
-                // per-thread register operands issues every 3 cycles instead of 2
-                double m1[R], m2[R];
-#pragma unroll
-                for (int r = 0; r < R; ++r) { m1[r] = ei[r] * zri[r]; m2[r] = ei[r] * zrr[r]; }
-#pragma unroll
-                for (int r = 0; r < R; ++r) { const double e0 = er[r]; er[r] = fma(e0, zrr[r], -m1[r]); ei[r] = fma(e0, zri[r], m2[r]); }
+                for (int q = 0; q < nadv; ++q) advance_e<R>(er, ei, zrr, zri);
+            } else {
+                advance_e<R>(er, ei, zrr, zri);
             }
-            double tr[R], ti[R];
-            {
-                const double2 u3 = cp[3], u2 = cp[2], u1 = cp[1], u0 = cp[0];
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(u3.x, dx[r], u2.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(u3.y, dx[r], u2.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], u1.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], u1.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], u0.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], u0.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) { hre[r] = fma(tr[r], er[r], hre[r]); him[r] = fma(ti[r], er[r], him[r]); }
-            }
-            {
-                const double2 v3 = cp[7], v2 = cp[6], v1 = cp[5], v0 = cp[4];
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(v3.x, dx[r], v2.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(v3.y, dx[r], v2.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], v1.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], v1.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) tr[r] = fma(tr[r], dx[r], v0.x);
-#pragma unroll
-                for (int r = R - 1; r >= 0; --r) ti[r] = fma(ti[r], dx[r], v0.y);
-#pragma unroll
-                for (int r = 0; r < R; ++r) { hre[r] = fma(tr[r], ei[r], hre[r]); him[r] = fma(ti[r], ei[r], him[r]); }
-            }
+            accumulate_pair<R>(cp, er, ei, are, aim);
+            ++gi; cp += 8; spec >>= 1;
         }
     }
 
+    // ---- h = acc_0 + dx (acc_1 + dx (acc_2 + dx acc_3)), once per sample
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        long long i = i_begin + r * kSumThreads + tid;
-        if (i < i_end) __stcs(&h[i], make_double2(hre[r], him[r]));
+        const long long i = i_begin + r * kSumThreads + tid;
+        if (i < i_end) {
+            const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
+            const double hr = fma(fma(fma(are[3][r], dx, are[2][r]), dx, are[1][r]), dx, are[0][r]);
+            const double hi = fma(fma(fma(aim[3][r], dx, aim[2][r]), dx, aim[1][r]), dx, aim[0][r]);
+            __stcs(&h[i], make_double2(hr, hi));
+        }
     }
     }   // persistent tile loop
 }
@@ -549,8 +560,8 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
-    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * 4;
-    few_sum_kernel<kSumR><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
+    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
+    few_sum_kernel<kSumR, kSumBlocksPerSm><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
         t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
