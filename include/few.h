@@ -136,8 +136,11 @@ int few_waveform(few_ctx* ctx, const double* t, const double* phase, const doubl
                  double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): copies inputs host->device
- * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform, copies h
- * (and keep_idx/n_keep if not NULL) device->host and synchronises.  Not re-entrant on one context.  `scale_host` may be NULL.  Returns the device status as well. */
+ * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform and delivers h
+ * (and keep_idx/n_keep if not NULL) to the host, then synchronises.  If h_host is page-locked (cudaHostAlloc /
+ * cudaHostRegister / torch pin_memory) the summation kernel stores into it directly, so the device->host transfer overlaps
+ * the computation; pageable h_host is filled by a copy after the kernels.  Not re-entrant on one context.  `scale_host` may
+ * be NULL.  Returns the device status as well. */
 int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
                       const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
                       const double* phi_host, const double* scale_host, double eps, double t0, double dt,

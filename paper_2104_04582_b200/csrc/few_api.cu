@@ -75,6 +75,8 @@ extern "C" int few_destroy(few_ctx* ctx)
     }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    for (int g = 0; g < kHostGroups; ++g) if (ctx->ev_group[g]) cudaEventDestroy(ctx->ev_group[g]);
     cudaFree(ctx->host_arena);
     delete ctx;
     return FEW_OK;
@@ -200,12 +202,25 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     const size_t b_t = (size_t)n_src * n_t * 8, b_ph = b_t * 2, b_amp = (size_t)n_src * n_t * n_modes * 16;
     const size_t b_lmn = (size_t)n_modes * 4, b_ang = (size_t)n_src * 8, b_h = (size_t)n_src * n_samples * 16;
     const size_t b_keep = (size_t)n_src * n_modes * 4, b_nk = (size_t)n_src * 4;
-    const size_t ws_bytes = few_waveform_workspace(n_src, n_t, n_modes, n_samples);
+    const int group_max = (n_src + kHostGroups - 1) / kHostGroups > 1 ? (n_src + kHostGroups - 1) / kHostGroups : 1;
+    const size_t ws_bytes = few_waveform_workspace(n_src < kHostGroups ? 1 : group_max, n_t, n_modes, n_samples);
+    // If h_host is pinned (page-locked, hence device-accessible under unified addressing) the summation kernel stores the
+    // waveform straight into it: the device->host transfer then rides on the kernel's own coalesced streaming stores and
+    // overlaps the FP64 work, instead of following it as a separate copy.  Pageable memory takes the staged path.
+    double* h_mapped = nullptr;
+    if (n_samples) {
+        cudaPointerAttributes attr;
+        if (cudaPointerGetAttributes(&attr, h_host) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer)
+            h_mapped = static_cast<double*>(attr.devicePointer);
+        else
+            (void)cudaGetLastError();
+    }
+    const size_t b_h_dev = h_mapped ? 0 : b_h;
     // one device allocation, carved
     size_t total = 0;
     few_carver sz(nullptr);
     sz.take<char>(b_t); sz.take<char>(b_ph); sz.take<char>(b_amp); sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_lmn);
-    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_h); sz.take<char>(b_keep); sz.take<char>(b_nk);
+    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_h_dev); sz.take<char>(b_keep); sz.take<char>(b_nk);
     sz.take<char>(ws_bytes);
     total = sz.off;
     // device arena and stream are kept in the context between calls (grow-only), so a steady-state call allocates nothing
@@ -214,7 +229,11 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
         FEW_CUDA_CHECK(cudaMalloc(&ctx->host_arena, total));
         ctx->host_arena_bytes = total;
     }
-    if (!ctx->host_stream) FEW_CUDA_CHECK(cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
+    if (!ctx->host_stream) {
+        FEW_CUDA_CHECK(cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
+        FEW_CUDA_CHECK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        for (int g = 0; g < kHostGroups; ++g) FEW_CUDA_CHECK(cudaEventCreateWithFlags(&ctx->ev_group[g], cudaEventDisableTiming));
+    }
     void* dev = ctx->host_arena;
     cudaStream_t st = ctx->host_stream;
     int rc = FEW_OK;
@@ -223,23 +242,41 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph); double* d_amp = (double*)c.take<char>(b_amp);
     int* d_l = (int*)c.take<char>(b_lmn); int* d_m = (int*)c.take<char>(b_lmn); int* d_n = (int*)c.take<char>(b_lmn);
     double* d_th = (double*)c.take<char>(b_ang); double* d_phi = (double*)c.take<char>(b_ang); double* d_sc = (double*)c.take<char>(b_ang);
-    double* d_h = (double*)c.take<char>(b_h); int* d_keep = (int*)c.take<char>(b_keep); int* d_nk = (int*)c.take<char>(b_nk);
+    double* d_h = (double*)c.take<char>(b_h_dev); int* d_keep = (int*)c.take<char>(b_keep); int* d_nk = (int*)c.take<char>(b_nk);
     void* d_ws = c.take<char>(ws_bytes);
-#define FEW_H2D(dst, src, bytes) if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st)
-    FEW_H2D(d_t, t_host, b_t); FEW_H2D(d_ph, phase_host, b_ph); FEW_H2D(d_amp, amp_host, b_amp);
+    // Sources are independent, so a batch is cut into up to kHostGroups groups: the inputs of every group go host->device
+    // on a copy stream, and group g's kernels start as soon as ITS inputs have landed, i.e. while later groups are still in
+    // flight over PCIe.  (One source: one group; its 6 MB of inputs precede everything.)
+    const int n_groups = n_src < kHostGroups ? n_src : kHostGroups;
+    cudaStream_t cs = ctx->copy_stream;
+#define FEW_H2D(dst, src, bytes) if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, cs)
     FEW_H2D(d_l, l_host, b_lmn); FEW_H2D(d_m, m_host, b_lmn); FEW_H2D(d_n, n_host, b_lmn);
-    FEW_H2D(d_th, theta_host, b_ang); FEW_H2D(d_phi, phi_host, b_ang);
-    if (scale_host) FEW_H2D(d_sc, scale_host, b_ang);
+    for (int g = 0; g < n_groups && e == cudaSuccess; ++g) {
+        const size_t s0 = (size_t)n_src * g / n_groups, s1 = (size_t)n_src * (g + 1) / n_groups, ns = s1 - s0;
+        FEW_H2D(d_t + s0 * n_t, t_host + s0 * n_t, ns * n_t * 8);
+        FEW_H2D(d_ph + s0 * n_t * 2, phase_host + s0 * n_t * 2, ns * n_t * 16);
+        FEW_H2D(d_th + s0, theta_host + s0, ns * 8); FEW_H2D(d_phi + s0, phi_host + s0, ns * 8);
+        if (scale_host) FEW_H2D(d_sc + s0, scale_host + s0, ns * 8);
+        FEW_H2D(d_amp + s0 * n_t * n_modes * 2, amp_host + s0 * n_t * n_modes * 2, ns * n_t * n_modes * 16);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_group[g], cs);
+    }
 #undef FEW_H2D
-    if (e == cudaSuccess) {
-        rc = few_waveform(ctx, d_t, d_ph, d_amp, d_l, d_m, d_n, d_th, d_phi, scale_host ? d_sc : nullptr, eps, t0, dt, n_samples,
-                          n_src, n_t, n_modes, d_h, d_keep, d_nk, d_ws, ws_bytes, st);
-        if (rc == FEW_OK) {
-            if (n_samples) e = cudaMemcpyAsync(h_host, d_h, b_h, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess && keep_idx_host) e = cudaMemcpyAsync(keep_idx_host, d_keep, b_keep, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess && n_keep_host) e = cudaMemcpyAsync(n_keep_host, d_nk, b_nk, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) rc = few_device_status(ctx, nullptr, st);   // synchronises
-        }
+    double* h_out = h_mapped ? h_mapped : d_h;
+    for (int g = 0; g < n_groups && e == cudaSuccess && rc == FEW_OK; ++g) {
+        const size_t s0 = (size_t)n_src * g / n_groups, s1 = (size_t)n_src * (g + 1) / n_groups, ns = s1 - s0;
+        e = cudaStreamWaitEvent(st, ctx->ev_group[g], 0);
+        if (e != cudaSuccess) break;
+        rc = few_waveform(ctx, d_t + s0 * n_t, d_ph + s0 * n_t * 2, d_amp + s0 * n_t * n_modes * 2, d_l, d_m, d_n, d_th + s0, d_phi + s0,
+                          scale_host ? d_sc + s0 : nullptr, eps, t0, dt, n_samples, (int)ns, n_t, n_modes,
+                          h_out + s0 * (size_t)n_samples * 2, d_keep + s0 * n_modes, d_nk + s0, d_ws, ws_bytes, st);
+        if (rc == FEW_OK && n_samples && !h_mapped)
+            e = cudaMemcpyAsync(h_host + s0 * (size_t)n_samples * 2, d_h + s0 * (size_t)n_samples * 2, ns * (size_t)n_samples * 16,
+                                cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess && rc == FEW_OK) {
+        if (keep_idx_host) e = cudaMemcpyAsync(keep_idx_host, d_keep, b_keep, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && n_keep_host) e = cudaMemcpyAsync(n_keep_host, d_nk, b_nk, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) rc = few_device_status(ctx, nullptr, st);   // synchronises
     }
     if (e != cudaSuccess) { few_set_error("few_waveform_host: %s", cudaGetErrorString(e)); rc = FEW_ERR_CUDA; }
     cudaStreamSynchronize(st);

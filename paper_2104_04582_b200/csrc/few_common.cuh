@@ -5,6 +5,8 @@
 #include <stdio.h>
 #include "few.h"
 
+constexpr int kHostGroups = 8;   // few_waveform_host: source groups whose input copies overlap earlier groups' kernels
+
 struct few_ctx {
     int device;
     int sm_count;
@@ -17,7 +19,8 @@ struct few_ctx {
     cudaEvent_t ev_fork, ev_join[2];
     void* host_arena;      // few_waveform_host: grow-only device arena (inputs, h, workspace), freed by few_destroy
     size_t host_arena_bytes;
-    cudaStream_t host_stream;
+    cudaStream_t host_stream, copy_stream;   // few_waveform_host: kernels / host->device copies
+    cudaEvent_t ev_group[8];                 // inputs of source group g have landed
 };
 
 void few_set_error(const char* fmt, ...);

@@ -306,16 +306,31 @@ def test_many_l_per_pair_and_n_gaps(api):
     assert nk[0] == len(l) and rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
 
 
-def test_whole_path_host_buffers(api):
+@pytest.mark.parametrize("pinned_out", [True, False])
+def test_whole_path_host_buffers(api, pinned_out):
+    """few_waveform_host: pinned h is written by the summation kernel itself (mapped stores), pageable h by a copy."""
     w = synth.make_config(1, n_samples=4_000, t0=1_000_000.0)
     f = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
     keep = torch.empty((1, w.n_modes), dtype=torch.int32).pin_memory(); nk = torch.empty((1,), dtype=torch.int32).pin_memory()
+    out = torch.full((1, w.n_samples), float("nan"), dtype=torch.complex128)
+    out = out.pin_memory() if pinned_out else out
     h = api.few_waveform_host(f(w.t), f(w.phase), f(w.amp), f(w.l), f(w.m), f(w.n), f(w.theta), f(w.phi), w.eps, w.t0, w.dt,
-                              w.n_samples, keep_idx=keep, n_keep=nk).numpy()
+                              w.n_samples, out=out, keep_idx=keep, n_keep=nk).numpy()
     hd, keepd, nkd = run_gpu_chain(api, w)
     assert np.array_equal(h, hd) and nk[0].item() == nkd[0] and np.array_equal(keep.numpy(), keepd)
     ref_k = oracle_with_gpu_keep(w, 0, keepd[0][: nkd[0]], [(0, w.n_samples)])[0]
     assert rel_l2(h[0], ref_k) <= REL_L2_TOL
+
+
+def test_host_buffers_batch_in_source_groups(api):
+    """few_waveform_host cuts a batch into source groups (copy/compute overlap): results equal the one-shot device chain."""
+    w = synth.make_config(3, n_src=11, n_samples=3_000, t0=2_000_000.0)
+    f = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
+    keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32).pin_memory(); nk = torch.empty((w.n_src,), dtype=torch.int32).pin_memory()
+    h = api.few_waveform_host(f(w.t), f(w.phase), f(w.amp), f(w.l), f(w.m), f(w.n), f(w.theta), f(w.phi), w.eps, w.t0, w.dt,
+                              w.n_samples, keep_idx=keep, n_keep=nk).numpy()
+    hd, keepd, nkd = run_gpu_chain(api, w)
+    assert np.array_equal(nk.numpy(), nkd) and np.array_equal(keep.numpy(), keepd) and np.array_equal(h, hd)
 
 
 # ------------------------------------------------------------------------------------------- full size, sampled
