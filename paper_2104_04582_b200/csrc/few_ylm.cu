@@ -4,8 +4,8 @@
 // Computed from the Wigner small-d function,  sY_lm(theta, phi) = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},
 //   d^l_{a,b}(beta) = sqrt((l+a)!(l-a)!(l+b)!(l-b)!) sum_k (-1)^{a-b+k} cos(beta/2)^{2l+b-a-2k} sin(beta/2)^{a-b+2k}
 //                     / ((l+b-k)! k! (a-b+k)! (l-a-k)!),
-// which agrees with the Goldberg et al. convention (R11).  The same __host__ __device__ routine backs the host
-// helper few_ylm.
+// which agrees with the Goldberg et al. convention (R11).  few_ylm_m2 backs the host helper few_ylm; the device
+// kernel evaluates the same sum from shared tables.
 #include <math.h>
 #include "few_common.cuh"
 
@@ -51,9 +51,11 @@ extern "C" int few_ylm(int l, int m, double theta, double phi, double* out_host)
 }
 
 // One block per source.  The harmonics depend on (l, m) only -- 117 values for l <= 10 against 3843 modes -- so the block
-// first tabulates -2Y_{l,m} for 2 <= l <= max l, |m| <= l in shared memory (one thread per entry) and every mode looks its
-// two values up.
-constexpr int kYlmThreads = 256;
+// first tabulates -2Y_{l,m} for 2 <= l <= max l, |m| <= l in shared memory (one thread per entry, reading factorials and the
+// powers of cos(theta/2), sin(theta/2) from small shared tables built in parallel) and every mode looks its two values up.
+// Same sum, same operation order as few_ylm_m2.
+constexpr int kYlmThreads = 1024;
+constexpr int kYlmPow = 2 * FEW_MAX_L + 3;       // powers 0 .. 2l + 2
 __host__ __device__ static inline int few_ylm_slot(int l, int m) { return l * l - 4 + m + l; }   // l >= 2, |m| <= l
 
 __global__ void __launch_bounds__(kYlmThreads)
@@ -62,9 +64,14 @@ few_ylm_modes_kernel(const double* __restrict__ theta, const double* __restrict_
                      double2* __restrict__ ylm_plus, double2* __restrict__ ylm_minus, int* status)
 {
     extern __shared__ double2 ylm_table[];
+    __shared__ double fact_s[kYlmPow], chp[kYlmPow], shp[kYlmPow];
     __shared__ int lmax_s;
     const int s = blockIdx.x, tid = threadIdx.x;
     if (tid == 0) lmax_s = 2;
+    const double th = theta[s], ph = phi[s];
+    if (tid < kYlmPow) fact_s[tid] = few_fact(tid);
+    else if (tid < 2 * kYlmPow) chp[tid - kYlmPow] = few_ipow(cos(0.5 * th), tid - kYlmPow);
+    else if (tid < 3 * kYlmPow) shp[tid - 2 * kYlmPow] = few_ipow(sin(0.5 * th), tid - 2 * kYlmPow);
     __syncthreads();
     int lm = 2;
     bool bad = false;
@@ -73,18 +80,26 @@ few_ylm_modes_kernel(const double* __restrict__ theta, const double* __restrict_
         if (lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj) bad = true; else lm = lj > lm ? lj : lm;
     }
     if (bad) atomicOr(status, FEW_DEV_BAD_MODE);
-    atomicMax(&lmax_s, lm);
+    lm = __reduce_max_sync(0xffffffffu, lm);
+    if ((tid & 31) == 0 && lm > 2) atomicMax(&lmax_s, lm);
     __syncthreads();
     const int lmax = lmax_s, n_tab = (lmax + 1) * (lmax + 1) - 4;
-    const double th = theta[s], ph = phi[s];
     for (int idx = tid; idx < n_tab; idx += kYlmThreads) {
         int ll = (int)sqrt((double)(idx + 4));
         while (ll * ll > idx + 4) --ll;
         while ((ll + 1) * (ll + 1) <= idx + 4) ++ll;
         const int mm = idx - (ll * ll - 4) - ll;
-        double2 y;
-        few_ylm_m2(ll, mm, th, ph, &y.x, &y.y);
-        ylm_table[idx] = y;
+        const int a = mm, b = 2;
+        const int k0 = (b - a) > 0 ? (b - a) : 0, k1 = (ll + b) < (ll - a) ? (ll + b) : (ll - a);
+        double tot = 0.0;
+        for (int k = k0; k <= k1; ++k) {
+            const double term = chp[2 * ll + b - a - 2 * k] * shp[a - b + 2 * k] /
+                                (fact_s[ll + b - k] * fact_s[k] * fact_s[a - b + k] * fact_s[ll - a - k]);
+            tot += ((a - b + k) & 1) ? -term : term;
+        }
+        const double d = sqrt(fact_s[ll + a] * fact_s[ll - a] * fact_s[ll + b] * fact_s[ll - b]) * tot;
+        const double v = sqrt((2.0 * ll + 1.0) / (4.0 * 3.14159265358979323846)) * d;
+        ylm_table[idx] = make_double2(v * cos(mm * ph), v * sin(mm * ph));
     }
     __syncthreads();
     for (int j = tid; j < n_modes; j += kYlmThreads) {
