@@ -10,13 +10,19 @@
 //
 // What the procedure defines is a SET, and the set is fixed by one number: C_{r-1} of an entry is G(key) = the summed power
 // of all entries with a strictly larger key (plus earlier ties), G is monotone in the key, so the kept entries are exactly
-// those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernel therefore does an MSB-first radix SELECT on
-// the order-preserving 64-bit pattern of the FP64 power instead of a full radix sort: each of the 63 bit steps is one masked
-// block reduction over powers held in registers (one block of 256 threads per row, nothing but the row's amplitudes read
-// from HBM, no scratch).  Ties at kappa are resolved by entry index with a second, 14-step select.  The owners of the kept
-// entries are OR-ed into a per-source bitmap; a last kernel compacts it into ascending keep_idx and n_keep.
-// (A stable in-shared-memory LSD radix sort + scan, the first version of this file, gave the same sets at 128 us per
-// 7137-entry row; this one takes ~5 us.  See DESIGN.md section 5.)
+// those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernel therefore SELECTS instead of sorting the
+// whole row (one block of 256 threads per row, powers held in registers, nothing but the row's amplitudes read from HBM):
+//   1. coarse: the key's top 11 bits are the binary exponent of the power.  An 11-step MSB-first search, each step one
+//      masked block reduction, finds the exponent bucket B in which the cumulative sum crosses the threshold.  Every entry
+//      in a higher bucket is kept, every entry in a lower one dropped.
+//   2. fine: the (typically ~100-200) entries of bucket B are compacted into shared memory, rank-sorted by (power
+//      descending, entry index ascending) and cumulatively summed in that order on top of the power above the bucket: this
+//      is the definition's sort + cumsum, applied only where it can change the answer.  Ties need no special case.
+//   3. fallback (more than kBucketMax entries in the bucket, e.g. a row of equal powers): a 63-step MSB-first radix select
+//      on the full 64-bit pattern, ties at kappa resolved by entry index with a 14-step select.
+// The owners of the kept entries are OR-ed into a per-source bitmap; a last kernel compacts it into ascending keep_idx
+// and n_keep.  (History: in-shared-memory LSD radix sort + scan 128 us per 7137-entry row; 63-step
+// select alone 44 us; this version see profiles/.)
 #include "few_common.cuh"
 
 namespace {
@@ -24,6 +30,7 @@ namespace {
 constexpr int kSelThreads = 256;
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kPrepThreads = 1024;
+constexpr int kBucketMax = 512;   // entries of the threshold's exponent bucket that the fine step sorts in shared memory
 
 struct sel_layout {
     int* owner;       // [n_modes]   owner mode of mirror entry e - n_modes   (shared by sources)
@@ -151,6 +158,9 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
     extern __shared__ double a2_s[];                 // [n_modes] |A_j|^2
     __shared__ sel_red red;
     __shared__ unsigned bitmap_s[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
+    __shared__ double bkt_p[kBucketMax], srt_p[kBucketMax];
+    __shared__ int bkt_e[kBucketMax], srt_e[kBucketMax];
+    __shared__ int bkt_count;
     const int tid = threadIdx.x;
     const int src = blockIdx.y, k = blockIdx.x;
     const int n_ent = *L.n_entries;
@@ -159,6 +169,7 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
     const double* y2 = L.y2 + (size_t)src * 2 * n_modes;
     const int words = sel_words(n_modes);
     for (int w = tid; w < words; w += kSelThreads) bitmap_s[w] = 0u;
+    if (tid == 0) bkt_count = 0;
     int slot = 0;
     auto entry_of = [&](int i) { return i < NP ? i * kSelThreads + tid : n_modes + (i - NP) * kSelThreads + tid; };
     auto valid = [&](int i) { return i < NP ? i * kSelThreads + tid < n_modes : entry_of(i) < n_ent; };
@@ -210,12 +221,66 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
         for (int i = 0; i < EPT; ++i) if (key[i] == kappa) { long long c = -(long long)entry_of(i); best = c > best ? c : best; }
         iota = (int)(-block_max_ll(best, red, slot));
     } else {
-        // G(c) = sum of powers with key > c is monotone non-increasing in c (the fixed reduction tree keeps that exactly);
+        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x and
+        // g(0) = total >= thr; B = the largest x with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
+        long long B = 0;
+        for (int b = 10; b >= 0; --b) {
+            const long long cand = (B | (1ll << b)) << 52;
+            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] >= cand ? __longlong_as_double(key[i]) : 0.0;
+            const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
+            if (!(g < thr)) B |= 1ll << b;
+        }
+        const long long k_lo = B << 52, k_hi = B >= 2047 ? 0x7fffffffffffffffLL : (B + 1) << 52;   // bucket B = keys in [k_lo, k_hi)
+        double ga = 0.0; long long nb = 0;
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) { ga += key[i] >= k_hi ? __longlong_as_double(key[i]) : 0.0; nb += (key[i] >= k_lo && key[i] < k_hi) ? 1 : 0; }
+        const double g_above = block_sum(ga, red, slot);           // < thr by construction
+        const long long n_bkt = block_sum_ll(nb, red, slot);
+        if (n_bkt <= kBucketMax) {
+            // ---- 2. fine: sort + cumulative sum of the bucket's entries, exactly as the definition orders them
+#pragma unroll
+            for (int i = 0; i < EPT; ++i)
+                if (key[i] >= k_lo && key[i] < k_hi) {
+                    const int pos = atomicAdd(&bkt_count, 1);
+                    bkt_p[pos] = __longlong_as_double(key[i]); bkt_e[pos] = entry_of(i);
+                }
+            __syncthreads();
+            const int M = (int)n_bkt;
+            for (int q = tid; q < M; q += kSelThreads) {
+                const double pq = bkt_p[q]; const int eq = bkt_e[q];
+                int rank = 0;
+                for (int r = 0; r < M; ++r) { const double pr = bkt_p[r]; rank += (pr > pq || (pr == pq && bkt_e[r] < eq)) ? 1 : 0; }
+                srt_p[rank] = pq; srt_e[rank] = eq;
+            }
+            __syncthreads();
+            if (tid < 32) {
+                // warp 0: C_{r-1} = g_above + (sum of the sorted entries before r), lane l owning positions [16 l, 16 l + 16)
+                constexpr int kPer = kBucketMax / 32;
+                double loc = 0.0;
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) { const int r = tid * kPer + u; loc += r < M ? srt_p[r] : 0.0; }
+                double incl = loc;
+                for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += v; }
+                double c = g_above + (incl - loc);
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) {
+                    const int r = tid * kPer + u;
+                    if (r < M) {
+                        if (c < thr) { const int e = srt_e[r]; const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&bitmap_s[j >> 5], 1u << (j & 31)); }
+                        c += srt_p[r];
+                    }
+                }
+            }
+            kappa = k_hi - 1; iota = -1;                             // below: key > kappa keeps everything above the bucket
+        } else {
+        // ---- 3. fallback.  G(c) = sum of powers with key > c is monotone non-increasing in c (the fixed reduction tree keeps that exactly);
         // build the largest c with G(c) >= thr bit by bit, then kappa = c + 1.
         long long lo = 0;
         for (int b = 62; b >= 0; --b) {
             const long long cand = lo | (1ll << b);
-            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
+            double g4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] > cand ? __longlong_as_double(key[i]) : 0.0;
             const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
@@ -245,6 +310,7 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
                 }
                 iota = lo_i + 1;
             }
+        }
         }
     }
 
