@@ -129,11 +129,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
                     const double* __restrict__ scale, double t0, double dt, long long N, int n_t, int n_modes,
                     sum_layout L, int* status)
 {
-    extern __shared__ unsigned plan_smem[];
-    unsigned* ukey = plan_smem;                                   // [n_modes] unsorted keys
-    unsigned* skey = ukey + n_modes;                              // [n_modes] sorted keys
-    int* uj = reinterpret_cast<int*>(skey + n_modes);             // [n_modes]
-    int* sj = uj + n_modes;                                       // [n_modes]
+    extern __shared__ unsigned long long plan_sorted[];           // [n_pow2] (key << 32 | mode index), sorted ascending
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
 
@@ -174,18 +170,25 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
             atomicOr(status, FEW_DEV_BAD_MODE);
             lj = 2; mj = 0; an = 0; nj = 0; j = ok ? j : 0;
         }
-        ukey[q] = ((unsigned)mj << 21) | ((nj < 0 ? 1u : 0u) << 20) | ((unsigned)an << 8) | (unsigned)lj;
-        uj[q] = j;
+        const unsigned key = ((unsigned)mj << 21) | ((nj < 0 ? 1u : 0u) << 20) | ((unsigned)an << 8) | (unsigned)lj;
+        plan_sorted[q] = ((unsigned long long)key << 32) | (unsigned)j;
     }
+    int n_pow2 = 1;
+    while (n_pow2 < K) n_pow2 <<= 1;
+    for (int q = K + tid; q < n_pow2; q += kPlanThreads) plan_sorted[q] = ~0ull;      // padding sorts to the end
     __syncthreads();
-    // ---- (c) rank sort (keys are unique for a valid mode list; ties fall back to list position)
-    for (int q = tid; q < K; q += kPlanThreads) {
-        unsigned key = ukey[q];
-        int rank = 0;
-        for (int p = 0; p < K; ++p) { unsigned kp = ukey[p]; rank += (kp < key || (kp == key && p < q)) ? 1 : 0; }
-        skey[rank] = key; sj[rank] = uj[q];
+    // ---- (c) bitonic sort in shared memory (keys are unique for a valid mode list; duplicates order by mode index)
+    for (int size = 2; size <= n_pow2; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int q = tid; q < (n_pow2 >> 1); q += kPlanThreads) {
+                const int lo = ((q & ~(stride - 1)) << 1) | (q & (stride - 1)), hi = lo | stride;
+                const unsigned long long a = plan_sorted[lo], b = plan_sorted[hi];
+                const bool up = (lo & size) == 0;
+                if ((a > b) == up) { plan_sorted[lo] = b; plan_sorted[hi] = a; }
+            }
+            __syncthreads();
+        }
     }
-    __syncthreads();
     // ---- (d) pairs: chunked scan of "new (m, n)" flags; descriptors; per-mode fold constants
     if (tid == 0) carry_s = 0;
     __syncthreads();
@@ -199,7 +202,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         bool new_run = false, new_sub = false, new_grp = false;
         unsigned key = 0, prev = 0;
         if (r < K) {
-            key = skey[r]; prev = r ? skey[r - 1] : 0u;
+            key = (unsigned)(plan_sorted[r] >> 32); prev = r ? (unsigned)(plan_sorted[r - 1] >> 32) : 0u;
             new_run = r == 0 || key_m(key) != key_m(prev);
             new_sub = new_run || key_dir(key) != key_dir(prev);
             new_grp = new_sub || key_absn(key) != key_absn(prev);
@@ -207,7 +210,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         int total, incl = plan_block_scan(new_grp ? 1 : 0, warp_sums, &total);
         int carry = carry_s;
         if (r < K) {
-            int j = sj[r];
+            int j = (int)(unsigned)(plan_sorted[r] & 0xffffffffull);
             oj[r] = j;
             if (new_grp) {
                 int g = carry + incl - 1;
@@ -514,7 +517,12 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     }   // persistent tile loop
 }
 
-size_t plan_smem_bytes(int n_modes) { return (size_t)n_modes * 16 + 16; }
+size_t plan_smem_bytes(int n_modes)
+{
+    size_t p = 1;
+    while (p < (size_t)n_modes) p <<= 1;
+    return p * 8;
+}
 
 }  // namespace
 
