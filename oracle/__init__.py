@@ -10,6 +10,10 @@ Functions (each follows the passage cited in few_oracle.c):
   ylm(l, m, theta, phi)       O2
   select_modes(...)           O3
   sum_waveform(...)           O4                  PAPER.md:155-159, Eq. (9), Eq. (10)
+  frame(qS, phiS, qK, phiK)   O5                  PAPER.md:69-102 Eq. (4)-(8)
+  frame_apply(h, factor)      O5
+  inner(d, h, dt)             O6                  PAPER.md:283-296 Eq. (15)-(17), PSD = 1
+  sum_direct(...)             O7
   waveform(workload)          chain O2 -> O3 -> O1 -> O4 in the paper's pipeline order
 """
 from __future__ import annotations
@@ -55,6 +59,10 @@ def lib():
         L.oracle_sum_waveform.argtypes = [_dp, _dp, C.c_void_p, _ip, _ip, _ip, _ip, C.c_int, _dp, _dp, C.c_double,
                                           C.c_int, C.c_double, C.c_double, C.c_longlong, C.c_longlong, C.c_int,
                                           C.c_int, _dp]
+        L.oracle_frame.argtypes = [C.c_double] * 5 + [_dp]
+        L.oracle_frame_apply.argtypes = [_dp, C.c_longlong, _dp, _dp]
+        L.oracle_inner.argtypes = [_dp, _dp, C.c_longlong, C.c_double, _dp]
+        L.oracle_sum_direct.argtypes = [_dp, _dp, _ip, _ip, _ip, _dp, _dp, C.c_double, C.c_int, C.c_longlong, C.c_int, _dp]
         L.oracle_num_threads.restype = C.c_int
         L.oracle_set_threads.argtypes = [C.c_int]
         _lib = L
@@ -139,6 +147,50 @@ def sum_waveform(t, coef_amp, coef_phase_ext, l, m, n, keep_idx, ylm_plus, ylm_m
                                    _ptr(k, _ip), 0 if k is None else len(k), _ptr(yp), _ptr(ym), float(scale),
                                    int(bool(fold)), float(t0), float(dt), int(i0), int(n_samples), n_t, n_modes, _ptr(h))
     if rc: raise ValueError(_ERR[rc])
+    return h.view(np.complex128)[:, 0]
+
+
+def frame(qS: float, phiS: float, qK: float, phiK: float, mu_over_dl: float = 1.0):
+    """O5.  -> (theta_src, phi_src, factor) with factor = -(mu/d_L) exp(+2 i psi) (complex)."""
+    out = np.empty(4)
+    lib().oracle_frame(float(qS), float(phiS), float(qK), float(phiK), float(mu_over_dl), _ptr(out))
+    return float(out[0]), float(out[1]), complex(out[2], out[3])
+
+
+def frame_apply(h, factor: complex):
+    """O5.  h complex128 [n] -> factor * h."""
+    hin = np.ascontiguousarray(h, np.complex128).reshape(-1)
+    out = np.empty_like(hin)
+    f = np.array([factor.real, factor.imag])
+    lib().oracle_frame_apply(_ptr(hin.view(np.float64)), hin.shape[0], _ptr(f), _ptr(out.view(np.float64)))
+    return out.reshape(np.shape(h))
+
+
+def inner(d, h, dt: float):
+    """O6.  -> (<d|h>, imaginary companion, <h|h>) for PSD = 1."""
+    d = np.ascontiguousarray(d, np.complex128).reshape(-1); h = np.ascontiguousarray(h, np.complex128).reshape(-1)
+    assert d.shape == h.shape
+    out = np.empty(3)
+    lib().oracle_inner(_ptr(d.view(np.float64)), _ptr(h.view(np.float64)), d.shape[0], float(dt), _ptr(out))
+    return float(out[0]), float(out[1]), float(out[2])
+
+
+def overlap(a, b, dt: float = 1.0) -> float:
+    """Eq. (17) with O6's inner product."""
+    ab = inner(a, b, dt)[0]
+    return ab / np.sqrt(inner(a, a, dt)[0] * inner(b, b, dt)[0])
+
+
+def sum_direct(amp, phase, l, m, n, ylm_plus, ylm_minus, scale: float = 1.0, fold: bool = True):
+    """O7.  amp [N, K] complex128, phase [N, 2] float64 -> h complex128 [N]."""
+    a = _c2d(amp); N, K = amp.shape
+    ph = np.ascontiguousarray(phase, np.float64); assert ph.shape == (N, 2)
+    l, m, n = (np.ascontiguousarray(x, np.int32) for x in (l, m, n))
+    yp = _c2d(ylm_plus)
+    ym = _c2d(ylm_minus if ylm_minus is not None else np.zeros(K, np.complex128))
+    h = np.empty((N, 2), np.float64)
+    lib().oracle_sum_direct(_ptr(a), _ptr(ph), _ptr(l, _ip), _ptr(m, _ip), _ptr(n, _ip), _ptr(yp), _ptr(ym), float(scale),
+                            int(bool(fold)), N, K, _ptr(h))
     return h.view(np.complex128)[:, 0]
 
 

@@ -16,6 +16,11 @@
  *   oracle_select_modes      : P8 brute-force prefix enumeration on tiny inputs + invariants.
  *   oracle_sum_waveform      : P4 closed form, P5 m -> -m fold vs explicit negative-m list, P7 mpmath brute
  *                              force (config 0), P9 real-linearity, P10 time translation / batch independence.
+ *   oracle_frame / _apply    : P12 wave-frame geometry rebuilt from Eq. (4)-(7) with cross products, spin-2 tensor
+ *                              projection, norm preservation, invariance under a common rotation about z.
+ *   oracle_inner             : P13 Parseval against the frequency-domain form of Eq. (16) (numpy FFT), overlap(a,a)=1.
+ *   oracle_sum_direct        : P14 closed form, mpmath brute force, agreement with the interpolated sum on inputs
+ *                              that are exactly cubic per segment.
  * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC few_oracle.c -o libfew_oracle.so -lm
@@ -296,6 +301,118 @@ int oracle_sum_waveform(const double *t, const double *coef_amp, const ext *coef
                     hr += zr * Wr + zi * Wi;                             /* Y- conj(W) */
                     hi += -zr * Wi + zi * Wr;
                 }
+            }
+        }
+        h[2 * i] = (double)(hr * scale);
+        h[2 * i + 1] = (double)(hi * scale);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O5 -- detector (solar-system-barycentre) frame, sec. II A, Eq. (4)-(8), and the mu/d_L
+ * prefactor of Eq. (10).  NEXT-1 of SURVEY.md section 8(f).
+ *  Eq. (4)  R = (sin qS cos phiS, sin qS sin phiS, cos qS)           line of sight to the source
+ *  Eq. (5)  S = (sin qK cos phiK, sin qK sin phiK, cos qK)           MBH spin direction
+ *  PAPER.md:96  "This convention leads to phi_src = -pi/2 always ... cos theta_src = -R.S"
+ *  PAPER.md:98  "a rotation angle of pi/2 is applied. This rotation is equivalent to a phase shift of pi"
+ *               -> factor e^{i pi} = -1
+ *  PAPER.md:100 "The rotation to the solar system baricenter frame is twice the polarization angle, psi"
+ *  Eq. (8)  prints psi = N/D with N = cos qS sin qK cos(phiS-phiK) - sin qS cos qK, D = sin qK sin(phiS-phiK):
+ *           an angle equated to a ratio; the kludge construction the paper follows defines psi through its
+ *           tangent, tan psi = N/D (R22).  psi = atan2(N, D); only 2 psi mod 2 pi enters, so the
+ *           branch of the arctangent is immaterial.  N = D = 0 (S parallel to R, wave frame undefined): psi = 0.
+ *  h_+^SSB - i h_x^SSB = e^{+2 i psi} (h_+ - i h_x): what the spin-2 combination h_+ - i h_x does when the polarisation
+ *  basis is rotated by psi about the propagation direction z_w = -R, from the wave frame (x_w, y_w) of Eq. (6) to the
+ *  right-handed pair (e_theta, -e_phi) at the sky position; Eq. (8)'s psi is exactly that angle (x_w = cos psi e_theta +
+ *  sin psi e_phi), pinned geometrically in P12 (R22).
+ * out[0] = theta_src, out[1] = phi_src, (out[2], out[3]) = factor = -(mu/d_L) e^{+2 i psi}.
+ * All in extended precision, rounded once.
+ * ------------------------------------------------------------------------------------------------ */
+int oracle_frame(double qS, double phiS, double qK, double phiK, double mu_over_dl, double out[4])
+{
+    ext R[3] = { sinl((ext)qS) * cosl((ext)phiS), sinl((ext)qS) * sinl((ext)phiS), cosl((ext)qS) };
+    ext S[3] = { sinl((ext)qK) * cosl((ext)phiK), sinl((ext)qK) * sinl((ext)phiK), cosl((ext)qK) };
+    ext c = -(R[0] * S[0] + R[1] * S[1] + R[2] * S[2]);
+    if (c > 1) c = 1;
+    if (c < -1) c = -1;
+    ext N = cosl((ext)qS) * sinl((ext)qK) * cosl((ext)phiS - (ext)phiK) - sinl((ext)qS) * cosl((ext)qK);
+    ext D = sinl((ext)qK) * sinl((ext)phiS - (ext)phiK);
+    ext psi = (N == 0 && D == 0) ? 0 : atan2l(N, D);
+    out[0] = (double)acosl(c);
+    out[1] = (double)(-acosl(-1.0L) / 2);
+    out[2] = (double)(-(ext)mu_over_dl * cosl(2 * psi));
+    out[3] = (double)(-(ext)mu_over_dl * sinl(2 * psi));
+    return 0;
+}
+
+/* h_out = factor * h_in (complex), extended-precision products, rounded once. */
+int oracle_frame_apply(const double *h_in, long long n, const double factor[2], double *h_out)
+{
+    for (long long i = 0; i < n; ++i) {
+        ext a = h_in[2 * i], b = h_in[2 * i + 1], fr = factor[0], fi = factor[1];
+        h_out[2 * i] = (double)(fr * a - fi * b);
+        h_out[2 * i + 1] = (double)(fr * b + fi * a);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O6 -- inner products with the PSD set to 1 (Eq. (15)-(17); "setting the PSD to 1 for all
+ * frequencies to avoid noise-weighting").  NEXT-2 of SURVEY.md section 8(f).
+ * Eq. (16) <a|b> = 4 Re int_0^inf conj(a~) b~ / S_n df.  With S_n = 1 and real a(t), b(t) sampled at dt, Parseval
+ * gives <a|b> = 2 dt sum_i a_i b_i; the two polarisations of h = h_+ - i h_x are summed (R23), so for complex
+ * series  <a|b> = 2 dt Re sum_i conj(a_i) b_i.  The imaginary part of the same sum is returned too (it is what a
+ * phase-maximised overlap needs and costs nothing).
+ * out[0] = <d|h>, out[1] = 2 dt Im sum conj(d_i) h_i, out[2] = <h|h>.  Sums in extended precision, index order.
+ * ------------------------------------------------------------------------------------------------ */
+int oracle_inner(const double *d, const double *h, long long n, double dt, double out[3])
+{
+    ext re = 0, im = 0, hh = 0;
+    for (long long i = 0; i < n; ++i) {
+        ext dr = d[2 * i], di = d[2 * i + 1], hr = h[2 * i], hi = h[2 * i + 1];
+        re += dr * hr + di * hi;
+        im += dr * hi - di * hr;
+        hh += hr * hr + hi * hi;
+    }
+    out[0] = (double)(2 * (ext)dt * re);
+    out[1] = (double)(2 * (ext)dt * im);
+    out[2] = (double)(2 * (ext)dt * hh);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O7 -- direct summation (sec. III C: "performs a direct summation with amplitude and trajectory
+ * information at the array density provided"; "combining the phase and amplitude information at
+ * each time point in the data stream without interpolating any of these quantities").  NEXT-3 of SURVEY.md 8(f).
+ *  h_i = scale * sum_j [ Y+_j W_ij + (m_j > 0) (-1)^{l_j} Y-_j conj(W_ij) ],
+ *  W_ij = A_ij exp(-i (m_j Phi_phi,i + n_j Phi_r,i))      (Eq. (10) with the Eq. (9) fold)
+ * amp[N][K][2] (modes fastest: the amplitude module's [n_t, n_modes] layout, at dense n_t = N);
+ * phase[N][2] = (Phi_phi, Phi_r) in FP64 as given; the angle m Phi_phi + n Phi_r is formed and reduced in
+ * extended precision (exact for the FP64 inputs to 2^-64 relative); accumulation over j in extended precision.
+ * ------------------------------------------------------------------------------------------------ */
+int oracle_sum_direct(const double *amp, const double *phase, const int *l, const int *m, const int *n,
+                      const double *ylm_plus, const double *ylm_minus, double scale, int fold,
+                      long long N, int K, double *h)
+{
+    long long i;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < N; ++i) {
+        ext hr = 0, hi = 0;
+        ext Pphi = phase[2 * i], Pr = phase[2 * i + 1];
+        const double *a = amp + (size_t)i * K * 2;
+        for (int j = 0; j < K; ++j) {
+            ext th = (ext)m[j] * Pphi + (ext)n[j] * Pr;
+            ext Er = cosl(th), Ei = -sinl(th);
+            ext Wr = (ext)a[2 * j] * Er - (ext)a[2 * j + 1] * Ei, Wi = (ext)a[2 * j] * Ei + (ext)a[2 * j + 1] * Er;
+            ext yr = ylm_plus[2 * j], yi = ylm_plus[2 * j + 1];
+            hr += yr * Wr - yi * Wi;
+            hi += yr * Wi + yi * Wr;
+            if (fold && m[j] > 0) {
+                ext sg = (l[j] % 2) ? -1.0L : 1.0L;
+                ext zr = sg * ylm_minus[2 * j], zi = sg * ylm_minus[2 * j + 1];
+                hr += zr * Wr + zi * Wi;
+                hi += -zr * Wi + zi * Wr;
             }
         }
         h[2 * i] = (double)(hr * scale);

@@ -225,10 +225,11 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
         // g(0) = total >= thr; B = the largest x with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
         long long B = 0;
         for (int b = 10; b >= 0; --b) {
-            const long long cand = (B | (1ll << b)) << 52;
+            const int cand_hi = (int)((B | (1ll << b)) << 20);   // the bucket lives in the key's high word: one 32-bit compare
             double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
 #pragma unroll
-            for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] >= cand ? __longlong_as_double(key[i]) : 0.0;
+            for (int i = 0; i < EPT; ++i)
+                if ((int)(key[i] >> 32) >= cand_hi) g4[i & 3] += __longlong_as_double(key[i]);
             const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
             if (!(g < thr)) B |= 1ll << b;
         }
