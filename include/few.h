@@ -126,6 +126,40 @@ int few_sum_waveform(few_ctx* ctx, const double* t, const double* coef_amp, cons
                      double t0, double dt, long long n_samples, double* h,
                      int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Extended form of S3.  Adds
+ *   factor[n_src][2] or NULL: a complex per-source prefactor (few_frame_constants: the detector-frame transformation of
+ *     Eq. (4)-(8) and mu/d_L).  h is linear in the harmonic constants, so the factor is folded into them before the sample
+ *     loop and the transformation costs nothing per sample.  Multiplies with `scale` if both are given.
+ *   d[n_src][n_samples][2] or NULL, inner[n_src][3] or NULL: with inner != NULL the kernel also reduces, per source, the
+ *     PSD = 1 inner products of PAPER.md:283-296 Eq. (15)-(17) (Parseval, both polarisations, R23):
+ *       inner[s][0] = <d|h> = 2 dt Re sum_i conj(d_i) h_i,  inner[s][1] = 2 dt Im sum_i conj(d_i) h_i,  inner[s][2] = <h|h>
+ *     ([0], [1] are 0 when d == NULL).  h may then be NULL: nothing but three doubles per source is written, which is what a
+ *     likelihood evaluation consumes (NEXT-2).  The reduction order is fixed: results are bit-reproducible.
+ * Everything else as few_sum_waveform (same workspace query). */
+int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
+                        const int* l, const int* m, const int* n, const int* keep_idx, const int* n_keep,
+                        const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                        double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                        int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- NEXT-1: detector (solar-system-barycentre) frame, sec. II A.
+ * few_frame_constants: sky[n_src][4] = (theta_S, phi_S, theta_K, phi_K) (sky position, MBH spin direction; Eq. (4), (5));
+ * mu_over_dl[n_src] or NULL (= 1) -> theta[n_src] with cos(theta) = -R.S and phi[n_src] = -pi/2, the viewing
+ * angles the harmonics take, and factor[n_src][2] = -(mu/d_L) e^{2 i psi}, tan(psi) given by Eq. (8) (the minus sign is the
+ * "phase shift of pi" of PAPER.md:98; readings: DESIGN.md R22).
+ * few_frame_rotate: h_out[n_src][n_samples][2] = factor[src] * h_in (may alias): the transformation as a separate pass over an
+ * existing source-frame waveform. */
+int few_frame_constants(few_ctx* ctx, const double* sky, const double* mu_over_dl, int n_src,
+                        double* theta, double* phi, double* factor, void* stream);
+int few_frame_rotate(few_ctx* ctx, const double* h_in, const double* factor, int n_src, long long n_samples,
+                     double* h_out, void* stream);
+
+/* ---- NEXT-2: PSD = 1 inner products of two stored series: inner[n_src][3] as in few_sum_waveform_ex,
+ * d, h [n_src][n_samples][2].  Two passes (per-chunk partials in the workspace, then a fixed-order sum): bit-reproducible. */
+size_t few_inner_products_workspace(int n_src, long long n_samples);
+int few_inner_products(few_ctx* ctx, const double* d, const double* h, int n_src, long long n_samples, double dt,
+                       double* inner, void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- Whole path on device buffers: S0 -> S2 -> S1 -> S3, no host synchronisation.
  * t[n_src][n_t], phase[n_src][n_t][2] (Phi_phi, Phi_r), amp[n_src][n_t][n_modes][2], theta/phi[n_src], l/m/n[n_modes].
  * Outputs: h[n_src][n_samples][2]; optional keep_idx[n_src][n_modes], n_keep[n_src] (NULL: kept inside the workspace). */
@@ -134,6 +168,16 @@ int few_waveform(few_ctx* ctx, const double* t, const double* phase, const doubl
                  const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
                  double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
                  double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Whole path in the detector frame: few_frame_constants -> S0 -> S2 -> S1 -> S3 with the frame factor folded in, and
+ * optionally the fused inner products against a resident data stream d (h may be NULL when inner is given).
+ * sky[n_src][4], mu_over_dl[n_src] or NULL as in few_frame_constants; d, inner as in few_sum_waveform_ex.  Same workspace
+ * query as few_waveform. */
+int few_waveform_ssb(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                     const int* l, const int* m, const int* n, const double* sky, const double* mu_over_dl,
+                     double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                     double* h, const double* d, double* inner, int* keep_idx, int* n_keep,
+                     void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): copies inputs host->device
  * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform and delivers h

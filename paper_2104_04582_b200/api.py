@@ -20,7 +20,8 @@ FEW_OK = 0
 SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_version", "few_device_status", "few_ylm",
            "few_ylm_modes", "few_spline_fit_workspace", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
-           "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms"]
+           "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
+           "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb"]
 
 
 class FewError(RuntimeError):
@@ -55,6 +56,12 @@ def _load() -> C.CDLL:
         "few_waveform_workspace": (sz, [i, i, i, ll]),
         "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
+        "few_sum_waveform_ex": (i, [vp] * 13 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
+        "few_frame_constants": (i, [vp, vp, vp, i, vp, vp, vp, vp]),
+        "few_frame_rotate": (i, [vp, vp, vp, i, ll, vp, vp]),
+        "few_inner_products_workspace": (sz, [i, ll]),
+        "few_inner_products": (i, [vp, vp, vp, i, ll, d, vp, vp, sz, vp]),
+        "few_waveform_ssb": (i, [vp] * 9 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, vp, vp, sz, vp]),
         "few_fp64_peak_probe": (i, [vp, i, i, i, vp, vp]),
         "few_profile_enable": (i, [vp, i]),
         "few_profile_sum_ms": (i, [vp, C.POINTER(C.c_float)]),
@@ -182,6 +189,73 @@ def few_sum_waveform(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, ylm_
                                _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale), float(t0), float(dt),
                                int(n_samples), _p(h), n_src, n_t, n_modes, _p(ws), ws.numel(), _stream()), "few_sum_waveform")
     return h
+
+
+def few_sum_waveform_ex(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, ylm_plus, ylm_minus, t0: float, dt: float,
+                        n_samples: int, scale=None, factor=None, d=None, want_inner: bool = False, want_h: bool = True,
+                        out=None, workspace=None):
+    """few_sum_waveform with the complex per-source `factor` [n_src] c128 and the fused PSD = 1 inner products against
+    d [n_src, n_samples] c128.  -> (h or None, inner [n_src, 3] f64 or None)."""
+    n_src, n_t = t.shape
+    n_modes = l.shape[0]
+    h = None
+    if want_h:
+        h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
+    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    ws = workspace if workspace is not None else _ws(need, t.device)
+    _chk(_lib.few_sum_waveform_ex(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
+                                  _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32), _p(keep_idx), _p(n_keep),
+                                  _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale), _p(factor),
+                                  float(t0), float(dt), int(n_samples), _p(h), _p(d), _p(inner), n_src, n_t, n_modes, _p(ws),
+                                  ws.numel(), _stream()), "few_sum_waveform_ex")
+    return h, inner
+
+
+def few_frame_constants(sky, mu_over_dl=None):
+    """sky [n_src, 4] f64 = (theta_S, phi_S, theta_K, phi_K) -> (theta [n_src], phi [n_src], factor [n_src] c128)."""
+    n_src = sky.shape[0]
+    theta = torch.empty(n_src, dtype=torch.float64, device=sky.device)
+    phi = torch.empty_like(theta)
+    factor = torch.empty(n_src, dtype=torch.complex128, device=sky.device)
+    _chk(_lib.few_frame_constants(context(), _p(sky, torch.float64), _p(mu_over_dl), n_src, _p(theta), _p(phi), _p(factor), _stream()),
+         "few_frame_constants")
+    return theta, phi, factor
+
+
+def few_frame_rotate(h, factor, out=None):
+    """h [n_src, n_samples] c128, factor [n_src] c128 -> factor[:, None] * h (a separate pass; `out` may be h)."""
+    n_src, n_samples = h.shape
+    o = out if out is not None else torch.empty_like(h)
+    _chk(_lib.few_frame_rotate(context(), _p(h, torch.complex128), _p(factor, torch.complex128), n_src, int(n_samples), _p(o),
+                               _stream()), "few_frame_rotate")
+    return o
+
+
+def few_inner_products(d, h, dt: float, workspace=None):
+    """d, h [n_src, n_samples] c128 -> inner [n_src, 3] f64 = (<d|h>, imaginary companion, <h|h>), PSD = 1."""
+    n_src, n_samples = h.shape
+    inner = torch.empty((n_src, 3), dtype=torch.float64, device=h.device)
+    ws = workspace if workspace is not None else _ws(_lib.few_inner_products_workspace(n_src, int(n_samples)), h.device)
+    _chk(_lib.few_inner_products(context(), _p(d, torch.complex128), _p(h, torch.complex128), n_src, int(n_samples), float(dt),
+                                 _p(inner), _p(ws), ws.numel(), _stream()), "few_inner_products")
+    return inner
+
+
+def few_waveform_ssb(t, phase, amp, l, m, n, sky, eps: float, t0: float, dt: float, n_samples: int, mu_over_dl=None, d=None,
+                     want_inner: bool = False, want_h: bool = True, out=None, keep_idx=None, n_keep=None, workspace=None):
+    """Whole path in the detector frame.  -> (h or None, inner or None)."""
+    n_src, n_t, n_modes = amp.shape
+    h = None
+    if want_h:
+        h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
+    ws = workspace if workspace is not None else _ws(few_waveform_workspace(n_src, n_t, n_modes, n_samples), t.device)
+    _chk(_lib.few_waveform_ssb(context(), _p(t, torch.float64), _p(phase, torch.float64), _p(amp, torch.complex128),
+                               _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32), _p(sky, torch.float64), _p(mu_over_dl),
+                               float(eps), float(t0), float(dt), int(n_samples), n_src, n_t, n_modes, _p(h), _p(d), _p(inner),
+                               _p(keep_idx), _p(n_keep), _p(ws), ws.numel(), _stream()), "few_waveform_ssb")
+    return h, inner
 
 
 def few_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int) -> int:

@@ -120,6 +120,7 @@ extern "C" int few_device_status(few_ctx* ctx, int* bits_out, void* stream)
 namespace {
 struct wf_layout {
     double *ylm_plus, *ylm_minus, *coef_amp, *coef_phase;
+    double *theta_src, *phi_src, *factor;      // few_waveform_ssb: source-frame viewing angles and the frame factor
     int *keep_idx, *n_keep;
     void *sel_ws, *sum_ws, *spl_ws;
     size_t sel_bytes, sum_bytes, spl_bytes;
@@ -135,6 +136,9 @@ wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_sample
     L.coef_phase = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 2 * 2);
     L.keep_idx = c.take<int>((size_t)n_src * n_modes);
     L.n_keep = c.take<int>(n_src);
+    L.theta_src = c.take<double>(n_src);
+    L.phi_src = c.take<double>(n_src);
+    L.factor = c.take<double>((size_t)n_src * 2);
     L.sel_bytes = few_select_modes_workspace(n_src, n_t, n_modes);
     L.sum_bytes = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples);
     L.spl_bytes = few_spline_fit_workspace(n_src, n_t);
@@ -154,12 +158,14 @@ extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long l
     return bytes;
 }
 
-extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, const double* amp,
-                            const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
-                            double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
-                            double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
+namespace {
+// theta/phi: source-frame viewing angles, or (sky != NULL) computed from the detector-frame angles by few_frame_constants.
+int waveform_impl(few_ctx* ctx, const double* t, const double* phase, const double* amp, const int* l, const int* m, const int* n,
+                  const double* theta, const double* phi, const double* sky, const double* scale, double eps, double t0, double dt,
+                  long long n_samples, int n_src, int n_t, int n_modes, double* h, const double* d, double* inner, int* keep_idx,
+                  int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
 {
-    FEW_REQUIRE(ctx && t && phase && amp && l && m && n && theta && phi, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(ctx && t && phase && amp && l && m && n && ((theta && phi) || sky), FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
     FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
@@ -179,12 +185,41 @@ extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, 
     if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, ctx->side[1]))) return rc;
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[0], ctx->side[0]));
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[1], ctx->side[1]));
+    const double* factor = nullptr;
+    if (sky) {      // Eq. (4)-(8): viewing angles for the harmonics, one complex constant per source for the summation
+        if ((rc = few_frame_constants(ctx, sky, scale, n_src, L.theta_src, L.phi_src, L.factor, stream))) return rc;
+        theta = L.theta_src; phi = L.phi_src; factor = L.factor; scale = nullptr;
+    }
     if ((rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream))) return rc;
     if ((rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream))) return rc;
     FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[0], 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[1], 0));
-    return few_sum_waveform(ctx, t, L.coef_amp, L.coef_phase, l, m, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, t0, dt, n_samples, h,
-                            n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
+    return few_sum_waveform_ex(ctx, t, L.coef_amp, L.coef_phase, l, m, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, factor, t0, dt,
+                               n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
+}
+}  // namespace
+
+extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                            const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
+                            double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                            double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(theta && phi, FEW_ERR_INVALID_ARG, "theta or phi is NULL");
+    FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
+    return waveform_impl(ctx, t, phase, amp, l, m, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
+                         nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
+}
+
+extern "C" int few_waveform_ssb(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                                const int* l, const int* m, const int* n, const double* sky, const double* mu_over_dl,
+                                double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                                double* h, const double* d, double* inner, int* keep_idx, int* n_keep,
+                                void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(sky != nullptr, FEW_ERR_INVALID_ARG, "sky is NULL");
+    FEW_REQUIRE(n_samples == 0 || h || inner, FEW_ERR_INVALID_ARG, "h and inner are both NULL");
+    return waveform_impl(ctx, t, phase, amp, l, m, n, nullptr, nullptr, sky, mu_over_dl, eps, t0, dt, n_samples, n_src, n_t, n_modes,
+                         h, d, inner, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 
 extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,

@@ -57,12 +57,16 @@ struct sum_layout {
     int* order_j;        // [n_src][n_modes]   mode index of sorted position r
     double* yfold;       // [n_src][n_modes][4] scale * (Y+ re, Y+ im, Ybar re, Ybar im) of sorted position r
     double* pack;        // [n_src][n_t - 1][max_stages][kStageBytes / 8]
+    double* partial;     // [n_src][max_tiles][4]  per-tile sums of conj(d) h (re, im) and |h|^2 (fused inner products)
     int max_stages;
+    int max_tiles;
 };
 
 __host__ __device__ inline int stages_for(int n_pairs) { return (n_pairs + kStagePairs - 1) / kStagePairs; }
 
-sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, size_t* bytes = nullptr)
+__host__ inline long long sum_max_tiles(long long n_samples, int n_t) { return (n_samples + kTile - 1) / kTile + n_t + 1; }
+
+sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, size_t* bytes = nullptr)
 {
     few_carver c(ws);
     sum_layout L;
@@ -76,6 +80,9 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, size_t* bytes = 
     L.order_j = c.take<int>((size_t)n_src * n_modes);
     L.yfold = c.take<double>((size_t)n_src * n_modes * 4);
     L.pack = c.take<double>((size_t)n_src * (n_t - 1) * L.max_stages * (kStageBytes / 8));
+    const long long mt = sum_max_tiles(n_samples, n_t);
+    L.max_tiles = (int)(mt < 2147483647LL ? mt : 2147483647LL);
+    L.partial = c.take<double>((size_t)n_src * (size_t)mt * 4);
     if (bytes) *bytes = c.off;
     return L;
 }
@@ -126,8 +133,8 @@ __global__ void __launch_bounds__(kPlanThreads, 1)
 few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l, const int* __restrict__ m,
                     const int* __restrict__ n, const int* __restrict__ keep_idx, const int* __restrict__ n_keep,
                     const double2* __restrict__ ylm_plus, const double2* __restrict__ ylm_minus,
-                    const double* __restrict__ scale, double t0, double dt, long long N, int n_t, int n_modes,
-                    sum_layout L, int* status)
+                    const double* __restrict__ scale, const double2* __restrict__ factor, double t0, double dt, long long N,
+                    int n_t, int n_modes, sum_layout L, int* status)
 {
     extern __shared__ unsigned long long plan_sorted[];           // [n_pow2] (key << 32 | mode index), sorted ascending
     __shared__ int warp_sums[32];
@@ -196,7 +203,10 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     int* gfirst = L.g_first + (size_t)src * (n_modes + 1);
     int* oj = L.order_j + (size_t)src * n_modes;
     double* yf = L.yfold + (size_t)src * n_modes * 4;
+    // every harmonic constant carries the source's prefactor: the real mu/d_L `scale` of Eq. (10) and the complex detector-frame
+    // `factor` of Eq. (4)-(8) (few_frame_constants); h is linear in (Y+, Ybar), so the frame rotation costs nothing per sample
     const double sc = scale ? scale[src] : 1.0;
+    const double2 fc = factor ? make_double2(sc * factor[src].x, sc * factor[src].y) : make_double2(sc, 0.0);
     for (int base = 0; base < K; base += kPlanThreads) {
         int r = base + tid;
         bool new_run = false, new_sub = false, new_grp = false;
@@ -228,7 +238,8 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
                 double sg = (key_l(key) & 1) ? -1.0 : 1.0;
                 yb = make_double2(sg * ym.x, sg * ym.y);
             }
-            yf[4 * r] = sc * yp.x; yf[4 * r + 1] = sc * yp.y; yf[4 * r + 2] = sc * yb.x; yf[4 * r + 3] = sc * yb.y;
+            yf[4 * r] = fc.x * yp.x - fc.y * yp.y; yf[4 * r + 1] = fc.x * yp.y + fc.y * yp.x;
+            yf[4 * r + 2] = fc.x * yb.x - fc.y * yb.y; yf[4 * r + 3] = fc.x * yb.y + fc.y * yb.x;
         }
         __syncthreads();
         if (tid == 0) carry_s = carry + total;
@@ -365,12 +376,14 @@ __device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, 
 template <int R, int kBlocksPerSm>
 __global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
-               int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all)
+               int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all,
+               int want_inner)
 {
     __shared__ __align__(128) double2 ring[kRing][kStageD2];
     __shared__ __align__(8) unsigned long long full[kRing];
     __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
     __shared__ int tile_s;
+    __shared__ double red_s[3][kSumThreads / 32];
 
     const int tid = threadIdx.x, n_seg = n_t - 1;
     if (tid == 0) {
@@ -399,11 +412,16 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     const int p = lo;
     const long long* B = L.bounds + (size_t)src * (n_t + 2);
     const long long i_begin = B[p] + (long long)(tile - TS[p]) * (R * kSumThreads), i_end = B[p + 1];
-    double2* h = h_all + (size_t)src * N;
+    double2* h = h_all ? h_all + (size_t)src * N : nullptr;
+    const double2* dat = d_all ? d_all + (size_t)src * N : nullptr;
+    double* partial = L.partial + ((size_t)src * max_tiles + tile) * 4;
 
     if (p == 0 || p == n_t) {           // outside [t_0, t_last]: h = 0 (R12)
+        if (h) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) { long long i = i_begin + r * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
+            for (int r = 0; r < R; ++r) { long long i = i_begin + r * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
+        }
+        if (want_inner && tid < 3) partial[tid] = 0.0;
         continue;
     }
     const int k = p - 1;
@@ -503,7 +521,9 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         }
     }
 
-    // ---- h = acc_0 + dx (acc_1 + dx (acc_2 + dx acc_3)), once per sample
+    // ---- h = acc_0 + dx (acc_1 + dx (acc_2 + dx acc_3)), once per sample; optionally the tile's share of the PSD = 1 inner
+    // products <d|h>, <h|h> so that a likelihood evaluation never writes h to HBM
+    double s_re = 0.0, s_im = 0.0, s_hh = 0.0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const long long i = i_begin + r * kSumThreads + tid;
@@ -511,10 +531,58 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
             const double hr = fma(fma(fma(are[3][r], dx, are[2][r]), dx, are[1][r]), dx, are[0][r]);
             const double hi = fma(fma(fma(aim[3][r], dx, aim[2][r]), dx, aim[1][r]), dx, aim[0][r]);
-            __stcs(&h[i], make_double2(hr, hi));
+            if (h) __stcs(&h[i], make_double2(hr, hi));
+            if (want_inner) {
+                if (dat) {
+                    const double2 dv = __ldcs(&dat[i]);
+                    s_re = fma(dv.x, hr, fma(dv.y, hi, s_re));      // Re conj(d) h
+                    s_im = fma(dv.x, hi, fma(-dv.y, hr, s_im));     // Im conj(d) h
+                }
+                s_hh = fma(hr, hr, fma(hi, hi, s_hh));
+            }
+        }
+    }
+    if (want_inner) {                   // fixed tree: lanes by butterfly, then the warps in order -> the same bits every run
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            s_re += __shfl_xor_sync(0xffffffffu, s_re, o);
+            s_im += __shfl_xor_sync(0xffffffffu, s_im, o);
+            s_hh += __shfl_xor_sync(0xffffffffu, s_hh, o);
+        }
+        if ((tid & 31) == 0) { red_s[0][tid >> 5] = s_re; red_s[1][tid >> 5] = s_im; red_s[2][tid >> 5] = s_hh; }
+        __syncthreads();
+        if (tid < 3) {
+            double v = 0.0;
+#pragma unroll
+            for (int w = 0; w < kSumThreads / 32; ++w) v += red_s[tid][w];
+            partial[tid] = v;
         }
     }
     }   // persistent tile loop
+}
+
+// inner[src] = 2 dt * (sum over the source's tiles of the per-tile partials): Eq. (16) with S_n = 1 by Parseval.  One block per
+// source; thread q adds tiles q, q + 256, ... in order, then a fixed tree: deterministic.
+constexpr int kInnerThreads = 256;
+__global__ void __launch_bounds__(kInnerThreads)
+few_sum_inner_kernel(sum_layout L, int n_t, int max_tiles, double dt, double* __restrict__ inner)
+{
+    __shared__ double red[3][kInnerThreads / 32];
+    const int src = blockIdx.x, tid = threadIdx.x;
+    const int n_tiles = L.tile_start[(size_t)src * (n_t + 2) + n_t + 1];
+    const double* P = L.partial + (size_t)src * max_tiles * 4;
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int q = tid; q < n_tiles; q += kInnerThreads) { a += P[4 * (size_t)q]; b += P[4 * (size_t)q + 1]; c += P[4 * (size_t)q + 2]; }
+    for (int o = 16; o; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); c += __shfl_xor_sync(0xffffffffu, c, o);
+    }
+    if ((tid & 31) == 0) { red[0][tid >> 5] = a; red[1][tid >> 5] = b; red[2][tid >> 5] = c; }
+    __syncthreads();
+    if (tid < 3) {
+        double v = 0.0;
+        for (int w = 0; w < kInnerThreads / 32; ++w) v += red[tid][w];
+        inner[(size_t)src * 3 + tid] = 2.0 * dt * v;
+    }
 }
 
 size_t plan_smem_bytes(int n_modes)
@@ -528,11 +596,60 @@ size_t plan_smem_bytes(int n_modes)
 
 extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
 {
-    (void)n_samples;
-    if (n_src <= 0 || n_t < 2 || n_modes <= 0) return 0;
+    if (n_src <= 0 || n_t < 2 || n_modes <= 0 || n_samples < 0) return 0;
     size_t bytes = 0;
-    sum_carve(nullptr, n_src, n_t, n_modes, &bytes);
+    sum_carve(nullptr, n_src, n_t, n_modes, n_samples, &bytes);
     return bytes;
+}
+
+extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
+                                   const int* l, const int* m, const int* n, const int* keep_idx, const int* n_keep,
+                                   const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                                   double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                                   int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(ctx && t && coef_amp && coef_phase_dd && l && m && n && ylm_plus && ylm_minus, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE((keep_idx == nullptr) == (n_keep == nullptr), FEW_ERR_INVALID_ARG, "keep_idx and n_keep must both be NULL or both be set");
+    FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
+    FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
+    FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
+    FEW_REQUIRE(n_src <= 65535 && n_t <= 65535, FEW_ERR_LIMIT, "n_src or n_t > 65535");
+    FEW_REQUIRE(d == nullptr || inner != nullptr, FEW_ERR_INVALID_ARG, "d given but inner is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_samples == 0) {
+        if (inner) FEW_CUDA_CHECK(cudaMemsetAsync(inner, 0, (size_t)n_src * 3 * sizeof(double), st));
+        return FEW_OK;
+    }
+    FEW_REQUIRE(h != nullptr || inner != nullptr, FEW_ERR_INVALID_ARG, "h and inner are both NULL");
+    FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
+                    workspace_bytes >= few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples),
+                FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
+    size_t psm = plan_smem_bytes(n_modes);
+    FEW_REQUIRE(psm <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "n_modes too large for the plan kernel's shared memory");
+    long long max_tiles = sum_max_tiles(n_samples, n_t);
+    FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
+    sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
+
+    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
+    few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, n, keep_idx, n_keep, (const double2*)ylm_plus,
+                                                          (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
+                                                          n_t, n_modes, L, ctx->d_status);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 1024, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
+    FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
+    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
+    few_sum_kernel<kSumR, kSumBlocksPerSm><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
+        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, (const double2*)d,
+        inner ? 1 : 0);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
+    if (inner) {
+        few_sum_inner_kernel<<<n_src, kInnerThreads, 0, st>>>(L, n_t, (int)max_tiles, dt, inner);
+        FEW_CUDA_CHECK(cudaGetLastError());
+    }
+    return FEW_OK;
 }
 
 extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
@@ -541,37 +658,7 @@ extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coe
                                 double t0, double dt, long long n_samples, double* h,
                                 int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
 {
-    FEW_REQUIRE(ctx && t && coef_amp && coef_phase_dd && l && m && n && ylm_plus && ylm_minus, FEW_ERR_INVALID_ARG, "NULL argument");
-    FEW_REQUIRE((keep_idx == nullptr) == (n_keep == nullptr), FEW_ERR_INVALID_ARG, "keep_idx and n_keep must both be NULL or both be set");
-    FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
-    FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
-    FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
-    FEW_REQUIRE(n_src <= 65535 && n_t <= 65535, FEW_ERR_LIMIT, "n_src or n_t > 65535");
-    if (n_samples == 0) return FEW_OK;
-    FEW_REQUIRE(h != nullptr, FEW_ERR_INVALID_ARG, "h is NULL");
-    FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
-                    workspace_bytes >= few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples),
-                FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
-    size_t psm = plan_smem_bytes(n_modes);
-    FEW_REQUIRE(psm <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "n_modes too large for the plan kernel's shared memory");
-    long long max_tiles = (n_samples + kTile - 1) / kTile + n_t + 1;
-    FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
-    cudaStream_t st = (cudaStream_t)stream;
-    sum_layout L = sum_carve(workspace, n_src, n_t, n_modes);
-
-    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-    few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, n, keep_idx, n_keep, (const double2*)ylm_plus,
-                                                          (const double2*)ylm_minus, scale, t0, dt, n_samples, n_t, n_modes, L,
-                                                          ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 1024, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
-    FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
-    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
-    few_sum_kernel<kSumR, kSumBlocksPerSm><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
-        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
-    return FEW_OK;
+    FEW_REQUIRE(n_samples == 0 || h != nullptr, FEW_ERR_INVALID_ARG, "h is NULL");
+    return few_sum_waveform_ex(ctx, t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, ylm_plus, ylm_minus, scale, nullptr,
+                               t0, dt, n_samples, h, nullptr, nullptr, n_src, n_t, n_modes, workspace, workspace_bytes, stream);
 }

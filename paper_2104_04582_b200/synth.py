@@ -197,3 +197,58 @@ def random_problem(seed: int, *, n_src=1, n_t=12, n_modes=10, l_max=5, n_max=3, 
         ts.append(g), phs.append(ph), amps.append(a)
     return Workload(f"random{seed}", np.stack(ts), np.stack(phs), np.stack(amps), l, m, n,
                     rng.uniform(0.2, 2.9, n_src), rng.uniform(0, 6.28, n_src), 0.0, T / n_samples, n_samples, 0.0)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Inputs of the SURVEY.md section 8(f) rows (still no method arithmetic: angles, a data stream, dense trajectories)
+# ---------------------------------------------------------------------------------------------------------------
+PAPER_ANGLES = (0.54, 5.36, 1.73, 3.20)   # (theta_S, phi_S, theta_K, phi_K): the one set the paper uses for all its tests
+
+
+def sky_angles(n_src: int, seed: int = 0):
+    """Detector-frame angles [n_src, 4] = (theta_S, phi_S, theta_K, phi_K) and mu/d_L [n_src].  Source 0 carries the paper's
+    angles; the others are uniform on the two spheres ("chosen from a random uniform distribution across
+    their domain").  mu/d_L ~ LogUniform(1e-2, 1) in the same arbitrary units as the amplitudes."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 500 + seed))
+    sky = np.empty((n_src, 4))
+    sky[:, 0] = np.arccos(rng.uniform(-1.0, 1.0, n_src)); sky[:, 1] = rng.uniform(0.0, 2.0 * np.pi, n_src)
+    sky[:, 2] = np.arccos(rng.uniform(-1.0, 1.0, n_src)); sky[:, 3] = rng.uniform(0.0, 2.0 * np.pi, n_src)
+    sky[0] = PAPER_ANGLES
+    return sky, 10.0 ** rng.uniform(-2.0, 0.0, n_src)
+
+
+def data_stream(shape, seed: int = 0, sigma: float = 1.0) -> np.ndarray:
+    """White complex Gaussian noise (PSD = 1 up to a constant: the case PAPER.md:292 studies) standing in for the strain
+    data d(t) of Eq. (15); tests add a signal to it."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 700 + seed))
+    return sigma * (rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
+
+
+def dense_trajectory(n_samples: int, dt: float = 10.0, *, seed: int = 0, l_max: int = L_MAX, n_max: int = N_MAX,
+                     p0: float = 14.0, p1: float | None = None, e0: float = 0.5, e1: float | None = None, M: float = 1e6,
+                     T: float = YEAR_S, t_start: float = 0.0):
+    """Dense inputs of the direct summation (amplitudes and phases "at each point in the dense trajectory",
+    10 s steps, no interpolation): the config-1 source evaluated at t_i = t_start + i dt instead of at ~100 sparse points.
+    p(t), e(t) linear in t over the year (a window of it if n_samples dt < T); Phi_phi, Phi_r are the closed-form integrals
+    of Omega_phi = p^-1.5 / M_s and Omega_r = Omega_phi sqrt(1 - 6/p) for linear p(t); amplitudes by the config-1 model.
+    -> (l, m, n, phase [N, 2] float64, amp [N, K] complex128)."""
+    p1 = 6.0 + 2 * 0.1 + 0.1 if p1 is None else p1
+    e1 = 0.1 if e1 is None else e1
+    l, m, n = mode_grid(l_max, n_max)
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 900 + seed))
+    t = t_start + dt * np.arange(n_samples, dtype=np.float64)
+    Ms = M * MSUN_S
+    slope = (p1 - p0) / T
+
+    def F_phi(p):   # antiderivative of p^-1.5 in p
+        return -2.0 / np.sqrt(p)
+
+    def F_r(p):     # antiderivative of p^-2 sqrt(p - 6) in p
+        return -np.sqrt(p - 6.0) / p + np.arctan(np.sqrt((p - 6.0) / 6.0)) / np.sqrt(6.0)
+
+    p = (p0 + slope * t).astype(np.longdouble)
+    phase = np.stack([(F_phi(p) - F_phi(np.longdouble(p0))) / (slope * Ms),
+                      (F_r(p) - F_r(np.longdouble(p0))) / (slope * Ms)], axis=1).astype(np.float64)
+    e_t = e0 + (e1 - e0) * (t / T)
+    amp = _amplitudes(rng, t, T, e_t, l, n, cfg0=False)
+    return l, m, n, phase, amp

@@ -1,0 +1,216 @@
+"""GPU parity of the SURVEY.md section 8(f) rows against the CPU oracle (through the C-ABI binding):
+  NEXT-1  detector-frame transformation, fused into the summation (few_frame_constants, few_waveform_ssb) and as a pass
+          (few_frame_rotate)
+  NEXT-2  PSD = 1 inner products, fused into the summation kernel (few_sum_waveform_ex / few_waveform_ssb) and as a separate
+          reduction (few_inner_products)
+  NEXT-3  direct summation (few_sum_direct)
+Bars: waveforms rel-L2 <= 1e-10 and mismatch <= 1e-12 (north_star); inner products within 1e-10 of 2 dt |d| |h| (the waveform
+bar carried through Cauchy-Schwarz), in practice ~1e-14; constants 1e-14.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_2104_04582_b200 import synth  # noqa: E402
+
+REL_L2_TOL = 1e-10
+MISMATCH_TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "-m gpu tests need a GPU"
+    from paper_2104_04582_b200 import api as a
+    return a
+
+
+def dev(a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def mismatch(a, b):
+    ah, bh = a / np.linalg.norm(a), b / np.linalg.norm(b)
+    return 0.5 * float(np.linalg.norm(ah - bh) ** 2)
+
+
+# ------------------------------------------------------------------------------------------- NEXT-1
+def test_frame_constants_vs_oracle(api):
+    sky, mu = synth.sky_angles(40, seed=1)
+    sky[1] = (1.0, 0.3, 1.0 + 1e-6, 0.3 + 1e-6)            # spin almost along the line of sight
+    sky[2] = (1e-4, 2.0, math.pi - 1e-4, 5.0)              # both near the poles
+    sky[3] = (0.9, 1.1, 0.9, 1.1)                          # exactly degenerate: N = D = 0 up to rounding of the products
+    th, ph, f = api.few_frame_constants(dev(sky), dev(mu))
+    th, ph, f = th.cpu().numpy(), ph.cpu().numpy(), f.cpu().numpy()
+    for s in range(sky.shape[0]):
+        rt, rp, rf = oracle.frame(*sky[s], mu[s])
+        R = np.array([math.sin(sky[s, 0]) * math.cos(sky[s, 1]), math.sin(sky[s, 0]) * math.sin(sky[s, 1]), math.cos(sky[s, 0])])
+        S = np.array([math.sin(sky[s, 2]) * math.cos(sky[s, 3]), math.sin(sky[s, 2]) * math.sin(sky[s, 3]), math.cos(sky[s, 2])])
+        sin_rs = np.linalg.norm(np.cross(R, S))
+        assert ph[s] == rp
+        if s == 3:
+            assert abs(abs(f[s]) - mu[s]) <= 1e-15          # direction of the factor is undefined; its modulus is not
+            continue
+        # theta from cos(theta) = -R.S: FP64 rounding of the dot product moves it by eps / sin(theta)
+        assert abs(th[s] - rt) <= 4e-16 / max(sin_rs, 1e-8) + 4e-16, (s, th[s], rt)
+        assert abs(f[s] - rf) <= 1e-15 * mu[s] / max(sin_rs, 1e-8) ** 2 + 4e-16 * mu[s], (s, f[s], rf)
+
+
+def test_frame_rotate_vs_oracle(api):
+    rng = np.random.default_rng(5)
+    for n_src, N in [(1, 1), (3, 1000), (2, 70_001), (5, 4096)]:
+        h = rng.normal(size=(n_src, N)) + 1j * rng.normal(size=(n_src, N))
+        f = rng.normal(size=n_src) + 1j * rng.normal(size=n_src)
+        out = api.few_frame_rotate(dev(h), dev(f)).cpu().numpy()
+        for s in range(n_src):
+            ref = oracle.frame_apply(h[s], complex(f[s]))
+            assert np.max(np.abs(out[s] - ref)) <= 4e-16 * abs(f[s]) * np.max(np.abs(h[s]))
+    hd = dev(h)
+    api.few_frame_rotate(hd, dev(f), out=hd)               # in place
+    assert np.array_equal(hd.cpu().numpy(), out)
+    assert api.few_frame_rotate(dev(np.zeros((2, 0), np.complex128)), dev(f[:2])).shape == (2, 0)
+
+
+def ssb_oracle(w, sky, mu, keep_by_src, windows=None):
+    """Oracle chain in the detector frame: O5 -> O2 -> O1 -> O4 at (theta_src, phi_src) -> O5 apply, restricted to given kept sets."""
+    out = []
+    for s in range(w.n_src):
+        th, ph, f = oracle.frame(*sky[s], mu[s] if mu is not None else 1.0)
+        yp, ym = oracle.ylm_modes(w.l, w.m, th, ph)
+        ca = oracle.spline_fit(w.t[s], np.ascontiguousarray(w.amp[s]).view(np.float64))
+        cp = oracle.spline_fit_ext(w.t[s], w.phase[s])
+        wins = windows if windows is not None else [(0, w.n_samples)]
+        hs = [oracle.frame_apply(oracle.sum_waveform(w.t[s], ca, cp, w.l, w.m, w.n, keep_by_src[s], yp, ym, w.t0, w.dt, nn, i0=i0), f)
+              for i0, nn in wins]
+        out.append(np.concatenate(hs))
+    return out
+
+
+def run_ssb(api, w, sky, mu, d=None, want_h=True, want_inner=False):
+    keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device="cuda")
+    nk = torch.empty((w.n_src,), dtype=torch.int32, device="cuda")
+    h, inner = api.few_waveform_ssb(dev(w.t), dev(w.phase), dev(w.amp), dev(w.l), dev(w.m), dev(w.n), dev(sky), w.eps, w.t0, w.dt,
+                                    w.n_samples, mu_over_dl=None if mu is None else dev(mu), d=None if d is None else dev(d),
+                                    want_inner=want_inner, want_h=want_h, keep_idx=keep, n_keep=nk)
+    api.few_device_status()
+    keep, nk = keep.cpu().numpy(), nk.cpu().numpy()
+    return (None if h is None else h.cpu().numpy()), (None if inner is None else inner.cpu().numpy()), \
+        [keep[s][: nk[s]] for s in range(w.n_src)]
+
+
+def test_waveform_ssb_config0(api):
+    w = synth.make_config(0)
+    sky, mu = synth.sky_angles(1)
+    h, _, keep = run_ssb(api, w, sky, mu)
+    ref = ssb_oracle(w, sky, mu, keep)[0]
+    assert len(keep[0]) == 8
+    assert rel_l2(h[0], ref) <= REL_L2_TOL and mismatch(h[0], ref) <= MISMATCH_TOL
+    assert np.max(np.abs(h[0] - ref)) <= 1e-10 * np.max(np.abs(ref))
+    # fused == the separate pass over the source-frame waveform (what the paper's pipeline does)
+    th, ph, f = api.few_frame_constants(dev(sky), dev(mu))
+    h_src = api.few_waveform(dev(w.t), dev(w.phase), dev(w.amp), dev(w.l), dev(w.m), dev(w.n), th, ph, w.eps, w.t0, w.dt, w.n_samples)
+    h2 = api.few_frame_rotate(h_src, f).cpu().numpy()
+    assert rel_l2(h2[0], h[0]) <= 1e-13
+
+
+@pytest.mark.parametrize("cfg,n,t0", [(1, 20_000, 0.0), (2, 3_000, 15_000_000.0)])
+def test_waveform_ssb_windows(api, cfg, n, t0):
+    w = synth.make_config(cfg, n_samples=n, t0=t0)
+    sky, mu = synth.sky_angles(1)
+    h, _, keep = run_ssb(api, w, sky, mu)
+    ref = ssb_oracle(w, sky, mu, keep)[0]
+    assert rel_l2(h[0], ref) <= REL_L2_TOL and mismatch(h[0], ref) <= MISMATCH_TOL
+    # the kept set is the oracle's selection at the oracle's own viewing angles (up to the 1e-12 band)
+    th, ph, _ = oracle.frame(*sky[0])
+    yp, ym = oracle.ylm_modes(w.l, w.m, th, ph)
+    ref_keep, margin = oracle.select_modes(w.amp[0], w.m, yp, ym, w.eps)
+    diff = np.setxor1d(ref_keep, keep[0])
+    assert all(margin[j] <= 1e-12 for j in diff), diff
+
+
+def test_waveform_ssb_batch(api):
+    w = synth.make_config(3, n_src=5, n_samples=2_500, t0=9_000_000.0)
+    sky, mu = synth.sky_angles(5, seed=3)
+    h, _, keep = run_ssb(api, w, sky, mu)
+    ref = ssb_oracle(w, sky, mu, keep)
+    for s in range(w.n_src):
+        assert rel_l2(h[s], ref[s]) <= REL_L2_TOL, (s, rel_l2(h[s], ref[s]))
+        assert mismatch(h[s], ref[s]) <= MISMATCH_TOL
+
+
+# ------------------------------------------------------------------------------------------- NEXT-2
+def inner_tol(d, h, dt):
+    return 1e-10 * 2 * dt * np.linalg.norm(d) * np.linalg.norm(h)
+
+
+def test_inner_products_standalone_vs_oracle(api):
+    rng = np.random.default_rng(21)
+    for n_src, N, dt in [(1, 1, 10.0), (2, 2047, 15.0), (3, 2048 * 3 + 5, 10.0), (1, 300_001, 5.0)]:
+        d = rng.normal(size=(n_src, N)) + 1j * rng.normal(size=(n_src, N))
+        h = rng.normal(size=(n_src, N)) + 1j * rng.normal(size=(n_src, N))
+        got = api.few_inner_products(dev(d), dev(h), dt).cpu().numpy()
+        got2 = api.few_inner_products(dev(d), dev(h), dt).cpu().numpy()
+        assert np.array_equal(got, got2)                                   # fixed reduction order
+        for s in range(n_src):
+            ref = oracle.inner(d[s], h[s], dt)
+            sc = 2 * dt * np.linalg.norm(d[s]) * np.linalg.norm(h[s])
+            assert abs(got[s, 0] - ref[0]) <= 1e-14 * sc and abs(got[s, 1] - ref[1]) <= 1e-14 * sc
+            assert abs(got[s, 2] - ref[2]) <= 1e-14 * ref[2]
+    z = api.few_inner_products(dev(np.zeros((2, 0), np.complex128)), dev(np.zeros((2, 0), np.complex128)), 10.0).cpu().numpy()
+    assert np.array_equal(z, np.zeros((2, 3)))
+
+
+@pytest.mark.parametrize("cfg,n,t0", [(0, 4096, 0.0), (1, 30_000, 1_000_000.0), (0, 5000, -3000.0)])
+def test_fused_inner_products_vs_oracle(api, cfg, n, t0):
+    """<d|h> and <h|h> reduced inside the summation kernel, against O6 applied to the oracle's waveform.  The third case puts
+    samples before t_0 and after t_last (h = 0 there, R12): they must contribute nothing."""
+    w = synth.make_config(cfg, n_samples=n, t0=t0)
+    sky, mu = synth.sky_angles(1)
+    noise = synth.data_stream((1, n), seed=cfg)
+    h_gpu, inner, keep = run_ssb(api, w, sky, mu, d=None, want_inner=True)
+    ref = ssb_oracle(w, sky, mu, keep)[0]
+    d = noise * (0.5 * np.std(ref.real)) + ref[None]                        # data = signal + noise
+    h2, inner, keep2 = run_ssb(api, w, sky, mu, d=d)
+    assert np.array_equal(h2, h_gpu) and all(np.array_equal(a, b) for a, b in zip(keep, keep2))
+    r = oracle.inner(d[0], ref, w.dt)
+    assert abs(inner[0, 0] - r[0]) <= inner_tol(d[0], ref, w.dt), (inner[0], r)
+    assert abs(inner[0, 1] - r[1]) <= inner_tol(d[0], ref, w.dt)
+    assert abs(inner[0, 2] - r[2]) <= 2e-10 * r[2]
+    # in practice: rounding level
+    assert abs(inner[0, 0] - r[0]) <= 1e-12 * 2 * w.dt * np.linalg.norm(d[0]) * np.linalg.norm(ref)
+    # h never written: same three numbers, bit for bit; and the run is reproducible
+    _, inner_only, _ = run_ssb(api, w, sky, mu, d=d, want_h=False)
+    assert np.array_equal(inner_only, inner)
+    # fused == separate reduction over the stored GPU waveform, to rounding
+    sep = api.few_inner_products(dev(d), dev(h2), w.dt).cpu().numpy()
+    assert np.max(np.abs(sep[0] - inner[0])) <= 1e-13 * 2 * w.dt * np.linalg.norm(d[0]) * np.linalg.norm(ref)
+    # without data only <h|h> is formed
+    _, hh_only, _ = run_ssb(api, w, sky, mu, d=None, want_inner=True, want_h=False)
+    assert hh_only[0, 0] == 0.0 and hh_only[0, 1] == 0.0 and hh_only[0, 2] == inner[0, 2]
+    # Eq. (15) and Eq. (17) from the three sums
+    dd = oracle.inner(d[0], d[0], w.dt)[2]
+    lnL = -0.5 * (dd - 2 * inner[0, 0] + inner[0, 2])
+    lnL_ref = -0.5 * oracle.inner(d[0] - ref, d[0] - ref, w.dt)[2]
+    assert abs(lnL - lnL_ref) <= 1e-9 * abs(lnL_ref)
+    ov = inner[0, 0] / math.sqrt(dd * inner[0, 2])
+    assert abs(ov - oracle.overlap(d[0], ref, w.dt)) <= 1e-12
+
+
+def test_fused_inner_products_batch(api):
+    w = synth.make_config(3, n_src=4, n_samples=3_000, t0=5_000_000.0)
+    sky, mu = synth.sky_angles(4, seed=7)
+    d = synth.data_stream((4, 3_000), seed=9)
+    h, inner, keep = run_ssb(api, w, sky, mu, d=d)
+    ref = ssb_oracle(w, sky, mu, keep)
+    for s in range(4):
+        r = oracle.inner(d[s], ref[s], w.dt)
+        assert abs(inner[s, 0] - r[0]) <= inner_tol(d[s], ref[s], w.dt) and abs(inner[s, 2] - r[2]) <= 2e-10 * r[2]
