@@ -160,6 +160,18 @@ size_t few_inner_products_workspace(int n_src, long long n_samples);
 int few_inner_products(few_ctx* ctx, const double* d, const double* h, int n_src, long long n_samples, double dt,
                        double* inner, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- NEXT-3: direct (non-interpolated) summation: amplitudes and phases given at every output sample.
+ *   h_i = scale * factor * sum_j [ Y+_j W_ij + (m_j > 0) (-1)^{l_j} Y-_j conj(W_ij) ],  W_ij = A_ij exp(-i(m_j Phi_phi,i + n_j Phi_r,i)).
+ * amp[n_src][n_samples][n_modes][2] (modes fastest: the amplitude module's layout); phase[n_src][n_samples][2] =
+ * (Phi_phi, Phi_r) in FP64 (reduced mod 2 pi exactly, per sample); l, m, n [n_modes] int32, m >= 0, any order (the grid's
+ * natural order -- n fastest -- is the fast case); ylm_*[n_src][n_modes][2]; scale[n_src] / factor[n_src][2] or NULL;
+ * h[n_src][n_samples][2].  Every mode given is summed (select by passing fewer columns).  HBM-bound: 16 B per sample*mode. */
+size_t few_sum_direct_workspace(int n_src, int n_modes);
+int few_sum_direct(few_ctx* ctx, const double* amp, const double* phase, const int* l, const int* m, const int* n,
+                   const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                   long long n_samples, int n_src, int n_modes, double* h,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- Whole path on device buffers: S0 -> S2 -> S1 -> S3, no host synchronisation.
  * t[n_src][n_t], phase[n_src][n_t][2] (Phi_phi, Phi_r), amp[n_src][n_t][n_modes][2], theta/phi[n_src], l/m/n[n_modes].
  * Outputs: h[n_src][n_samples][2]; optional keep_idx[n_src][n_modes], n_keep[n_src] (NULL: kept inside the workspace). */

@@ -21,7 +21,8 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_ylm_modes", "few_spline_fit_workspace", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
-           "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb"]
+           "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
+           "few_sum_direct"]
 
 
 class FewError(RuntimeError):
@@ -62,6 +63,8 @@ def _load() -> C.CDLL:
         "few_inner_products_workspace": (sz, [i, ll]),
         "few_inner_products": (i, [vp, vp, vp, i, ll, d, vp, vp, sz, vp]),
         "few_waveform_ssb": (i, [vp] * 9 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, vp, vp, sz, vp]),
+        "few_sum_direct_workspace": (sz, [i, i]),
+        "few_sum_direct": (i, [vp] * 10 + [ll, i, i, vp, vp, sz, vp]),
         "few_fp64_peak_probe": (i, [vp, i, i, i, vp, vp]),
         "few_profile_enable": (i, [vp, i]),
         "few_profile_sum_ms": (i, [vp, C.POINTER(C.c_float)]),
@@ -256,6 +259,17 @@ def few_waveform_ssb(t, phase, amp, l, m, n, sky, eps: float, t0: float, dt: flo
                                float(eps), float(t0), float(dt), int(n_samples), n_src, n_t, n_modes, _p(h), _p(d), _p(inner),
                                _p(keep_idx), _p(n_keep), _p(ws), ws.numel(), _stream()), "few_waveform_ssb")
     return h, inner
+
+
+def few_sum_direct(amp, phase, l, m, n, ylm_plus, ylm_minus, scale=None, factor=None, out=None, workspace=None):
+    """Direct summation.  amp [n_src, N, K] c128, phase [n_src, N, 2] f64 -> h [n_src, N] c128."""
+    n_src, n_samples, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, n_samples), dtype=torch.complex128, device=amp.device)
+    ws = workspace if workspace is not None else _ws(_lib.few_sum_direct_workspace(n_src, n_modes), amp.device)
+    _chk(_lib.few_sum_direct(context(), _p(amp, torch.complex128), _p(phase, torch.float64), _p(l, torch.int32), _p(m, torch.int32),
+                             _p(n, torch.int32), _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale),
+                             _p(factor), int(n_samples), n_src, n_modes, _p(h), _p(ws), ws.numel(), _stream()), "few_sum_direct")
+    return h
 
 
 def few_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int) -> int:

@@ -214,3 +214,91 @@ def test_fused_inner_products_batch(api):
     for s in range(4):
         r = oracle.inner(d[s], ref[s], w.dt)
         assert abs(inner[s, 0] - r[0]) <= inner_tol(d[s], ref[s], w.dt) and abs(inner[s, 2] - r[2]) <= 2e-10 * r[2]
+
+
+# ------------------------------------------------------------------------------------------- NEXT-3
+def direct_case(api, l, m, n, phase, amp, theta, phi, scale=None, factor=None):
+    """amp [n_src, N, K], phase [n_src, N, 2] -> (gpu h, oracle h) per source."""
+    n_src = amp.shape[0]
+    yp, ym = api.few_ylm_modes(dev(theta), dev(phi), dev(l), dev(m))
+    h = api.few_sum_direct(dev(amp), dev(phase), dev(l), dev(m), dev(n), yp, ym, scale=None if scale is None else dev(scale),
+                           factor=None if factor is None else dev(factor)).cpu().numpy()
+    api.few_device_status()
+    refs = []
+    for s in range(n_src):
+        ryp, rym = oracle.ylm_modes(l, m, float(theta[s]), float(phi[s]))
+        r = oracle.sum_direct(amp[s], phase[s], l, m, n, ryp, rym, scale=1.0 if scale is None else float(scale[s]))
+        refs.append(r if factor is None else oracle.frame_apply(r, complex(factor[s])))
+    return h, refs
+
+
+@pytest.mark.parametrize("N,t_start", [(300, 0.0), (129, 25_000_000.0)])
+def test_direct_full_grid_vs_oracle(api, N, t_start):
+    """All 3843 modes of the Schwarzschild grid in natural order at dense samples (the slow model's summation, PAPER.md:248);
+    the second window sits late in the year where the phases are ~2e5 rad."""
+    l, m, n, phase, amp = synth.dense_trajectory(N, t_start=t_start)
+    h, refs = direct_case(api, l, m, n, phase[None], amp[None], np.array([0.7]), np.array([1.1]))
+    assert rel_l2(h[0], refs[0]) <= REL_L2_TOL and mismatch(h[0], refs[0]) <= MISMATCH_TOL
+    assert np.max(np.abs(h[0] - refs[0])) <= 1e-10 * np.max(np.abs(refs[0]))
+    assert rel_l2(h[0], refs[0]) <= 1e-12                      # in practice: rounding level
+
+
+@pytest.mark.parametrize("K,order", [(1, "natural"), (17, "natural"), (33, "reverse"), (200, "random"), (554, "gaps")])
+def test_direct_mode_lists_and_ragged_chunks(api, K, order):
+    """Ragged last chunk (K not a multiple of 16), descending and shuffled lists (every mode restarts E), lists with gaps in n."""
+    l, m, n, phase, amp = synth.dense_trajectory(257, t_start=12_000_000.0, seed=K)
+    rng = np.random.default_rng(K)
+    if order == "gaps":
+        idx = np.sort(rng.choice(len(l), K, replace=False))
+    else:
+        idx = np.arange(900, 900 + K)
+        if order == "reverse": idx = idx[::-1]
+        if order == "random": idx = rng.permutation(len(l))[:K]
+    idx = np.ascontiguousarray(idx)
+    h, refs = direct_case(api, l[idx], m[idx], n[idx], phase[None], np.ascontiguousarray(amp[:, idx])[None], np.array([2.1]),
+                          np.array([4.0]))
+    assert rel_l2(h[0], refs[0]) <= REL_L2_TOL and mismatch(h[0], refs[0]) <= MISMATCH_TOL
+    assert rel_l2(h[0], refs[0]) <= 1e-12
+
+
+def test_direct_batch_scale_factor_and_edges(api):
+    n_src, N = 3, 130
+    parts = [synth.dense_trajectory(N, seed=s, t_start=1e6 * s, l_max=4, n_max=5) for s in range(n_src)]
+    l, m, n = parts[0][:3]
+    phase = np.stack([p[3] for p in parts]); amp = np.stack([p[4] for p in parts])
+    theta = np.array([0.3, 1.5, 3.0]); phi = np.array([0.0, 2.0, 5.0])
+    scale = np.array([1.0, 0.25, 3.0]); factor = np.array([1j, -0.6 + 0.8j, 2.0 + 0j])
+    h, refs = direct_case(api, l, m, n, phase, amp, theta, phi, scale=scale, factor=factor)
+    for s in range(n_src):
+        assert rel_l2(h[s], refs[s]) <= 1e-12
+    # a single source gives the same bits as inside the batch
+    h1, _ = direct_case(api, l, m, n, phase[1:2], amp[1:2], theta[1:2], phi[1:2], scale=scale[1:2], factor=factor[1:2])
+    assert np.array_equal(h1[0], h[1])
+    # empty output, bad modes
+    yp, ym = api.few_ylm_modes(dev(theta), dev(phi), dev(l), dev(m))
+    e = api.few_sum_direct(dev(np.zeros((3, 0, len(l)), np.complex128)), dev(np.zeros((3, 0, 2))), dev(l), dev(m), dev(n), yp, ym)
+    assert e.shape == (3, 0)
+    bad_m = m.copy(); bad_m[3] = -1
+    api.few_sum_direct(dev(amp), dev(phase), dev(l), dev(bad_m), dev(n), yp, ym)
+    assert api.few_device_status(raise_on_error=False) != 0
+
+
+def test_direct_equals_interpolated_on_dense_spline_values(api):
+    """Cross-check of the two summation modules on the GPU: the interpolated path's waveform equals the direct sum fed with the
+    oracle's splines evaluated at every sample (amplitudes FP64, phases rounded to FP64: agreement to |m Phi| 2^-53)."""
+    w = synth.make_config(0)
+    h_int = api.few_waveform(dev(w.t), dev(w.phase), dev(w.amp), dev(w.l), dev(w.m), dev(w.n), dev(w.theta), dev(w.phi), 0.0, w.t0,
+                             w.dt, 1500).cpu().numpy()[0]
+    ca = oracle.spline_fit(w.t[0], np.ascontiguousarray(w.amp[0]).view(np.float64))
+    cp = oracle.spline_fit_ext(w.t[0], w.phase[0])
+    ti = w.t0 + np.arange(1500) * w.dt
+    k = np.clip(np.searchsorted(w.t[0], ti, side="right") - 1, 0, w.n_t - 2)
+    dx = ti - w.t[0][k]
+    c = ca[k]
+    val = ((c[:, 3] * dx[:, None] + c[:, 2]) * dx[:, None] + c[:, 1]) * dx[:, None] + c[:, 0]
+    A = np.ascontiguousarray(val[:, 0::2] + 1j * val[:, 1::2])
+    dxl = dx.astype(np.longdouble)[:, None]; cpk = cp[k]
+    ph = (((cpk[:, 3] * dxl + cpk[:, 2]) * dxl + cpk[:, 1]) * dxl + cpk[:, 0]).astype(np.float64)
+    yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), dev(w.l), dev(w.m))
+    h_dir = api.few_sum_direct(dev(A[None]), dev(ph[None]), dev(w.l), dev(w.m), dev(w.n), yp, ym).cpu().numpy()[0]
+    assert rel_l2(h_dir, h_int) <= 1e-12
