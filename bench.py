@@ -108,7 +108,7 @@ def time_stages(api, torch, w, g, flush, reps: int = 10):
     """Each C-ABI stage timed alone with CUDA events (L2 flushed before every launch); GB/s = algorithmic bytes / time:
     S1 reads 8 B and writes 32 B per knot and system; S2 reads the 16 B complex amplitude of every mode at every step."""
     yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
-    keep, nk = api.few_select_modes(g["amp"], g["m"], yp, ym, max(w.eps, 1e-5))
+    keep, nk = api.few_select_modes(g["amp"], g["m"], yp, ym, w.eps)       # eps <= 0: the identity list (all modes)
     y_amp = torch.view_as_real(g["amp"]).reshape(w.n_src, w.n_t, -1)
     coef = api.few_spline_fit(g["t"], y_amp)
     cdd = api.few_spline_fit_dd(g["t"], g["phase"])
@@ -138,6 +138,67 @@ def time_stages(api, torch, w, g, flush, reps: int = 10):
         if name in nbytes:
             out[name]["algorithmic_bytes"] = nbytes[name]
             out[name]["gbs"] = nbytes[name] / (float(np.mean(ts)) * 1e-3) / 1e9
+    return out
+
+
+def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: int = 1 << 18):
+    """SURVEY.md 8(f) rows, each timed with CUDA events after an L2 flush: the detector-frame whole path (NEXT-1) against the
+    source-frame one and against the separate rotation pass; the likelihood step with the inner products fused and h never
+    written (NEXT-2) against the separate reduction; the direct summation (NEXT-3) against the HBM roofline."""
+    from paper_2104_04582_b200 import synth
+    dev = g["t"].device
+    sky_h, mu_h = synth.sky_angles(w.n_src)
+    sky, mu = torch.as_tensor(sky_h).to(dev), torch.as_tensor(mu_h).to(dev)
+    h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
+    d = torch.randn((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
+    ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=dev)
+    ipws = torch.empty(max(api._lib.few_inner_products_workspace(w.n_src, w.n_samples), 256), dtype=torch.uint8, device=dev)
+    th, ph, fac = api.few_frame_constants(sky, mu)
+    args_ = (g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"])
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.mean(ts))
+
+    out = {}
+    out["source_frame_step_ms"] = timed(lambda: api.few_waveform(*args_, th, ph, w.eps, w.t0, w.dt, w.n_samples, out=h, workspace=ws))
+    out["ssb_step_ms_fused"] = timed(lambda: api.few_waveform_ssb(*args_, sky, w.eps, w.t0, w.dt, w.n_samples, mu_over_dl=mu, out=h,
+                                                                  workspace=ws))
+    ms = timed(lambda: api.few_frame_rotate(h, fac, out=h))
+    nb = 32.0 * w.n_src * w.n_samples
+    out["frame_rotate_pass"] = {"ms": ms, "algorithmic_bytes": nb, "gbs": nb / ms / 1e6, "hbm_frac": nb / ms / 1e6 / hbm_gbs}
+    out["likelihood_step_ms_fused_no_h"] = timed(lambda: api.few_waveform_ssb(*args_, sky, w.eps, w.t0, w.dt, w.n_samples, mu_over_dl=mu,
+                                                                              d=d, want_h=False, workspace=ws))
+    out["likelihood_step_ms_fused_with_h"] = timed(lambda: api.few_waveform_ssb(*args_, sky, w.eps, w.t0, w.dt, w.n_samples,
+                                                                                mu_over_dl=mu, d=d, out=h, workspace=ws))
+    ms = timed(lambda: api.few_inner_products(d, h, w.dt, workspace=ipws))
+    out["inner_products_pass"] = {"ms": ms, "algorithmic_bytes": nb, "gbs": nb / ms / 1e6, "hbm_frac": nb / ms / 1e6 / hbm_gbs}
+    del h, d, ws
+    # direct summation: the full 3843-mode grid at every sample (the slow model's summation, PAPER.md:248); amplitudes are
+    # device-generated noise of the workload's shape (the kernel has no data-dependent path), phases ramp to ~2e5 rad
+    l_h, m_h, n_h = synth.mode_grid()
+    K, N = len(l_h), int(direct_samples)
+    amp = torch.empty((1, N, K), dtype=torch.complex128, device=dev)
+    ar = torch.view_as_real(amp)
+    for c0 in range(0, N, 1 << 14):
+        ar[0, c0:c0 + (1 << 14)].normal_()
+    tt = torch.arange(N, dtype=torch.float64, device=dev) * 10.0
+    phase = torch.stack([tt * 6.9e-3, tt * 3.8e-3], dim=1)[None].contiguous()
+    l_d, m_d, n_d = (torch.as_tensor(x).to(dev) for x in (l_h, m_h, n_h))
+    yp, ym = api.few_ylm_modes(g["theta"][:1], g["phi"][:1], l_d, m_d)
+    hd = torch.empty((1, N), dtype=torch.complex128, device=dev)
+    dws = torch.empty(max(api._lib.few_sum_direct_workspace(1, K), 256), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: api.few_sum_direct(amp, phase, l_d, m_d, n_d, yp, ym, out=hd, workspace=dws))
+    nb = 16.0 * N * K
+    out["direct_sum"] = {"ms": ms, "n_samples": N, "n_modes": K, "algorithmic_bytes": nb, "gbs": nb / ms / 1e6,
+                         "hbm_frac": nb / ms / 1e6 / hbm_gbs, "evals_per_s": N * K / (ms * 1e-3),
+                         "note": "16 B per sample*mode evaluation; L2 flushed; inputs 16 GB >> L2"}
     return out
 
 
@@ -178,6 +239,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--eps", type=float, default=None)
     ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
+    ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows: detector frame, fused inner products, direct sum")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
@@ -287,12 +349,17 @@ def main():
     if args.stages and rank == 0:
         stages = time_stages(api, torch, w, g, flush)
 
+    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
+    nxt = None
+    if args.next and rank == 0:
+        del h
+        nxt = time_next(api, torch, w, g, flush, hbm_gbs)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
     sum_ms_avg = float(np.mean(sum_ms))
     peak_tflops = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     achieved_tflops = pair_evals_per_step * FLOP_PER_PAIR / (sum_ms_avg * 1e-3) / 1e12
@@ -327,6 +394,8 @@ def main():
                 v["hbm_frac"] = v["gbs"] / hbm_gbs
         out["stages"] = stages
         out["stages_hbm_peak_gbs"] = hbm_gbs
+    if nxt is not None:
+        out["next"] = nxt
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

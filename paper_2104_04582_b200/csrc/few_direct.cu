@@ -9,11 +9,13 @@
 //
 // Bound: HBM.  Every amplitude is read exactly once, 16 B per sample*mode evaluation, against ~12 FP64 instructions.
 // Design: one thread per sample, a block owns kDirTile consecutive samples and walks the K modes in chunks of kDirChunk.  A
-// chunk of the tile is kDirTile rows of 256 contiguous bytes in HBM; warp 0 fetches each row with one 1-D TMA bulk copy
-// (cp.async.bulk + mbarrier, SASS UBLKCP) into a shared-memory stage whose rows are padded by 16 B, so that thread i reading
-// "its" row with 128-bit loads is bank-conflict free: the transposition from the mode-fastest HBM layout to the
-// sample-per-thread register layout costs no instruction.  A ring of kDirStages stages keeps >= 2 stages (70 KB per block) in
-// flight.  Mode constants travel with the chunk (one more bulk copy of 768 B).
+// chunk of the tile is kDirTile rows of 256 contiguous bytes in HBM; the block copies them with 16-byte cp.async (LDGSTS: a
+// half-warp per row, so every request is a full 256-byte segment) into a shared-memory stage whose rows are padded by 16 B,
+// so that thread i reading "its" row with 128-bit loads is bank-conflict free: the transposition from the mode-fastest HBM
+// layout to the sample-per-thread register layout costs no instruction.  A ring of kDirStages stages (cp.async commit groups)
+// keeps 2 stages = 70 KB per block in flight.  Mode constants travel with the chunk (48 more 16-byte pieces).
+// (First version: one 1-D TMA bulk copy per 256-byte row.  ncu: 1.6 TB/s, warps parked at the barrier -- the TMA unit retires
+// about one bulk request per 40 cycles per SM, so 256-byte requests cap at ~1.9 TB/s chip-wide; profiles/r01c_direct.md.)
 // exp(-i(m Phi_phi + n Phi_r)) = Z_phi^m Z_r^n with Z = exp(-i Phi) from ONE full-range sincos per phase and sample; along a
 // mode list in the grid's natural order (n fastest) E advances by one complex multiplication per mode; jumps in (m, n) restart
 // from Z_phi^m and a binary power of Z_r (block-uniform branch, once per (l, m) run of the full grid).
@@ -36,30 +38,12 @@ struct dir_cst {          // 48 B per mode
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+__device__ __forceinline__ void cp_async16(void* dst, const void* src)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
-{
-    unsigned ok;
-    do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok)
-                     : "r"(smem_u32(bar)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // z^e for e >= 0 by binary powering (e is block-uniform)
 __device__ __forceinline__ void cpow(double zr, double zi, int e, double* pr, double* pi)
@@ -116,7 +100,6 @@ few_direct_kernel(const double2* __restrict__ amp_all, const double2* __restrict
                   long long N, int K, int K_pad, double2* __restrict__ h_all)
 {
     extern __shared__ __align__(128) unsigned char dsm[];
-    __shared__ __align__(8) unsigned long long full[kDirStages];
     const int tid = threadIdx.x, src = blockIdx.y;
     const long long i0 = (long long)blockIdx.x * kDirTile;
     const int rows = (int)((N - i0) < kDirTile ? (N - i0) : kDirTile);
@@ -124,28 +107,22 @@ few_direct_kernel(const double2* __restrict__ amp_all, const double2* __restrict
     const unsigned char* cst_g = reinterpret_cast<const unsigned char*>(cst_all + (size_t)src * K_pad);
     const int n_chunks = K_pad / kDirChunk;
 
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < kDirStages; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-
-    // warp 0 issues stage c: one bulk copy per row (lane r, r + 32, ...) plus the chunk's constants
+    // stage c: piece p = tid + kDirTile * u is the 16 bytes of mode c*16 + (p & 15) of row p >> 4
     auto issue = [&](int c) {
         unsigned char* st = dsm + (size_t)(c % kDirStages) * kDirStageBytes;
-        unsigned long long* bar = &full[c % kDirStages];
         const int cnt = (K - c * kDirChunk) < kDirChunk ? (K - c * kDirChunk) : kDirChunk;     // ragged last chunk
-        const unsigned row_bytes = (unsigned)cnt * 16u;
-        if (tid == 0) mbar_expect_tx(bar, row_bytes * (unsigned)rows + kDirCstBytes);
-        __syncwarp();
-        if (tid == 0) bulk_g2s(st + kDirTile * kDirRowBytes, cst_g + (size_t)c * kDirCstBytes, kDirCstBytes, bar);
-        for (int r = tid; r < rows; r += 32)
-            bulk_g2s(st + r * kDirRowBytes, amp + (size_t)r * K + (size_t)c * kDirChunk, row_bytes, bar);
+        const int q = tid & (kDirChunk - 1);
+        const double2* g = amp + (size_t)c * kDirChunk + q;
+        if (q < cnt) {
+#pragma unroll
+            for (int u = 0; u < kDirChunk; ++u) {
+                const int r = (tid >> 4) + u * (kDirTile / kDirChunk);
+                if (r < rows) cp_async16(st + r * kDirRowBytes + q * 16, g + (size_t)r * K);
+            }
+        }
+        if (tid < kDirCstBytes / 16) cp_async16(st + kDirTile * kDirRowBytes + tid * 16, cst_g + (size_t)c * kDirCstBytes + tid * 16);
     };
-    if (tid < 32)
-        for (int c = 0; c < kDirStages - 1 && c < n_chunks; ++c) issue(c);
+    for (int c = 0; c < kDirStages - 1; ++c) { if (c < n_chunks) issue(c); cp_async_commit(); }
 
     // per-sample phase factors (overlaps the first copies)
     double zpr = 1.0, zpi = 0.0, zrr = 1.0, zri = 0.0;
@@ -160,9 +137,10 @@ few_direct_kernel(const double2* __restrict__ amp_all, const double2* __restrict
     double er = 1.0, ei = 0.0, hr = 0.0, hi = 0.0;
 
     for (int c = 0; c < n_chunks; ++c) {
-        __syncthreads();                                            // stage c-1 fully consumed: its slot may be refilled
-        if (tid < 32 && c + kDirStages - 1 < n_chunks) issue(c + kDirStages - 1);
-        mbar_wait(&full[c % kDirStages], (unsigned)(c / kDirStages) & 1u);
+        cp_async_wait<kDirStages - 2>();                            // this thread's pieces of stage c have landed
+        __syncthreads();                                            // ... everyone's have; stage c-1 is fully consumed
+        if (c + kDirStages - 1 < n_chunks) issue(c + kDirStages - 1);
+        cp_async_commit();                                          // one group per iteration, empty or not
         const unsigned char* st = dsm + (size_t)(c % kDirStages) * kDirStageBytes;
         const double2* row = reinterpret_cast<const double2*>(st + tid * kDirRowBytes);
         const dir_cst* cs = reinterpret_cast<const dir_cst*>(st + kDirTile * kDirRowBytes);

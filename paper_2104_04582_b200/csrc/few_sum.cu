@@ -373,12 +373,12 @@ __device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, 
     }
 }
 
-template <int R, int kBlocksPerSm>
+template <int R, int kBlocksPerSm, bool kInner>
 __global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
-               int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all,
-               int want_inner)
+               int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all)
 {
+    constexpr bool want_inner = kInner;      // the inner-product epilogue is compiled out of the plain waveform kernel
     __shared__ __align__(128) double2 ring[kRing][kStageD2];
     __shared__ __align__(8) unsigned long long full[kRing];
     __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
@@ -640,9 +640,13 @@ extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* 
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
     const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
-    few_sum_kernel<kSumR, kSumBlocksPerSm><<<(unsigned)(want < resident ? want : resident), kSumThreads, 0, st>>>(
-        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, (const double2*)d,
-        inner ? 1 : 0);
+    const unsigned grid = (unsigned)(want < resident ? want : resident);
+    if (inner)
+        few_sum_kernel<kSumR, kSumBlocksPerSm, true><<<grid, kSumThreads, 0, st>>>(
+            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, (const double2*)d);
+    else
+        few_sum_kernel<kSumR, kSumBlocksPerSm, false><<<grid, kSumThreads, 0, st>>>(
+            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, nullptr);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     if (inner) {
