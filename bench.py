@@ -33,6 +33,9 @@ FLOP_PER_PAIR = 38.0          # executed algorithm: per sa
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
 GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
 GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch, from the `ncu --set full` captures summarised in
+# profiles/r01c_kernels.md (the coefficient stream and h stay in the 126 MB L2 while the kernel runs)
+SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 4.78e6, "config2_1yr_allmodes": 10.39e6}
 
 
 def load_peaks():
@@ -365,7 +368,8 @@ def main():
     achieved_tflops = pair_evals_per_step * FLOP_PER_PAIR / (sum_ms_avg * 1e-3) / 1e12
     nominal_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "few_sum_kernel", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / peak_tflops, "traffic": None,
+                "frac": achieved_tflops / peak_tflops,
+                "traffic": SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if args.eps is None else None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
