@@ -14,6 +14,7 @@ Functions (each follows the passage cited in few_oracle.c):
   frame_apply(h, factor)      O5
   inner(d, h, dt)             O6                  PAPER.md:283-296 Eq. (15)-(17), PSD = 1
   sum_direct(...)             O7
+  sum_waveform_kerr(...)      O8                  PAPER.md:54 Eq. (1), 438-444 Eq. (19), Eq. (9) with k
   waveform(workload)          chain O2 -> O3 -> O1 -> O4 in the paper's pipeline order
 """
 from __future__ import annotations
@@ -63,6 +64,9 @@ def lib():
         L.oracle_frame_apply.argtypes = [_dp, C.c_longlong, _dp, _dp]
         L.oracle_inner.argtypes = [_dp, _dp, C.c_longlong, C.c_double, _dp]
         L.oracle_sum_direct.argtypes = [_dp, _dp, _ip, _ip, _ip, _dp, _dp, C.c_double, C.c_int, C.c_longlong, C.c_int, _dp]
+        L.oracle_sum_waveform_kerr.argtypes = [_dp, _dp, C.c_void_p, C.c_int, _ip, _ip, _ip, _ip, _ip, C.c_int, _dp, _dp,
+                                               C.c_double, C.c_int, C.c_double, C.c_double, C.c_longlong, C.c_longlong,
+                                               C.c_int, C.c_int, _dp]
         L.oracle_num_threads.restype = C.c_int
         L.oracle_set_threads.argtypes = [C.c_int]
         _lib = L
@@ -191,6 +195,28 @@ def sum_direct(amp, phase, l, m, n, ylm_plus, ylm_minus, scale: float = 1.0, fol
     h = np.empty((N, 2), np.float64)
     lib().oracle_sum_direct(_ptr(a), _ptr(ph), _ptr(l, _ip), _ptr(m, _ip), _ptr(n, _ip), _ptr(yp), _ptr(ym), float(scale),
                             int(bool(fold)), N, K, _ptr(h))
+    return h.view(np.complex128)[:, 0]
+
+
+def sum_waveform_kerr(t, coef_amp, coef_phase_ext, l, m, k, n, keep_idx, ylm_plus, ylm_minus, t0, dt, n_samples,
+                      scale: float = 1.0, fold: bool = True, i0: int = 0):
+    """O8.  coef_phase_ext [n_t-1, 4, n_ph] longdouble with n_ph = 3 (Phi_phi, Phi_theta, Phi_r) or 2; k int32 [n_modes] or None."""
+    t = np.ascontiguousarray(t, np.float64)
+    ca = np.ascontiguousarray(coef_amp, np.float64)
+    cp = np.ascontiguousarray(coef_phase_ext, np.longdouble)
+    l, m, n = (np.ascontiguousarray(x, np.int32) for x in (l, m, n))
+    kk = None if k is None else np.ascontiguousarray(k, np.int32)
+    n_t, n_modes, n_ph = t.shape[0], l.shape[0], cp.shape[2]
+    assert ca.shape == (n_t - 1, 4, 2 * n_modes) and cp.shape == (n_t - 1, 4, n_ph)
+    kp = None if keep_idx is None else np.ascontiguousarray(keep_idx, np.int32)
+    yp = _c2d(ylm_plus)
+    ym = _c2d(ylm_minus if ylm_minus is not None else np.zeros(n_modes, np.complex128))
+    h = np.empty((int(n_samples), 2), np.float64)
+    rc = lib().oracle_sum_waveform_kerr(_ptr(t), _ptr(ca), cp.ctypes.data, n_ph, _ptr(l, _ip), _ptr(m, _ip), _ptr(kk, _ip),
+                                        _ptr(n, _ip), _ptr(kp, _ip), 0 if kp is None else len(kp), _ptr(yp), _ptr(ym),
+                                        float(scale), int(bool(fold)), float(t0), float(dt), int(i0), int(n_samples), n_t,
+                                        n_modes, _ptr(h))
+    if rc: raise ValueError(_ERR.get(rc, f"oracle error {rc}"))
     return h.view(np.complex128)[:, 0]
 
 

@@ -21,6 +21,8 @@
  *   oracle_inner             : P13 Parseval against the frequency-domain form of Eq. (16) (numpy FFT), overlap(a,a)=1.
  *   oracle_sum_direct        : P14 closed form, mpmath brute force, agreement with the interpolated sum on inputs
  *                              that are exactly cubic per segment.
+ *   oracle_sum_waveform_kerr : P15 equals oracle_sum_waveform for k = 0 / two phases, single-mode closed form with k,
+ *                              (-1)^(l+k) fold vs the explicit (l,-m,-k,-n) list, mpmath brute force with three phases.
  * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC few_oracle.c -o libfew_oracle.so -lm
@@ -413,6 +415,74 @@ int oracle_sum_direct(const double *amp, const double *phase, const int *l, cons
                 ext zr = sg * ylm_minus[2 * j], zi = sg * ylm_minus[2 * j + 1];
                 hr += zr * Wr + zi * Wi;
                 hi += -zr * Wi + zi * Wr;
+            }
+        }
+        h[2 * i] = (double)(hr * scale);
+        h[2 * i + 1] = (double)(hi * scale);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O8 -- interpolated summation with the polar index k and the third phase (generic Kerr shape), Eq. (1):
+ * "Phi_mkn = m Phi_phi + k Phi_theta + n Phi_r", Eq. (19): with the spheroidal harmonics projected on
+ * spherical ones "h = mu/d_L sum_lmkn A_lmkn(t) -2Y_lm(theta, phi) exp(-i Phi_mkn(t))", and Eq. (9) in full:
+ * "A_{l,-m,-k,-n} = (-1)^{(l+k)} A*_lmkn".  NEXT-4 of SURVEY.md section 8(f).
+ *  h(t_i) = scale * sum_{j kept} [ Y+_j W_j + (m_j > 0) (-1)^{l_j + k_j} Y-_j conj(W_j) ],
+ *  W_j = A_j(t_i) exp(-i (m_j Phi_phi + k_j Phi_theta + n_j Phi_r)).
+ * Everything else exactly as O4 (sample times, segment lookup, extended-precision phases, FP64 amplitudes, accumulation
+ * order).  coef_phase[n_t-1][4][n_ph] with n_ph = 3: (Phi_phi, Phi_theta, Phi_r); n_ph = 2: (Phi_phi, Phi_r), k ignored
+ * in the angle -- then the function is O4 apart from the fold sign, which is pinned against O4 with k = 0.
+ * ------------------------------------------------------------------------------------------------ */
+int oracle_sum_waveform_kerr(const double *t, const double *coef_amp, const ext *coef_phase, int n_ph,
+                             const int *l, const int *m, const int *k, const int *n, const int *keep_idx, int n_keep,
+                             const double *ylm_plus, const double *ylm_minus, double scale, int fold,
+                             double t0, double dt, long long i0, long long n_samples,
+                             int n_t, int n_modes, double *h)
+{
+    if (n_t < 4) return -1;
+    if (n_ph != 2 && n_ph != 3) return -3;
+    const int n_sys = 2 * n_modes;
+    const int K = keep_idx ? n_keep : n_modes;
+    long long i;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < n_samples; ++i) {
+        double prod = (double)(i0 + i) * dt;
+        double ti = t0 + prod;
+        ext hr = 0, hi = 0;
+        if (ti >= t[0] && ti <= t[n_t - 1]) {
+            int lo = 0, hi_k = n_t - 1;
+            while (hi_k - lo > 1) {
+                int mid = (lo + hi_k) / 2;
+                if (t[mid] <= ti) lo = mid; else hi_k = mid;
+            }
+            int seg = lo > n_t - 2 ? n_t - 2 : lo;
+            double dx = ti - t[seg];
+            const ext *cp = coef_phase + (size_t)seg * 4 * n_ph;
+            ext x = dx, P[3] = {0, 0, 0};
+            for (int q = 0; q < n_ph; ++q)
+                P[q] = ((cp[3 * n_ph + q] * x + cp[2 * n_ph + q]) * x + cp[n_ph + q]) * x + cp[q];
+            ext Pphi = P[0], Pth = n_ph == 3 ? P[1] : 0, Pr = n_ph == 3 ? P[2] : P[1];
+            const double *ca = coef_amp + (size_t)seg * 4 * n_sys;
+            for (int q = 0; q < K; ++q) {
+                int j = keep_idx ? keep_idx[q] : q;
+                const double *c0 = ca + 2 * (size_t)j, *c1 = c0 + n_sys, *c2 = c1 + n_sys, *c3 = c2 + n_sys;
+                double Ar = ((c3[0] * dx + c2[0]) * dx + c1[0]) * dx + c0[0];
+                double Ai = ((c3[1] * dx + c2[1]) * dx + c1[1]) * dx + c0[1];
+                int kj = (n_ph == 3 && k) ? k[j] : 0;
+                ext th = (ext)m[j] * Pphi + (ext)kj * Pth + (ext)n[j] * Pr;
+                ext Er = cosl(th), Ei = -sinl(th);
+                ext Wr = (ext)Ar * Er - (ext)Ai * Ei, Wi = (ext)Ar * Ei + (ext)Ai * Er;
+                ext yr = ylm_plus[2 * j], yi = ylm_plus[2 * j + 1];
+                hr += yr * Wr - yi * Wi;
+                hi += yr * Wi + yi * Wr;
+                if (fold && m[j] > 0) {                                  /* Eq. (9): (-1)^(l+k) */
+                    int par = l[j] + (k ? k[j] : 0);
+                    ext sg = (par % 2) ? -1.0L : 1.0L;
+                    ext zr = sg * ylm_minus[2 * j], zi = sg * ylm_minus[2 * j + 1];
+                    hr += zr * Wr + zi * Wi;
+                    hi += -zr * Wi + zi * Wr;
+                }
             }
         }
         h[2 * i] = (double)(hr * scale);

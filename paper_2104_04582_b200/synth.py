@@ -52,6 +52,7 @@ class Workload:
     dt: float
     n_samples: int
     eps: float
+    k: np.ndarray | None = None     # polar index per mode (Kerr-shaped workloads: phase then has 3 columns, Phi_phi, Phi_theta, Phi_r)
 
     @property
     def n_src(self): return self.t.shape[0]
@@ -252,3 +253,47 @@ def dense_trajectory(n_samples: int, dt: float = 10.0, *, seed: int = 0, l_max: 
     e_t = e0 + (e1 - e0) * (t / T)
     amp = _amplitudes(rng, t, T, e_t, l, n, cfg0=False)
     return l, m, n, phase, amp
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Kerr-shaped workload: polar index k and a third phase, ~10x the modes
+# ---------------------------------------------------------------------------------------------------------------
+def kerr_mode_grid(l_max: int = L_MAX, k_max: int = 5, n_max: int = N_MAX):
+    """(l, m, k, n) int32 arrays, m >= 0 only: l slowest, then m, then k in [-k_max, k_max], n fastest.  Full grid:
+    63 (l, m) x 11 x 61 = 42 273 modes, "roughly an order of magnitude" more than Schwarzschild's 3843."""
+    ls, ms, ks, ns = [], [], [], []
+    for l in range(L_MIN, l_max + 1):
+        for m in range(0, l + 1):
+            for k in range(-k_max, k_max + 1):
+                for n in range(-n_max, n_max + 1):
+                    ls.append(l), ms.append(m), ks.append(k), ns.append(n)
+    return tuple(np.asarray(x, np.int32) for x in (ls, ms, ks, ns))
+
+
+def make_kerr(*, n_samples: int = 3_155_760, n_t: int = 100, l_max: int = L_MAX, k_max: int = 5, n_max: int = N_MAX,
+              eps: float = 1e-5, t0: float = 0.0, seed: int = 0) -> Workload:
+    """Config-1 trajectory with a third, polar phase and the k index.  Nothing here is Kerr physics: the shapes are.
+    Omega_theta = Omega_phi sqrt(1 - 3/p) lies between Omega_r and Omega_phi as the polar frequency does;
+    |A_lmkn| = config-1 model x exp(-|k| / 1.5) (power concentrated at small |k|), each mode with its own seeded
+    modulation and phase.  Phases by the same composite Simpson rule as the other configs."""
+    l, m, k, n = kerr_mode_grid(l_max, k_max, n_max)
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 40 + seed))
+    T, p0, p1, e0, e1, M = YEAR_S, 14.0, 6.0 + 2 * 0.1 + 0.1, 0.5, 0.1, 1e6
+    t = sparse_grid(T, n_t, uniform=False)
+    e_t = e0 + (e1 - e0) * (t / T)
+    ph2 = _phases(t, T, p0, p1, M)
+    Ms = M * MSUN_S
+    # Phi_theta: Simpson with 256 sub-steps per interval, as _phases does for the other two
+    pth = np.zeros(n_t)
+    acc = np.longdouble(0)
+    for q in range(n_t - 1):
+        hh = (t[q + 1] - t[q]) / 256
+        x = t[q] + hh * np.arange(257); xm = x[:-1] + 0.5 * hh
+        f = lambda tt: (p0 + (p1 - p0) * tt / T) ** -1.5 / Ms * np.sqrt(1.0 - 3.0 / (p0 + (p1 - p0) * tt / T))
+        fa, fm = f(x), f(xm)
+        acc += np.sum(((hh / 6.0) * (fa[:-1] + 4.0 * fm + fa[1:])).astype(np.longdouble))
+        pth[q + 1] = float(acc)
+    phase = np.stack([ph2[:, 0], pth, ph2[:, 1]], axis=1)
+    amp = _amplitudes(rng, t, T, e_t, l, n, cfg0=False) * np.exp(-np.abs(k) / 1.5)[None, :]
+    return Workload(f"kerr_shaped_{len(l)}modes", t[None], phase[None], amp[None], l, m, n, np.array([0.7]), np.array([1.1]),
+                    float(t0), 10.0, int(n_samples), float(eps), k=k)

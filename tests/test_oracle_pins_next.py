@@ -241,3 +241,76 @@ def test_p14_direct_mpmath_bruteforce_and_fold():
             le.append(lj); me.append(-mj); ne.append(-nj); cols.append((-1) ** lj * np.conj(amp[:, j])); ypl.append(ym[j])
     h2 = oracle.sum_direct(np.stack(cols, axis=1), phase, le, me, ne, np.array(ypl), None, scale=0.5, fold=False)
     assert np.max(np.abs(h2 - got)) <= 1e-14 * np.max(np.sum(np.abs(amp), axis=1))
+
+
+# ---------------------------------------------------------------- P15: Kerr-shaped summation (k index, third phase)
+def _kerr_small(seed=1):
+    w = synth.make_kerr(n_samples=300, n_t=12, l_max=3, k_max=2, n_max=2, t0=2_000_000.0, seed=seed)
+    yp, ym = oracle.ylm_modes(w.l, w.m, 0.7, 1.1)
+    ca = oracle.spline_fit(w.t[0], np.ascontiguousarray(w.amp[0]).view(np.float64))
+    cp = oracle.spline_fit_ext(w.t[0], w.phase[0])
+    return w, yp, ym, ca, cp
+
+
+def test_p15_kerr_sum_reduces_to_schwarzschild_sum():
+    """k = 0 everywhere (or two phases): O8 is O4, bit for bit."""
+    w, yp, ym, ca, cp = _kerr_small()
+    k0 = np.zeros_like(w.k)
+    cp2 = np.ascontiguousarray(cp[:, :, [0, 2]])
+    ref = oracle.sum_waveform(w.t[0], ca, cp2, w.l, w.m, w.n, None, yp, ym, w.t0, w.dt, w.n_samples)
+    assert np.array_equal(oracle.sum_waveform_kerr(w.t[0], ca, cp, w.l, w.m, k0, w.n, None, yp, ym, w.t0, w.dt, w.n_samples), ref)
+    assert np.array_equal(oracle.sum_waveform_kerr(w.t[0], ca, cp2, w.l, w.m, None, w.n, None, yp, ym, w.t0, w.dt, w.n_samples), ref)
+
+
+@pytest.mark.parametrize("l,m,k,n", [(2, 2, 1, 0), (3, 1, -2, 4), (4, 0, 3, -1), (5, 5, -1, -3)])
+def test_p15_kerr_single_mode_closed_form(l, m, k, n):
+    """Constant amplitude, linear phases (splines of lines are exact): h = a Y+ e^{-i w t} + [m>0] (-1)^{l+k} conj(a) Y- e^{+i w t},
+    w = m Om_phi + k Om_theta + n Om_r."""
+    t = np.linspace(0.0, 5000.0, 9)
+    om = np.array([3.1e-3, 2.3e-3, 1.9e-3])
+    a = 0.6 * np.exp(-0.4j)
+    ca = oracle.spline_fit(t, np.tile(np.array([[a.real, a.imag]]), (9, 1)))
+    cp = oracle.spline_fit_ext(t, t[:, None] * om[None, :])
+    yp, ym = oracle.ylm_modes([l], [m], 1.0, 2.0)
+    got = oracle.sum_waveform_kerr(t, ca, cp, [l], [m], [k], [n], None, yp, ym, 0.0, 12.5, 400)
+    ti = 12.5 * np.arange(400)
+    wt = (m * om[0] + k * om[1] + n * om[2]) * ti
+    want = a * yp[0] * np.exp(-1j * wt) + ((-1) ** (l + k) * np.conj(a) * ym[0] * np.exp(1j * wt) if m > 0 else 0.0)
+    assert np.max(np.abs(got - want)) <= 1e-13
+
+
+def test_p15_kerr_fold_equals_explicit_mirror_list_and_mpmath():
+    """Eq. (9) with k: the folded sum equals the un-folded sum over a list that also holds (l, -m, -k, -n) with amplitude
+    (-1)^{l+k} conj(A) and harmonic Y_{l,-m}; one sample recomputed with 40-digit mpmath from the extended coefficients."""
+    mp = pytest.importorskip("mpmath")
+    w, yp, ym, ca, cp = _kerr_small(seed=2)
+    h = oracle.sum_waveform_kerr(w.t[0], ca, cp, w.l, w.m, w.k, w.n, None, yp, ym, w.t0, w.dt, w.n_samples)
+    le, me, ke, ne, ypl, cols = [], [], [], [], [], []
+    A = np.ascontiguousarray(w.amp[0])
+    for j in range(w.n_modes):
+        le.append(w.l[j]); me.append(w.m[j]); ke.append(w.k[j]); ne.append(w.n[j]); ypl.append(yp[j]); cols.append(A[:, j])
+        if w.m[j] > 0:
+            le.append(w.l[j]); me.append(-w.m[j]); ke.append(-w.k[j]); ne.append(-w.n[j]); ypl.append(ym[j])
+            cols.append((-1) ** int(w.l[j] + w.k[j]) * np.conj(A[:, j]))
+    ca2 = oracle.spline_fit(w.t[0], np.ascontiguousarray(np.stack(cols, axis=1)).view(np.float64))
+    h2 = oracle.sum_waveform_kerr(w.t[0], ca2, cp, le, me, ke, ne, None, np.array(ypl), None, w.t0, w.dt, w.n_samples, fold=False)
+    assert np.max(np.abs(h2 - h)) <= 1e-13 * np.max(np.abs(h))
+    # mpmath at one sample
+    mp.mp.dps = 40
+    i = 137
+    ti = w.t0 + i * w.dt
+    seg = int(np.searchsorted(w.t[0], ti, side="right") - 1)
+    dx = mp.mpf(float(ti - w.t[0][seg]))
+    horner = lambda c: ((c[3] * dx + c[2]) * dx + c[1]) * dx + c[0]
+    ld = lambda x: mp.mpf(float(x)) + mp.mpf(float(x - np.longdouble(float(x))))      # exact: 64-bit mantissa = two doubles
+    P = [horner([ld(cp[seg, p, q]) for p in range(4)]) for q in range(3)]
+    tot = mp.mpc(0)
+    for j in range(w.n_modes):
+        Ar = horner([mp.mpf(float(ca[seg, p, 2 * j])) for p in range(4)])
+        Ai = horner([mp.mpf(float(ca[seg, p, 2 * j + 1])) for p in range(4)])
+        th = int(w.m[j]) * P[0] + int(w.k[j]) * P[1] + int(w.n[j]) * P[2]
+        W = mp.mpc(Ar, Ai) * mp.expj(-th)
+        tot += mp.mpc(float(yp[j].real), float(yp[j].imag)) * W
+        if w.m[j] > 0:
+            tot += (-1) ** int(w.l[j] + w.k[j]) * mp.mpc(float(ym[j].real), float(ym[j].imag)) * mp.conj(W)
+    assert abs(complex(tot) - h[i]) <= 1e-13 * np.max(np.abs(h))
