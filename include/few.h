@@ -45,7 +45,7 @@ enum {
     FEW_ERR_INVALID_ARG = -1,     /* NULL pointer, non-positive size, bad flag */
     FEW_ERR_TOO_FEW_POINTS = -2,  /* n_t < 4: a not-a-knot cubic spline needs 4 knots */
     FEW_ERR_NOT_INCREASING = -3,  /* t not strictly increasing (reported by few_device_status) */
-    FEW_ERR_BAD_MODE = -4,        /* l < 2, |m| > l, m < 0, |n| > FEW_MAX_ABS_N, l > FEW_MAX_L (few_device_status / few_ylm) */
+    FEW_ERR_BAD_MODE = -4,        /* l < 2, |m| > l, m < 0, |n| > FEW_MAX_ABS_N, |k| > FEW_MAX_ABS_K, l > FEW_MAX_L (few_device_status / few_ylm) */
     FEW_ERR_WORKSPACE = -5,       /* workspace NULL, misaligned or smaller than the query says */
     FEW_ERR_CUDA = -6,            /* a CUDA runtime call failed; few_last_error() has the text */
     FEW_ERR_LIMIT = -7            /* size beyond a documented limit (FEW_MAX_*) */
@@ -56,6 +56,7 @@ enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
 
 #define FEW_MAX_L 16            /* l <= 16: the explicit Wigner-d sum in FP64 is accurate to 5e-15 for l <= 10 (the paper's range) and 1e-12 at l = 16 */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
+#define FEW_MAX_ABS_K 63        /* |k| <= 63 (polar index of Kerr-shaped mode lists, few_sum_waveform_kerr) */
 #define FEW_MAX_NT_SPLINE 736   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
 
@@ -141,6 +142,20 @@ int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, c
                         const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
                         double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
                         int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- NEXT-4: the summation for Kerr-shaped mode lists, Eq. (1) "Phi_mkn = m Phi_phi + k Phi_theta + n Phi_r",
+ * PAPER.md:438-444 Eq. (19) (spheroidal harmonics projected on -2Y_lm, so the harmonic constants stay S0's), Eq. (9) in full:
+ *   h_i = scale * factor * sum_{j kept} [ Y+_j W_j + (m_j > 0) (-1)^{l_j + k_j} Y-_j conj(W_j) ],
+ *   W_j = A_j(t_i) exp(-i(m_j Phi_phi + k_j Phi_theta + n_j Phi_r)).
+ * n_phase = 3: coef_phase_dd[n_src][n_t-1][4][3][2] from few_spline_fit_dd with n_sys = 3, systems (Phi_phi, Phi_theta, Phi_r);
+ * k[n_modes] int32, |k| <= FEW_MAX_ABS_K, or NULL (= 0).  n_phase = 2, k = NULL is few_sum_waveform_ex exactly.
+ * Kept lists longer than 16384 modes are ordered in the workspace instead of shared memory (same result).
+ * All other arguments, the workspace query and the error behaviour as few_sum_waveform_ex. */
+int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd, int n_phase,
+                          const int* l, const int* m, const int* k, const int* n, const int* keep_idx, const int* n_keep,
+                          const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                          double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                          int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- NEXT-1: detector (solar-system-barycentre) frame, sec. II A.
  * few_frame_constants: sky[n_src][4] = (theta_S, phi_S, theta_K, phi_K) (sky position, MBH spin direction; Eq. (4), (5));

@@ -22,7 +22,7 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
            "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
-           "few_sum_direct"]
+           "few_sum_direct", "few_sum_waveform_kerr"]
 
 
 class FewError(RuntimeError):
@@ -58,6 +58,7 @@ def _load() -> C.CDLL:
         "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
         "few_sum_waveform_ex": (i, [vp] * 13 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
+        "few_sum_waveform_kerr": (i, [vp, vp, vp, vp, i] + [vp] * 10 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
         "few_frame_constants": (i, [vp, vp, vp, i, vp, vp, vp, vp]),
         "few_frame_rotate": (i, [vp, vp, vp, i, ll, vp, vp]),
         "few_inner_products_workspace": (sz, [i, ll]),
@@ -212,6 +213,28 @@ def few_sum_waveform_ex(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, y
                                   _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale), _p(factor),
                                   float(t0), float(dt), int(n_samples), _p(h), _p(d), _p(inner), n_src, n_t, n_modes, _p(ws),
                                   ws.numel(), _stream()), "few_sum_waveform_ex")
+    return h, inner
+
+
+def few_sum_waveform_kerr(t, coef_amp, coef_phase_dd, l, m, k, n, keep_idx, n_keep, ylm_plus, ylm_minus, t0: float, dt: float,
+                          n_samples: int, scale=None, factor=None, d=None, want_inner: bool = False, want_h: bool = True,
+                          out=None, workspace=None):
+    """Summation for Kerr-shaped mode lists: coef_phase_dd [n_src, n_t-1, 4, n_phase, 2] with n_phase = 3 (Phi_phi, Phi_theta,
+    Phi_r) or 2; k [n_modes] i32 or None.  -> (h or None, inner or None)."""
+    n_src, n_t = t.shape
+    n_modes = l.shape[0]
+    n_phase = int(coef_phase_dd.shape[3])
+    h = None
+    if want_h:
+        h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
+    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    ws = workspace if workspace is not None else _ws(need, t.device)
+    _chk(_lib.few_sum_waveform_kerr(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
+                                    n_phase, _p(l, torch.int32), _p(m, torch.int32), _p(k), _p(n, torch.int32), _p(keep_idx),
+                                    _p(n_keep), _p(ylm_plus, torch.complex128), _p(ylm_minus, torch.complex128), _p(scale),
+                                    _p(factor), float(t0), float(dt), int(n_samples), _p(h), _p(d), _p(inner), n_src, n_t, n_modes,
+                                    _p(ws), ws.numel(), _stream()), "few_sum_waveform_kerr")
     return h, inner
 
 

@@ -27,6 +27,7 @@
 namespace {
 
 constexpr int kPlanThreads = 1024;
+constexpr int kPlanSmemElems = 16384;         // 128 KB of (key, mode) words: the plan kernel's in-shared-memory sort capacity
 constexpr int kSumThreads = 128;
 #ifndef FEW_SUM_R
 #define FEW_SUM_R 4
@@ -45,7 +46,8 @@ constexpr int kAdvShift = 1, kAdvBits = 12;   // number of E steps before this p
 constexpr int kNewSub = 1 << 13;              // restart E from Z_phi^m (n changes sign or m changes)
 constexpr int kDirNeg = 1 << 14;              // walk with conj(Z_r)
 constexpr int kDmShift = 15, kDmBits = 7;     // m increment of a new run
-constexpr int kNewRun = 1 << 22;
+constexpr int kNewRun = 1 << 22;               // new (m, k) run
+constexpr int kKShift = 23, kKBits = 7;       // polar index of the run, offset by 64 (Kerr-shaped lists, |k| <= FEW_MAX_ABS_K)
 
 struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
@@ -58,6 +60,8 @@ struct sum_layout {
     double* yfold;       // [n_src][n_modes][4] scale * (Y+ re, Y+ im, Ybar re, Ybar im) of sorted position r
     double* pack;        // [n_src][n_t - 1][max_stages][kStageBytes / 8]
     double* partial;     // [n_src][max_tiles][4]  per-tile sums of conj(d) h (re, im) and |h|^2 (fused inner products)
+    unsigned long long* sortbuf;   // [n_src][sort_pow2] plan-kernel sort array when the mode list exceeds shared memory (else empty)
+    int sort_pow2;
     int max_stages;
     int max_tiles;
 };
@@ -83,6 +87,10 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samp
     const long long mt = sum_max_tiles(n_samples, n_t);
     L.max_tiles = (int)(mt < 2147483647LL ? mt : 2147483647LL);
     L.partial = c.take<double>((size_t)n_src * (size_t)mt * 4);
+    int p2 = 1;
+    while (p2 < n_modes) p2 <<= 1;
+    L.sort_pow2 = p2 > kPlanSmemElems ? p2 : 0;
+    L.sortbuf = c.take<unsigned long long>((size_t)n_src * L.sort_pow2);
     if (bytes) *bytes = c.off;
     return L;
 }
@@ -123,20 +131,40 @@ __device__ __forceinline__ int plan_block_scan(int v, int* warp_sums, int* total
     return res;
 }
 
-// sort key: m | sign(n) | |n| | l  (ascending): runs of equal m, inside them n = 0, 1, 2, ... then -1, -2, ...
-__device__ __forceinline__ int key_m(unsigned k) { return (int)(k >> 21); }
-__device__ __forceinline__ int key_dir(unsigned k) { return (int)(k >> 20) & 1; }
-__device__ __forceinline__ int key_absn(unsigned k) { return (int)(k >> 8) & 0xfff; }
-__device__ __forceinline__ int key_l(unsigned k) { return (int)(k & 0xff); }
+// sort key: m | k + 64 | sign(n) | |n| | l  (ascending): runs of equal (m, k), inside them n = 0, 1, 2, ... then -1, -2, ...
+__device__ __forceinline__ int key_m(unsigned k) { return (int)(k >> 25); }
+__device__ __forceinline__ int key_k(unsigned k) { return (int)((k >> 18) & 0x7f) - 64; }
+__device__ __forceinline__ unsigned key_run(unsigned k) { return k >> 18; }
+__device__ __forceinline__ int key_dir(unsigned k) { return (int)(k >> 17) & 1; }
+__device__ __forceinline__ int key_absn(unsigned k) { return (int)(k >> 5) & 0xfff; }
+__device__ __forceinline__ int key_l(unsigned k) { return (int)(k & 0x1f); }
+
+// Bitonic compare-exchange steps on buf[0, n) (n a power of two), which holds elements [c0, c0 + n) of the whole array: for
+// size = size_first, 2 size_first, ..., size_last the strides min(size, n)/2 ... 1.  Direction from the GLOBAL index.
+__device__ void plan_bitonic_steps(unsigned long long* buf, int c0, int n, int size_first, int size_last)
+{
+    for (int size = size_first; size <= size_last; size <<= 1) {
+        for (int stride = (size < n ? size : n) >> 1; stride > 0; stride >>= 1) {
+            for (int q = threadIdx.x; q < (n >> 1); q += kPlanThreads) {
+                const int lo = ((q & ~(stride - 1)) << 1) | (q & (stride - 1)), hi = lo | stride;
+                const unsigned long long a = buf[lo], b = buf[hi];
+                const bool up = ((lo + c0) & size) == 0;
+                if ((a > b) == up) { buf[lo] = b; buf[hi] = a; }
+            }
+            __syncthreads();
+        }
+    }
+}
 
 __global__ void __launch_bounds__(kPlanThreads, 1)
 few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l, const int* __restrict__ m,
-                    const int* __restrict__ n, const int* __restrict__ keep_idx, const int* __restrict__ n_keep,
+                    const int* __restrict__ kpol, const int* __restrict__ n, const int* __restrict__ keep_idx, const int* __restrict__ n_keep,
                     const double2* __restrict__ ylm_plus, const double2* __restrict__ ylm_minus,
                     const double* __restrict__ scale, const double2* __restrict__ factor, double t0, double dt, long long N,
-                    int n_t, int n_modes, sum_layout L, int* status)
+                    int n_t, int n_modes, int smem_elems, sum_layout L, int* status)
 {
-    extern __shared__ unsigned long long plan_sorted[];           // [n_pow2] (key << 32 | mode index), sorted ascending
+    extern __shared__ unsigned long long plan_smem[];             // [smem_elems]
+    unsigned long long* plan_sorted;                              // [n_pow2] (key << 32 | mode index), sorted ascending
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
 
@@ -168,32 +196,53 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
 
     // ---- (b) kept modes -> keys
     const int K = n_keep ? min(max(n_keep[src], 0), n_modes) : n_modes;
+    int n_pow2 = 1;
+    while (n_pow2 < K) n_pow2 <<= 1;
+    // the sort runs in shared memory when the kept list fits (always for the Schwarzschild grid), else in the workspace with
+    // the short-stride steps done chunk by chunk in shared memory (Kerr-shaped lists with > 16384 kept modes)
+    const bool in_smem = n_pow2 <= smem_elems;
+    plan_sorted = in_smem ? plan_smem : L.sortbuf + (size_t)src * L.sort_pow2;
     for (int q = tid; q < K; q += kPlanThreads) {
         int j = keep_idx ? keep_idx[(size_t)src * n_modes + q] : q;
         bool ok = j >= 0 && j < n_modes;
-        int lj = ok ? l[j] : 2, mj = ok ? m[j] : 0, nj = ok ? n[j] : 0;
+        int lj = ok ? l[j] : 2, mj = ok ? m[j] : 0, nj = ok ? n[j] : 0, kj = (ok && kpol) ? kpol[j] : 0;
         int an = nj < 0 ? -nj : nj;
-        if (!ok || lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj || an > FEW_MAX_ABS_N) {
+        if (!ok || lj < 2 || lj > FEW_MAX_L || mj < 0 || mj > lj || an > FEW_MAX_ABS_N || kj < -FEW_MAX_ABS_K || kj > FEW_MAX_ABS_K) {
             atomicOr(status, FEW_DEV_BAD_MODE);
-            lj = 2; mj = 0; an = 0; nj = 0; j = ok ? j : 0;
+            lj = 2; mj = 0; an = 0; nj = 0; kj = 0; j = ok ? j : 0;
         }
-        const unsigned key = ((unsigned)mj << 21) | ((nj < 0 ? 1u : 0u) << 20) | ((unsigned)an << 8) | (unsigned)lj;
+        const unsigned key = ((unsigned)mj << 25) | ((unsigned)(kj + 64) << 18) | ((nj < 0 ? 1u : 0u) << 17) | ((unsigned)an << 5) |
+                             (unsigned)lj;
         plan_sorted[q] = ((unsigned long long)key << 32) | (unsigned)j;
     }
-    int n_pow2 = 1;
-    while (n_pow2 < K) n_pow2 <<= 1;
     for (int q = K + tid; q < n_pow2; q += kPlanThreads) plan_sorted[q] = ~0ull;      // padding sorts to the end
     __syncthreads();
-    // ---- (c) bitonic sort in shared memory (keys are unique for a valid mode list; duplicates order by mode index)
-    for (int size = 2; size <= n_pow2; size <<= 1) {
-        for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            for (int q = tid; q < (n_pow2 >> 1); q += kPlanThreads) {
-                const int lo = ((q & ~(stride - 1)) << 1) | (q & (stride - 1)), hi = lo | stride;
-                const unsigned long long a = plan_sorted[lo], b = plan_sorted[hi];
-                const bool up = (lo & size) == 0;
-                if ((a > b) == up) { plan_sorted[lo] = b; plan_sorted[hi] = a; }
+    // ---- (c) bitonic sort (keys are unique for a valid mode list; duplicates order by mode index)
+    if (in_smem) {
+        plan_bitonic_steps(plan_sorted, 0, n_pow2, 2, n_pow2);
+    } else {
+        const int CH = smem_elems;
+        auto chunk_pass = [&](int size_first, int size_last) {
+            for (int c0 = 0; c0 < n_pow2; c0 += CH) {
+                for (int q = tid; q < CH; q += kPlanThreads) plan_smem[q] = plan_sorted[c0 + q];
+                __syncthreads();
+                plan_bitonic_steps(plan_smem, c0, CH, size_first, size_last);
+                for (int q = tid; q < CH; q += kPlanThreads) plan_sorted[c0 + q] = plan_smem[q];
+                __syncthreads();
             }
-            __syncthreads();
+        };
+        chunk_pass(2, CH);
+        for (int size = 2 * CH; size <= n_pow2; size <<= 1) {
+            for (int stride = size >> 1; stride >= CH; stride >>= 1) {             // long strides: straight through L2
+                for (int q = tid; q < (n_pow2 >> 1); q += kPlanThreads) {
+                    const int lo = ((q & ~(stride - 1)) << 1) | (q & (stride - 1)), hi = lo | stride;
+                    const unsigned long long a = plan_sorted[lo], b = plan_sorted[hi];
+                    const bool up = (lo & size) == 0;
+                    if ((a > b) == up) { plan_sorted[lo] = b; plan_sorted[hi] = a; }
+                }
+                __syncthreads();
+            }
+            chunk_pass(size, size);
         }
     }
     // ---- (d) pairs: chunked scan of "new (m, n)" flags; descriptors; per-mode fold constants
@@ -213,7 +262,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         unsigned key = 0, prev = 0;
         if (r < K) {
             key = (unsigned)(plan_sorted[r] >> 32); prev = r ? (unsigned)(plan_sorted[r - 1] >> 32) : 0u;
-            new_run = r == 0 || key_m(key) != key_m(prev);
+            new_run = r == 0 || key_run(key) != key_run(prev);
             new_sub = new_run || key_dir(key) != key_dir(prev);
             new_grp = new_sub || key_absn(key) != key_absn(prev);
         }
@@ -227,15 +276,15 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
                 int nadv = new_sub ? key_absn(key) : key_absn(key) - key_absn(prev);
                 int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
                 int d = (nadv << kAdvShift) | (new_sub ? kNewSub : 0) | (key_dir(key) ? kDirNeg : 0) | (dm << kDmShift) |
-                        (new_run ? kNewRun : 0);
+                        (new_run ? kNewRun : 0) | ((key_k(key) + 64) << kKShift);
                 if (new_sub || nadv != 1) d |= 1;
                 desc[g] = d;
                 gfirst[g] = r;
             }
             double2 yp = ylm_plus[(size_t)src * n_modes + j], yb = make_double2(0.0, 0.0);
-            if (key_m(key) > 0) {                       // Eq. (9): the (l,-m,-n) mirror, Ybar = (-1)^l Y_{l,-m}
+            if (key_m(key) > 0) {                       // Eq. (9): the (l,-m,-k,-n) mirror, Ybar = (-1)^(l+k) Y_{l,-m}
                 double2 ym = ylm_minus[(size_t)src * n_modes + j];
-                double sg = (key_l(key) & 1) ? -1.0 : 1.0;
+                double sg = ((key_l(key) + key_k(key)) & 1) ? -1.0 : 1.0;
                 yb = make_double2(sg * ym.x, sg * ym.y);
             }
             yf[4 * r] = fc.x * yp.x - fc.y * yp.y; yf[4 * r + 1] = fc.x * yp.y + fc.y * yp.x;
@@ -373,7 +422,9 @@ __device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, 
     }
 }
 
-template <int R, int kBlocksPerSm, bool kInner>
+// kKerr: Kerr-shaped mode lists (Eq. (1), Eq. (19)): a third phase factor Z_theta and runs of equal (m, k) with
+// E restarting from Z_phi^m Z_theta^k; two more per-thread stashes live in dynamic shared memory.  The hot loop is the same.
+template <int R, int kBlocksPerSm, bool kInner, bool kKerr>
 __global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
                int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all)
@@ -384,6 +435,8 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
     __shared__ int tile_s;
     __shared__ double red_s[3][kSumThreads / 32];
+    extern __shared__ double2 stash_dyn[];      // kKerr: [R][kSumThreads] Z_theta, then [R][kSumThreads] Z_phi^m Z_theta^k
+    constexpr int n_ph = kKerr ? 3 : 2;
 
     const int tid = threadIdx.x, n_seg = n_t - 1;
     if (tid == 0) {
@@ -439,7 +492,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
 
     // ---- per-sample setup (overlaps the first copies): dx and the two phase factors
     const double tk = t_all[(size_t)src * n_t + k];
-    const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 8;     // [4][2] dd
+    const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 4 * n_ph;     // [4][n_ph] dd
     double zrr[R], zri[R], er[R], ei[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -447,8 +500,14 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         if (i >= i_end) i = i_end - 1;                              // tail lanes recompute the last sample, never store
         const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
         double zpr, zpi;
-        phase_factor(cph + 0, 2, dx, &zpr, &zpi);
-        phase_factor(cph + 1, 2, dx, &zrr[r], &zri[r]);
+        phase_factor(cph + 0, n_ph, dx, &zpr, &zpi);
+        phase_factor(cph + n_ph - 1, n_ph, dx, &zrr[r], &zri[r]);
+        if (kKerr) {
+            double ztr, zti;
+            phase_factor(cph + 1, n_ph, dx, &ztr, &zti);
+            stash_dyn[r * kSumThreads + tid] = make_double2(ztr, zti);
+            stash_dyn[(R + r) * kSumThreads + tid] = make_double2(1.0, 0.0);
+        }
         // Z_phi and the run's Z_phi^m are needed only when m or the sign of n changes: parked in shared memory, not registers
         stash_zp[r][tid] = make_double2(zpr, zpi);
         stash_pm[r][tid] = make_double2(1.0, 0.0);
@@ -499,13 +558,24 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                             pm.x = a;
                         }
                         stash_pm[r][tid] = pm;
+                        if (kKerr) {                                // base of the run: Z_phi^m Z_theta^k (k < 0: conjugate powers)
+                            const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                            double2 zt = stash_dyn[r * kSumThreads + tid];
+                            if (kk < 0) zt.y = -zt.y;
+                            for (int q = 0; q < (kk < 0 ? -kk : kk); ++q) {
+                                double a = pm.x * zt.x - pm.y * zt.y;
+                                pm.y = pm.x * zt.y + pm.y * zt.x;
+                                pm.x = a;
+                            }
+                            stash_dyn[(R + r) * kSumThreads + tid] = pm;
+                        }
                     }
                 }
                 if (d & kNewSub) {
                     const bool want_neg = (d & kDirNeg) != 0;
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        const double2 pm = stash_pm[r][tid];
+                        const double2 pm = kKerr ? stash_dyn[(R + r) * kSumThreads + tid] : stash_pm[r][tid];
                         er[r] = pm.x; ei[r] = pm.y;
                         if (want_neg != neg) zri[r] = -zri[r];
                     }
@@ -585,11 +655,11 @@ few_sum_inner_kernel(sum_layout L, int n_t, int max_tiles, double dt, double* __
     }
 }
 
-size_t plan_smem_bytes(int n_modes)
+int plan_smem_elems(int n_modes)
 {
-    size_t p = 1;
-    while (p < (size_t)n_modes) p <<= 1;
-    return p * 8;
+    int p = 1;
+    while (p < n_modes) p <<= 1;
+    return p < kPlanSmemElems ? p : kPlanSmemElems;
 }
 
 }  // namespace
@@ -602,12 +672,14 @@ extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, lo
     return bytes;
 }
 
-extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
-                                   const int* l, const int* m, const int* n, const int* keep_idx, const int* n_keep,
-                                   const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
-                                   double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
-                                   int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
+extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd, int n_phase,
+                                     const int* l, const int* m, const int* k, const int* n, const int* keep_idx, const int* n_keep,
+                                     const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                                     double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                                     int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
 {
+    FEW_REQUIRE(n_phase == 2 || n_phase == 3, FEW_ERR_INVALID_ARG, "n_phase must be 2 (Phi_phi, Phi_r) or 3 (Phi_phi, Phi_theta, Phi_r)");
+    FEW_REQUIRE(n_phase == 3 || k == nullptr, FEW_ERR_INVALID_ARG, "a polar index k needs the third phase (n_phase = 3)");
     FEW_REQUIRE(ctx && t && coef_amp && coef_phase_dd && l && m && n && ylm_plus && ylm_minus, FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE((keep_idx == nullptr) == (n_keep == nullptr), FEW_ERR_INVALID_ARG, "keep_idx and n_keep must both be NULL or both be set");
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
@@ -624,16 +696,17 @@ extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* 
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
                     workspace_bytes >= few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
-    size_t psm = plan_smem_bytes(n_modes);
-    FEW_REQUIRE(psm <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "n_modes too large for the plan kernel's shared memory");
+    const int plan_elems = plan_smem_elems(n_modes);
+    const size_t psm = (size_t)plan_elems * 8;
+    FEW_REQUIRE(psm <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "plan kernel's shared memory exceeds the device limit");
     long long max_tiles = sum_max_tiles(n_samples, n_t);
     FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
     sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
 
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-    few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, n, keep_idx, n_keep, (const double2*)ylm_plus,
+    few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
-                                                          n_t, n_modes, L, ctx->d_status);
+                                                          n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
     few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 1024, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
@@ -641,12 +714,20 @@ extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* 
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
     const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
     const unsigned grid = (unsigned)(want < resident ? want : resident);
-    if (inner)
-        few_sum_kernel<kSumR, kSumBlocksPerSm, true><<<grid, kSumThreads, 0, st>>>(
-            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, (const double2*)d);
-    else
-        few_sum_kernel<kSumR, kSumBlocksPerSm, false><<<grid, kSumThreads, 0, st>>>(
-            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, nullptr);
+    const size_t kerr_smem = 2 * (size_t)kSumR * kSumThreads * sizeof(double2);      // Z_theta and run-base stashes
+#define FEW_SUM_LAUNCH(INNER, KERR, SMEM, DPTR)                                                                                   \
+    few_sum_kernel<kSumR, kSumBlocksPerSm, INNER, KERR><<<grid, kSumThreads, SMEM, st>>>(                                         \
+        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, DPTR)
+    if (n_phase == 3) {     // static + dynamic shared memory exceeds the 48 KB default: opt in
+        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_kernel<kSumR, kSumBlocksPerSm, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kerr_smem));
+        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_kernel<kSumR, kSumBlocksPerSm, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kerr_smem));
+        if (inner) FEW_SUM_LAUNCH(true, true, kerr_smem, (const double2*)d);
+        else FEW_SUM_LAUNCH(false, true, kerr_smem, nullptr);
+    } else {
+        if (inner) FEW_SUM_LAUNCH(true, false, 0, (const double2*)d);
+        else FEW_SUM_LAUNCH(false, false, 0, nullptr);
+    }
+#undef FEW_SUM_LAUNCH
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     if (inner) {
@@ -654,6 +735,16 @@ extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* 
         FEW_CUDA_CHECK(cudaGetLastError());
     }
     return FEW_OK;
+}
+
+extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,
+                                   const int* l, const int* m, const int* n, const int* keep_idx, const int* n_keep,
+                                   const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                                   double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                                   int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return few_sum_waveform_kerr(ctx, t, coef_amp, coef_phase_dd, 2, l, m, nullptr, n, keep_idx, n_keep, ylm_plus, ylm_minus, scale,
+                                 factor, t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, workspace, workspace_bytes, stream);
 }
 
 extern "C" int few_sum_waveform(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,

@@ -302,3 +302,69 @@ def test_direct_equals_interpolated_on_dense_spline_values(api):
     yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), dev(w.l), dev(w.m))
     h_dir = api.few_sum_direct(dev(A[None]), dev(ph[None]), dev(w.l), dev(w.m), dev(w.n), yp, ym).cpu().numpy()[0]
     assert rel_l2(h_dir, h_int) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------- NEXT-4 (summation part)
+def kerr_gpu_and_oracle(api, w, keep=None, theta=0.7, phi=1.1):
+    """S0 + S1 (amplitudes FP64, three phases double-double) + Kerr-shaped S3 on the GPU; O2 + O1 + O8 on the CPU."""
+    th, ph = dev(np.array([theta])), dev(np.array([phi]))
+    yp, ym = api.few_ylm_modes(th, ph, dev(w.l), dev(w.m))
+    coef = api.few_spline_fit(dev(w.t), dev(w.amp))
+    cdd = api.few_spline_fit_dd(dev(w.t), dev(w.phase))
+    assert cdd.shape[3] == 3
+    kd = nk = None
+    if keep is not None:
+        pad = np.full((1, w.n_modes), -1, np.int32); pad[0, : len(keep)] = keep
+        kd, nk = dev(pad), dev(np.array([len(keep)], np.int32))
+    h, _ = api.few_sum_waveform_kerr(dev(w.t), coef, cdd, dev(w.l), dev(w.m), dev(w.k), dev(w.n), kd, nk, yp, ym, w.t0, w.dt, w.n_samples)
+    api.few_device_status()
+    ryp, rym = oracle.ylm_modes(w.l, w.m, theta, phi)
+    ca = oracle.spline_fit(w.t[0], np.ascontiguousarray(w.amp[0]).view(np.float64))
+    cp = oracle.spline_fit_ext(w.t[0], w.phase[0])
+    ref = oracle.sum_waveform_kerr(w.t[0], ca, cp, w.l, w.m, w.k, w.n, keep, ryp, rym, w.t0, w.dt, w.n_samples)
+    return h.cpu().numpy()[0], ref
+
+
+def test_kerr_sum_small_all_modes(api):
+    w = synth.make_kerr(n_samples=3000, n_t=30, l_max=4, k_max=2, n_max=3, t0=20_000_000.0)
+    h, ref = kerr_gpu_and_oracle(api, w)
+    assert rel_l2(h, ref) <= REL_L2_TOL and mismatch(h, ref) <= MISMATCH_TOL
+    assert np.max(np.abs(h - ref)) <= 1e-10 * np.max(np.abs(ref))
+
+
+def test_kerr_sum_full_grid_sorted_in_workspace(api):
+    """All 42 273 modes of the Kerr-shaped grid: the kept list (65 536 padded) exceeds the plan kernel's shared memory, so the
+    ordering runs through the workspace; 7381 (m, k, n) runs of E."""
+    w = synth.make_kerr(n_samples=700, t0=15_000_000.0)
+    assert w.n_modes == 42273
+    h, ref = kerr_gpu_and_oracle(api, w)
+    assert rel_l2(h, ref) <= REL_L2_TOL and mismatch(h, ref) <= MISMATCH_TOL
+
+
+@pytest.mark.parametrize("n_keep", [5000, 20000])
+def test_kerr_sum_kept_subsets(api, n_keep):
+    """Random kept subsets with gaps in k and n: 5000 sorts in shared memory, 20 000 (32 768 padded) through the workspace."""
+    w = synth.make_kerr(n_samples=600, t0=3_000_000.0)
+    keep = np.sort(np.random.default_rng(n_keep).choice(w.n_modes, n_keep, replace=False)).astype(np.int32)
+    h, ref = kerr_gpu_and_oracle(api, w, keep=keep, theta=2.0, phi=5.0)
+    assert rel_l2(h, ref) <= REL_L2_TOL and mismatch(h, ref) <= MISMATCH_TOL
+
+
+def test_kerr_sum_reduces_to_schwarzschild_path(api):
+    """n_phase = 2, k = NULL gives few_sum_waveform's bits; k = 0 with three phases gives the same waveform to rounding."""
+    w = synth.make_config(1, n_samples=4000, t0=9_000_000.0)
+    g = dict(t=dev(w.t), l=dev(w.l), m=dev(w.m), n=dev(w.n))
+    yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), g["l"], g["m"])
+    coef = api.few_spline_fit(g["t"], dev(w.amp))
+    c2 = api.few_spline_fit_dd(g["t"], dev(w.phase))
+    h_ref = api.few_sum_waveform(g["t"], coef, c2, g["l"], g["m"], g["n"], None, None, yp, ym, w.t0, w.dt, w.n_samples).cpu().numpy()
+    h2, _ = api.few_sum_waveform_kerr(g["t"], coef, c2, g["l"], g["m"], None, g["n"], None, None, yp, ym, w.t0, w.dt, w.n_samples)
+    assert np.array_equal(h2.cpu().numpy(), h_ref)
+    ph3 = np.stack([w.phase[..., 0], 0.77 * w.phase[..., 0], w.phase[..., 1]], axis=-1)
+    c3 = api.few_spline_fit_dd(g["t"], dev(ph3))
+    k0 = dev(np.zeros(w.n_modes, np.int32))
+    h3, _ = api.few_sum_waveform_kerr(g["t"], coef, c3, g["l"], g["m"], k0, g["n"], None, None, yp, ym, w.t0, w.dt, w.n_samples)
+    assert rel_l2(h3.cpu().numpy()[0], h_ref[0]) <= 1e-13
+    bad = np.zeros(w.n_modes, np.int32); bad[5] = 64
+    api.few_sum_waveform_kerr(g["t"], coef, c3, g["l"], g["m"], dev(bad), g["n"], None, None, yp, ym, w.t0, w.dt, 16)
+    assert api.few_device_status(raise_on_error=False) != 0
