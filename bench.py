@@ -58,7 +58,7 @@ class ClockSampler:
     def _run(self):
         try:
             proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                     "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                     "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             return
         try:
@@ -202,6 +202,34 @@ def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: i
     out["direct_sum"] = {"ms": ms, "n_samples": N, "n_modes": K, "algorithmic_bytes": nb, "gbs": nb / ms / 1e6,
                          "hbm_frac": nb / ms / 1e6 / hbm_gbs, "evals_per_s": N * K / (ms * 1e-3),
                          "note": "16 B per sample*mode evaluation; L2 flushed; inputs 16 GB >> L2"}
+    del amp, hd, phase
+    # Kerr-shaped list (NEXT-4, summation part): 42 273 modes = 7381 (m, k, n) triples, third phase, one year at dt = 10 s;
+    # all modes, then the 4000 strongest at mid-trajectory (a kept list of the size selection would hand over)
+    wk = synth.make_kerr()
+    tk = torch.as_tensor(wk.t).to(dev)
+    coef = api.few_spline_fit(tk, torch.as_tensor(wk.amp).to(dev))
+    cdd = api.few_spline_fit_dd(tk, torch.as_tensor(wk.phase).to(dev))
+    lk, mk, kk, nk_ = (torch.as_tensor(x).to(dev) for x in (wk.l, wk.m, wk.k, wk.n))
+    ypk, ymk = api.few_ylm_modes(g["theta"][:1], g["phi"][:1], lk, mk)
+    hk = torch.empty((1, wk.n_samples), dtype=torch.complex128, device=dev)
+    kws = torch.empty(api._lib.few_sum_waveform_workspace(1, wk.n_t, wk.n_modes, wk.n_samples), dtype=torch.uint8, device=dev)
+    out["kerr_shaped_sum"] = {}
+    for label, n_keep in (("all_modes", None), ("kept_4000", 4000)):
+        keep = nkeep = None
+        triples = len({(int(a), int(b), int(c)) for a, b, c in zip(wk.m, wk.k, wk.n)})
+        if n_keep is not None:
+            idx = np.sort(np.argsort(-np.abs(wk.amp[0, wk.n_t // 2]))[:n_keep]).astype(np.int32)
+            pad = np.full((1, wk.n_modes), -1, np.int32); pad[0, :n_keep] = idx
+            keep, nkeep = torch.as_tensor(pad).to(dev), torch.as_tensor(np.array([n_keep], np.int32)).to(dev)
+            triples = len({(int(wk.m[j]), int(wk.k[j]), int(wk.n[j])) for j in idx})
+        api.few_profile_enable(True)
+        ms = timed(lambda: api.few_sum_waveform_kerr(tk, coef, cdd, lk, mk, kk, nk_, keep, nkeep, ypk, ymk, wk.t0, wk.dt, wk.n_samples,
+                                                     out=hk, workspace=kws))
+        kern_ms = api.few_profile_sum_ms()
+        K = wk.n_modes if n_keep is None else n_keep
+        fl = FLOP_PER_PAIR * wk.n_samples * triples
+        out["kerr_shaped_sum"][label] = {"ms": ms, "sum_kernel_ms": kern_ms, "kept_modes": K, "mkn_triples": triples,
+                                         "evals_per_s": wk.n_samples * K / (ms * 1e-3), "tflops_executed": fl / (kern_ms * 1e-3) / 1e12}
     return out
 
 
@@ -300,6 +328,13 @@ def main():
     probe_flops = api.few_fp64_peak_probe(148 * 8, 256, 20000, sink)
     e1.record(); torch.cuda.synchronize()
     fp64_measured_tflops = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
+    # the hot loop's own instruction mix (72 DFMA + 8 DMUL per pair step, coefficients from shared memory) and nothing else,
+    # at the sum kernel's launch shape (3 blocks of 128 threads per SM): the ceiling of that instruction form on this chip
+    api.few_fp64_mix_probe(148 * 3, 2000, sink)
+    torch.cuda.synchronize(); e0.record()
+    mix_flops = api.few_fp64_mix_probe(148 * 3, 20000, sink)
+    e1.record(); torch.cuda.synchronize()
+    fp64_mix_tflops = mix_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
 
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
@@ -372,6 +407,7 @@ def main():
                 "traffic": SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if args.eps is None else None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
+                "peak_measured_hot_mix_probe": fp64_mix_tflops, "frac_of_hot_mix_probe": achieved_tflops / fp64_mix_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
                 "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {pair_evals_per_step:.4g} "
                                f"pair evaluations per launch ({pairs} pairs from {K_kept} kept modes)",

@@ -223,6 +223,13 @@ int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_ho
  * to sink[blocks*threads].  FLOPs = 2 * 16 * iters * blocks * threads. */
 int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double* sink, void* stream);
 
+/* ---- Measurement aid: the instruction mix of few_sum_kernel's hot loop and nothing else: `blocks` x 128
+ * threads, each running `iters` pair steps for 4 samples = 72 DFMA + 8 DMUL per step, the 8 complex coefficients of a step
+ * read from shared memory with broadcast 128-bit loads.  seed[16] (device) fills the coefficient table; one double per thread
+ * is written to sink[blocks*128].  FLOPs = 152 * iters * blocks * 128.  What it sustains is the ceiling of this instruction
+ * form (three register operands per DFMA) on the device, below the register-resident DFMA-chain figure. */
+int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream);
+
 /* ---- Measurement aid: with profiling on, few_sum_waveform (also inside few_waveform) brackets its hot kernel
  * (few_sum_kernel, the dominant launch of the path) with two CUDA events on the caller's stream.  few_profile_sum_ms
  * waits for the closing event of the most recent launch and writes its duration in milliseconds to ms_host.

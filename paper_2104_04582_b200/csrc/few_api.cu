@@ -345,3 +345,63 @@ extern "C" int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int it
     FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// FP64 instruction-mix probe: the hot loop of few_sum_kernel stripped of everything else -- per (m, n) pair and thread, for
+// 4 samples, E <- E Z_r (8 DMUL + 8 DFMA) and acc_p += e_r U_p + e_i V_p (64 DFMA) with the 8 complex coefficients read from
+// shared memory by broadcast 128-bit loads, 128 threads per block.  What this sustains is the ceiling of that instruction form
+// (three register operands per DFMA, one of them block-uniform) on this chip; DESIGN.md section 5.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) few_fp64_mix_kernel(int iters, double* sink, const double* seed)
+{
+    __shared__ __align__(16) double2 cs[256];
+    for (int i = threadIdx.x; i < 256; i += 128) cs[i] = make_double2(seed[(2 * i) & 15] * (1 + i), seed[(2 * i + 1) & 15] * (1 + i));
+    __syncthreads();
+    constexpr int R = 4;
+    double are[4][R], aim[4][R], er[R], ei[R], zr[R], zi[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        sincos(1e-3 * (threadIdx.x + 128 * r + 1), &zi[r], &zr[r]);
+        er[r] = 1.0; ei[r] = 0.0;
+    }
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < R; ++r) are[p][r] = aim[p][r] = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        const double2* cp = cs + (it & 31) * 8;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double m1 = ei[r] * zi[r], m2 = ei[r] * zr[r], e0 = er[r];
+            er[r] = fma(e0, zr[r], -m1);
+            ei[r] = fma(e0, zi[r], m2);
+        }
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const double2 u = cp[p];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { are[p][r] = fma(er[r], u.x, are[p][r]); aim[p][r] = fma(er[r], u.y, aim[p][r]); }
+        }
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const double2 v = cp[4 + p];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { are[p][r] = fma(ei[r], v.x, are[p][r]); aim[p][r] = fma(ei[r], v.y, aim[p][r]); }
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < R; ++r) s += are[p][r] + aim[p][r];
+    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream)
+{
+    FEW_REQUIRE(ctx && sink && seed, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(blocks > 0 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
+    few_fp64_mix_kernel<<<blocks, 128, 0, (cudaStream_t)stream>>>(iters, sink, seed);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    return FEW_OK;
+}
