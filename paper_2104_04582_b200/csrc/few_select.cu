@@ -37,11 +37,15 @@ struct sel_layout {
     int* n_entries;   // [1]
     double* y2;       // [n_src][2 n_modes]  |Y|^2 per entry
     unsigned* bitmap; // [n_src][words]
+    int* mirror_e;    // [n_modes]   entry index of the mirror of mode j, -1 if it has none   (shared by sources)
+    double* y2m;      // [n_src][n_modes]    |Y_{l,-m}|^2 by mode (the mirror's weight beside the primary's)
+    int* fb_list;     // [n_src * n_t]       rows left to the general kernel by the fast one
+    int* fb_count;    // [1]
 };
 
 __host__ __device__ inline int sel_words(int n_modes) { return (n_modes + 31) / 32; }
 
-sel_layout sel_carve(void* ws, int n_src, int n_modes, size_t* bytes = nullptr)
+sel_layout sel_carve(void* ws, int n_src, int n_t, int n_modes, size_t* bytes = nullptr)
 {
     few_carver c(ws);
     sel_layout L;
@@ -49,6 +53,10 @@ sel_layout sel_carve(void* ws, int n_src, int n_modes, size_t* bytes = nullptr)
     L.n_entries = c.take<int>(1);
     L.y2 = c.take<double>((size_t)n_src * 2 * n_modes);
     L.bitmap = c.take<unsigned>((size_t)n_src * sel_words(n_modes));
+    L.mirror_e = c.take<int>(n_modes);
+    L.y2m = c.take<double>((size_t)n_src * n_modes);
+    L.fb_list = c.take<int>((size_t)n_src * n_t);
+    L.fb_count = c.take<int>(1);
     if (bytes) *bytes = c.off;
     return L;
 }
@@ -95,18 +103,22 @@ few_select_prepare_kernel(const int* __restrict__ m, const double2* __restrict__
         if (j < n_modes) {
             double2 yp = with_y ? ylm_plus[(size_t)src * n_modes + j] : make_double2(1.0, 0.0);
             y2[j] = __dadd_rn(__dmul_rn(yp.x, yp.x), __dmul_rn(yp.y, yp.y));
+            double w_m = 0.0;
             if (flag) {
                 int e = carry + incl - 1;
                 if (src == 0) L.owner[e] = j;
                 double2 ym = ylm_minus[(size_t)src * n_modes + j];
-                y2[n_modes + e] = __dadd_rn(__dmul_rn(ym.x, ym.x), __dmul_rn(ym.y, ym.y));
+                w_m = __dadd_rn(__dmul_rn(ym.x, ym.x), __dmul_rn(ym.y, ym.y));
+                y2[n_modes + e] = w_m;
             }
+            if (src == 0) L.mirror_e[j] = flag ? n_modes + carry + incl - 1 : -1;
+            L.y2m[(size_t)src * n_modes + j] = w_m;
         }
         __syncthreads();
         if (tid == 0) carry_s = carry + total;
         __syncthreads();
     }
-    if (src == 0 && tid == 0) *L.n_entries = n_modes + carry_s;
+    if (src == 0 && tid == 0) { *L.n_entries = n_modes + carry_s; *L.fb_count = 0; }
     for (int w = tid; w < sel_words(n_modes); w += kPrepThreads) L.bitmap[(size_t)src * sel_words(n_modes) + w] = 0u;
 }
 
@@ -148,31 +160,174 @@ __device__ __forceinline__ long long block_max_ll(long long v, sel_red& s, int& 
     return r;
 }
 
-// One (source, step) row.  Register slot i of thread tid holds primary entry j = i*256 + tid for i < NP = ceil(n_modes/256)
-// and mirror entry n_modes + (i - NP)*256 + tid after that, so every global load of the row is coalesced and independent
-// of the others; |A|^2 goes through shared memory once so that the mirrors need no second, dependent gather from HBM.
+// ---- shared state of one row's selection
+struct sel_shared {
+    sel_red red;
+    unsigned bitmap[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
+    double bkt_p[kBucketMax], srt_p[kBucketMax];
+    int bkt_e[kBucketMax], srt_e[kBucketMax];
+    int bkt_count;
+};
+
+// The selection proper, on entry powers held in registers: key[i] = bit pattern of the power of the thread's i-th entry (-1 =
+// empty slot), entry_of(i) its entry index, thr = (1 - eps) * (total power of the row) > 0 or <= 0 for the degenerate case.
+// The entries passed need not be the whole row: any superset of the kept entries whose total is >= thr gives the same set,
+// because C_{r-1} of an entry is the summed power of the entries before it in the order and every such entry is itself kept.
+// Marks the owners of the kept entries in S.bitmap (caller zeroes it and S.bkt_count, then __syncthreads).
+template <int EPT, class EntOf>
+__device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf entry_of, double thr, int b_lo, int b_hi, int n_modes,
+                                            const int* __restrict__ owner, sel_shared& S, int& slot)
+{
+    const int tid = threadIdx.x;
+    long long kappa;            // kept  <=>  key > kappa  or  (key == kappa and entry index <= iota)
+    int iota = 0x7fffffff;
+    if (!(thr > 0.0)) {
+        // eps >= 1 or an all-zero row: only rank 0 survives, i.e. the largest power with the lowest entry index
+        long long kmax_local = -1;
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) kmax_local = key[i] > kmax_local ? key[i] : kmax_local;
+        kappa = block_max_ll(kmax_local, S.red, slot);
+        long long best = -0x7fffffff;       // max of -index
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) if (key[i] == kappa) { long long c = -(long long)entry_of(i); best = c > best ? c : best; }
+        iota = (int)(-block_max_ll(best, S.red, slot));
+    } else {
+        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x and
+        // g(0) = total >= thr; B = the largest x with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
+        // The bucket is searched in [b_lo, b_hi] (the caller knows that g(b_lo) >= thr and that no key lies above bucket b_hi).
+        int s_lo = b_lo, s_hi = b_hi;
+        while (s_lo < s_hi) {
+            const int mid = (s_lo + s_hi + 1) >> 1;
+            const int cand_hi = mid << 20;                 // the bucket lives in the key's high word: one 32-bit compare
+            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
+#pragma unroll
+            for (int i = 0; i < EPT; ++i)
+                if ((int)(key[i] >> 32) >= cand_hi) g4[i & 3] += __longlong_as_double(key[i]);
+            const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), S.red, slot);
+            if (!(g < thr)) s_lo = mid; else s_hi = mid - 1;
+        }
+        const long long B = s_lo;
+        const long long k_lo = B << 52, k_hi = B >= 2047 ? 0x7fffffffffffffffLL : (B + 1) << 52;   // bucket B = keys in [k_lo, k_hi)
+        double ga = 0.0; long long nb = 0;
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) { ga += key[i] >= k_hi ? __longlong_as_double(key[i]) : 0.0; nb += (key[i] >= k_lo && key[i] < k_hi) ? 1 : 0; }
+        const double g_above = block_sum(ga, S.red, slot);           // < thr by construction
+        const long long n_bkt = block_sum_ll(nb, S.red, slot);
+        if (n_bkt <= kBucketMax) {
+            // ---- 2. fine: sort + cumulative sum of the bucket's entries, exactly as the definition orders them
+#pragma unroll
+            for (int i = 0; i < EPT; ++i)
+                if (key[i] >= k_lo && key[i] < k_hi) {
+                    const int pos = atomicAdd(&S.bkt_count, 1);
+                    S.bkt_p[pos] = __longlong_as_double(key[i]); S.bkt_e[pos] = entry_of(i);
+                }
+            __syncthreads();
+            const int M = (int)n_bkt;
+            for (int q = tid; q < M; q += kSelThreads) {
+                const double pq = S.bkt_p[q]; const int eq = S.bkt_e[q];
+                int rank = 0;
+                for (int r = 0; r < M; ++r) { const double pr = S.bkt_p[r]; rank += (pr > pq || (pr == pq && S.bkt_e[r] < eq)) ? 1 : 0; }
+                S.srt_p[rank] = pq; S.srt_e[rank] = eq;
+            }
+            __syncthreads();
+            if (tid < 32) {
+                // warp 0: C_{r-1} = g_above + (sum of the sorted entries before r), lane l owning positions [16 l, 16 l + 16)
+                constexpr int kPer = kBucketMax / 32;
+                double loc = 0.0;
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) { const int r = tid * kPer + u; loc += r < M ? S.srt_p[r] : 0.0; }
+                double incl = loc;
+                for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += v; }
+                double c = g_above + (incl - loc);
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) {
+                    const int r = tid * kPer + u;
+                    if (r < M) {
+                        if (c < thr) { const int e = S.srt_e[r]; const int j = e < n_modes ? e : owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); }
+                        c += S.srt_p[r];
+                    }
+                }
+            }
+            kappa = k_hi - 1; iota = -1;                             // below: key > kappa keeps everything above the bucket
+        } else {
+            // ---- 3. fallback.  G(c) = sum of powers with key > c is monotone non-increasing in c (the fixed reduction tree keeps
+            // that exactly); build the largest c with G(c) >= thr bit by bit, then kappa = c + 1.
+            long long lo = 0;
+            for (int b = 62; b >= 0; --b) {
+                const long long cand = lo | (1ll << b);
+                double g4[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] > cand ? __longlong_as_double(key[i]) : 0.0;
+                const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), S.red, slot);
+                if (!(g < thr)) lo = cand;
+            }
+            kappa = lo + 1;
+            // ties at kappa: the j-th (by entry index) is kept iff G(kappa) + j P < thr, accumulated one by one like the cumsum
+            double g = 0.0; long long nt = 0;
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) { g += key[i] > kappa ? __longlong_as_double(key[i]) : 0.0; nt += key[i] == kappa ? 1 : 0; }
+            g = block_sum(g, S.red, slot);
+            const long long n_tie = block_sum_ll(nt, S.red, slot);
+            if (n_tie > 1) {
+                const double p = __longlong_as_double(kappa);
+                long long keep_t = 0; double c = g;
+                while (keep_t < n_tie && c < thr) { ++keep_t; c += p; }      // every thread computes the same count
+                if (keep_t < n_tie) {
+                    // iota = the keep_t-th smallest entry index among the ties: 14-bit select on the index
+                    int lo_i = -1;                                           // largest index with count(ties <= index) < keep_t
+                    for (int b = 13; b >= 0; --b) {
+                        const int cand = lo_i < 0 ? (1 << b) - 1 : lo_i + (1 << b);
+                        long long cnt = 0;
+#pragma unroll
+                        for (int i = 0; i < EPT; ++i) cnt += (key[i] == kappa && entry_of(i) <= cand) ? 1 : 0;
+                        cnt = block_sum_ll(cnt, S.red, slot);
+                        if (cnt < keep_t) lo_i = cand;
+                    }
+                    iota = lo_i + 1;
+                }
+            }
+        }
+    }
+
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        if (key[i] >= 0) {
+            const int e = entry_of(i);
+            if (key[i] > kappa || (key[i] == kappa && e <= iota)) {
+                const int j = e < n_modes ? e : owner[e - n_modes];
+                atomicOr(&S.bitmap[j >> 5], 1u << (j & 31));
+            }
+        }
+    }
+}
+
+// General kernel, one (source, step) row per block pass: the whole row's keys in registers.  Register slot i of thread tid
+// holds primary entry j = i*256 + tid for i < NP = ceil(n_modes/256) and mirror entry n_modes + (i - NP)*256 + tid after that,
+// so every global load of the row is coalesced and independent of the others; |A|^2 goes through shared memory once so that
+// the mirrors need no second, dependent gather from HBM.  Rows come from the list the fast kernel leaves (rows whose
+// candidate list did not fit, or degenerate ones); with fb_list == NULL the grid is (n_t, n_src) and every row is done here.
 template <int EPT>
 __global__ void __launch_bounds__(kSelThreads)
-few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L)
+few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L, const int* __restrict__ fb_list,
+                      const int* __restrict__ fb_count)
 {
     extern __shared__ double a2_s[];                 // [n_modes] |A_j|^2
-    __shared__ sel_red red;
-    __shared__ unsigned bitmap_s[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
-    __shared__ double bkt_p[kBucketMax], srt_p[kBucketMax];
-    __shared__ int bkt_e[kBucketMax], srt_e[kBucketMax];
-    __shared__ int bkt_count;
+    __shared__ sel_shared S;
     const int tid = threadIdx.x;
-    const int src = blockIdx.y, k = blockIdx.x;
+    const int n_rows = fb_list ? *fb_count : 1;
+    for (int q = fb_list ? blockIdx.x : 0; q < n_rows; q += gridDim.x) {
+    const int row = fb_list ? fb_list[q] : blockIdx.y * n_t + blockIdx.x;
+    const int src = row / n_t, k = row - src * n_t;
     const int n_ent = *L.n_entries;
     const int NP = (n_modes + kSelThreads - 1) / kSelThreads;
     const double2* a = amp + ((size_t)src * n_t + k) * n_modes;
     const double* y2 = L.y2 + (size_t)src * 2 * n_modes;
     const int words = sel_words(n_modes);
-    for (int w = tid; w < words; w += kSelThreads) bitmap_s[w] = 0u;
-    if (tid == 0) bkt_count = 0;
+    __syncthreads();                                 // the previous row's shared state is no longer read
+    for (int w = tid; w < words; w += kSelThreads) S.bitmap[w] = 0u;
+    if (tid == 0) S.bkt_count = 0;
     int slot = 0;
     auto entry_of = [&](int i) { return i < NP ? i * kSelThreads + tid : n_modes + (i - NP) * kSelThreads + tid; };
-    auto valid = [&](int i) { return i < NP ? i * kSelThreads + tid < n_modes : entry_of(i) < n_ent; };
 
     // ---- entry powers (same separately rounded operations as the definition: |A|^2 = re*re + im*im, P = |A|^2 |Y|^2).
     // key = bit pattern of P as a signed 64-bit integer: monotone for P >= 0; empty slots get -1 (below every key).
@@ -205,128 +360,108 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
             }
         }
     }
-    const double total = block_sum(tot_local, red, slot);
-    const double thr = (1.0 - eps) * total;
+    const double total = block_sum(tot_local, S.red, slot);
+    select_core<EPT>(key, entry_of, (1.0 - eps) * total, 0, 2047, n_modes, L.owner, S, slot);
+    __syncthreads();
+    unsigned* gb = L.bitmap + (size_t)src * words;
+    for (int w = tid; w < words; w += kSelThreads)
+        if (S.bitmap[w]) atomicOr(&gb[w], S.bitmap[w]);
+    }
+}
 
-    long long kappa;            // kept  <=>  key > kappa  or  (key == kappa and entry index <= iota)
-    int iota = 0x7fffffff;
-    if (!(thr > 0.0)) {
-        // eps >= 1 or an all-zero row: only rank 0 survives, i.e. the largest power with the lowest entry index
-        long long kmax_local = -1;
+// Fast kernel, one (source, step) row per block.  An entry whose power is below tau = eps * total / (4 n_entries) is
+// certainly dropped: all such entries together hold less than eps * total / 4, so for each of them C_{r-1} > (1 - eps/4) total,
+// a margin far outside rounding.  Only the candidates (power >= tau: the kept entries and a margin, a few hundred of the
+// 7137) are compacted -- in a fixed order, so that every run adds the same numbers in the same order -- and go through
+// select_core at 8 entries per thread instead of 32.  The mirror entry of mode j is formed beside the primary from the same
+// |A_j|^2 (mirror_e[j] = its entry index, y2m[j] = |Y_{l,-m}|^2): no gather, no shared-memory copy of the row.
+// A row with more than kCandMax candidates (a flat spectrum) or a degenerate threshold is appended to fb_list for the
+// general kernel.
+constexpr int kCandMax = 2048;
+constexpr int kCandEpt = kCandMax / kSelThreads;
+
+template <int NPT>
+__global__ void __launch_bounds__(kSelThreads, NPT <= 16 ? 3 : 1)
+few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L)
+{
+    __shared__ sel_shared S;
+    __shared__ long long cand_k[kCandMax];
+    __shared__ int cand_e[kCandMax];
+    __shared__ int warp_sums[kSelWarps];
+    const int tid = threadIdx.x;
+    const int src = blockIdx.y, k = blockIdx.x;
+    const int n_ent = *L.n_entries;
+    const double2* a = amp + ((size_t)src * n_t + k) * n_modes;
+    const double* y2p = L.y2 + (size_t)src * 2 * n_modes;
+    const double* y2m = L.y2m + (size_t)src * n_modes;
+    const int words = sel_words(n_modes);
+    for (int w = tid; w < words; w += kSelThreads) S.bitmap[w] = 0u;
+    if (tid == 0) S.bkt_count = 0;
+    int slot = 0;
+
+    long long kp[NPT], km[NPT];
+    double t4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-        for (int i = 0; i < EPT; ++i) kmax_local = key[i] > kmax_local ? key[i] : kmax_local;
-        kappa = block_max_ll(kmax_local, red, slot);
-        long long best = -0x7fffffff;       // max of -index
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) if (key[i] == kappa) { long long c = -(long long)entry_of(i); best = c > best ? c : best; }
-        iota = (int)(-block_max_ll(best, red, slot));
-    } else {
-        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x and
-        // g(0) = total >= thr; B = the largest x with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
-        long long B = 0;
-        for (int b = 10; b >= 0; --b) {
-            const int cand_hi = (int)((B | (1ll << b)) << 20);   // the bucket lives in the key's high word: one 32-bit compare
-            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
-#pragma unroll
-            for (int i = 0; i < EPT; ++i)
-                if ((int)(key[i] >> 32) >= cand_hi) g4[i & 3] += __longlong_as_double(key[i]);
-            const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
-            if (!(g < thr)) B |= 1ll << b;
-        }
-        const long long k_lo = B << 52, k_hi = B >= 2047 ? 0x7fffffffffffffffLL : (B + 1) << 52;   // bucket B = keys in [k_lo, k_hi)
-        double ga = 0.0; long long nb = 0;
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) { ga += key[i] >= k_hi ? __longlong_as_double(key[i]) : 0.0; nb += (key[i] >= k_lo && key[i] < k_hi) ? 1 : 0; }
-        const double g_above = block_sum(ga, red, slot);           // < thr by construction
-        const long long n_bkt = block_sum_ll(nb, red, slot);
-        if (n_bkt <= kBucketMax) {
-            // ---- 2. fine: sort + cumulative sum of the bucket's entries, exactly as the definition orders them
-#pragma unroll
-            for (int i = 0; i < EPT; ++i)
-                if (key[i] >= k_lo && key[i] < k_hi) {
-                    const int pos = atomicAdd(&bkt_count, 1);
-                    bkt_p[pos] = __longlong_as_double(key[i]); bkt_e[pos] = entry_of(i);
-                }
-            __syncthreads();
-            const int M = (int)n_bkt;
-            for (int q = tid; q < M; q += kSelThreads) {
-                const double pq = bkt_p[q]; const int eq = bkt_e[q];
-                int rank = 0;
-                for (int r = 0; r < M; ++r) { const double pr = bkt_p[r]; rank += (pr > pq || (pr == pq && bkt_e[r] < eq)) ? 1 : 0; }
-                srt_p[rank] = pq; srt_e[rank] = eq;
+    for (int i = 0; i < NPT; ++i) {
+        kp[i] = km[i] = -1;
+        const int j = i * kSelThreads + tid;
+        if (j < n_modes) {
+            const double2 v = a[j];
+            const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
+            const double p = __dmul_rn(a2, y2p[j]);
+            kp[i] = __double_as_longlong(p);
+            t4[i & 1] += p;
+            if (L.mirror_e[j] >= 0) {
+                const double pm = __dmul_rn(a2, y2m[j]);
+                km[i] = __double_as_longlong(pm);
+                t4[2 + (i & 1)] += pm;
             }
-            __syncthreads();
-            if (tid < 32) {
-                // warp 0: C_{r-1} = g_above + (sum of the sorted entries before r), lane l owning positions [16 l, 16 l + 16)
-                constexpr int kPer = kBucketMax / 32;
-                double loc = 0.0;
-#pragma unroll
-                for (int u = 0; u < kPer; ++u) { const int r = tid * kPer + u; loc += r < M ? srt_p[r] : 0.0; }
-                double incl = loc;
-                for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += v; }
-                double c = g_above + (incl - loc);
-#pragma unroll
-                for (int u = 0; u < kPer; ++u) {
-                    const int r = tid * kPer + u;
-                    if (r < M) {
-                        if (c < thr) { const int e = srt_e[r]; const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&bitmap_s[j >> 5], 1u << (j & 31)); }
-                        c += srt_p[r];
-                    }
-                }
-            }
-            kappa = k_hi - 1; iota = -1;                             // below: key > kappa keeps everything above the bucket
-        } else {
-        // ---- 3. fallback.  G(c) = sum of powers with key > c is monotone non-increasing in c (the fixed reduction tree keeps that exactly);
-        // build the largest c with G(c) >= thr bit by bit, then kappa = c + 1.
-        long long lo = 0;
-        for (int b = 62; b >= 0; --b) {
-            const long long cand = lo | (1ll << b);
-            double g4[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-            for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] > cand ? __longlong_as_double(key[i]) : 0.0;
-            const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), red, slot);
-            if (!(g < thr)) lo = cand;
-        }
-        kappa = lo + 1;
-        // ties at kappa: the j-th (by entry index) is kept iff G(kappa) + j P < thr, accumulated one by one like the cumsum
-        double g = 0.0; long long nt = 0;
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) { g += key[i] > kappa ? __longlong_as_double(key[i]) : 0.0; nt += key[i] == kappa ? 1 : 0; }
-        g = block_sum(g, red, slot);
-        const long long n_tie = block_sum_ll(nt, red, slot);
-        if (n_tie > 1) {
-            const double p = __longlong_as_double(kappa);
-            long long keep_t = 0; double c = g;
-            while (keep_t < n_tie && c < thr) { ++keep_t; c += p; }      // every thread computes the same count
-            if (keep_t < n_tie) {
-                // iota = the keep_t-th smallest entry index among the ties: 14-bit select on the index
-                int lo_i = -1;                                           // largest index with count(ties <= index) < keep_t
-                for (int b = 13; b >= 0; --b) {
-                    const int cand = lo_i < 0 ? (1 << b) - 1 : lo_i + (1 << b);
-                    long long cnt = 0;
-#pragma unroll
-                    for (int i = 0; i < EPT; ++i) cnt += (key[i] == kappa && entry_of(i) <= cand) ? 1 : 0;
-                    cnt = block_sum_ll(cnt, red, slot);
-                    if (cnt < keep_t) lo_i = cand;
-                }
-                iota = lo_i + 1;
-            }
-        }
         }
     }
-
+    const double total = block_sum((t4[0] + t4[1]) + (t4[2] + t4[3]), S.red, slot);
+    const double thr = (1.0 - eps) * total;
+    const long long tau_key = __double_as_longlong(0.25 * eps * total / (double)n_ent);
+    int cnt = 0;
 #pragma unroll
-    for (int i = 0; i < EPT; ++i) {
-        const int e = entry_of(i);
-        if (valid(i) && (key[i] > kappa || (key[i] == kappa && e <= iota))) {
-            const int j = e < n_modes ? e : L.owner[e - n_modes];
-            atomicOr(&bitmap_s[j >> 5], 1u << (j & 31));
-        }
+    for (int i = 0; i < NPT; ++i) cnt += (kp[i] >= tau_key ? 1 : 0) + (km[i] >= tau_key ? 1 : 0);
+    int n_cand;
+    const int incl = block_scan_int<kSelThreads>(cnt, warp_sums, &n_cand);
+    if (!(thr > 0.0) || !(tau_key >= 0) || n_cand > kCandMax) {          // block-uniform: hand the row to the general kernel
+        if (tid == 0) L.fb_list[atomicAdd(L.fb_count, 1)] = src * n_t + k;
+        return;
+    }
+    int pos = incl - cnt;
+#pragma unroll
+    for (int i = 0; i < NPT; ++i) {
+        if (kp[i] >= tau_key) { cand_k[pos] = kp[i]; cand_e[pos] = i * kSelThreads + tid; ++pos; }
+        if (km[i] >= tau_key) { cand_k[pos] = km[i]; cand_e[pos] = L.mirror_e[i * kSelThreads + tid]; ++pos; }
+    }
+    __syncthreads();
+    long long ck[kCandEpt];
+    int ce[kCandEpt];
+    double tc = 0.0;
+#pragma unroll
+    for (int i = 0; i < kCandEpt; ++i) {
+        const int q = i * kSelThreads + tid;
+        ck[i] = q < n_cand ? cand_k[q] : -1;
+        ce[i] = q < n_cand ? cand_e[q] : 0x7fffffff;
+        tc += q < n_cand ? __longlong_as_double(ck[i]) : 0.0;
+    }
+    const double total_cand = block_sum(tc, S.red, slot);
+    if (total_cand < thr) {
+        // every candidate has C_{r-1} < thr: all kept
+#pragma unroll
+        for (int i = 0; i < kCandEpt; ++i)
+            if (ck[i] >= 0) { const int e = ce[i]; const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); }
+    } else {
+        // candidates lie in the exponent buckets of [tau, total]: ~log2(4 n_entries / eps) of them, 5-6 search steps instead of 11
+        select_core<kCandEpt>(ck, [&](int i) { return ce[i]; }, thr, (int)(tau_key >> 52), (int)(__double_as_longlong(total) >> 52), n_modes,
+                              L.owner, S, slot);
     }
     __syncthreads();
     unsigned* gb = L.bitmap + (size_t)src * words;
     for (int w = tid; w < words; w += kSelThreads)
-        if (bitmap_s[w]) atomicOr(&gb[w], bitmap_s[w]);
+        if (S.bitmap[w]) atomicOr(&gb[w], S.bitmap[w]);
 }
 
 // bitmap -> ascending keep_idx (padded with -1) and n_keep.  One block per source.  keep_all: identity list.
@@ -364,10 +499,9 @@ few_select_compact_kernel(sel_layout L, int n_modes, int keep_all, int* __restri
 
 extern "C" size_t few_select_modes_workspace(int n_src, int n_t, int n_modes)
 {
-    (void)n_t;
-    if (n_src <= 0 || n_modes <= 0) return 0;
+    if (n_src <= 0 || n_t <= 0 || n_modes <= 0) return 0;
     size_t bytes = 0;
-    sel_carve(nullptr, n_src, n_modes, &bytes);
+    sel_carve(nullptr, n_src, n_t, n_modes, &bytes);
     return bytes;
 }
 
@@ -390,17 +524,26 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
                     workspace_bytes >= few_select_modes_workspace(n_src, n_t, n_modes),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
-    L = sel_carve(workspace, n_src, n_modes);
+    L = sel_carve(workspace, n_src, n_t, n_modes);
     few_select_prepare_kernel<<<n_src, kPrepThreads, 0, st>>>(m, (const double2*)ylm_plus, (const double2*)ylm_minus, n_modes, L,
                                                            ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
     const dim3 grid(n_t, n_src);
+    constexpr int kNptMax = (FEW_MAX_SELECT_ENTRIES + kSelThreads - 1) / kSelThreads;
+    if (n_modes <= 16 * kSelThreads)
+        few_select_row_fast_kernel<16><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+    else
+        few_select_row_fast_kernel<kNptMax><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    // the rows the fast kernel left (usually none): a small persistent grid walks the list
+    const long long n_rows = (long long)n_t * n_src;
+    const unsigned fb_grid = (unsigned)(n_rows < 2LL * ctx->sm_count ? n_rows : 2LL * ctx->sm_count);
     const size_t smem = (size_t)n_modes * sizeof(double);
     constexpr int kEptMax = (FEW_MAX_SELECT_ENTRIES + kSelThreads - 1) / kSelThreads + 1;   // +1: primaries and mirrors are padded separately
     if (2 * ((n_modes + kSelThreads - 1) / kSelThreads) <= 32)
-        few_select_row_kernel<32><<<grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+        few_select_row_kernel<32><<<fb_grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L, L.fb_list, L.fb_count);
     else
-        few_select_row_kernel<kEptMax><<<grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+        few_select_row_kernel<kEptMax><<<fb_grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L, L.fb_list, L.fb_count);
     FEW_CUDA_CHECK(cudaGetLastError());
     few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
     FEW_CUDA_CHECK(cudaGetLastError());

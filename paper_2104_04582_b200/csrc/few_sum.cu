@@ -708,7 +708,7 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
                                                           n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
-    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 1024, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
+    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");

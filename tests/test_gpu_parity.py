@@ -173,6 +173,27 @@ def test_select_modes_tiny_and_ties(api):
                 check_keep(keep[s].cpu().numpy(), nk[s].item(), ref, margin, w.n_modes)
 
 
+def test_select_modes_flat_and_mixed_rows(api):
+    """Rows whose candidate list exceeds the fast kernel's capacity (flat spectra: every entry is above eps*total/(4 n)) go to
+    the general kernel through the device-side row list; a batch mixes such a source with an ordinary one, and one source
+    alternates flat and steep steps."""
+    w = synth.make_config(3, n_src=3, n_samples=8)
+    rng = np.random.default_rng(7)
+    amp = w.amp.copy()
+    flat = (rng.uniform(1.0, 2.0, amp[0].shape) * np.exp(1j * rng.uniform(0, 2 * np.pi, amp[0].shape)))
+    amp[0] = flat * 1e-3
+    amp[2, ::2] = flat[::2] * 1e-2                      # source 2: every other step flat
+    g = gpu_inputs(w)
+    yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
+    for eps in (1e-5, 1e-2):
+        keep, nk = api.few_select_modes(dev(amp), g["m"], yp, ym, eps)
+        api.few_device_status()
+        for s in range(w.n_src):
+            ref, margin = oracle.select_modes(amp[s], w.m, yp[s].cpu().numpy(), ym[s].cpu().numpy(), eps)
+            check_keep(keep[s].cpu().numpy(), nk[s].item(), ref, margin, w.n_modes)
+    assert nk[0].item() > 3000                             # the flat source keeps almost everything
+
+
 # ------------------------------------------------------------------------------------------- S3 and the whole path
 def run_gpu_chain(api, w):
     g = gpu_inputs(w)
