@@ -58,7 +58,7 @@ enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
 #define FEW_MAX_ABS_K 63        /* |k| <= 63 (polar index of Kerr-shaped mode lists, few_sum_waveform_kerr) */
 #define FEW_MAX_NT_SPLINE 736   /* n_t limit of few_spline_fit (one shared-memory column per system) */
-#define FEW_MAX_SELECT_ENTRIES 9728 /* n_modes + #(m>0) limit of few_select_modes (one row sorted in shared memory) */
+#define FEW_MAX_SELECT_MODES 131072 /* n_modes limit of few_select_modes (owner bitmap of a row in shared memory) */
 
 typedef struct few_ctx few_ctx;
 
@@ -105,7 +105,7 @@ int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y, int n_src,
  * ylm_plus == NULL (then ylm_minus is ignored): power = |A|^2, no mirror entries.
  * amp[n_src][n_t][n_modes][2]; m[n_modes]; ylm_*[n_src][n_modes][2];
  * keep_idx[n_src][n_modes] int32 ascending, padded with -1; n_keep[n_src] int32.
- * Limit: n_modes + #(m>0) <= FEW_MAX_SELECT_ENTRIES. */
+ * Rows of any length up to n_modes <= FEW_MAX_SELECT_MODES (a Kerr-shaped 42 273-mode row has 78 507 entries). */
 size_t few_select_modes_workspace(int n_src, int n_t, int n_modes);
 int few_select_modes(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
                      double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,

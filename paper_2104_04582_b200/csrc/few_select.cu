@@ -10,19 +10,24 @@
 //
 // What the procedure defines is a SET, and the set is fixed by one number: C_{r-1} of an entry is G(key) = the summed power
 // of all entries with a strictly larger key (plus earlier ties), G is monotone in the key, so the kept entries are exactly
-// those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernel therefore SELECTS instead of sorting the
-// whole row (one block of 256 threads per row, powers held in registers, nothing but the row's amplitudes read from HBM):
-//   1. coarse: the key's top 11 bits are the binary exponent of the power.  An 11-step MSB-first search, each step one
-//      masked block reduction, finds the exponent bucket B in which the cumulative sum crosses the threshold.  Every entry
+// those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernels therefore SELECT instead of sorting the row
+// (select_core, one block per row, nothing but the row's amplitudes read from HBM):
+//   1. coarse: the key's top 11 bits are the binary exponent of the power.  A binary search over the exponent buckets, each
+//      step one masked block reduction, finds the bucket B in which the cumulative sum crosses the threshold.  Every entry
 //      in a higher bucket is kept, every entry in a lower one dropped.
-//   2. fine: the (typically ~100-200) entries of bucket B are compacted into shared memory, rank-sorted by (power
-//      descending, entry index ascending) and cumulatively summed in that order on top of the power above the bucket: this
-//      is the definition's sort + cumsum, applied only where it can change the answer.  Ties need no special case.
-//   3. fallback (more than kBucketMax entries in the bucket, e.g. a row of equal powers): a 63-step MSB-first radix select
-//      on the full 64-bit pattern, ties at kappa resolved by entry index with a 14-step select.
+//   2. fine: the entries of bucket B are compacted into shared memory, rank-sorted by (power descending, entry index
+//      ascending) and cumulatively summed in that order on top of the power above the bucket: this is the definition's
+//      sort + cumsum, applied only where it can change the answer.  Ties need no special case.
+//   3. fallback (more entries in the bucket than the shared arrays hold, e.g. a row of equal powers): a 63-step MSB-first
+//      radix select on the full 64-bit pattern, ties at kappa resolved by entry index with an 18-step select.
+// select_core sees the row through an `Entries` policy with one member, for_each(f): f(key, entry index, chain):
+//   reg_entries     keys held in registers -- the fast kernel's candidates (few_select_row_fast_kernel: entries below
+//                   eps*total/(4 n) are certainly dropped; the few hundred to ~1500 others are compacted and selected);
+//   stream_entries  keys recomputed from the amplitudes on every pass (the row stays in L2) -- rows of any length: the
+//                   Kerr-shaped grid's 78 507 entries, and the rows the fast kernel hands over (flat spectra, degenerate eps).
 // The owners of the kept entries are OR-ed into a per-source bitmap; a last kernel compacts it into ascending keep_idx
 // and n_keep.  (History: in-shared-memory LSD radix sort + scan 128 us per 7137-entry row; 63-step
-// select alone 44 us; this version see profiles/.)
+// select alone 44 us; keys of the whole row in registers 26 us; this version see profiles/.)
 #include "few_common.cuh"
 
 namespace {
@@ -122,108 +127,135 @@ few_select_prepare_kernel(const int* __restrict__ m, const double2* __restrict__
     for (int w = tid; w < sel_words(n_modes); w += kPrepThreads) L.bitmap[(size_t)src * sel_words(n_modes) + w] = 0u;
 }
 
-// ---- block reductions over kSelThreads threads; every thread gets the result.  `slot` alternates between calls so that one
+// ---- block reductions over W warps; every thread gets the result.  `slot` alternates between calls so that one
 // __syncthreads per reduction suffices.
-struct sel_red { double d[2][kSelWarps]; long long i[2][kSelWarps]; };
+template <int W> struct sel_red { double d[2][W]; long long i[2][W]; };
 
-__device__ __forceinline__ double block_sum(double v, sel_red& s, int& slot)
+template <int W>
+__device__ __forceinline__ double block_sum(double v, sel_red<W>& s, int& slot)
 {
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0) s.d[slot][threadIdx.x >> 5] = v;
     __syncthreads();
     double r = 0.0;
 #pragma unroll
-    for (int w = 0; w < kSelWarps; ++w) r += s.d[slot][w];
+    for (int w = 0; w < W; ++w) r += s.d[slot][w];
     slot ^= 1;
     return r;
 }
-__device__ __forceinline__ long long block_sum_ll(long long v, sel_red& s, int& slot)
+template <int W>
+__device__ __forceinline__ long long block_sum_ll(long long v, sel_red<W>& s, int& slot)
 {
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0) s.i[slot][threadIdx.x >> 5] = v;
     __syncthreads();
     long long r = 0;
 #pragma unroll
-    for (int w = 0; w < kSelWarps; ++w) r += s.i[slot][w];
+    for (int w = 0; w < W; ++w) r += s.i[slot][w];
     slot ^= 1;
     return r;
 }
-__device__ __forceinline__ long long block_max_ll(long long v, sel_red& s, int& slot)
+template <int W>
+__device__ __forceinline__ long long block_max_ll(long long v, sel_red<W>& s, int& slot)
 {
     for (int o = 16; o; o >>= 1) { long long u = __shfl_xor_sync(0xffffffffu, v, o); v = u > v ? u : v; }
     if ((threadIdx.x & 31) == 0) s.i[slot][threadIdx.x >> 5] = v;
     __syncthreads();
     long long r = s.i[slot][0];
 #pragma unroll
-    for (int w = 1; w < kSelWarps; ++w) r = s.i[slot][w] > r ? s.i[slot][w] : r;
+    for (int w = 1; w < W; ++w) r = s.i[slot][w] > r ? s.i[slot][w] : r;
     slot ^= 1;
     return r;
 }
 
-// ---- shared state of one row's selection
+// ---- shared state of one row's selection: T threads, BK = capacity of the fine step, NW = words of the owner bitmap
+template <int T, int BK, int NW>
 struct sel_shared {
-    sel_red red;
-    unsigned bitmap[(FEW_MAX_SELECT_ENTRIES + 31) / 32];
-    double bkt_p[kBucketMax], srt_p[kBucketMax];
-    int bkt_e[kBucketMax], srt_e[kBucketMax];
+    sel_red<T / 32> red;
+    unsigned bitmap[NW];
+    double bkt_p[BK], srt_p[BK];
+    int bkt_e[BK], srt_e[BK];
     int bkt_count;
 };
 
-// The selection proper, on entry powers held in registers: key[i] = bit pattern of the power of the thread's i-th entry (-1 =
-// empty slot), entry_of(i) its entry index, thr = (1 - eps) * (total power of the row) > 0 or <= 0 for the degenerate case.
-// The entries passed need not be the whole row: any superset of the kept entries whose total is >= thr gives the same set,
-// because C_{r-1} of an entry is the summed power of the entries before it in the order and every such entry is itself kept.
-// Marks the owners of the kept entries in S.bitmap (caller zeroes it and S.bkt_count, then __syncthreads).
-template <int EPT, class EntOf>
-__device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf entry_of, double thr, int b_lo, int b_hi, int n_modes,
-                                            const int* __restrict__ owner, sel_shared& S, int& slot)
+// Entries policy 1: keys (bit patterns of the powers, -1 = empty slot) and entry indices in registers.
+template <int EPT>
+struct reg_entries {
+    const long long (&key)[EPT];
+    const int (&ent)[EPT];
+    __device__ __forceinline__ reg_entries(const long long (&k)[EPT], const int (&e)[EPT]) : key(k), ent(e) {}
+    template <class F> __device__ __forceinline__ void for_each(F f) const
+    {
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) if (key[i] >= 0) f(key[i], ent[i], i & 3);
+    }
+};
+
+// Entries policy 2: the row is re-read (L2) and the powers recomputed on every pass, with the same separately rounded
+// operations as the definition: |A|^2 = re*re + im*im, P = |A|^2 |Y|^2.  Primary of mode j = entry j; its mirror (m > 0) =
+// entry mirror_e[j], formed from the same |A_j|^2.  Thread tid owns modes tid, tid + T, ...: a fixed order per thread.
+template <int T>
+struct stream_entries {
+    const double2* a; const double* y2p; const double* y2m; const int* mirror_e; int n_modes;
+    template <class F> __device__ __forceinline__ void for_each(F f) const
+    {
+        for (int j = threadIdx.x; j < n_modes; j += T) {
+            const double2 v = a[j];
+            const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
+            f(__double_as_longlong(__dmul_rn(a2, y2p[j])), j, 0);
+            const int me = mirror_e[j];
+            if (me >= 0) f(__double_as_longlong(__dmul_rn(a2, y2m[j])), me, 1);
+        }
+    }
+};
+
+// The selection proper.  thr = (1 - eps) * (total power of the row) > 0, or <= 0 for the degenerate case (eps >= 1, zero row).
+// The entries E enumerates need not be the whole row: any superset of the kept entries whose total is >= thr gives the same
+// set, because C_{r-1} of an entry is the summed power of the entries before it in the order and each of those is itself
+// kept.  The threshold's exponent bucket is searched in [b_lo, b_hi]: the caller guarantees g(b_lo) >= thr and no key above
+// bucket b_hi.  Marks the owners of the kept entries in S.bitmap (caller zeroes it and S.bkt_count, then __syncthreads).
+template <int T, int BK, int NW, class Entries>
+__device__ __forceinline__ void select_core(const Entries& E, double thr, int b_lo, int b_hi, int n_modes,
+                                            const int* __restrict__ owner, sel_shared<T, BK, NW>& S, int& slot)
 {
     const int tid = threadIdx.x;
+    auto mark = [&](int e) { const int j = e < n_modes ? e : owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); };
     long long kappa;            // kept  <=>  key > kappa  or  (key == kappa and entry index <= iota)
     int iota = 0x7fffffff;
     if (!(thr > 0.0)) {
-        // eps >= 1 or an all-zero row: only rank 0 survives, i.e. the largest power with the lowest entry index
+        // only rank 0 survives, i.e. the largest power with the lowest entry index
         long long kmax_local = -1;
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) kmax_local = key[i] > kmax_local ? key[i] : kmax_local;
+        E.for_each([&](long long k, int, int) { kmax_local = k > kmax_local ? k : kmax_local; });
         kappa = block_max_ll(kmax_local, S.red, slot);
         long long best = -0x7fffffff;       // max of -index
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) if (key[i] == kappa) { long long c = -(long long)entry_of(i); best = c > best ? c : best; }
+        E.for_each([&](long long k, int e, int) { if (k == kappa) { const long long c = -(long long)e; best = c > best ? c : best; } });
         iota = (int)(-block_max_ll(best, S.red, slot));
     } else {
-        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x and
-        // g(0) = total >= thr; B = the largest x with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
-        // The bucket is searched in [b_lo, b_hi] (the caller knows that g(b_lo) >= thr and that no key lies above bucket b_hi).
+        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x;
+        // B = the largest x in [b_lo, b_hi] with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
         int s_lo = b_lo, s_hi = b_hi;
         while (s_lo < s_hi) {
             const int mid = (s_lo + s_hi + 1) >> 1;
             const int cand_hi = mid << 20;                 // the bucket lives in the key's high word: one 32-bit compare
-            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // four chains: the DADD latency, not its rate, bounds this loop
-#pragma unroll
-            for (int i = 0; i < EPT; ++i)
-                if ((int)(key[i] >> 32) >= cand_hi) g4[i & 3] += __longlong_as_double(key[i]);
+            double g4[4] = {0.0, 0.0, 0.0, 0.0};          // several chains: the DADD latency, not its rate, bounds this loop
+            E.for_each([&](long long k, int, int c) { if ((int)(k >> 32) >= cand_hi) g4[c] += __longlong_as_double(k); });
             const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), S.red, slot);
             if (!(g < thr)) s_lo = mid; else s_hi = mid - 1;
         }
         const long long B = s_lo;
         const long long k_lo = B << 52, k_hi = B >= 2047 ? 0x7fffffffffffffffLL : (B + 1) << 52;   // bucket B = keys in [k_lo, k_hi)
         double ga = 0.0; long long nb = 0;
-#pragma unroll
-        for (int i = 0; i < EPT; ++i) { ga += key[i] >= k_hi ? __longlong_as_double(key[i]) : 0.0; nb += (key[i] >= k_lo && key[i] < k_hi) ? 1 : 0; }
+        E.for_each([&](long long k, int, int) { ga += k >= k_hi ? __longlong_as_double(k) : 0.0; nb += (k >= k_lo && k < k_hi) ? 1 : 0; });
         const double g_above = block_sum(ga, S.red, slot);           // < thr by construction
         const long long n_bkt = block_sum_ll(nb, S.red, slot);
-        if (n_bkt <= kBucketMax) {
+        if (n_bkt <= BK) {
             // ---- 2. fine: sort + cumulative sum of the bucket's entries, exactly as the definition orders them
-#pragma unroll
-            for (int i = 0; i < EPT; ++i)
-                if (key[i] >= k_lo && key[i] < k_hi) {
-                    const int pos = atomicAdd(&S.bkt_count, 1);
-                    S.bkt_p[pos] = __longlong_as_double(key[i]); S.bkt_e[pos] = entry_of(i);
-                }
+            E.for_each([&](long long k, int e, int) {
+                if (k >= k_lo && k < k_hi) { const int pos = atomicAdd(&S.bkt_count, 1); S.bkt_p[pos] = __longlong_as_double(k); S.bkt_e[pos] = e; }
+            });
             __syncthreads();
             const int M = (int)n_bkt;
-            for (int q = tid; q < M; q += kSelThreads) {
+            for (int q = tid; q < M; q += T) {
                 const double pq = S.bkt_p[q]; const int eq = S.bkt_e[q];
                 int rank = 0;
                 for (int r = 0; r < M; ++r) { const double pr = S.bkt_p[r]; rank += (pr > pq || (pr == pq && S.bkt_e[r] < eq)) ? 1 : 0; }
@@ -231,19 +263,17 @@ __device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf e
             }
             __syncthreads();
             if (tid < 32) {
-                // warp 0: C_{r-1} = g_above + (sum of the sorted entries before r), lane l owning positions [16 l, 16 l + 16)
-                constexpr int kPer = kBucketMax / 32;
+                // warp 0: C_{r-1} = g_above + (sum of the sorted entries before r), lane l owning positions [kPer l, kPer (l + 1))
+                constexpr int kPer = BK / 32;
                 double loc = 0.0;
-#pragma unroll
                 for (int u = 0; u < kPer; ++u) { const int r = tid * kPer + u; loc += r < M ? S.srt_p[r] : 0.0; }
                 double incl = loc;
                 for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += v; }
                 double c = g_above + (incl - loc);
-#pragma unroll
                 for (int u = 0; u < kPer; ++u) {
                     const int r = tid * kPer + u;
                     if (r < M) {
-                        if (c < thr) { const int e = S.srt_e[r]; const int j = e < n_modes ? e : owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); }
+                        if (c < thr) mark(S.srt_e[r]);
                         c += S.srt_p[r];
                     }
                 }
@@ -256,16 +286,14 @@ __device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf e
             for (int b = 62; b >= 0; --b) {
                 const long long cand = lo | (1ll << b);
                 double g4[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int i = 0; i < EPT; ++i) g4[i & 3] += key[i] > cand ? __longlong_as_double(key[i]) : 0.0;
+                E.for_each([&](long long k, int, int c) { g4[c] += k > cand ? __longlong_as_double(k) : 0.0; });
                 const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), S.red, slot);
                 if (!(g < thr)) lo = cand;
             }
             kappa = lo + 1;
             // ties at kappa: the j-th (by entry index) is kept iff G(kappa) + j P < thr, accumulated one by one like the cumsum
             double g = 0.0; long long nt = 0;
-#pragma unroll
-            for (int i = 0; i < EPT; ++i) { g += key[i] > kappa ? __longlong_as_double(key[i]) : 0.0; nt += key[i] == kappa ? 1 : 0; }
+            E.for_each([&](long long k, int, int) { g += k > kappa ? __longlong_as_double(k) : 0.0; nt += k == kappa ? 1 : 0; });
             g = block_sum(g, S.red, slot);
             const long long n_tie = block_sum_ll(nt, S.red, slot);
             if (n_tie > 1) {
@@ -273,13 +301,12 @@ __device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf e
                 long long keep_t = 0; double c = g;
                 while (keep_t < n_tie && c < thr) { ++keep_t; c += p; }      // every thread computes the same count
                 if (keep_t < n_tie) {
-                    // iota = the keep_t-th smallest entry index among the ties: 14-bit select on the index
+                    // iota = the keep_t-th smallest entry index among the ties: 18-bit select on the index
                     int lo_i = -1;                                           // largest index with count(ties <= index) < keep_t
-                    for (int b = 13; b >= 0; --b) {
+                    for (int b = 17; b >= 0; --b) {
                         const int cand = lo_i < 0 ? (1 << b) - 1 : lo_i + (1 << b);
                         long long cnt = 0;
-#pragma unroll
-                        for (int i = 0; i < EPT; ++i) cnt += (key[i] == kappa && entry_of(i) <= cand) ? 1 : 0;
+                        E.for_each([&](long long k, int e, int) { cnt += (k == kappa && e <= cand) ? 1 : 0; });
                         cnt = block_sum_ll(cnt, S.red, slot);
                         if (cnt < keep_t) lo_i = cand;
                     }
@@ -288,84 +315,48 @@ __device__ __forceinline__ void select_core(const long long (&key)[EPT], EntOf e
             }
         }
     }
-
-#pragma unroll
-    for (int i = 0; i < EPT; ++i) {
-        if (key[i] >= 0) {
-            const int e = entry_of(i);
-            if (key[i] > kappa || (key[i] == kappa && e <= iota)) {
-                const int j = e < n_modes ? e : owner[e - n_modes];
-                atomicOr(&S.bitmap[j >> 5], 1u << (j & 31));
-            }
-        }
-    }
+    E.for_each([&](long long k, int e, int) { if (k > kappa || (k == kappa && e <= iota)) mark(e); });
 }
 
-// General kernel, one (source, step) row per block pass: the whole row's keys in registers.  Register slot i of thread tid
-// holds primary entry j = i*256 + tid for i < NP = ceil(n_modes/256) and mirror entry n_modes + (i - NP)*256 + tid after that,
-// so every global load of the row is coalesced and independent of the others; |A|^2 goes through shared memory once so that
-// the mirrors need no second, dependent gather from HBM.  Rows come from the list the fast kernel leaves (rows whose
-// candidate list did not fit, or degenerate ones); with fb_list == NULL the grid is (n_t, n_src) and every row is done here.
-template <int EPT>
-__global__ void __launch_bounds__(kSelThreads)
-few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L, const int* __restrict__ fb_list,
-                      const int* __restrict__ fb_count)
+// General kernel, one (source, step) row per block pass, rows of any length: every pass of select_core streams the row's
+// amplitudes (HBM once, then L2) and recomputes the powers.  Serves the Kerr-shaped grid (42 273 modes, 78 507 entries per
+// row: ~10 passes of 676 KB) and the rows the fast kernel leaves in fb_list (flat spectra, degenerate thresholds); with
+// fb_list == NULL the grid is (n_t, n_src) and every row is done here.
+constexpr int kStreamThreads = 1024;
+constexpr int kStreamBucket = 2048;
+constexpr int kStreamWords = FEW_MAX_SELECT_MODES / 32;
+using stream_shared = sel_shared<kStreamThreads, kStreamBucket, kStreamWords>;
+
+__global__ void __launch_bounds__(kStreamThreads)
+few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L,
+                             const int* __restrict__ fb_list, const int* __restrict__ fb_count)
 {
-    extern __shared__ double a2_s[];                 // [n_modes] |A_j|^2
-    __shared__ sel_shared S;
+    extern __shared__ __align__(16) unsigned char stream_smem[];
+    stream_shared& S = *reinterpret_cast<stream_shared*>(stream_smem);
     const int tid = threadIdx.x;
     const int n_rows = fb_list ? *fb_count : 1;
-    for (int q = fb_list ? blockIdx.x : 0; q < n_rows; q += gridDim.x) {
-    const int row = fb_list ? fb_list[q] : blockIdx.y * n_t + blockIdx.x;
-    const int src = row / n_t, k = row - src * n_t;
     const int n_ent = *L.n_entries;
-    const int NP = (n_modes + kSelThreads - 1) / kSelThreads;
-    const double2* a = amp + ((size_t)src * n_t + k) * n_modes;
-    const double* y2 = L.y2 + (size_t)src * 2 * n_modes;
     const int words = sel_words(n_modes);
-    __syncthreads();                                 // the previous row's shared state is no longer read
-    for (int w = tid; w < words; w += kSelThreads) S.bitmap[w] = 0u;
-    if (tid == 0) S.bkt_count = 0;
-    int slot = 0;
-    auto entry_of = [&](int i) { return i < NP ? i * kSelThreads + tid : n_modes + (i - NP) * kSelThreads + tid; };
-
-    // ---- entry powers (same separately rounded operations as the definition: |A|^2 = re*re + im*im, P = |A|^2 |Y|^2).
-    // key = bit pattern of P as a signed 64-bit integer: monotone for P >= 0; empty slots get -1 (below every key).
-    long long key[EPT];
-    double tot_local = 0.0;
-#pragma unroll
-    for (int i = 0; i < EPT; ++i) {
-        key[i] = -1;
-        if (i < NP) {
-            const int j = i * kSelThreads + tid;
-            if (j < n_modes) {
-                const double2 v = a[j];
-                const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
-                a2_s[j] = a2;
-                const double p = __dmul_rn(a2, y2[j]);
-                key[i] = __double_as_longlong(p);
-                tot_local += p;
-            }
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < EPT; ++i) {
-        if (i >= NP) {
-            const int e = n_modes + (i - NP) * kSelThreads + tid;
-            if (e < n_ent) {
-                const double p = __dmul_rn(a2_s[L.owner[e - n_modes]], y2[e]);
-                key[i] = __double_as_longlong(p);
-                tot_local += p;
-            }
-        }
-    }
-    const double total = block_sum(tot_local, S.red, slot);
-    select_core<EPT>(key, entry_of, (1.0 - eps) * total, 0, 2047, n_modes, L.owner, S, slot);
-    __syncthreads();
-    unsigned* gb = L.bitmap + (size_t)src * words;
-    for (int w = tid; w < words; w += kSelThreads)
-        if (S.bitmap[w]) atomicOr(&gb[w], S.bitmap[w]);
+    for (int q = fb_list ? blockIdx.x : 0; q < n_rows; q += gridDim.x) {
+        const int row = fb_list ? fb_list[q] : blockIdx.y * n_t + blockIdx.x;
+        const int src = row / n_t, k = row - src * n_t;
+        stream_entries<kStreamThreads> E{amp + ((size_t)src * n_t + k) * n_modes, L.y2 + (size_t)src * 2 * n_modes,
+                                         L.y2m + (size_t)src * n_modes, L.mirror_e, n_modes};
+        __syncthreads();                                 // the previous row's shared state is no longer read
+        for (int w = tid; w < words; w += kStreamThreads) S.bitmap[w] = 0u;
+        if (tid == 0) S.bkt_count = 0;
+        int slot = 0;
+        double t2[2] = {0.0, 0.0};
+        E.for_each([&](long long key, int, int c) { t2[c] += __longlong_as_double(key); });
+        const double total = block_sum((t2[0] + t2[1]) + (0.0 + 0.0), S.red, slot);      // the same tree as the core's g(0)
+        // buckets below that of tau = eps total / (4 n) hold less than eps total / 4 altogether: the search starts there
+        const long long tau_key = __double_as_longlong(0.25 * eps * total / (double)n_ent);
+        const int b_lo = (eps > 1e-10 && tau_key > 0) ? (int)(tau_key >> 52) : 0;
+        select_core(E, (1.0 - eps) * total, b_lo, (int)(__double_as_longlong(total) >> 52), n_modes, L.owner, S, slot);
+        __syncthreads();
+        unsigned* gb = L.bitmap + (size_t)src * words;
+        for (int w = tid; w < words; w += kStreamThreads)
+            if (S.bitmap[w]) atomicOr(&gb[w], S.bitmap[w]);
     }
 }
 
@@ -379,12 +370,14 @@ few_select_row_kernel(const double2* __restrict__ amp, int n_t, int n_modes, dou
 // general kernel.
 constexpr int kCandMax = 2048;
 constexpr int kCandEpt = kCandMax / kSelThreads;
+constexpr int kFastModes = 16 * kSelThreads;          // rows of up to 4096 modes: 16 primaries + 16 mirrors per thread
+constexpr int kFastWords = kFastModes / 32;
 
 template <int NPT>
-__global__ void __launch_bounds__(kSelThreads, NPT <= 16 ? 3 : 1)
+__global__ void __launch_bounds__(kSelThreads, 3)
 few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L)
 {
-    __shared__ sel_shared S;
+    __shared__ sel_shared<kSelThreads, kBucketMax, kFastWords> S;
     __shared__ long long cand_k[kCandMax];
     __shared__ int cand_e[kCandMax];
     __shared__ int warp_sums[kSelWarps];
@@ -426,7 +419,7 @@ few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes
     for (int i = 0; i < NPT; ++i) cnt += (kp[i] >= tau_key ? 1 : 0) + (km[i] >= tau_key ? 1 : 0);
     int n_cand;
     const int incl = block_scan_int<kSelThreads>(cnt, warp_sums, &n_cand);
-    if (!(thr > 0.0) || !(tau_key >= 0) || n_cand > kCandMax) {          // block-uniform: hand the row to the general kernel
+    if (!(thr > 0.0) || !(tau_key > 0) || !(eps > 1e-10) || n_cand > kCandMax) {   // block-uniform: hand the row to the general kernel
         if (tid == 0) L.fb_list[atomicAdd(L.fb_count, 1)] = src * n_t + k;
         return;
     }
@@ -455,8 +448,8 @@ few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes
             if (ck[i] >= 0) { const int e = ce[i]; const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); }
     } else {
         // candidates lie in the exponent buckets of [tau, total]: ~log2(4 n_entries / eps) of them, 5-6 search steps instead of 11
-        select_core<kCandEpt>(ck, [&](int i) { return ce[i]; }, thr, (int)(tau_key >> 52), (int)(__double_as_longlong(total) >> 52), n_modes,
-                              L.owner, S, slot);
+        select_core(reg_entries<kCandEpt>(ck, ce), thr, (int)(tau_key >> 52), (int)(__double_as_longlong(total) >> 52), n_modes, L.owner, S,
+                    slot);
     }
     __syncthreads();
     unsigned* gb = L.bitmap + (size_t)src * words;
@@ -520,7 +513,7 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
         FEW_CUDA_CHECK(cudaGetLastError());
         return FEW_OK;
     }
-    FEW_REQUIRE(2 * (long long)n_modes <= FEW_MAX_SELECT_ENTRIES, FEW_ERR_LIMIT, "2*n_modes > FEW_MAX_SELECT_ENTRIES");
+    FEW_REQUIRE(n_modes <= FEW_MAX_SELECT_MODES, FEW_ERR_LIMIT, "n_modes > FEW_MAX_SELECT_MODES");
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
                     workspace_bytes >= few_select_modes_workspace(n_src, n_t, n_modes),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
@@ -529,21 +522,20 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
                                                            ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
     const dim3 grid(n_t, n_src);
-    constexpr int kNptMax = (FEW_MAX_SELECT_ENTRIES + kSelThreads - 1) / kSelThreads;
-    if (n_modes <= 16 * kSelThreads)
+    FEW_REQUIRE(sizeof(stream_shared) <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "stream kernel's shared memory exceeds the device limit");
+    FEW_CUDA_CHECK(cudaFuncSetAttribute(few_select_row_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(stream_shared)));
+    if (n_modes <= kFastModes) {
         few_select_row_fast_kernel<16><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
-    else
-        few_select_row_fast_kernel<kNptMax><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    // the rows the fast kernel left (usually none): a small persistent grid walks the list
-    const long long n_rows = (long long)n_t * n_src;
-    const unsigned fb_grid = (unsigned)(n_rows < 2LL * ctx->sm_count ? n_rows : 2LL * ctx->sm_count);
-    const size_t smem = (size_t)n_modes * sizeof(double);
-    constexpr int kEptMax = (FEW_MAX_SELECT_ENTRIES + kSelThreads - 1) / kSelThreads + 1;   // +1: primaries and mirrors are padded separately
-    if (2 * ((n_modes + kSelThreads - 1) / kSelThreads) <= 32)
-        few_select_row_kernel<32><<<fb_grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L, L.fb_list, L.fb_count);
-    else
-        few_select_row_kernel<kEptMax><<<fb_grid, kSelThreads, smem, st>>>((const double2*)amp, n_t, n_modes, eps, L, L.fb_list, L.fb_count);
+        FEW_CUDA_CHECK(cudaGetLastError());
+        // the rows the fast kernel left (usually none): a small persistent grid walks the list
+        const long long n_rows = (long long)n_t * n_src;
+        const unsigned fb_grid = (unsigned)(n_rows < ctx->sm_count ? n_rows : ctx->sm_count);
+        few_select_row_stream_kernel<<<fb_grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t, n_modes, eps, L,
+                                                                                             L.fb_list, L.fb_count);
+    } else {
+        few_select_row_stream_kernel<<<grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t, n_modes, eps, L, nullptr,
+                                                                                          nullptr);
+    }
     FEW_CUDA_CHECK(cudaGetLastError());
     few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
     FEW_CUDA_CHECK(cudaGetLastError());

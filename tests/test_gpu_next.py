@@ -368,3 +368,59 @@ def test_kerr_sum_reduces_to_schwarzschild_path(api):
     bad = np.zeros(w.n_modes, np.int32); bad[5] = 64
     api.few_sum_waveform_kerr(g["t"], coef, c3, g["l"], g["m"], dev(bad), g["n"], None, None, yp, ym, w.t0, w.dt, 16)
     assert api.few_device_status(raise_on_error=False) != 0
+
+
+# ------------------------------------------------------------------------------------------- NEXT-4 (selection part)
+def _check_keep(keep_gpu, nk_gpu, ref_keep, margin):
+    k = keep_gpu[: int(nk_gpu)]
+    assert np.all(np.diff(k) > 0) and np.all(keep_gpu[int(nk_gpu):] == -1)
+    bad = [j for j in set(k.tolist()) ^ set(ref_keep.tolist()) if not margin[j] <= 1e-12]
+    assert not bad, f"kept sets differ outside the 1e-12 band: {bad[:10]} ({len(k)} vs {len(ref_keep)})"
+
+
+@pytest.mark.parametrize("eps", [1e-5, 1e-2, 0.7])
+def test_kerr_select_rows_of_78507_entries_vs_oracle(api, eps):
+    """Rows of the Kerr-shaped grid (42 273 modes + 36 234 mirrors) do not fit any block's registers: the streaming kernel
+    recomputes the powers from the amplitudes on every pass of the selection."""
+    w = synth.make_kerr(n_samples=8, n_t=24)
+    yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), dev(w.l), dev(w.m))
+    keep, nk = api.few_select_modes(dev(w.amp), dev(w.m), yp, ym, eps)
+    api.few_device_status()
+    ref, margin = oracle.select_modes(w.amp[0], w.m, yp[0].cpu().numpy(), ym[0].cpu().numpy(), eps)
+    _check_keep(keep[0].cpu().numpy(), nk[0].item(), ref, margin)
+    assert 0 < nk[0].item() < w.n_modes
+
+
+def test_kerr_select_flat_rows_and_ties(api):
+    """Equal powers on a long row: the threshold bucket holds far more entries than the fine step sorts, so the 63-step
+    select and the 18-bit index select for ties run on streamed keys."""
+    n_modes = 20000
+    amp = np.ones((1, 3, n_modes), np.complex128)
+    m = np.zeros(n_modes, np.int32)
+    keep, nk = api.few_select_modes(dev(amp), dev(m), None, None, 0.25)
+    api.few_device_status()
+    assert nk.item() == 15000 and np.array_equal(keep[0, :15000].cpu().numpy(), np.arange(15000))
+    rng = np.random.default_rng(3)
+    amp = rng.uniform(1.0, 1.4, (1, 3, n_modes)) * np.exp(1j * rng.uniform(0, 6.28, (1, 3, n_modes)))
+    m = rng.integers(0, 3, n_modes).astype(np.int32)
+    keep, nk = api.few_select_modes(dev(amp), dev(m), None, None, 0.1)
+    ref, margin = oracle.select_modes(amp[0], m, None, None, 0.1)
+    _check_keep(keep[0].cpu().numpy(), nk[0].item(), ref, margin)
+
+
+def test_kerr_whole_path_select_fit_sum(api):
+    """S0 + S2 (streamed rows) + S1 + Kerr-shaped S3 chained on the device against O2 + O3 + O1 + O8."""
+    w = synth.make_kerr(n_samples=500, n_t=24, t0=9_000_000.0)
+    yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), dev(w.l), dev(w.m))
+    keep, nk = api.few_select_modes(dev(w.amp), dev(w.m), yp, ym, 1e-4)
+    coef = api.few_spline_fit(dev(w.t), dev(w.amp))
+    cdd = api.few_spline_fit_dd(dev(w.t), dev(w.phase))
+    h, _ = api.few_sum_waveform_kerr(dev(w.t), coef, cdd, dev(w.l), dev(w.m), dev(w.k), dev(w.n), keep, nk, yp, ym, w.t0, w.dt, w.n_samples)
+    api.few_device_status()
+    kept = keep[0, : nk[0].item()].cpu().numpy()
+    ryp, rym = oracle.ylm_modes(w.l, w.m, float(w.theta[0]), float(w.phi[0]))
+    ca = oracle.spline_fit(w.t[0], np.ascontiguousarray(w.amp[0]).view(np.float64))
+    cp = oracle.spline_fit_ext(w.t[0], w.phase[0])
+    ref = oracle.sum_waveform_kerr(w.t[0], ca, cp, w.l, w.m, w.k, w.n, kept, ryp, rym, w.t0, w.dt, w.n_samples)
+    hh = h.cpu().numpy()[0]
+    assert rel_l2(hh, ref) <= REL_L2_TOL and mismatch(hh, ref) <= MISMATCH_TOL
