@@ -230,6 +230,28 @@ def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: i
         fl = FLOP_PER_PAIR * wk.n_samples * triples
         out["kerr_shaped_sum"][label] = {"ms": ms, "sum_kernel_ms": kern_ms, "kept_modes": K, "mkn_triples": triples,
                                          "evals_per_s": wk.n_samples * K / (ms * 1e-3), "tflops_executed": fl / (kern_ms * 1e-3) / 1e12}
+    # the Kerr-shaped chain on the device: S2 on 100 rows of 78 507 entries (streamed keys), S1 on 84 546 systems, S3 on the kept list
+    amp_k = torch.as_tensor(wk.amp).to(dev)
+    ph_k = torch.as_tensor(wk.phase).to(dev)
+    sel_ws = torch.empty(api._lib.few_select_modes_workspace(1, wk.n_t, wk.n_modes), dtype=torch.uint8, device=dev)
+    keep_k = torch.empty((1, wk.n_modes), dtype=torch.int32, device=dev)
+    nkeep_k = torch.empty((1,), dtype=torch.int32, device=dev)
+    ms_sel = timed(lambda: api.few_select_modes(amp_k, mk, ypk, ymk, wk.eps, keep_idx=keep_k, n_keep=nkeep_k, workspace=sel_ws))
+    ms_fit = timed(lambda: api.few_spline_fit(tk, amp_k, out=coef))
+    nb_sel, nb_fit = 16.0 * wk.n_t * wk.n_modes, 40.0 * wk.n_t * 2 * wk.n_modes
+
+    def chain():
+        api.few_select_modes(amp_k, mk, ypk, ymk, wk.eps, keep_idx=keep_k, n_keep=nkeep_k, workspace=sel_ws)
+        api.few_spline_fit(tk, amp_k, out=coef)
+        api.few_spline_fit_dd(tk, ph_k, out=cdd)
+        api.few_sum_waveform_kerr(tk, coef, cdd, lk, mk, kk, nk_, keep_k, nkeep_k, ypk, ymk, wk.t0, wk.dt, wk.n_samples, out=hk, workspace=kws)
+    ms_chain = timed(chain)
+    Kk = int(nkeep_k.item())
+    out["kerr_shaped_chain"] = {"eps": wk.eps, "kept_modes": Kk, "step_ms": ms_chain, "evals_per_s": wk.n_samples * Kk / (ms_chain * 1e-3),
+                                "select": {"ms": ms_sel, "rows": wk.n_t, "entries_per_row": int(wk.n_modes + np.count_nonzero(wk.m > 0)),
+                                           "algorithmic_bytes": nb_sel, "gbs": nb_sel / ms_sel / 1e6},
+                                "spline_fit": {"ms": ms_fit, "algorithmic_bytes": nb_fit, "gbs": nb_fit / ms_fit / 1e6,
+                                               "hbm_frac": nb_fit / ms_fit / 1e6 / hbm_gbs}}
     return out
 
 

@@ -169,11 +169,11 @@ def few_spline_fit_dd(t, y, out=None):
     return coef
 
 
-def few_select_modes(amp, m, ylm_plus, ylm_minus, eps: float, workspace=None):
+def few_select_modes(amp, m, ylm_plus, ylm_minus, eps: float, workspace=None, keep_idx=None, n_keep=None):
     """amp [n_src, n_t, n_modes] c128 -> (keep_idx [n_src, n_modes] i32 ascending, padded -1; n_keep [n_src] i32)."""
     n_src, n_t, n_modes = amp.shape
-    keep = torch.empty((n_src, n_modes), dtype=torch.int32, device=amp.device)
-    nk = torch.empty((n_src,), dtype=torch.int32, device=amp.device)
+    keep = keep_idx if keep_idx is not None else torch.empty((n_src, n_modes), dtype=torch.int32, device=amp.device)
+    nk = n_keep if n_keep is not None else torch.empty((n_src,), dtype=torch.int32, device=amp.device)
     need = _lib.few_select_modes_workspace(n_src, n_t, n_modes)
     ws = workspace if workspace is not None else _ws(need, amp.device)
     _chk(_lib.few_select_modes(context(), _p(amp, torch.complex128), _p(m, torch.int32), _p(ylm_plus), _p(ylm_minus), float(eps),
