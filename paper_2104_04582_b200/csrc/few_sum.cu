@@ -708,7 +708,10 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
                                                           n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_CUDA_CHECK(cudaGetLastError());
-    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), 256, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
+    // few blocks (one waveform): 1024 threads finish a segment's 4 x pairs items in one sweep; a batch fills the SMs with
+    // several 256-thread blocks each, which hides the dependent index -> coefficient loads better
+    const int pack_threads = (long long)(n_t - 1) * n_src < 2LL * ctx->sm_count ? 1024 : 256;
+    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), pack_threads, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
     FEW_CUDA_CHECK(cudaGetLastError());
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
