@@ -31,7 +31,7 @@ import numpy as np  # noqa: E402
 FLOP_PER_EVAL = 20.0          # nominal per-mode figure of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA)
 FLOP_PER_PAIR = 38.0          # executed algorithm: per sample and (m,n) pair 18 DFMA + 2 DMUL = 20 FP64 slots
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
-GPU_LAUNCHES_EPS = 9          # ylm 1 + select 3 + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
+GPU_LAUNCHES_EPS = 10         # ylm 1 + select 4 (prepare, fast, streamed rest, compact) + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
 GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch, from the `ncu --set full` captures summarised in
 # profiles/r01c_kernels.md (the coefficient stream and h stay in the 126 MB L2 while the kernel runs)
