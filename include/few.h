@@ -196,6 +196,14 @@ int few_waveform(few_ctx* ctx, const double* t, const double* phase, const doubl
                  double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
                  double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Whole path for Kerr-shaped mode lists (NEXT-4): phase[n_src][n_t][3] = (Phi_phi, Phi_theta, Phi_r), k[n_modes] the polar
+ * index; selection on rows of any length (streamed), three double-double phase fits, few_sum_waveform_kerr.  Everything else
+ * as few_waveform, same workspace query. */
+int few_waveform_kerr(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                      const int* l, const int* m, const int* k, const int* n, const double* theta, const double* phi,
+                      const double* scale, double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                      double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Whole path in the detector frame: few_frame_constants -> S0 -> S2 -> S1 -> S3 with the frame factor folded in, and
  * optionally the fused inner products against a resident data stream d (h may be NULL when inner is given).
  * sky[n_src][4], mu_over_dl[n_src] or NULL as in few_frame_constants; d, inner as in few_sum_waveform_ex.  Same workspace

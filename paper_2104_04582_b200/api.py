@@ -22,7 +22,7 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_fp64_mix_probe", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
            "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
-           "few_sum_direct", "few_sum_waveform_kerr"]
+           "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr"]
 
 
 class FewError(RuntimeError):
@@ -56,6 +56,7 @@ def _load() -> C.CDLL:
         "few_sum_waveform": (i, [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, d, d, ll, vp, i, i, i, vp, sz, vp]),
         "few_waveform_workspace": (sz, [i, i, i, ll]),
         "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
+        "few_waveform_kerr": (i, [vp] * 11 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
         "few_sum_waveform_ex": (i, [vp] * 13 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
         "few_sum_waveform_kerr": (i, [vp, vp, vp, vp, i] + [vp] * 10 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
@@ -310,6 +311,19 @@ def few_waveform(t, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: 
                            _p(m, torch.int32), _p(n, torch.int32), _p(theta, torch.float64), _p(phi, torch.float64), _p(scale),
                            float(eps), float(t0), float(dt), int(n_samples), n_src, n_t, n_modes, _p(h), _p(keep_idx), _p(n_keep),
                            _p(ws), ws.numel(), _stream()), "few_waveform")
+    return h
+
+
+def few_waveform_kerr(t, phase, amp, l, m, k, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int, scale=None,
+                      out=None, keep_idx=None, n_keep=None, workspace=None):
+    """Whole path for Kerr-shaped mode lists: phase [n_src, n_t, 3] = (Phi_phi, Phi_theta, Phi_r), k [n_modes] i32."""
+    n_src, n_t, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    ws = workspace if workspace is not None else _ws(few_waveform_workspace(n_src, n_t, n_modes, n_samples), t.device)
+    _chk(_lib.few_waveform_kerr(context(), _p(t, torch.float64), _p(phase, torch.float64), _p(amp, torch.complex128), _p(l, torch.int32),
+                                _p(m, torch.int32), _p(k, torch.int32), _p(n, torch.int32), _p(theta, torch.float64),
+                                _p(phi, torch.float64), _p(scale), float(eps), float(t0), float(dt), int(n_samples), n_src, n_t, n_modes,
+                                _p(h), _p(keep_idx), _p(n_keep), _p(ws), ws.numel(), _stream()), "few_waveform_kerr")
     return h
 
 

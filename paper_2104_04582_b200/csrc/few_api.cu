@@ -133,7 +133,7 @@ wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_sample
     L.ylm_plus = c.take<double>((size_t)n_src * n_modes * 2);
     L.ylm_minus = c.take<double>((size_t)n_src * n_modes * 2);
     L.coef_amp = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 2 * n_modes);
-    L.coef_phase = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 2 * 2);
+    L.coef_phase = c.take<double>((size_t)n_src * (n_t - 1) * 4 * 3 * 2);      // up to three phases (Kerr-shaped lists)
     L.keep_idx = c.take<int>((size_t)n_src * n_modes);
     L.n_keep = c.take<int>(n_src);
     L.theta_src = c.take<double>(n_src);
@@ -160,8 +160,8 @@ extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long l
 
 namespace {
 // theta/phi: source-frame viewing angles, or (sky != NULL) computed from the detector-frame angles by few_frame_constants.
-int waveform_impl(few_ctx* ctx, const double* t, const double* phase, const double* amp, const int* l, const int* m, const int* n,
-                  const double* theta, const double* phi, const double* sky, const double* scale, double eps, double t0, double dt,
+int waveform_impl(few_ctx* ctx, const double* t, const double* phase, int n_phase, const double* amp, const int* l, const int* m,
+                  const int* k, const int* n, const double* theta, const double* phi, const double* sky, const double* scale, double eps, double t0, double dt,
                   long long n_samples, int n_src, int n_t, int n_modes, double* h, const double* d, double* inner, int* keep_idx,
                   int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
 {
@@ -182,7 +182,7 @@ int waveform_impl(few_ctx* ctx, const double* t, const double* phase, const doub
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[0], ctx->ev_fork, 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[1], ctx->ev_fork, 0));
     if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]))) return rc;
-    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, 2, L.coef_phase, ctx->side[1]))) return rc;
+    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, n_phase, L.coef_phase, ctx->side[1]))) return rc;
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[0], ctx->side[0]));
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[1], ctx->side[1]));
     const double* factor = nullptr;
@@ -194,8 +194,8 @@ int waveform_impl(few_ctx* ctx, const double* t, const double* phase, const doub
     if ((rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream))) return rc;
     FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[0], 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[1], 0));
-    return few_sum_waveform_ex(ctx, t, L.coef_amp, L.coef_phase, l, m, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, factor, t0, dt,
-                               n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
+    return few_sum_waveform_kerr(ctx, t, L.coef_amp, L.coef_phase, n_phase, l, m, k, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, factor,
+                                 t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
 }
 }  // namespace
 
@@ -206,7 +206,18 @@ extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, 
 {
     FEW_REQUIRE(theta && phi, FEW_ERR_INVALID_ARG, "theta or phi is NULL");
     FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
-    return waveform_impl(ctx, t, phase, amp, l, m, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
+    return waveform_impl(ctx, t, phase, 2, amp, l, m, nullptr, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
+                         nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
+}
+
+extern "C" int few_waveform_kerr(few_ctx* ctx, const double* t, const double* phase, const double* amp,
+                                 const int* l, const int* m, const int* k, const int* n, const double* theta, const double* phi,
+                                 const double* scale, double eps, double t0, double dt, long long n_samples, int n_src, int n_t,
+                                 int n_modes, double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(theta && phi && k, FEW_ERR_INVALID_ARG, "theta, phi or k is NULL");
+    FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
+    return waveform_impl(ctx, t, phase, 3, amp, l, m, k, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
                          nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 
@@ -218,7 +229,7 @@ extern "C" int few_waveform_ssb(few_ctx* ctx, const double* t, const double* pha
 {
     FEW_REQUIRE(sky != nullptr, FEW_ERR_INVALID_ARG, "sky is NULL");
     FEW_REQUIRE(n_samples == 0 || h || inner, FEW_ERR_INVALID_ARG, "h and inner are both NULL");
-    return waveform_impl(ctx, t, phase, amp, l, m, n, nullptr, nullptr, sky, mu_over_dl, eps, t0, dt, n_samples, n_src, n_t, n_modes,
+    return waveform_impl(ctx, t, phase, 2, amp, l, m, nullptr, n, nullptr, nullptr, sky, mu_over_dl, eps, t0, dt, n_samples, n_src, n_t, n_modes,
                          h, d, inner, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 

@@ -424,3 +424,9 @@ def test_kerr_whole_path_select_fit_sum(api):
     ref = oracle.sum_waveform_kerr(w.t[0], ca, cp, w.l, w.m, w.k, w.n, kept, ryp, rym, w.t0, w.dt, w.n_samples)
     hh = h.cpu().numpy()[0]
     assert rel_l2(hh, ref) <= REL_L2_TOL and mismatch(hh, ref) <= MISMATCH_TOL
+    # the single C call (few_waveform_kerr: fits on side streams, nothing read back) gives the same bits
+    keep2 = torch.empty_like(keep); nk2 = torch.empty_like(nk)
+    h2 = api.few_waveform_kerr(dev(w.t), dev(w.phase), dev(w.amp), dev(w.l), dev(w.m), dev(w.k), dev(w.n), dev(w.theta), dev(w.phi),
+                               1e-4, w.t0, w.dt, w.n_samples, keep_idx=keep2, n_keep=nk2)
+    api.few_device_status()
+    assert torch.equal(keep2, keep) and torch.equal(nk2, nk) and torch.equal(h2, h)
