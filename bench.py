@@ -357,6 +357,12 @@ def main():
     mix_flops = api.few_fp64_mix_probe(148 * 3, 20000, sink)
     e1.record(); torch.cuda.synchronize()
     fp64_mix_tflops = mix_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
+    # the same arithmetic in FP64 tensor-core form (DMMA.8x8x4): what an MMA formulation of the summation could sustain
+    api.few_fp64_mma_probe(148 * 3, 2000, sink)
+    torch.cuda.synchronize(); e0.record()
+    mma_flops = api.few_fp64_mma_probe(148 * 3, 20000, sink)
+    e1.record(); torch.cuda.synchronize()
+    fp64_mma_tflops = mma_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
 
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
@@ -430,6 +436,7 @@ def main():
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
                 "peak_measured_hot_mix_probe": fp64_mix_tflops, "frac_of_hot_mix_probe": achieved_tflops / fp64_mix_tflops,
+                "peak_measured_mma_form_probe": fp64_mma_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
                 "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {pair_evals_per_step:.4g} "
                                f"pair evaluations per launch ({pairs} pairs from {K_kept} kept modes)",

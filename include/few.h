@@ -238,6 +238,12 @@ int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double
  * form (three register operands per DFMA) on the device, below the register-resident DFMA-chain figure. */
 int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream);
 
+/* ---- Measurement aid: the same arithmetic in FP64 tensor-core form (DMMA.8x8x4 = mma.sync.m8n8k4.f64): per warp step
+ * 4 sample groups x (a complex rotation per lane + two 8x8x4 MMAs whose B fragments come from shared memory).  Per thread and
+ * step 8 DMUL + 8 DFMA and 8 MMAs of 8 FMA per lane: FLOPs = 152 * iters * blocks * 128 (as few_fp64_mix_probe).  The ceiling of the
+ * MMA formulation of the summation. */
+int few_fp64_mma_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream);
+
 /* ---- Measurement aid: with profiling on, few_sum_waveform (also inside few_waveform) brackets its hot kernel
  * (few_sum_kernel, the dominant launch of the path) with two CUDA events on the caller's stream.  few_profile_sum_ms
  * waits for the closing event of the most recent launch and writes its duration in milliseconds to ms_host.

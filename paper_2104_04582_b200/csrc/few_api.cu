@@ -416,3 +416,57 @@ extern "C" int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* s
     FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// FP64 MMA-form probe: the same arithmetic as few_fp64_mix_kernel arranged for DMMA.8x8x4 (mma.sync.m8n8k4.f64): a warp holds
+// 8 samples x 4 pair streams per sample group (lane = 4 * sample + stream), rotates its E (2 DMUL + 2 DFMA per lane and group)
+// and contracts acc[8 samples][4 powers x re/im] += E_r[8 x 4] U[4 x 8], += E_i[8 x 4] V[4 x 8] with two DMMA whose B
+// fragments come from shared memory by one LDS.64 per lane.  4 sample groups per warp, 128 threads per block.
+// 20 FP64 lane-operations per sample and pair, as in the DFMA form (4 + 2 x 8 FMA).  DESIGN.md section 5.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void few_dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(128) few_fp64_mma_kernel(int iters, double* sink, const double* seed)
+{
+    __shared__ __align__(16) double cs[8 * 64];
+    for (int i = threadIdx.x; i < 8 * 64; i += 128) cs[i] = seed[i & 15] * (1 + i);
+    __syncthreads();
+    constexpr int G = 4;
+    const int lane = threadIdx.x & 31;
+    double c0[G], c1[G], er[G], ei[G], zr[G], zi[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        sincos(1e-3 * (threadIdx.x + 128 * g + 1), &zi[g], &zr[g]);
+        c0[g] = c1[g] = 0.0; er[g] = 1.0; ei[g] = 0.0;
+    }
+    for (int it = 0; it < iters; ++it) {
+        const double* f = cs + (it & 7) * 64;
+        const double u = f[lane], v = f[32 + lane];
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const double m1 = ei[g] * zi[g], m2 = ei[g] * zr[g], e0 = er[g];
+            er[g] = fma(e0, zr[g], -m1);
+            ei[g] = fma(e0, zi[g], m2);
+        }
+#pragma unroll
+        for (int g = 0; g < G; ++g) few_dmma884(c0[g], c1[g], er[g], u);
+#pragma unroll
+        for (int g = 0; g < G; ++g) few_dmma884(c0[g], c1[g], ei[g], v);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int g = 0; g < G; ++g) s += c0[g] + c1[g];
+    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int few_fp64_mma_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream)
+{
+    FEW_REQUIRE(ctx && sink && seed, FEW_ERR_INVALID_ARG, "NULL argument");
+    FEW_REQUIRE(blocks > 0 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
+    few_fp64_mma_kernel<<<blocks, 128, 0, (cudaStream_t)stream>>>(iters, sink, seed);
+    FEW_CUDA_CHECK(cudaGetLastError());
+    return FEW_OK;
+}
