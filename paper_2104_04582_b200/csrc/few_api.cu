@@ -446,15 +446,13 @@ __global__ void __launch_bounds__(128) few_fp64_mma_kernel(int iters, double* si
         const double* f = cs + (it & 7) * 64;
         const double u = f[lane], v = f[32 + lane];
 #pragma unroll
-        for (int g = 0; g < G; ++g) {
+        for (int g = 0; g < G; ++g) {               // per group: rotate, contract (the compiler pipelines the groups)
             const double m1 = ei[g] * zi[g], m2 = ei[g] * zr[g], e0 = er[g];
             er[g] = fma(e0, zr[g], -m1);
             ei[g] = fma(e0, zi[g], m2);
+            few_dmma884(c0[g], c1[g], er[g], u);
+            few_dmma884(c0[g], c1[g], ei[g], v);
         }
-#pragma unroll
-        for (int g = 0; g < G; ++g) few_dmma884(c0[g], c1[g], er[g], u);
-#pragma unroll
-        for (int g = 0; g < G; ++g) few_dmma884(c0[g], c1[g], ei[g], v);
     }
     double s = 0.0;
 #pragma unroll
