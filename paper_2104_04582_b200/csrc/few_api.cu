@@ -78,6 +78,7 @@ extern "C" int few_destroy(few_ctx* ctx)
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     for (int g = 0; g < kHostGroups; ++g) if (ctx->ev_group[g]) cudaEventDestroy(ctx->ev_group[g]);
     cudaFree(ctx->host_arena);
+    if (ctx->host_stage) cudaFreeHost(ctx->host_stage);
     delete ctx;
     return FEW_OK;
 }
@@ -262,11 +263,13 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
             (void)cudaGetLastError();
     }
     const size_t b_h_dev = h_mapped ? 0 : b_h;
-    // one device allocation, carved
+    // one device allocation, carved: the small inputs first and contiguous (they travel as one block), then amp, h, outputs
     size_t total = 0;
     few_carver sz(nullptr);
-    sz.take<char>(b_t); sz.take<char>(b_ph); sz.take<char>(b_amp); sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_lmn);
-    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_h_dev); sz.take<char>(b_keep); sz.take<char>(b_nk);
+    sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_t); sz.take<char>(b_ph);
+    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang);
+    const size_t small_bytes = sz.off;
+    sz.take<char>(b_amp); sz.take<char>(b_h_dev); sz.take<char>(b_keep); sz.take<char>(b_nk);
     sz.take<char>(ws_bytes);
     total = sz.off;
     // device arena and stream are kept in the context between calls (grow-only), so a steady-state call allocates nothing
@@ -274,6 +277,11 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
         if (ctx->host_arena) { FEW_CUDA_CHECK(cudaFree(ctx->host_arena)); ctx->host_arena = nullptr; ctx->host_arena_bytes = 0; }
         FEW_CUDA_CHECK(cudaMalloc(&ctx->host_arena, total));
         ctx->host_arena_bytes = total;
+    }
+    if (small_bytes > ctx->host_stage_bytes) {
+        if (ctx->host_stage) { FEW_CUDA_CHECK(cudaFreeHost(ctx->host_stage)); ctx->host_stage = nullptr; ctx->host_stage_bytes = 0; }
+        FEW_CUDA_CHECK(cudaHostAlloc(&ctx->host_stage, small_bytes, cudaHostAllocDefault));
+        ctx->host_stage_bytes = small_bytes;
     }
     if (!ctx->host_stream) {
         FEW_CUDA_CHECK(cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
@@ -285,28 +293,36 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     int rc = FEW_OK;
     cudaError_t e = cudaSuccess;
     few_carver c(dev);
-    double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph); double* d_amp = (double*)c.take<char>(b_amp);
     int* d_l = (int*)c.take<char>(b_lmn); int* d_m = (int*)c.take<char>(b_lmn); int* d_n = (int*)c.take<char>(b_lmn);
+    double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph);
     double* d_th = (double*)c.take<char>(b_ang); double* d_phi = (double*)c.take<char>(b_ang); double* d_sc = (double*)c.take<char>(b_ang);
+    double* d_amp = (double*)c.take<char>(b_amp);
     double* d_h = (double*)c.take<char>(b_h_dev); int* d_keep = (int*)c.take<char>(b_keep); int* d_nk = (int*)c.take<char>(b_nk);
     void* d_ws = c.take<char>(ws_bytes);
-    // Sources are independent, so a batch is cut into up to kHostGroups groups: the inputs of every group go host->device
-    // on a copy stream, and group g's kernels start as soon as ITS inputs have landed, i.e. while later groups are still in
-    // flight over PCIe.  (One source: one group; its 6 MB of inputs precede everything.)
+    // The small inputs (mode indices, sparse times, phases, angles: tens of KB) are gathered into a pinned staging block
+    // with the arena's own layout and go up as ONE copy; the amplitudes follow source group by source group.
+    // Sources are independent, so a batch is cut into up to kHostGroups groups: group g's kernels start as soon as ITS
+    // amplitudes have landed, i.e. while later groups are still in flight over PCIe.  (One source: one group.)
+    {
+        char* hs = static_cast<char*>(ctx->host_stage);
+        few_carver hc(hs);
+        memcpy(hc.take<char>(b_lmn), l_host, b_lmn); memcpy(hc.take<char>(b_lmn), m_host, b_lmn); memcpy(hc.take<char>(b_lmn), n_host, b_lmn);
+        memcpy(hc.take<char>(b_t), t_host, b_t); memcpy(hc.take<char>(b_ph), phase_host, b_ph);
+        memcpy(hc.take<char>(b_ang), theta_host, b_ang); memcpy(hc.take<char>(b_ang), phi_host, b_ang);
+        char* sc = hc.take<char>(b_ang);
+        if (scale_host) memcpy(sc, scale_host, b_ang);
+    }
     const int n_groups = n_src < kHostGroups ? n_src : kHostGroups;
     cudaStream_t cs = ctx->copy_stream;
-#define FEW_H2D(dst, src, bytes) if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, cs)
-    FEW_H2D(d_l, l_host, b_lmn); FEW_H2D(d_m, m_host, b_lmn); FEW_H2D(d_n, n_host, b_lmn);
+    // the staging block is reused by the next call: that call's memcpy must not overtake this copy, which the final
+    // synchronisation of this call guarantees
+    e = cudaMemcpyAsync(dev, ctx->host_stage, small_bytes, cudaMemcpyHostToDevice, cs);
     for (int g = 0; g < n_groups && e == cudaSuccess; ++g) {
         const size_t s0 = (size_t)n_src * g / n_groups, s1 = (size_t)n_src * (g + 1) / n_groups, ns = s1 - s0;
-        FEW_H2D(d_t + s0 * n_t, t_host + s0 * n_t, ns * n_t * 8);
-        FEW_H2D(d_ph + s0 * n_t * 2, phase_host + s0 * n_t * 2, ns * n_t * 16);
-        FEW_H2D(d_th + s0, theta_host + s0, ns * 8); FEW_H2D(d_phi + s0, phi_host + s0, ns * 8);
-        if (scale_host) FEW_H2D(d_sc + s0, scale_host + s0, ns * 8);
-        FEW_H2D(d_amp + s0 * n_t * n_modes * 2, amp_host + s0 * n_t * n_modes * 2, ns * n_t * n_modes * 16);
+        e = cudaMemcpyAsync(d_amp + s0 * n_t * n_modes * 2, amp_host + s0 * n_t * n_modes * 2, ns * n_t * n_modes * 16,
+                            cudaMemcpyHostToDevice, cs);
         if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_group[g], cs);
     }
-#undef FEW_H2D
     double* h_out = h_mapped ? h_mapped : d_h;
     for (int g = 0; g < n_groups && e == cudaSuccess && rc == FEW_OK; ++g) {
         const size_t s0 = (size_t)n_src * g / n_groups, s1 = (size_t)n_src * (g + 1) / n_groups, ns = s1 - s0;

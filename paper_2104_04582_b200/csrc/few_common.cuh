@@ -19,6 +19,8 @@ struct few_ctx {
     cudaEvent_t ev_fork, ev_join[2];
     void* host_arena;      // few_waveform_host: grow-only device arena (inputs, h, workspace), freed by few_destroy
     size_t host_arena_bytes;
+    void* host_stage;      // few_waveform_host: pinned staging block for the small inputs (one host->device copy instead of eight)
+    size_t host_stage_bytes;
     cudaStream_t host_stream, copy_stream;   // few_waveform_host: kernels / host->device copies
     cudaEvent_t ev_group[8];                 // inputs of source group g have landed
 };
