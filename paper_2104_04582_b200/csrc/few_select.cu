@@ -399,16 +399,16 @@ few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes
         kp[i] = km[i] = -1;
         const int j = i * kSelThreads + tid;
         if (j < n_modes) {
+            // branch-free, so that all of a thread's loads are in flight together (y2m is 0 where there is no mirror)
             const double2 v = a[j];
+            const double wp = y2p[j], wm = y2m[j];
+            const bool has_mirror = L.mirror_e[j] >= 0;
             const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
-            const double p = __dmul_rn(a2, y2p[j]);
+            const double p = __dmul_rn(a2, wp), pm = __dmul_rn(a2, wm);
             kp[i] = __double_as_longlong(p);
+            km[i] = has_mirror ? __double_as_longlong(pm) : -1;
             t4[i & 1] += p;
-            if (L.mirror_e[j] >= 0) {
-                const double pm = __dmul_rn(a2, y2m[j]);
-                km[i] = __double_as_longlong(pm);
-                t4[2 + (i & 1)] += pm;
-            }
+            t4[2 + (i & 1)] += has_mirror ? pm : 0.0;
         }
     }
     const double total = block_sum((t4[0] + t4[1]) + (t4[2] + t4[3]), S.red, slot);
