@@ -12,7 +12,7 @@
 // of all entries with a strictly larger key (plus earlier ties), G is monotone in the key, so the kept entries are exactly
 // those with key >= kappa, kappa = min{k : G(k) < (1-eps) C_last}.  The kernels therefore SELECT instead of sorting the row
 // (select_core, one block per row, nothing but the row's amplitudes read from HBM):
-//   1. coarse: the key's top 11 bits are the binary exponent of the power.  A binary search over the exponent buckets, each
+//   1. coarse: the key's top 14 bits are the binary exponent of the power and 3 mantissa bits.  A binary search over these buckets, each
 //      step one masked block reduction, finds the bucket B in which the cumulative sum crosses the threshold.  Every entry
 //      in a higher bucket is kept, every entry in a lower one dropped.
 //   2. fine: the entries of bucket B are compacted into shared memory, rank-sorted by (power descending, entry index
@@ -35,7 +35,8 @@ namespace {
 constexpr int kSelThreads = 256;
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kPrepThreads = 1024;
-constexpr int kBucketMax = 512;   // entries of the threshold's exponent bucket that the fine step sorts in shared memory
+constexpr int kBucketMax = 512;   // entries of the threshold's bucket that the fine step sorts in shared memory
+constexpr int kBucketShift = 49;  // bucket of a key = its top 14 bits: the power's binary exponent and 3 mantissa bits (an eighth of a binade)
 
 struct sel_layout {
     int* owner;       // [n_modes]   owner mode of mirror entry e - n_modes   (shared by sources)
@@ -231,19 +232,20 @@ __device__ __forceinline__ void select_core(const Entries& E, double thr, int b_
         E.for_each([&](long long k, int e, int) { if (k == kappa) { const long long c = -(long long)e; best = c > best ? c : best; } });
         iota = (int)(-block_max_ll(best, S.red, slot));
     } else {
-        // ---- 1. coarse: g(x) = sum of powers with exponent bucket >= x (bucket = key >> 52) is non-increasing in x;
+        // ---- 1. coarse: g(x) = sum of powers with bucket >= x (bucket = key >> kBucketShift) is non-increasing in x;
         // B = the largest x in [b_lo, b_hi] with g(x) >= thr (the fixed reduction tree keeps monotonicity exactly).
         int s_lo = b_lo, s_hi = b_hi;
         while (s_lo < s_hi) {
             const int mid = (s_lo + s_hi + 1) >> 1;
-            const int cand_hi = mid << 20;                 // the bucket lives in the key's high word: one 32-bit compare
+            const int cand_hi = mid << (kBucketShift - 32);   // the bucket lives in the key's high word: one 32-bit compare
             double g4[4] = {0.0, 0.0, 0.0, 0.0};          // several chains: the DADD latency, not its rate, bounds this loop
             E.for_each([&](long long k, int, int c) { if ((int)(k >> 32) >= cand_hi) g4[c] += __longlong_as_double(k); });
             const double g = block_sum((g4[0] + g4[1]) + (g4[2] + g4[3]), S.red, slot);
             if (!(g < thr)) s_lo = mid; else s_hi = mid - 1;
         }
         const long long B = s_lo;
-        const long long k_lo = B << 52, k_hi = B >= 2047 ? 0x7fffffffffffffffLL : (B + 1) << 52;   // bucket B = keys in [k_lo, k_hi)
+        const long long k_lo = B << kBucketShift;                   // bucket B = keys in [k_lo, k_hi)
+        const long long k_hi = B >= (1ll << (63 - kBucketShift)) - 1 ? 0x7fffffffffffffffLL : (B + 1) << kBucketShift;
         double ga = 0.0; long long nb = 0;
         E.for_each([&](long long k, int, int) { ga += k >= k_hi ? __longlong_as_double(k) : 0.0; nb += (k >= k_lo && k < k_hi) ? 1 : 0; });
         const double g_above = block_sum(ga, S.red, slot);           // < thr by construction
@@ -351,8 +353,8 @@ few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_mod
         const double total = block_sum((t2[0] + t2[1]) + (0.0 + 0.0), S.red, slot);      // the same tree as the core's g(0)
         // buckets below that of tau = eps total / (4 n) hold less than eps total / 4 altogether: the search starts there
         const long long tau_key = __double_as_longlong(0.25 * eps * total / (double)n_ent);
-        const int b_lo = (eps > 1e-10 && tau_key > 0) ? (int)(tau_key >> 52) : 0;
-        select_core(E, (1.0 - eps) * total, b_lo, (int)(__double_as_longlong(total) >> 52), n_modes, L.owner, S, slot);
+        const int b_lo = (eps > 1e-10 && tau_key > 0) ? (int)(tau_key >> kBucketShift) : 0;
+        select_core(E, (1.0 - eps) * total, b_lo, (int)(__double_as_longlong(total) >> kBucketShift), n_modes, L.owner, S, slot);
         __syncthreads();
         unsigned* gb = L.bitmap + (size_t)src * words;
         for (int w = tid; w < words; w += kStreamThreads)
@@ -448,7 +450,8 @@ few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes
             if (ck[i] >= 0) { const int e = ce[i]; const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); }
     } else {
         // candidates lie in the exponent buckets of [tau, total]: ~log2(4 n_entries / eps) of them, 5-6 search steps instead of 11
-        select_core(reg_entries<kCandEpt>(ck, ce), thr, (int)(tau_key >> 52), (int)(__double_as_longlong(total) >> 52), n_modes, L.owner, S,
+        select_core(reg_entries<kCandEpt>(ck, ce), thr, (int)(tau_key >> kBucketShift), (int)(__double_as_longlong(total) >> kBucketShift), n_modes,
+                    L.owner, S,
                     slot);
     }
     __syncthreads();
