@@ -375,3 +375,20 @@ def test_full_size_sampled_parity(api, cfg):
     idx = np.arange(7, N, 4099 if cfg == 1 else 40_009)
     one = np.concatenate(oracle_with_gpu_keep(w, 0, keep[0][: nk[0]], [(int(i), 1) for i in idx]))
     assert rel_l2(h[0][idx], one) <= REL_L2_TOL
+
+
+def test_fp64_probes_run_and_are_ordered(api):
+    """The three measurement aids of bench.py launch and give finite sinks; their known ordering on this chip (register-resident
+    DFMA chains > MMA form > three-operand DFMA form) is what DESIGN.md section 5 builds on."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    rates = {}
+    for name, fn in (("dfma", lambda it: api.few_fp64_peak_probe(148 * 8, 256, it)),
+                     ("mix", lambda it: api.few_fp64_mix_probe(148 * 3, it)),
+                     ("mma", lambda it: api.few_fp64_mma_probe(148 * 3, it))):
+        fn(500); torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record(); flops = fn(5000); b.record(); torch.cuda.synchronize()
+        rates[name] = flops / (a.elapsed_time(b) * 1e-3) / 1e12
+    api.few_device_status()
+    assert all(np.isfinite(v) and v > 1.0 for v in rates.values()), rates
+    assert rates["dfma"] > rates["mma"] > rates["mix"], rates
