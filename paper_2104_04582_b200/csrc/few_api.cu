@@ -404,16 +404,20 @@ __global__ void __launch_bounds__(128) few_fp64_mix_kernel(int iters, double* si
             ei[r] = fma(e0, zi[r], m2);
         }
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
+        for (int p = 0; p < 4; ++p) {               // the kernel's order: samples walked in alternating directions
             const double2 u = cp[p];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { are[p][r] = fma(er[r], u.x, are[p][r]); aim[p][r] = fma(er[r], u.y, aim[p][r]); }
+            for (int r = 0; r < R; ++r) are[p][r] = fma(er[r], u.x, are[p][r]);
+#pragma unroll
+            for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(er[r], u.y, aim[p][r]);
         }
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             const double2 v = cp[4 + p];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { are[p][r] = fma(ei[r], v.x, are[p][r]); aim[p][r] = fma(ei[r], v.y, aim[p][r]); }
+            for (int r = 0; r < R; ++r) are[p][r] = fma(ei[r], v.x, are[p][r]);
+#pragma unroll
+            for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(ei[r], v.y, aim[p][r]);
         }
     }
     double s = 0.0;

@@ -402,8 +402,9 @@ __device__ __forceinline__ void advance_e(double (&er)[R], double (&ei)[R], cons
 }
 
 // acc_p += e_r U_p + e_i V_p for the four powers p of dx.  Every DFMA has one block-uniform operand (a coefficient, shared by
-// the R samples of the thread) and two per-thread ones: the form the FP64 pipe sustains at one warp instruction per two
-// cycles (three fresh per-thread register operands cost three).
+// the R samples of the thread) and two per-thread ones.  A DFMA that reads three registers none of which sits in the
+// operand-reuse cache costs the FP64 pipe about one cycle more than the usual two, so the R samples are
+// walked in alternating directions from one coefficient to the next: where the coefficient changes, e stays the same.
 template <int R>
 __device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, const double (&er)[R], const double (&ei)[R],
                                                 double (&are)[4][R], double (&aim)[4][R])
@@ -412,13 +413,17 @@ __device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, 
     for (int p = 0; p < 4; ++p) {
         const double2 u = cp[p];
 #pragma unroll
-        for (int r = 0; r < R; ++r) { are[p][r] = fma(er[r], u.x, are[p][r]); aim[p][r] = fma(er[r], u.y, aim[p][r]); }
+        for (int r = 0; r < R; ++r) are[p][r] = fma(er[r], u.x, are[p][r]);
+#pragma unroll
+        for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(er[r], u.y, aim[p][r]);
     }
 #pragma unroll
     for (int p = 0; p < 4; ++p) {
         const double2 v = cp[4 + p];
 #pragma unroll
-        for (int r = 0; r < R; ++r) { are[p][r] = fma(ei[r], v.x, are[p][r]); aim[p][r] = fma(ei[r], v.y, aim[p][r]); }
+        for (int r = 0; r < R; ++r) are[p][r] = fma(ei[r], v.x, are[p][r]);
+#pragma unroll
+        for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(ei[r], v.y, aim[p][r]);
     }
 }
 
