@@ -34,8 +34,8 @@ DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (pub
 GPU_LAUNCHES_EPS = 10         # ylm 1 + select 4 (prepare, fast, streamed rest, compact) + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
 GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch, from the `ncu --set full` captures summarised in
-# profiles/r01d_kernels.md (config 1) and profiles/r01c_kernels.md (config 2) (the coefficient stream and h stay in the 126 MB L2 while the kernel runs)
-SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 4.56e6, "config2_1yr_allmodes": 10.39e6}
+# profiles/r01d_kernels.md (the coefficient stream and h stay in the 126 MB L2 while the kernel runs)
+SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 4.84e6, "config2_1yr_allmodes": 10.62e6}
 
 
 def load_peaks():
