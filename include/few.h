@@ -18,9 +18,15 @@
  *   - Pointers are DEVICE pointers (on the context's device) unless the name or comment says "host".
  *   - Ownership: the caller owns every input, output and workspace buffer.  The library keeps only a few KB of
  *     state in few_ctx (plus, if few_waveform_host is used, its device arena).  Workspace sizes come from the *_workspace() queries; workspaces need 256-byte alignment.
- *   - All work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as void*; NULL = legacy
+ *   - All work is ordered on the caller's stream (`stream` is a cudaStream_t passed as void*; NULL = legacy
  *     default stream).  No device-pointer call synchronises; n_keep stays on the device so S2 -> S1 -> S3 chain
  *     without a host round trip.  Only few_waveform_host and few_device_status synchronise.
+ *     few_waveform, few_waveform_kerr and few_waveform_ssb run the two spline fits on two internal streams of the
+ *     context, forked from and joined back into the caller's stream with events (on every return path, failing or not).
+ *   - Threading and devices: a few_ctx serves ONE host thread at a time (its internal streams, events, profiling pair and
+ *     host arena are not locked); use one context per thread.  Device-pointer entry points expect the context's device to
+ *     be the calling thread's current device; few_create and few_waveform_host switch to it themselves and restore the
+ *     caller's current device before returning.
  *   - Shapes are validated on the host (FEW_ERR_INVALID_ARG, FEW_ERR_TOO_FEW_POINTS, FEW_ERR_LIMIT).  Data that
  *     lives on the device (t increasing, (l,m,n) validity) is checked by the kernels, which OR a FEW_DEV_* bit into a
  *     device status word read back by few_device_status().  Outputs are unspecified when a bit is set.
@@ -218,7 +224,7 @@ int few_waveform_ssb(few_ctx* ctx, const double* t, const double* phase, const d
  * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform and delivers h
  * (and keep_idx/n_keep if not NULL) to the host, then synchronises.  If h_host is page-locked (cudaHostAlloc /
  * cudaHostRegister / torch pin_memory) the summation kernel stores into it directly, so the device->host transfer overlaps
- * the computation; pageable h_host is filled by a copy after the kernels.  Not re-entrant on one context.  `scale_host` may
+ * the computation; pageable h_host is filled by a copy after the kernels.  Like every call, not re-entrant on one context.  `scale_host` may
  * be NULL.  Returns the device status as well. */
 int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
                       const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
@@ -231,25 +237,16 @@ int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_ho
  * to sink[blocks*threads].  FLOPs = 2 * 16 * iters * blocks * threads. */
 int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int iters, double* sink, void* stream);
 
-/* ---- Measurement aid: the instruction mix of few_sum_kernel's hot loop and nothing else: `blocks` x 128
- * threads, each running `iters` pair steps for 4 samples = 72 DFMA + 8 DMUL per step, the 8 complex coefficients of a step
- * read from shared memory with broadcast 128-bit loads.  seed[16] (device) fills the coefficient table; one double per thread
- * is written to sink[blocks*128].  FLOPs = 152 * iters * blocks * 128.  What it sustains is the ceiling of this instruction
- * form (three register operands per DFMA) on the device, below the register-resident DFMA-chain figure. */
-int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream);
-
-/* ---- Measurement aid: the same arithmetic in FP64 tensor-core form (DMMA.8x8x4 = mma.sync.m8n8k4.f64): per warp step
- * 4 sample groups x (a complex rotation per lane + two 8x8x4 MMAs whose B fragments come from shared memory).  Per thread and
- * step 8 DMUL + 8 DFMA and 8 MMAs of 8 FMA per lane: FLOPs = 152 * iters * blocks * 128 (as few_fp64_mix_probe).  The ceiling of the
- * MMA formulation of the summation. */
-int few_fp64_mma_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream);
-
 /* ---- Measurement aid: with profiling on, few_sum_waveform (also inside few_waveform) brackets its hot kernel
  * (few_sum_kernel, the dominant launch of the path) with two CUDA events on the caller's stream.  few_profile_sum_ms
  * waits for the closing event of the most recent launch and writes its duration in milliseconds to ms_host.
  * FEW_ERR_INVALID_ARG if profiling is off or nothing was launched since it was switched on. */
 int few_profile_enable(few_ctx* ctx, int on);
 int few_profile_sum_ms(few_ctx* ctx, float* ms_host);
+
+/* ---- Measurement aid: number of kernels this library has launched through `ctx` since few_create (every launch site
+ * counts itself), written to count_host.  bench.py reports the difference over its timed region as `gpu_launches`. */
+int few_launch_count(few_ctx* ctx, long long* count_host);
 
 #ifdef __cplusplus
 }

@@ -20,7 +20,7 @@ FEW_OK = 0
 SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_version", "few_device_status", "few_ylm",
            "few_ylm_modes", "few_spline_fit_workspace", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
-           "few_fp64_peak_probe", "few_fp64_mix_probe", "few_fp64_mma_probe", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
+           "few_fp64_peak_probe", "few_launch_count", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
            "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
            "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr"]
 
@@ -68,8 +68,7 @@ def _load() -> C.CDLL:
         "few_sum_direct_workspace": (sz, [i, i]),
         "few_sum_direct": (i, [vp] * 10 + [ll, i, i, vp, vp, sz, vp]),
         "few_fp64_peak_probe": (i, [vp, i, i, i, vp, vp]),
-        "few_fp64_mix_probe": (i, [vp, i, i, vp, vp, vp]),
-        "few_fp64_mma_probe": (i, [vp, i, i, vp, vp, vp]),
+        "few_launch_count": (i, [vp, C.POINTER(C.c_longlong)]),
         "few_profile_enable": (i, [vp, i]),
         "few_profile_sum_ms": (i, [vp, C.POINTER(C.c_float)]),
     }
@@ -356,18 +355,11 @@ def few_fp64_peak_probe(blocks: int, threads: int, iters: int, sink=None):
     return 2.0 * 16 * iters * blocks * threads   # FLOPs launched
 
 
-def few_fp64_mix_probe(blocks: int, iters: int, sink=None):
-    sink = sink if sink is not None else torch.empty(blocks * 128, dtype=torch.float64, device="cuda")
-    seed = torch.linspace(-2e-3, 4e-3, 16, dtype=torch.float64, device=sink.device)
-    _chk(_lib.few_fp64_mix_probe(context(), blocks, iters, _p(sink), _p(seed), _stream()), "few_fp64_mix_probe")
-    return 152.0 * iters * blocks * 128   # FLOPs launched (72 DFMA + 8 DMUL per thread and step)
-
-
-def few_fp64_mma_probe(blocks: int, iters: int, sink=None):
-    sink = sink if sink is not None else torch.empty(blocks * 128, dtype=torch.float64, device="cuda")
-    seed = torch.linspace(-2e-3, 4e-3, 16, dtype=torch.float64, device=sink.device)
-    _chk(_lib.few_fp64_mma_probe(context(), blocks, iters, _p(sink), _p(seed), _stream()), "few_fp64_mma_probe")
-    return 152.0 * iters * blocks * 128   # FLOPs per thread and step: 8 DMUL + 8 DFMA x 2 + 8 MMA x 8 FMA x 2 (as the mix probe)
+def few_launch_count(device: int | None = None) -> int:
+    """Kernels launched by the library through this device's context so far."""
+    n = C.c_longlong(0)
+    _chk(_lib.few_launch_count(context(device), C.byref(n)), "few_launch_count")
+    return int(n.value)
 
 
 def few_profile_enable(on: bool = True) -> None:

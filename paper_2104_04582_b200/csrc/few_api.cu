@@ -39,9 +39,11 @@ extern "C" int few_create(few_ctx** out, int device)
     int count = 0;
     FEW_CUDA_CHECK(cudaGetDeviceCount(&count));
     FEW_REQUIRE(device >= 0 && device < count, FEW_ERR_INVALID_ARG, "no such CUDA device");
+    int prev_device = 0;
+    FEW_CUDA_CHECK(cudaGetDevice(&prev_device));
     FEW_CUDA_CHECK(cudaSetDevice(device));
-    few_ctx* c = new (std::nothrow) few_ctx();
-    FEW_REQUIRE(c != nullptr, FEW_ERR_INVALID_ARG, "out of host memory");
+    few_ctx* c = new (std::nothrow) few_ctx();          // value-initialised: every handle starts as NULL
+    if (c == nullptr) { cudaSetDevice(prev_device); few_set_error("few_create: out of host memory"); return FEW_ERR_INVALID_ARG; }
     c->device = device;
     cudaError_t e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -56,9 +58,11 @@ extern "C" int few_create(few_ctx** out, int device)
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         few_set_error("few_create: %s", cudaGetErrorString(e));
-        delete c;
+        few_destroy(c);                                 // releases whatever was created (the rest is NULL)
+        cudaSetDevice(prev_device);
         return FEW_ERR_CUDA;
     }
+    cudaSetDevice(prev_device);                         // the caller's current device is left as it was
     *out = c;
     return FEW_OK;
 }
@@ -97,6 +101,13 @@ extern "C" int few_profile_sum_ms(few_ctx* ctx, float* ms_host)
     FEW_REQUIRE(ctx->profile && ctx->profile_valid, FEW_ERR_INVALID_ARG, "profiling is off or no summation was launched");
     FEW_CUDA_CHECK(cudaEventSynchronize(ctx->ev_sum[1]));
     FEW_CUDA_CHECK(cudaEventElapsedTime(ms_host, ctx->ev_sum[0], ctx->ev_sum[1]));
+    return FEW_OK;
+}
+
+extern "C" int few_launch_count(few_ctx* ctx, long long* count_host)
+{
+    FEW_REQUIRE(ctx && count_host, FEW_ERR_INVALID_ARG, "NULL argument");
+    *count_host = ctx->launches;
     return FEW_OK;
 }
 
@@ -172,29 +183,39 @@ int waveform_impl(few_ctx* ctx, const double* t, const double* phase, int n_phas
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
                     workspace_bytes >= few_waveform_workspace(n_src, n_t, n_modes, n_samples),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
+    // every limit a sub-call checks is checked HERE, before anything is enqueued: once the side streams are forked, an early
+    // return would leave them running into a workspace the caller is free to release
+    FEW_REQUIRE(n_src <= 65535 && n_t <= 65535, FEW_ERR_LIMIT, "n_src or n_t > 65535");
+    FEW_REQUIRE(n_t <= FEW_MAX_NT_SPLINE, FEW_ERR_LIMIT, "n_t > FEW_MAX_NT_SPLINE");
+    FEW_REQUIRE(n_modes <= FEW_MAX_SELECT_MODES, FEW_ERR_LIMIT, "n_modes > FEW_MAX_SELECT_MODES");
+    FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
+    FEW_REQUIRE(d == nullptr || inner != nullptr, FEW_ERR_INVALID_ARG, "d given but inner is NULL");
     wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, nullptr);
     int* kidx = keep_idx ? keep_idx : L.keep_idx;
     int* nk = n_keep ? n_keep : L.n_keep;
     // The spline fits depend on the inputs only, so they run on two side streams beside harmonics + mode selection and
     // join before the summation (fork/join with events: nothing synchronises the host, and the pattern is graph-capturable).
+    // A few_ctx serves ONE host thread at a time: the side streams and the fork/join events are the context's (few.h).
     cudaStream_t st = (cudaStream_t)stream;
-    int rc;
     FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_fork, st));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[0], ctx->ev_fork, 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[1], ctx->ev_fork, 0));
-    if ((rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]))) return rc;
-    if ((rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, n_phase, L.coef_phase, ctx->side[1]))) return rc;
-    FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[0], ctx->side[0]));
-    FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_join[1], ctx->side[1]));
+    // from here on every path, failing or not, joins the side streams back into the caller's stream before returning
+    int rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]);
+    if (rc == FEW_OK) rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, n_phase, L.coef_phase, ctx->side[1]);
     const double* factor = nullptr;
-    if (sky) {      // Eq. (4)-(8): viewing angles for the harmonics, one complex constant per source for the summation
-        if ((rc = few_frame_constants(ctx, sky, scale, n_src, L.theta_src, L.phi_src, L.factor, stream))) return rc;
+    if (rc == FEW_OK && sky) {      // Eq. (4)-(8): viewing angles for the harmonics, one complex constant per source for the summation
+        rc = few_frame_constants(ctx, sky, scale, n_src, L.theta_src, L.phi_src, L.factor, stream);
         theta = L.theta_src; phi = L.phi_src; factor = L.factor; scale = nullptr;
     }
-    if ((rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream))) return rc;
-    if ((rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream))) return rc;
-    FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[0], 0));
-    FEW_CUDA_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[1], 0));
+    if (rc == FEW_OK) rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream);
+    if (rc == FEW_OK) rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream);
+    cudaError_t je = cudaEventRecord(ctx->ev_join[0], ctx->side[0]);
+    if (je == cudaSuccess) je = cudaEventRecord(ctx->ev_join[1], ctx->side[1]);
+    if (je == cudaSuccess) je = cudaStreamWaitEvent(st, ctx->ev_join[0], 0);
+    if (je == cudaSuccess) je = cudaStreamWaitEvent(st, ctx->ev_join[1], 0);
+    if (rc != FEW_OK) return rc;
+    if (je != cudaSuccess) { few_set_error("few_waveform: joining the spline-fit streams failed: %s", cudaGetErrorString(je)); return FEW_ERR_CUDA; }
     return few_sum_waveform_kerr(ctx, t, L.coef_amp, L.coef_phase, n_phase, l, m, k, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, factor,
                                  t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
 }
@@ -245,6 +266,11 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
     FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
     FEW_REQUIRE(n_samples == 0 || h_host, FEW_ERR_INVALID_ARG, "h_host is NULL");
+    struct device_guard {           // the context's device is current inside the call; the caller's is restored on every return
+        int prev = -1;
+        ~device_guard() { if (prev >= 0) cudaSetDevice(prev); }
+    } guard;
+    FEW_CUDA_CHECK(cudaGetDevice(&guard.prev));
     FEW_CUDA_CHECK(cudaSetDevice(ctx->device));
     const size_t b_t = (size_t)n_src * n_t * 8, b_ph = b_t * 2, b_amp = (size_t)n_src * n_t * n_modes * 16;
     const size_t b_lmn = (size_t)n_modes * 4, b_ang = (size_t)n_src * 8, b_h = (size_t)n_src * n_samples * 16;
@@ -369,122 +395,6 @@ extern "C" int few_fp64_peak_probe(few_ctx* ctx, int blocks, int threads, int it
     FEW_REQUIRE(ctx && sink, FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE(blocks > 0 && threads > 0 && threads <= 1024 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
     few_fp64_peak_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    return FEW_OK;
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// FP64 instruction-mix probe: the hot loop of few_sum_kernel stripped of everything else -- per (m, n) pair and thread, for
-// 4 samples, E <- E Z_r (8 DMUL + 8 DFMA) and acc_p += e_r U_p + e_i V_p (64 DFMA) with the 8 complex coefficients read from
-// shared memory by broadcast 128-bit loads, 128 threads per block.  What this sustains is the ceiling of that instruction form
-// (three register operands per DFMA, one of them block-uniform) on this chip; DESIGN.md section 5.
-// ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) few_fp64_mix_kernel(int iters, double* sink, const double* seed)
-{
-    __shared__ __align__(16) double2 cs[256];
-    for (int i = threadIdx.x; i < 256; i += 128) cs[i] = make_double2(seed[(2 * i) & 15] * (1 + i), seed[(2 * i + 1) & 15] * (1 + i));
-    __syncthreads();
-    constexpr int R = 4;
-    double are[4][R], aim[4][R], er[R], ei[R], zr[R], zi[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        sincos(1e-3 * (threadIdx.x + 128 * r + 1), &zi[r], &zr[r]);
-        er[r] = 1.0; ei[r] = 0.0;
-    }
-#pragma unroll
-    for (int p = 0; p < 4; ++p)
-#pragma unroll
-        for (int r = 0; r < R; ++r) are[p][r] = aim[p][r] = 0.0;
-    for (int it = 0; it < iters; ++it) {
-        const double2* cp = cs + (it & 31) * 8;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const double m1 = ei[r] * zi[r], m2 = ei[r] * zr[r], e0 = er[r];
-            er[r] = fma(e0, zr[r], -m1);
-            ei[r] = fma(e0, zi[r], m2);
-        }
-#pragma unroll
-        for (int p = 0; p < 4; ++p) {               // the kernel's order: samples walked in alternating directions
-            const double2 u = cp[p];
-#pragma unroll
-            for (int r = 0; r < R; ++r) are[p][r] = fma(er[r], u.x, are[p][r]);
-#pragma unroll
-            for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(er[r], u.y, aim[p][r]);
-        }
-#pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const double2 v = cp[4 + p];
-#pragma unroll
-            for (int r = 0; r < R; ++r) are[p][r] = fma(ei[r], v.x, are[p][r]);
-#pragma unroll
-            for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(ei[r], v.y, aim[p][r]);
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int p = 0; p < 4; ++p)
-#pragma unroll
-        for (int r = 0; r < R; ++r) s += are[p][r] + aim[p][r];
-    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-extern "C" int few_fp64_mix_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream)
-{
-    FEW_REQUIRE(ctx && sink && seed, FEW_ERR_INVALID_ARG, "NULL argument");
-    FEW_REQUIRE(blocks > 0 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
-    few_fp64_mix_kernel<<<blocks, 128, 0, (cudaStream_t)stream>>>(iters, sink, seed);
-    FEW_CUDA_CHECK(cudaGetLastError());
-    return FEW_OK;
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// FP64 MMA-form probe: the same arithmetic as few_fp64_mix_kernel arranged for DMMA.8x8x4 (mma.sync.m8n8k4.f64): a warp holds
-// 8 samples x 4 pair streams per sample group (lane = 4 * sample + stream), rotates its E (2 DMUL + 2 DFMA per lane and group)
-// and contracts acc[8 samples][4 powers x re/im] += E_r[8 x 4] U[4 x 8], += E_i[8 x 4] V[4 x 8] with two DMMA whose B
-// fragments come from shared memory by one LDS.64 per lane.  4 sample groups per warp, 128 threads per block.
-// 20 FP64 lane-operations per sample and pair, as in the DFMA form (4 + 2 x 8 FMA).  DESIGN.md section 5.
-// ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void few_dmma884(double& c0, double& c1, double a, double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-__global__ void __launch_bounds__(128) few_fp64_mma_kernel(int iters, double* sink, const double* seed)
-{
-    __shared__ __align__(16) double cs[8 * 64];
-    for (int i = threadIdx.x; i < 8 * 64; i += 128) cs[i] = seed[i & 15] * (1 + i);
-    __syncthreads();
-    constexpr int G = 4;
-    const int lane = threadIdx.x & 31;
-    double c0[G], c1[G], er[G], ei[G], zr[G], zi[G];
-#pragma unroll
-    for (int g = 0; g < G; ++g) {
-        sincos(1e-3 * (threadIdx.x + 128 * g + 1), &zi[g], &zr[g]);
-        c0[g] = c1[g] = 0.0; er[g] = 1.0; ei[g] = 0.0;
-    }
-    for (int it = 0; it < iters; ++it) {
-        const double* f = cs + (it & 7) * 64;
-        const double u = f[lane], v = f[32 + lane];
-#pragma unroll
-        for (int g = 0; g < G; ++g) {               // per group: rotate, contract (the compiler pipelines the groups)
-            const double m1 = ei[g] * zi[g], m2 = ei[g] * zr[g], e0 = er[g];
-            er[g] = fma(e0, zr[g], -m1);
-            ei[g] = fma(e0, zi[g], m2);
-            few_dmma884(c0[g], c1[g], er[g], u);
-            few_dmma884(c0[g], c1[g], ei[g], v);
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int g = 0; g < G; ++g) s += c0[g] + c1[g];
-    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-extern "C" int few_fp64_mma_probe(few_ctx* ctx, int blocks, int iters, double* sink, const double* seed, void* stream)
-{
-    FEW_REQUIRE(ctx && sink && seed, FEW_ERR_INVALID_ARG, "NULL argument");
-    FEW_REQUIRE(blocks > 0 && iters > 0, FEW_ERR_INVALID_ARG, "bad launch shape");
-    few_fp64_mma_kernel<<<blocks, 128, 0, (cudaStream_t)stream>>>(iters, sink, seed);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

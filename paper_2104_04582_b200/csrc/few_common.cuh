@@ -14,6 +14,7 @@ struct few_ctx {
     int* d_status;       // device status word (FEW_DEV_* bits)
     int profile;         // few_profile_enable
     int profile_valid;   // a sum kernel was bracketed since profiling was switched on
+    long long launches;  // kernels launched through this context so far (few_launch_count)
     cudaEvent_t ev_sum[2];
     cudaStream_t side[2];  // few_waveform: the two spline fits run beside harmonics + mode selection
     cudaEvent_t ev_fork, ev_join[2];
@@ -34,6 +35,13 @@ void few_set_error(const char* fmt, ...);
             few_set_error("%s failed at %s:%d: %s", #expr, __FILE__, __LINE__, cudaGetErrorString(_e)); \
             return FEW_ERR_CUDA;                                                                 \
         }                                                                                        \
+    } while (0)
+
+// after every kernel launch: count it (few_launch_count) and pick up a launch error
+#define FEW_LAUNCHED(ctx)                                                                        \
+    do {                                                                                         \
+        ++(ctx)->launches;                                                                       \
+        FEW_CUDA_CHECK(cudaGetLastError());                                                      \
     } while (0)
 
 #define FEW_REQUIRE(cond, code, msg)                                                             \

@@ -15,7 +15,7 @@
 // layout to the sample-per-thread register layout costs no instruction.  A ring of kDirStages stages (cp.async commit groups)
 // keeps 2 stages = 70 KB per block in flight.  Mode constants travel with the chunk (48 more 16-byte pieces).
 // (First version: one 1-D TMA bulk copy per 256-byte row.  ncu: 1.6 TB/s, warps parked at the barrier -- the TMA unit retires
-// about one bulk request per 40 cycles per SM, so 256-byte requests cap at ~1.9 TB/s chip-wide; profiles/r01c_direct.md.)
+// about one bulk request per 40 cycles per SM, so 256-byte requests cap at ~1.9 TB/s chip-wide; profiles/r01c_kernels.md, section few_direct_kernel.)
 // exp(-i(m Phi_phi + n Phi_r)) = Z_phi^m Z_r^n with Z = exp(-i Phi) from ONE full-range sincos per phase and sample; along a
 // mode list in the grid's natural order (n fastest) E advances by one complex multiplication per mode; jumps in (m, n) restart
 // from Z_phi^m and a binary power of Z_r (block-uniform branch, once per (l, m) run of the full grid).
@@ -202,11 +202,11 @@ extern "C" int few_sum_direct(few_ctx* ctx, const double* amp, const double* pha
     dir_cst* cst = static_cast<dir_cst*>(workspace);
     few_direct_prepare_kernel<<<n_src, 256, 0, st>>>(l, m, n, (const double2*)ylm_plus, (const double2*)ylm_minus, scale,
                                                      (const double2*)factor, n_modes, K_pad, cst, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     const size_t smem = (size_t)kDirStages * kDirStageBytes;
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_direct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     few_direct_kernel<<<dim3((unsigned)tiles, n_src), kDirTile, smem, st>>>((const double2*)amp, (const double2*)phase, cst, n_samples,
                                                                            n_modes, K_pad, (double2*)h);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

@@ -131,7 +131,7 @@ extern "C" int few_frame_constants(few_ctx* ctx, const double* sky, const double
     FEW_REQUIRE(ctx && sky && theta && phi && factor, FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE(n_src > 0, FEW_ERR_INVALID_ARG, "n_src must be positive");
     few_frame_constants_kernel<<<(n_src + 127) / 128, 128, 0, (cudaStream_t)stream>>>(sky, mu_over_dl, n_src, theta, phi, (double2*)factor);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }
 
@@ -147,7 +147,7 @@ extern "C" int few_frame_rotate(few_ctx* ctx, const double* h_in, const double* 
     if ((long long)n_src * per_src > cap) per_src = cap / n_src > 1 ? cap / n_src : 1;
     few_frame_rotate_kernel<<<dim3((unsigned)per_src, n_src), 256, 0, (cudaStream_t)stream>>>((const double2*)h_in, (const double2*)factor,
                                                                                            n_samples, (double2*)h_out);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }
 
@@ -172,8 +172,8 @@ extern "C" int few_inner_products(few_ctx* ctx, const double* d, const double* h
     FEW_REQUIRE(nc < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
     few_inner_partial_kernel<<<dim3((unsigned)nc, n_src), kIpThreads, 0, st>>>((const double2*)d, (const double2*)h, n_samples, (int)nc,
                                                                              (double*)workspace);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     few_inner_final_kernel<<<n_src, kIpThreads, 0, st>>>((const double*)workspace, (int)nc, dt, inner);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

@@ -27,7 +27,7 @@
 //                   Kerr-shaped grid's 78 507 entries, and the rows the fast kernel hands over (flat spectra, degenerate eps).
 // The owners of the kept entries are OR-ed into a per-source bitmap; a last kernel compacts it into ascending keep_idx
 // and n_keep.  (History: in-shared-memory LSD radix sort + scan 128 us per 7137-entry row; 63-step
-// select alone 44 us; keys of the whole row in registers 26 us; this version see profiles/.)
+// select alone 44 us; keys of the whole row in registers 26 us; this version ~11 us, profiles/r01d_kernels.md.)
 #include "few_common.cuh"
 
 namespace {
@@ -513,7 +513,7 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
     sel_layout L{};
     if (!(eps > 0.0)) {       // R6: eps <= 0 keeps every mode, nothing is sorted
         few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 1, keep_idx, n_keep);
-        FEW_CUDA_CHECK(cudaGetLastError());
+        FEW_LAUNCHED(ctx);
         return FEW_OK;
     }
     FEW_REQUIRE(n_modes <= FEW_MAX_SELECT_MODES, FEW_ERR_LIMIT, "n_modes > FEW_MAX_SELECT_MODES");
@@ -523,13 +523,13 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
     L = sel_carve(workspace, n_src, n_t, n_modes);
     few_select_prepare_kernel<<<n_src, kPrepThreads, 0, st>>>(m, (const double2*)ylm_plus, (const double2*)ylm_minus, n_modes, L,
                                                            ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     const dim3 grid(n_t, n_src);
     FEW_REQUIRE(sizeof(stream_shared) <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "stream kernel's shared memory exceeds the device limit");
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_select_row_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(stream_shared)));
     if (n_modes <= kFastModes) {
         few_select_row_fast_kernel<16><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
-        FEW_CUDA_CHECK(cudaGetLastError());
+        FEW_LAUNCHED(ctx);
         // the rows the fast kernel left (usually none): a small persistent grid walks the list
         const long long n_rows = (long long)n_t * n_src;
         const unsigned fb_grid = (unsigned)(n_rows < ctx->sm_count ? n_rows : ctx->sm_count);
@@ -539,8 +539,8 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
         few_select_row_stream_kernel<<<grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t, n_modes, eps, L, nullptr,
                                                                                           nullptr);
     }
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

@@ -11,7 +11,7 @@
 // few_spline_factor_kernel (one block per source): the matrix depends on the grid only, so its Thomas factorisation (no
 // pivoting) is done ONCE per source into six per-knot arrays in the caller's workspace -- a serial chain of n_t divisions
 // that would otherwise sit on the critical path of every block of the fit kernel (it cost as much as the block's whole
-// HBM time, profiles/r01b_spline_cfg3.md).
+// HBM time: 0.477 ms before, 0.372 ms with the pre-kernel on config 3; the capture of this version is in profiles/r01c_kernels.md, section few_spline_fit_kernel).
 // few_spline_fit_kernel (FP64, thousands of systems): one thread per system, systems fastest in memory so every global
 // access of a warp is a contiguous row.  The kernel is HBM-bound (8 B read + 32 B written per knot and system); see the
 // comment at the kernel.  No cuSPARSE.
@@ -342,13 +342,13 @@ extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, in
         dim3 grid((n_sys + W - 1) / W, n_src);
         FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes_lat(W)));
         few_spline_fit_kernel<true><<<grid, W, bytes_lat(W), st>>>(t, nullptr, y, n_t, n_sys, coef, ctx->d_status);
-        FEW_CUDA_CHECK(cudaGetLastError());
+        FEW_LAUNCHED(ctx);
         return FEW_OK;
     }
     // Throughput regime.  Block width W (systems per block): as wide as possible (longer contiguous rows per store) while at
     // least two blocks fit an SM and the grid still covers every SM twice.
     few_spline_factor_kernel<<<n_src, 128, (size_t)6 * n_t * sizeof(double), st>>>(t, n_t, fac, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     auto bytes = [&](int w) { return (size_t)n_t * (48 + 8 * (size_t)w); };
     int W = 128;
     while (W > 32 && (bytes(W) > half || total / W < 2LL * ctx->sm_count)) W >>= 1;
@@ -356,7 +356,7 @@ extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, in
     dim3 grid((n_sys + W - 1) / W, n_src);
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes(W)));
     few_spline_fit_kernel<false><<<grid, W, bytes(W), st>>>(t, fac, y, n_t, n_sys, coef, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }
 
@@ -370,6 +370,6 @@ extern "C" int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y,
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_dd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     dim3 grid((n_sys + kDdSys - 1) / kDdSys, n_src);
     few_spline_fit_dd_kernel<<<grid, kDdThreads, bytes, (cudaStream_t)stream>>>(t, y, n_t, n_sys, coef_dd, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

@@ -712,12 +712,12 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
                                                           n_t, n_modes, plan_elems, L, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     // few blocks (one waveform): 1024 threads finish a segment's 4 x pairs items in one sweep; a batch fills the SMs with
     // several 256-thread blocks each, which hides the dependent index -> coefficient loads better
     const int pack_threads = (long long)(n_t - 1) * n_src < 2LL * ctx->sm_count ? 1024 : 256;
     few_sum_pack_kernel<<<dim3(n_t - 1, n_src), pack_threads, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
     const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
@@ -736,11 +736,11 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
         else FEW_SUM_LAUNCH(false, false, 0, nullptr);
     }
 #undef FEW_SUM_LAUNCH
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     if (ctx->profile) { FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[1], st)); ctx->profile_valid = 1; }
     if (inner) {
         few_sum_inner_kernel<<<n_src, kInnerThreads, 0, st>>>(L, n_t, (int)max_tiles, dt, inner);
-        FEW_CUDA_CHECK(cudaGetLastError());
+        FEW_LAUNCHED(ctx);
     }
     return FEW_OK;
 }

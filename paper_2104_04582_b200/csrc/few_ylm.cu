@@ -120,6 +120,6 @@ extern "C" int few_ylm_modes(few_ctx* ctx, const double* theta, const double* ph
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_ylm_modes_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     few_ylm_modes_kernel<<<n_src, kYlmThreads, smem, (cudaStream_t)stream>>>(theta, phi, l, m, n_src, n_modes, (double2*)ylm_plus,
                                                                            (double2*)ylm_minus, ctx->d_status);
-    FEW_CUDA_CHECK(cudaGetLastError());
+    FEW_LAUNCHED(ctx);
     return FEW_OK;
 }

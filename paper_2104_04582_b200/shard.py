@@ -5,7 +5,8 @@ Every dense sample is independent given the (small) spline coefficients, and eve
  - whole sources of a batch (`shard_sources`), or
  - contiguous sample ranges of one long waveform (`shard_samples`): each rank repeats the cheap S0-S2-S1 steps on the
    sparse inputs and sums only its own range [i0, i0 + n) by passing t0 + i0*dt as its t0.
-Pure host logic; used by bench.py (one process per GPU) and tested with gloo on CPU.
+Pure host logic (no kernels, no torch): `bench.py --gpus N --config 3|4` shards the GPU path with it (one process per GPU),
+and `tests/test_abi_and_host.py` covers it with a world_size-2 gloo run on CPU.
 """
 from __future__ import annotations
 
@@ -28,7 +29,9 @@ def shard_sources(n_src: int, rank: int, world: int) -> tuple[int, int]:
 
 
 def shard_samples(n_samples: int, rank: int, world: int, align: int = 256) -> tuple[int, int]:
-    """Sample range of a rank, aligned to the summation kernel's tile so no tile straddles two ranks."""
+    """Sample range of a rank.  Any split gives the same bits as the unsharded call (every sample's arithmetic depends on
+    its own t_i only; the kernel re-clips its tiles to each call's range), so `align` is cosmetic: it keeps shard
+    boundaries on multiples of 256 samples so that the ranks' stores start on 4 KB boundaries of h."""
     return shard_range(n_samples, rank, world, align)
 
 

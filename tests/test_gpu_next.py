@@ -374,8 +374,8 @@ def test_kerr_sum_reduces_to_schwarzschild_path(api):
 def _check_keep(keep_gpu, nk_gpu, ref_keep, margin):
     k = keep_gpu[: int(nk_gpu)]
     assert np.all(np.diff(k) > 0) and np.all(keep_gpu[int(nk_gpu):] == -1)
-    bad = [j for j in set(k.tolist()) ^ set(ref_keep.tolist()) if not margin[j] <= 1e-12]
-    assert not bad, f"kept sets differ outside the 1e-12 band: {bad[:10]} ({len(k)} vs {len(ref_keep)})"
+    bad = sorted(set(k.tolist()) ^ set(ref_keep.tolist()))        # identical sets: no band (margins are generic here)
+    assert not bad, f"kept sets differ: {bad[:10]} ({len(k)} vs {len(ref_keep)}; margins {[margin[j] for j in bad[:10]]})"
 
 
 @pytest.mark.parametrize("eps", [1e-5, 1e-2, 0.7])

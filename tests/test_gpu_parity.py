@@ -80,13 +80,17 @@ def test_spline_fit_vs_oracle(api, n_t, n_sys, uniform):
         ref = oracle.spline_fit(t[s], y[s])
         h = np.diff(t[s])[:, None]
         assert np.array_equal(coef[s][:, 0], y[s][:-1])                 # c0 is a bit copy
-        # compare c_p h^p, i.e. each term's contribution at the end of its segment, against the size of the data.  The two
-        # sides share no arithmetic order (FMA contraction, reciprocals), so the bound scales with the system's conditioning.
-        cond = max(1.0, float(h.max() / h.min()))
+        # compare c_p h^p, i.e. each term's contribution at the end of its segment, against the size of the data.  Observed on
+        # B200 (round 2): source 0 (the workloads' grid family: uniform / R17 shrinking steps) <= 4.1e-15
+        # in every case; source 1 (random sorted knots, h_max/h_min 6 ... 1.1e4 with near-coincident knots, where both FP64
+        # solves lose digits to conditioning) <= 5.8e-12.  Bars = ~10x those observations, flat (no scaling by h_max/h_min).
+        bar = 5e-14 if s == 0 else 6e-11
         for p in (1, 2, 3):
             err = np.abs(coef[s][:, p] - ref[:, p]) * h ** p
             scale = np.max(np.abs(y[s]), axis=0)[None, :]
-            assert np.max(err / scale) <= 1e-12 * cond, (s, p, np.max(err / scale))
+            obs = float(np.max(err / scale))
+            print(f"S1 observed n_t={n_t} n_sys={n_sys} src={s} p={p} h_max/h_min={float(h.max() / h.min()):.3g}: max err/scale = {obs:.3e}")
+            assert obs <= bar, (s, p, obs)
 
 
 def test_spline_fit_dd_vs_oracle_ext(api):
@@ -117,13 +121,17 @@ def test_spline_errors(api):
 
 
 # ------------------------------------------------------------------------------------------- S2
-def check_keep(keep_gpu, nk_gpu, ref_keep, margin, n_modes):
+def check_keep(keep_gpu, nk_gpu, ref_keep, margin, n_modes, band=0.0):
+    """Kept sets must be IDENTICAL (band = 0: the default, used for every BASELINE config and every other case whose
+    margins are generic).  Only the constructed threshold-hit case passes band = BAND: there a mode whose cumulative power
+    lies within 1e-12 (relative to the step's total) of the threshold may differ (north_star); `margin` is the oracle's pinned
+    distance to the threshold (tests/test_oracle_pins.py::test_p8_margin_*).  Returns the modes that differ."""
     k = keep_gpu[: int(nk_gpu)]
     assert np.all(np.diff(k) > 0) and np.all(keep_gpu[int(nk_gpu):] == -1)
-    diff = set(k.tolist()) ^ set(ref_keep.tolist())
-    bad = [j for j in diff if not margin[j] <= BAND]
-    assert not bad, f"kept sets differ outside the 1e-12 band: {bad[:10]} ({len(k)} vs {len(ref_keep)})"
-    return len(diff)
+    diff = sorted(set(k.tolist()) ^ set(ref_keep.tolist()))
+    bad = [j for j in diff if not (band > 0.0 and margin[j] <= band)]
+    assert not bad, f"kept sets differ: {bad[:10]} ({len(k)} vs {len(ref_keep)}; margins {[margin[j] for j in bad[:10]]})"
+    return diff
 
 
 @pytest.mark.parametrize("cfg,eps", [(1, 1e-5), (1, 1e-2), (4, 1e-3), (1, 0.5)])
@@ -192,6 +200,32 @@ def test_select_modes_flat_and_mixed_rows(api):
             ref, margin = oracle.select_modes(amp[s], w.m, yp[s].cpu().numpy(), ym[s].cpu().numpy(), eps)
             check_keep(keep[s].cpu().numpy(), nk[s].item(), ref, margin, w.n_modes)
     assert nk[0].item() > 3000                             # the flat source keeps almost everything
+
+
+def test_select_modes_constructed_threshold_hit_uses_the_band(api):
+    """The one place the 1e-12 band (north_star) is allowed: eps is chosen so that, in step 0, the cumulative power in front
+    of one entry equals (1 - eps) total up to the rounding of eps.  Whether that entry's mode is kept is decided by the
+    summation order (oracle: sequential, extended; kernel: tree, FP64), so the two sets may differ by exactly that mode --
+    and by nothing else."""
+    from fractions import Fraction
+    rng = np.random.default_rng(2104)
+    n_modes, n_t = 600, 4
+    amp = (rng.normal(size=(1, n_t, n_modes)) + 1j * rng.normal(size=(1, n_t, n_modes))) * 10.0 ** rng.uniform(-4, 0, (1, n_t, n_modes))
+    m = np.zeros(n_modes, np.int32)
+    p0 = amp[0, 0].real ** 2 + amp[0, 0].imag ** 2
+    order = sorted(range(n_modes), key=lambda e: (-p0[e], e))
+    fr = [Fraction(float(p0[e])) for e in order]
+    total = sum(fr)
+    r = 37                                                   # the entry of rank 37 sits exactly on the threshold
+    eps = float(1 - sum(fr[:r]) / total)
+    target = order[r]
+    ref, margin = oracle.select_modes(amp[0], m, None, None, eps)
+    assert margin[target] <= 1e-15                           # the construction worked (pinned margin)
+    assert np.sum(margin <= BAND) == 1                       # and no other mode is anywhere near a threshold
+    keep, nk = api.few_select_modes(dev(amp), dev(m), None, None, eps)
+    api.few_device_status()
+    diff = check_keep(keep[0].cpu().numpy(), nk[0].item(), ref, margin, n_modes, band=BAND)
+    assert diff in ([], [target])
 
 
 # ------------------------------------------------------------------------------------------- S3 and the whole path
@@ -377,18 +411,92 @@ def test_full_size_sampled_parity(api, cfg):
     assert rel_l2(h[0][idx], one) <= REL_L2_TOL
 
 
-def test_fp64_probes_run_and_are_ordered(api):
-    """The three measurement aids of bench.py launch and give finite sinks; their known ordering on this chip (register-resident
-    DFMA chains > MMA form > three-operand DFMA form) is what DESIGN.md section 5 builds on."""
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-    rates = {}
-    for name, fn in (("dfma", lambda it: api.few_fp64_peak_probe(148 * 8, 256, it)),
-                     ("mix", lambda it: api.few_fp64_mix_probe(148 * 3, it)),
-                     ("mma", lambda it: api.few_fp64_mma_probe(148 * 3, it))):
-        fn(500); torch.cuda.synchronize()
-        a, b = ev(), ev()
-        a.record(); flops = fn(5000); b.record(); torch.cuda.synchronize()
-        rates[name] = flops / (a.elapsed_time(b) * 1e-3) / 1e12
+def knot_windows(w, s, knots, n_win):
+    """Sample windows of n_win samples centred on the first dense sample at or after the given sparse knots of source s."""
+    out = []
+    for k in knots:
+        i = int(math.ceil((w.t[s][k] - w.t0) / w.dt))
+        out.append((min(max(i - n_win // 2, 0), w.n_samples - n_win), n_win))
+    return out
+
+
+def test_config3_full_size_sampled_parity_device_and_host_paths(api):
+    """BASELINE config 3 exactly as bench.py times it: 64 sources x 1 051 920 samples, one few_waveform call, and the same
+    through few_waveform_host (8 source groups, h stored by the kernel into a 1.08 GB pinned host buffer).  Kept sets of all
+    64 sources must equal the oracle's; the waveform is recomputed by the oracle on windows at the first and last samples of
+    every source and at segment boundaries, with the three sources whose phases end highest (59, 35, 9: 1.0-1.3e6 rad, the
+    precision worst case of SURVEY H1) covered by several windows each including the end of the trajectory."""
+    w = synth.make_config(3)
+    assert w.n_src == 64 and w.n_samples == 1_051_920
+    worst = [int(s) for s in np.argsort(-w.phase[:, -1, 0])[:3]]
+    assert w.phase[worst[0], -1, 0] > 1.2e6
+    g = gpu_inputs(w)
+    keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device="cuda")
+    nk = torch.empty((w.n_src,), dtype=torch.int32, device="cuda")
+    h = api.few_waveform(g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
+                         w.n_samples, keep_idx=keep, n_keep=nk)
     api.few_device_status()
-    assert all(np.isfinite(v) and v > 1.0 for v in rates.values()), rates
-    assert rates["dfma"] > rates["mma"] > rates["mix"], rates
+    yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
+    yp, ym, keep_h, nk_h = yp.cpu().numpy(), ym.cpu().numpy(), keep.cpu().numpy(), nk.cpu().numpy()
+    N = w.n_samples
+    worst_err = 0.0
+    for s in range(w.n_src):
+        ref, margin = oracle.select_modes(w.amp[s], w.m, yp[s], ym[s], w.eps)      # the GPU's harmonics: bit-equal powers
+        check_keep(keep_h[s], nk_h[s], ref, margin, w.n_modes)                   # identical, no band
+        if s in worst:
+            wins = [(0, 192), (N - 192, 192)] + knot_windows(w, s, [1, 2, 40, 77, 78], 192) + [(i0, 64) for i0 in range(50_021, N - 64, N // 9)]
+        else:
+            wins = [(0, 48), (N - 48, 48)] + knot_windows(w, s, [1 + s % 70, 78], 48)
+        refs = np.concatenate(oracle_with_gpu_keep(w, s, keep_h[s][: nk_h[s]], wins))
+        got = torch.cat([h[s, i0:i0 + nn] for i0, nn in wins]).cpu().numpy()
+        e = rel_l2(got, refs)
+        worst_err = max(worst_err, e)
+        assert e <= REL_L2_TOL and mismatch(got, refs) <= MISMATCH_TOL, (s, e)
+        assert np.max(np.abs(got - refs)) <= 3e-10 * np.max(np.abs(refs)), s
+    print(f"config 3 full size: worst windowed rel-L2 over 64 sources {worst_err:.3e}; kept {int(nk_h.sum())}")
+    assert bool(torch.isfinite(torch.view_as_real(h)).all())
+    # host path: pinned inputs and a pinned 1.08 GB output written by the kernel's own stores
+    f = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
+    keep2 = torch.empty((w.n_src, w.n_modes), dtype=torch.int32).pin_memory(); nk2 = torch.empty((w.n_src,), dtype=torch.int32).pin_memory()
+    h_host = torch.full((w.n_src, N), float("nan"), dtype=torch.complex128).pin_memory()
+    api.few_waveform_host(f(w.t), f(w.phase), f(w.amp), f(w.l), f(w.m), f(w.n), f(w.theta), f(w.phi), w.eps, w.t0, w.dt, N,
+                          out=h_host, keep_idx=keep2, n_keep=nk2)
+    assert np.array_equal(nk2.numpy(), nk_h) and np.array_equal(keep2.numpy(), keep_h)
+    for s0 in range(0, w.n_src, 8):                       # bit-equal to the device-resident call, compared on the device
+        assert torch.equal(h_host[s0:s0 + 8].cuda(), h[s0:s0 + 8]), s0
+
+
+@pytest.mark.parametrize("eps", [1e-2, 1e-3, 1e-4, 1e-5, 0.0])
+def test_config4_full_size_sampled_parity_eps_sweep(api, eps):
+    """BASELINE config 4 at full size (12 623 040 samples, 300 knots: ~24.7 k tiles over 301 pseudo-segments) for every eps
+    of the sweep bench.py times; windows include the first and last 256 samples and the knots 1, 150 and 298."""
+    w = synth.make_config(4, eps=eps)
+    assert w.n_samples == 12_623_040 and w.n_t == 300
+    h, keep, nk = run_gpu_chain(api, w)
+    yp, ym = api.few_ylm_modes(dev(w.theta), dev(w.phi), dev(w.l), dev(w.m))
+    ref, margin = oracle.select_modes(w.amp[0], w.m, yp[0].cpu().numpy(), ym[0].cpu().numpy(), eps)
+    check_keep(keep[0], nk[0], ref, margin, w.n_modes)
+    N = w.n_samples
+    n_win = 256 if eps > 0 else 64
+    wins = [(0, n_win), (N - 256, 256)] + knot_windows(w, 0, [1, 150, 298], n_win) + [(i0, 32) for i0 in range(400_009, N - 32, N // 7)]
+    refs = np.concatenate(oracle_with_gpu_keep(w, 0, keep[0][: nk[0]], wins))
+    got = np.concatenate([h[0][i0:i0 + nn] for i0, nn in wins])
+    assert rel_l2(got, refs) <= REL_L2_TOL and mismatch(got, refs) <= MISMATCH_TOL, (eps, rel_l2(got, refs))
+    assert np.max(np.abs(got - refs)) <= 3e-10 * np.max(np.abs(refs))
+    idx = np.arange(11, N, 250_007)
+    one = np.concatenate(oracle_with_gpu_keep(w, 0, keep[0][: nk[0]], [(int(i), 1) for i in idx]))
+    assert rel_l2(h[0][idx], one) <= REL_L2_TOL
+    assert np.all(np.isfinite(h.view(np.float64)))
+    print(f"config 4 eps={eps:g}: kept {int(nk[0])}, windowed rel-L2 {rel_l2(got, refs):.3e}")
+
+
+def test_fp64_peak_probe_runs(api):
+    """The one measurement aid left in the ABI (the roofline denominator bench.py prints beside the nominal peak) launches,
+    writes finite values and sustains a plausible FP64 rate; no throughput ordering is asserted."""
+    sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
+    api.few_fp64_peak_probe(148 * 8, 256, 500, sink); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); flops = api.few_fp64_peak_probe(148 * 8, 256, 5000, sink); b.record(); torch.cuda.synchronize()
+    rate = flops / (a.elapsed_time(b) * 1e-3) / 1e12
+    api.few_device_status()
+    assert bool(torch.isfinite(sink).all()) and rate > 1.0, rate

@@ -408,6 +408,70 @@ def test_p8_ties_broken_by_entry_index():
     assert list(k) == [0, 1, 2]
 
 
+def brute_margin(P, owner, eps, n_modes):
+    """The oracle's `margin` output by its definition, in exact rational arithmetic: for every mode the minimum, over the
+    steps and over the mode's entries of rank r >= 1, of |C_{r-1} - (1 - eps) total| / total (C = inclusive cumulative sum in
+    descending-power order, ties by entry index).  inf for a mode that is rank 0 in every step, and for eps <= 0."""
+    out = [math.inf] * n_modes
+    if eps <= 0:
+        return out
+    one_minus = 1 - Fraction(eps)
+    for row in P:
+        order = sorted(range(len(row)), key=lambda e: (-row[e], e))
+        fr = [Fraction(float(row[e])) for e in order]
+        total = sum(fr)
+        c = Fraction(0)
+        for r, e in enumerate(order):
+            if r >= 1 and total > 0:
+                d = abs(c - one_minus * total) / total
+                out[owner[e]] = min(out[owner[e]], float(d))
+            c += fr[r]
+    return out
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_p8_margin_is_the_distance_to_the_threshold(seed):
+    """`margin[j]` is what the GPU set-parity tests lean on (a kept-set difference is excused only inside the 1e-12 band), so it
+    is pinned like the set itself: exact rationals on tiny rows, both power variants, five eps, plus eps <= 0 and a mode
+    that is the strongest entry of every step (no rank >= 1 entry: inf)."""
+    rng = np.random.default_rng(50 + seed)
+    nm, nt = 7, 3
+    m = rng.integers(0, 3, nm).astype(np.int32)
+    amp = (rng.normal(size=(nt, nm)) + 1j * rng.normal(size=(nt, nm))) * 10.0 ** rng.uniform(-3, 0, (nt, nm))
+    amp[:, 2] = 50.0                                        # mode 2 is rank 0 in every step ...
+    m[2] = 0                                                # ... and has no mirror entry
+    yp = rng.normal(size=nm) + 1j * rng.normal(size=nm); ym = rng.normal(size=nm) + 1j * rng.normal(size=nm)
+    yp[2] = 1.0
+    owner = list(range(nm)) + [j for j in range(nm) if m[j] > 0]
+    P = np.concatenate([np.abs(amp) ** 2 * np.abs(yp) ** 2, (np.abs(amp) ** 2 * np.abs(ym) ** 2)[:, m > 0]], axis=1)
+    for eps in (0.5, 1e-1, 1e-2, 1e-4, 1e-9):
+        _, margin = oracle.select_modes(amp, m, yp, ym, eps)
+        want = brute_margin(P, owner, eps, nm)
+        assert margin[2] == math.inf and want[2] == math.inf
+        for j in range(nm):
+            if j != 2:
+                assert abs(margin[j] - want[j]) <= 1e-15, (eps, j, margin[j], want[j])
+        _, margin0 = oracle.select_modes(amp, m, None, None, eps)
+        want0 = brute_margin(np.abs(amp) ** 2, list(range(nm)), eps, nm)
+        assert all(abs(a - b) <= 1e-15 for a, b in zip(np.delete(margin0, 2), np.delete(want0, 2)))
+    _, margin = oracle.select_modes(amp, m, yp, ym, 0.0)
+    assert np.all(np.isinf(margin))
+
+
+def test_p8_margin_of_a_constructed_threshold_hit():
+    """A row built so that C_{r-1} equals (1 - eps) total up to rounding: the margin of the rank-r mode is ~1e-17, far
+    inside the 1e-12 band, and every other mode is far outside it (the case the GPU band test is built on)."""
+    p = np.array([0.5, 0.25, 0.125, 0.0625, 0.03125, 0.03125])            # total = 1 exactly; C = .5 .75 .875 .9375 ...
+    amp = np.sqrt(p)[None, :].astype(np.complex128)
+    m = np.zeros(6, np.int32)
+    eps = 0.125                                                           # (1 - eps) total = 0.875 = C_2 exactly
+    keep, margin = oracle.select_modes(amp, m, None, None, eps)
+    want = brute_margin(np.abs(amp) ** 2, list(range(6)), eps, 6)
+    assert abs(margin[3] - want[3]) <= 1e-15 and margin[3] <= 1e-15       # rank 3 sees C_2 = threshold
+    assert list(keep) == [0, 1, 2] or list(keep) == [0, 1, 2, 3]          # C_2 < 0.875 decided by rounding of |a|^2
+    assert all(margin[j] > 1e-3 for j in (1, 2, 4, 5))
+
+
 def test_p8_mismatch_scales_like_eps_paper_fig3():
     """PAPER.md:300 (Fig. 3): mismatch ~1e-2 at eps=1e-1 falling as a power law.  On the synthetic model the
     kept-vs-all-modes mismatch must fall roughly linearly with eps (order-of-magnitude pin of O3 + O4 together)."""
