@@ -6,8 +6,15 @@
 A step is ONE pass of the whole hot path (S0 harmonics, S2 mode selection, S1 spline fits, S3 summation; DESIGN.md
 section 1) over one synthetic workload: by default BASELINE.json configs[1], the one-year single-source waveform with
 eps = 1e-5 that the metric "ms per 1-yr FP64 waveform; sample*mode evals/s; % of FP64 roofline" is quoted on.
-With N > 1 every rank runs its own copy of the workload (independent waveforms, as in an MCMC: weak scaling, no
-data-path collective); value = total sample*mode evaluations of all ranks / max-over-ranks time.
+After the headline measurement the default run (N = 1, no flag) also times, for a few steps each, the other BASELINE
+configurations the perf targets are stated on and reports them under `also`: config 2 (all modes: the FP64 roofline
+probe), config 3 (64-source batch: spline fit and selection against HBM, host-buffer call), config 4 at eps = 1e-2 and 0.
+
+With N > 1 the path shards with no data-path collective:
+  --config 1 (default), 2   every rank runs its own copy of the workload (independent waveforms of an MCMC): "replicas", weak
+  --config 3                rank r takes sources shard_sources(64, r, N): strong scaling by source
+  --config 4                rank r takes samples shard_samples(N_samples, r, N) and repeats S0-S2-S1: strong scaling by time range
+value = total sample*mode evaluations of all ranks / max-over-ranks time.
 
 Prints ONE JSON line (see the keys at the bottom).  `--impl reference` times the CPU oracle instead (rank 0 only).
 """
@@ -31,11 +38,28 @@ import numpy as np  # noqa: E402
 FLOP_PER_EVAL = 20.0          # nominal per-mode figure of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA)
 FLOP_PER_PAIR = 38.0          # executed algorithm: per sample and (m,n) pair 18 DFMA + 2 DMUL = 20 FP64 slots
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
-GPU_LAUNCHES_EPS = 10         # ylm 1 + select 4 (prepare, fast, streamed rest, compact) + spline 1 (+1 factor kernel when batched) + spline_dd 1 + sum 3
-GPU_LAUNCHES_ALL = 7          # eps <= 0: select is a single list-fill kernel
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch, from the `ncu --set full` captures summarised in
-# profiles/r01d_kernels.md (the coefficient stream and h stay in the 126 MB L2 while the kernel runs)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch: static figures from `ncu --set full` captures (the
+# run itself does not measure them); the coefficient stream and h stay in the 126 MB L2 while the kernel runs
 SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 4.84e6, "config2_1yr_allmodes": 10.62e6}
+SUM_KERNEL_DRAM_TRAFFIC_SOURCE = "profiles/r01d_kernels.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum; static, not measured by this run)"
+
+
+def config_dict(w, **extra):
+    """The `config` object: the same keys in the repo arm and in the reference arm."""
+    d = {"workload": w.name, "n_src": int(w.n_src), "n_t": int(w.n_t), "n_modes": int(w.n_modes), "n_samples": int(w.n_samples),
+         "dt": float(w.dt), "eps": float(w.eps)}
+    d.update(extra)
+    return d
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def load_peaks():
@@ -84,12 +108,15 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "reasons": reasons, "samples": len(rows)}
 
 
-def oracle_sample(w, target_s: float):
+def oracle_sample(w, target_s: float, threads: int | None = None, max_samples: int = 1 << 22):
     """Times the CPU oracle, as it stands, on a bounded contiguous slice of the workload (whole path: harmonics,
-    selection, spline fits, summation).  Returns (evals/s, description, cores, seconds)."""
+    selection, spline fits, summation).  threads = None: all host cores.  Returns (evals/s, description, cores, seconds, n, K)."""
     import oracle
     from paper_2104_04582_b200 import synth
     oracle.build()
+    all_cores = oracle.num_threads()
+    if threads is not None:
+        oracle.set_threads(threads)
     cores = oracle.num_threads()
     mid = (w.n_samples // 2) // 256 * 256
 
@@ -100,11 +127,94 @@ def oracle_sample(w, target_s: float):
         _, parts = oracle.waveform(ws, return_parts=True)
         return time.perf_counter() - t0, len(parts[0]["keep_idx"])
 
-    t_cal, K = run(4096)
-    rate = 4096 * K / t_cal
-    n = int(min(max(target_s * rate / K, 4096), w.n_samples - mid, 1 << 22))
-    t_run, K = run(n)
+    try:
+        # two calibration sizes separate the fixed cost (harmonics, selection, fits) from the per-sample cost
+        n1, n2 = (2048, 16384) if threads is None else (256, 2048)
+        t1, K = run(n1)
+        t2, K = run(n2)
+        per_sample = max((t2 - t1) / (n2 - n1), 1e-9)
+        fixed = max(t1 - per_sample * n1, 0.0)
+        n = int(min(max((target_s - fixed) / per_sample, n2), w.n_samples - mid, max_samples))
+        t_run, K = run(n)
+    finally:
+        if threads is not None:
+            oracle.set_threads(all_cores)
     return n * K / t_run, f"{n} contiguous samples of source 0 from sample {mid}, whole path, K={K}", cores, t_run, n, K
+
+
+def kept_structure(w, keep_h, nk_h):
+    """(kept modes, (m, n) pairs) summed over the sources: bookkeeping for the roofline (the kernel sums all l of an (m, n) pair
+    into one pair of splines before the sample loop)."""
+    K = int(nk_h.sum())
+    pairs = sum(len({(int(w.m[j]), int(w.n[j])) for j in keep_h[s, : nk_h[s]]}) for s in range(w.n_src))
+    return K, pairs
+
+
+class Bench:
+    """One workload resident on the device, and the timed step over it."""
+
+    def __init__(self, api, torch, w, dev):
+        self.api, self.torch, self.w, self.dev = api, torch, w, dev
+        host = dict(t=w.t, phase=w.phase, amp=w.amp, l=w.l, m=w.m, n=w.n, theta=w.theta, phi=w.phi)
+        self.pinned = {k: torch.as_tensor(np.ascontiguousarray(v)).pin_memory() for k, v in host.items()}
+        self.g = {k: v.to(dev) for k, v in self.pinned.items()}
+        self.h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
+        self.keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device=dev)
+        self.nk = torch.empty((w.n_src,), dtype=torch.int32, device=dev)
+        self.ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=dev)
+
+    def step(self):
+        g, w = self.g, self.w
+        self.api.few_waveform(g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
+                              w.n_samples, out=self.h, keep_idx=self.keep, n_keep=self.nk, workspace=self.ws)
+
+    def warm(self, n, flush):
+        for _ in range(n):
+            flush.fill_(1); self.step()
+        self.api.few_device_status()
+        self.K, self.pairs = kept_structure(self.w, self.keep.cpu().numpy(), self.nk.cpu().numpy())
+
+    def timed(self, steps, flush, barrier=None):
+        """steps timed steps, L2 flushed before each (outside the event pair), CUDA events on the launch stream; the library's
+        own event pair around the hot kernel gives its duration.  Returns (step ms list, hot-kernel ms list, launches)."""
+        torch, api = self.torch, self.api
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        sum_ms = []
+        if barrier:
+            barrier()
+        n0 = api.few_launch_count()
+        for a, b in ev:
+            flush.fill_(1)
+            a.record(); self.step(); b.record()
+            sum_ms.append(api.few_profile_sum_ms())       # waits for this step's hot kernel
+        launches = api.few_launch_count() - n0
+        if barrier:
+            barrier()
+        else:
+            torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev], sum_ms, launches
+
+    def e2e(self, reps, device_index):
+        """The same step through few_waveform_host (C ABI, HOST pointers): H2D + kernels + D2H inside the call."""
+        torch, api, w, p = self.torch, self.api, self.w, self.pinned
+        h_host = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128).pin_memory()
+        call = lambda: api.few_waveform_host(p["t"], p["phase"], p["amp"], p["l"], p["m"], p["n"], p["theta"], p["phi"], w.eps, w.t0,
+                                             w.dt, w.n_samples, out=h_host, device=device_index)
+        call()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            call()                           # synchronous: returns after the D2H copy completed
+        sec = (time.perf_counter() - t0) / reps
+        h2d = sum(v.numel() * v.element_size() for v in p.values())
+        return sec, int(h2d), int(h_host.numel() * 16)
+
+
+def sum_kernel_roofline(w, pairs, kernel_ms, sm_max_mhz):
+    """FP64 ALU roofline of few_sum_kernel: executed flops of the formulation / time, against the nominal pipe."""
+    peak = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    achieved = float(w.n_samples) * pairs * FLOP_PER_PAIR / (kernel_ms * 1e-3) / 1e12
+    return achieved, peak
 
 
 def time_stages(api, torch, w, g, flush, reps: int = 10):
@@ -261,7 +371,7 @@ def reference_arm(args):
     if rank != 0:
         return 0
     from paper_2104_04582_b200 import synth
-    w = synth.make_config(args.config)
+    w = synth.make_config(args.config, eps=args.eps)
     per_step = max(6.0, min(30.0, 120.0 / max(args.steps + args.warmup, 1)))
     vals, times = [], []
     desc = cores = None
@@ -270,15 +380,81 @@ def reference_arm(args):
         if i >= args.warmup:
             vals.append(v); times.append(t_run)
     value = float(np.mean(vals))
-    out = {"impl": "reference", "metric": "sample*mode evaluations per second (1-yr FP64 waveform, whole hot path)", "value": value,
+    out = {"impl": "reference", "metric": METRIC, "value": value,
            "unit": "evals/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "n_samples_full": w.n_samples, "eps": w.eps,
-                                                            "n_modes": w.n_modes, "n_t": w.n_t},
-           "cpu_baseline": {"value": value, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc},
+           "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": parallelism_label(w, args.config, args.gpus)[1], "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "config": config_dict(w, parallelism=parallelism_label(w, args.config, args.gpus)[0]),
+           "cpu_baseline": {"value": value, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "cpu_model": cpu_model()},
            "e2e": {"value": value, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(out), flush=True)
     return 0
+
+
+METRIC = "sample*mode evaluations per second (1-yr FP64 waveform, whole hot path)"
+
+
+def parallelism_label(w, config: int, world: int):
+    """(label, scaling) of the split `--gpus world --config config` runs; the same in both arms."""
+    if world == 1:
+        return "single GPU", "weak"
+    if config == 3:
+        return f"by source, {world} x {w.n_src // world} sources, no collective", "strong"
+    if config == 4:
+        return f"by contiguous time range, {world} x ~{w.n_samples // world} samples, S0-S2-S1 repeated per rank, no collective", "strong"
+    return f"{world} independent replicas (one waveform per GPU, an MCMC's walkers), no collective", "weak"
+
+
+def shard_workload(w, config: int, rank: int, world: int):
+    """The rank's share of the workload.  No data-path collective."""
+    from paper_2104_04582_b200 import synth
+    from paper_2104_04582_b200.shard import shard_samples, shard_sources, shard_t0
+    if world > 1 and config == 3:
+        s0, sc = shard_sources(w.n_src, rank, world)
+        return synth.Workload(w.name, w.t[s0:s0 + sc], w.phase[s0:s0 + sc], w.amp[s0:s0 + sc], w.l, w.m, w.n, w.theta[s0:s0 + sc],
+                              w.phi[s0:s0 + sc], w.t0, w.dt, w.n_samples, w.eps)
+    if world > 1 and config == 4:
+        i0, cnt = shard_samples(w.n_samples, rank, world)
+        return synth.Workload(w.name, w.t, w.phase, w.amp, w.l, w.m, w.n, w.theta, w.phi, shard_t0(w.t0, w.dt, i0), w.dt, cnt, w.eps)
+    return w
+
+
+def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
+    """The other BASELINE configurations the perf targets are stated on, a few steps each (N = 1 default run only)."""
+    from paper_2104_04582_b200 import synth
+    out = {}
+
+    def short(w, steps=4, warm=3):
+        b = Bench(api, torch, w, dev)
+        b.warm(warm, flush)
+        step_ms, sum_ms, launches = b.timed(steps, flush)
+        kms = float(np.mean(sum_ms))
+        ach, peak = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz)
+        r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "steps": steps,
+             "ms_per_step": float(np.mean(step_ms)), "kernel_ms": kms, "tflops": ach, "frac": ach / peak,
+             "evals_per_s": float(w.n_samples) * b.K / (float(np.mean(step_ms)) * 1e-3), "gpu_launches_per_step": launches / steps}
+        return b, r
+
+    b, out["config2"] = short(synth.make_config(2))
+    del b
+    for eps, key in ((1e-2, "config4_eps1e-2"), (0.0, "config4_eps0")):
+        b, out[key] = short(synth.make_config(4, eps=eps), steps=3)
+        del b
+    torch.cuda.empty_cache()
+    w3 = synth.make_config(3)
+    b, r = short(w3, steps=3)
+    st = time_stages(api, torch, w3, b.g, flush, reps=5)
+    for name, key in (("S1_spline_fit", "S1"), ("S2_select_modes", "S2")):
+        r[key] = {"ms": st[name]["ms_avg"], "gbs": st[name]["gbs"], "hbm_frac": st[name]["gbs"] / hbm_gbs,
+                  "algorithmic_bytes": st[name]["algorithmic_bytes"]}
+    r["output_bytes"] = 16.0 * w3.n_src * w3.n_samples
+    del b.h
+    sec, h2d, d2h = b.e2e(2, local)
+    r["e2e_ms"] = 1e3 * sec
+    r["e2e_h2d_bytes"], r["e2e_d2h_bytes"] = h2d, d2h
+    out["config3"] = r
+    del b
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -286,10 +462,11 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = headline; 2, 3, 4 for profiling)")
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = headline; 2, 3, 4 for profiling and sharded scaling)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the short runs of configs 2, 3, 4 that the default run appends")
     ap.add_argument("--eps", type=float, default=None)
     ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows: detector frame, fused inner products, direct sum")
@@ -311,20 +488,12 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    w = synth.make_config(args.config, eps=args.eps)
-    host = dict(t=w.t, phase=w.phase, amp=w.amp, l=w.l, m=w.m, n=w.n, theta=w.theta, phi=w.phi)
-    pinned = {k: torch.as_tensor(np.ascontiguousarray(v)).pin_memory() for k, v in host.items()}
-    g = {k: v.to(dev) for k, v in pinned.items()}
-    h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
-    keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device=dev)
-    nk = torch.empty((w.n_src,), dtype=torch.int32, device=dev)
-    ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=dev)
+    w_full = synth.make_config(args.config, eps=args.eps)
+    w = shard_workload(w_full, args.config, rank, world)
+    parallelism, scaling = parallelism_label(w_full, args.config, world)
+    bench = Bench(api, torch, w, dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)            # > 126 MB L2
     api.few_profile_enable(True)
-
-    def step():
-        api.few_waveform(g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
-                         w.n_samples, out=h, keep_idx=keep, n_keep=nk, workspace=ws)
 
     def barrier():
         torch.cuda.synchronize()
@@ -332,15 +501,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        flush.fill_(1); step()
-    api.few_device_status()
-    K_kept = int(nk.sum().item())            # kept modes summed over sources
+    bench.warm(args.warmup, flush)
+    K_kept, pairs = bench.K, bench.pairs
     evals_per_step = float(w.n_samples) * K_kept
-    # (m, n) pairs among the kept modes (bookkeeping for the roofline: the kernel sums all l of a pair into one spline pair)
-    keep_h, nk_h = keep.cpu().numpy(), nk.cpu().numpy()
-    pairs = sum(len({(int(w.m[j]), int(w.n[j])) for j in keep_h[s, : nk_h[s]]}) for s in range(w.n_src))
-    pair_evals_per_step = float(w.n_samples) * pairs
 
     # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
     sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
@@ -350,40 +513,19 @@ def main():
     probe_flops = api.few_fp64_peak_probe(148 * 8, 256, 20000, sink)
     e1.record(); torch.cuda.synchronize()
     fp64_measured_tflops = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
-    # the hot loop's own instruction mix (72 DFMA + 8 DMUL per pair step, coefficients from shared memory) and nothing else,
-    # at the sum kernel's launch shape (3 blocks of 128 threads per SM): the ceiling of that instruction form on this chip
-    api.few_fp64_mix_probe(148 * 3, 2000, sink)
-    torch.cuda.synchronize(); e0.record()
-    mix_flops = api.few_fp64_mix_probe(148 * 3, 20000, sink)
-    e1.record(); torch.cuda.synchronize()
-    fp64_mix_tflops = mix_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
-    # the same arithmetic in FP64 tensor-core form (DMMA.8x8x4): what an MMA formulation of the summation could sustain
-    api.few_fp64_mma_probe(148 * 3, 2000, sink)
-    torch.cuda.synchronize(); e0.record()
-    mma_flops = api.few_fp64_mma_probe(148 * 3, 20000, sink)
-    e1.record(); torch.cuda.synchronize()
-    fp64_mma_tflops = mma_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
 
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start(); time.sleep(0.3)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    sum_ms = []
-    barrier()
     t_begin = time.perf_counter()
-    for a, b in ev:
-        flush.fill_(1)                      # L2 flush between timed iterations (outside the event pair)
-        a.record(); step(); b.record()
-        sum_ms.append(api.few_profile_sum_ms())     # waits for this step's hot kernel: its own CUDA events on the launch stream
-    barrier()
+    step_ms, sum_ms, launches = bench.timed(args.steps, flush, barrier)
     t_end = time.perf_counter()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-        ev_all = torch.tensor([evals_per_step], dtype=torch.float64, device=dev)
+        ev_all = torch.tensor([evals_per_step, float(K_kept), float(pairs)], dtype=torch.float64, device=dev)
         dist.all_reduce(ev_all, op=dist.ReduceOp.SUM)
-        evals_all = float(ev_all.item())
+        evals_all = float(ev_all[0].item())
     else:
         evals_all = evals_per_step
     clocks = sampler.stop(t_begin, t_end) if sampler else None
@@ -393,33 +535,28 @@ def main():
     # e2e: the same metric through the C-ABI call with HOST buffers (H2D of the inputs and D2H of h inside the timed region)
     e2e = None
     if not args.no_e2e:
-        h_host = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128).pin_memory()
-        p = pinned
-        call = lambda: api.few_waveform_host(p["t"], p["phase"], p["amp"], p["l"], p["m"], p["n"], p["theta"], p["phi"], w.eps, w.t0,
-                                             w.dt, w.n_samples, out=h_host, device=local)
-        call()
-        n_e2e = max(3, min(args.steps, 10))
         barrier()
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            call()                           # synchronous: returns after the D2H copy completed
-        t_e2e = torch.tensor([(time.perf_counter() - t0) / n_e2e], dtype=torch.float64, device=dev)
+        sec, h2d, d2h = bench.e2e(max(3, min(args.steps, 10)), local)
+        t_e2e = torch.tensor([sec], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-        h2d = sum(v.numel() * v.element_size() for v in pinned.values())
         e2e = {"value": evals_all / float(t_e2e.item()), "unit": "evals/s", "ms_per_step": 1e3 * float(t_e2e.item()),
-               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h_host.numel() * 16),
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "note": "few_waveform_host (C ABI, host pointers): H2D of the sparse inputs + kernels + D2H of h, pinned host buffers"}
 
+    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
     stages = None
     if args.stages and rank == 0:
-        stages = time_stages(api, torch, w, g, flush)
-
-    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
+        stages = time_stages(api, torch, w, bench.g, flush)
     nxt = None
     if args.next and rank == 0:
-        del h
-        nxt = time_next(api, torch, w, g, flush, hbm_gbs)
+        del bench.h
+        nxt = time_next(api, torch, w, bench.g, flush, hbm_gbs)
+    also = None
+    if world == 1 and args.config == 1 and args.eps is None and not args.no_also:
+        del bench
+        torch.cuda.empty_cache()
+        also = also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local)
 
     if rank != 0:
         if world > 1:
@@ -427,36 +564,35 @@ def main():
         return 0
 
     sum_ms_avg = float(np.mean(sum_ms))
-    peak_tflops = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    achieved_tflops = pair_evals_per_step * FLOP_PER_PAIR / (sum_ms_avg * 1e-3) / 1e12
+    achieved_tflops, peak_tflops = sum_kernel_roofline(w, pairs, sum_ms_avg, sm_max_mhz)
     nominal_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
+    traffic = SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if (args.eps is None and world == 1) else None
     roofline = {"bound": "alu", "kernel": "few_sum_kernel", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / peak_tflops,
-                "traffic": SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if args.eps is None else None,
+                "frac": achieved_tflops / peak_tflops, "traffic": traffic,
+                "traffic_source": SUM_KERNEL_DRAM_TRAFFIC_SOURCE if traffic is not None else None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
-                "peak_measured_hot_mix_probe": fp64_mix_tflops, "frac_of_hot_mix_probe": achieved_tflops / fp64_mix_tflops,
-                "peak_measured_mma_form_probe": fp64_mma_tflops,
-                "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / ms_per_step,
-                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {pair_evals_per_step:.4g} "
-                               f"pair evaluations per launch ({pairs} pairs from {K_kept} kept modes)",
+                "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / float(np.mean(step_ms)),
+                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {float(w.n_samples) * pairs:.4g} "
+                               f"pair evaluations per launch on this rank ({pairs} pairs from {K_kept} kept modes)",
                 "nominal_per_mode": {"achieved": nominal_tflops, "frac": nominal_tflops / peak_tflops,
                                      "note": "20 flop per sample*mode evaluation (per-mode formulation); exceeds the executed "
                                              "figure because all l of an (m,n) pair are summed into one spline before the sample loop"}}
     cpu = None
     if not args.no_cpu_baseline:
         v, desc, cores, t_run, n, K = oracle_sample(w, 12.0)
-        cpu = {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": t_run}
-    out = {"metric": "sample*mode evaluations per second (1-yr FP64 waveform, whole hot path)", "value": value, "unit": "evals/s",
+        cpu = {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": t_run, "cpu_model": cpu_model()}
+        v1, desc1, cores1, t1, n1, K1 = oracle_sample(w, 8.0, threads=1, max_samples=1 << 18)
+        cpu["one_core"] = {"value": v1, "unit": "evals/s", "cores": cores1, "sample": desc1, "seconds": t1,
+                           "note": "the paper's CPU convention is one core (PAPER.md:332, 378)"}
+    out = {"metric": METRIC, "value": value, "unit": "evals/s",
            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": w.name, "n_src": w.n_src, "n_t": w.n_t, "n_modes": w.n_modes, "n_samples": w.n_samples, "dt": w.dt,
-                      "eps": w.eps, "kept_modes": K_kept, "mn_pairs": pairs, "l2": "flushed between timed steps (256 MiB write)",
-                      "parallelism": f"{world} independent replicas" if world > 1 else "single GPU"},
-           "ms_per_waveform": ms_per_step / w.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-           "gpu_launches": ((GPU_LAUNCHES_EPS if w.eps > 0 else GPU_LAUNCHES_ALL) + (0 if (2 * w.n_modes * w.n_src + 31) // 32 <= 148 * (232448 // (w.n_t * 608)) else 1)) * args.steps,
-           "clocks": clocks,
-           "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
+           "scaling": scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": config_dict(w_full, parallelism=parallelism),
+           "kept_modes": K_kept, "mn_pairs": pairs, "timing": "L2 flushed between timed steps (256 MiB write); CUDA events on the launch stream; max over ranks",
+           "ms_per_waveform": ms_per_step / w_full.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+           "gpu_launches": int(launches), "gpu_launches_note": "counted by the library at its launch sites (few_launch_count) over the timed steps of this rank",
+           "clocks": clocks, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
     if stages is not None:
         for v in stages.values():
             if "gbs" in v:
@@ -465,6 +601,9 @@ def main():
         out["stages_hbm_peak_gbs"] = hbm_gbs
     if nxt is not None:
         out["next"] = nxt
+    if also is not None:
+        out["also"] = also
+        out["also_hbm_peak_gbs"] = hbm_gbs
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
