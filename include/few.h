@@ -58,7 +58,7 @@ enum {
 };
 
 /* bits of the device status word */
-enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2 };
+enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_SPARSE_LIST = 4 };
 
 #define FEW_MAX_L 16            /* l <= 16: the explicit Wigner-d sum in FP64 is accurate to 5e-15 for l <= 10 (the paper's range) and 1e-12 at l = 16 */
 #define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */

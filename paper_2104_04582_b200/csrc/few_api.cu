@@ -122,6 +122,7 @@ extern "C" int few_device_status(few_ctx* ctx, int* bits_out, void* stream)
     if (bits_out) *bits_out = bits;
     if (bits & FEW_DEV_NOT_INCREASING) { few_set_error("device check: sparse times not strictly increasing"); return FEW_ERR_NOT_INCREASING; }
     if (bits & FEW_DEV_BAD_MODE) { few_set_error("device check: invalid (l, m, n) or kept-mode index"); return FEW_ERR_BAD_MODE; }
+    if (bits & FEW_DEV_SPARSE_LIST) { few_set_error("device check: kept-mode list too sparse in (m, k, |n|) for the summation's step capacity"); return FEW_ERR_LIMIT; }
     return FEW_OK;
 }
 

@@ -4,24 +4,31 @@
 //    ... only compute modes for m >= 0 ... the modes in a single time step are combined."
 //   h(t_i) = scale * sum_{j kept} [ Y+_j W_j + (m_j>0) (-1)^{l_j} Y-_j conj(W_j) ],  W_j = A_j(t_i) exp(-i(m_j Phi_phi + n_j Phi_r)).
 //
-// Algebra used (exact): with E = exp(-i theta) = e_r + i e_i and Ybar = (-1)^l Y- (0 for m = 0),
-//   Y+ A E + Ybar conj(A) conj(E) = e_r U + e_i V,   U = Y+ A + Ybar conj(A),   V = i (Y+ A - Ybar conj(A)).
-// U and V are linear in A's spline coefficients, and E depends on (m, n) only, so all kept l of one (m, n) PAIR are summed
-// into one pair of complex cubics (U_mn, V_mn) per sparse segment BEFORE the sample loop.  The hot loop then costs, per
-// sample and pair, 12 DFMA (two complex cubic Horners) + 4 DFMA (h += e_r U + e_i V) + 4 (E *= Z_r), with no per-l state.
+// Algebra used (exact).  With E = exp(-i theta), Ybar = (-1)^(l+k) Y- (0 for m = 0), a mode contributes
+// alpha E + beta conj(E), alpha = Y+ A, beta = Ybar conj(A): complex cubics in dx (linear in A's spline coefficients).  E depends
+// on (m, k, n) only, so all kept l of one (m, k, n) are summed into one (alpha, beta) per sparse segment BEFORE the sample loop.
+// Further, E_{m,k,+-nu} = P rho^(+-nu) with P = exp(-i(m Phi_phi + k Phi_theta)) (one per RUN (m, k)) and
+// rho^nu = exp(-i nu Phi_r) = c_nu + i s_nu, so the two signs of n share (c_nu, s_nu) -- a UNIT (m, k, nu):
+//   sum over the run = P_r S + i P_i D,   S = sum_nu c_nu B1c_nu + s_nu B1s_nu,   D = sum_nu c_nu B2c_nu + s_nu B2s_nu,
+//   B1c = (alpha+ + alpha-) + (beta+ + beta-),   B1s = i(alpha+ - alpha-) + i(beta- - beta+),
+//   B2c = (alpha+ + alpha-) - (beta+ + beta-),   B2s = i(alpha+ - alpha-) - i(beta- - beta+).
+// S and D are [samples] x [4 powers of dx x (re, im)] = sum over units of [samples x units] . [units x 8]: a small dense FP64
+// contraction per sample tile, executed as DMMA.8x8x4 (mma.sync.m8n8k4.f64) on the FP64 pipe -- 8 samples x 4 consecutive nu
+// per instruction; a lane carries (c_nu, s_nu) of ONE sample and ONE of the four nu and steps it by rho^4 (2 DMUL + 2 DFMA)
+// between the 4 DMMAs of a step.  Per sample and unit: 32 FMA in DMMAs + 4 scalar FP64 operations (40 scalar operations in
+// the per-(m,n)-pair DFMA form this replaces).  The same IEEE FMA arithmetic on the same pipe; what changes is that a DMMA
+// reads 4 registers per 8 FMA where a DFMA reads 3 per FMA, which is what held the DFMA form at 0.75 of the pipe.
 //
 // Three launches per call, all on the caller's stream, nothing read back to the host:
 //   1. few_sum_plan_kernel  (one block per source): clips the dense sample grid to the sparse segments and prefix-sums
 //        the per-segment tile counts (every block of the sum kernel works inside ONE segment, so its coefficients are
-//        block-uniform); orders the kept modes by (m, sign n, |n|, l), finds the pairs and describes how E_mn = Z_phi^m Z_r^n
-//        is reached from the previous pair (walking n upward from 0 with Z_r, then downward with conj Z_r).
-//   2. few_sum_pack_kernel  (one block per source and segment): forms (U_mn, V_mn) from the kept modes' spline coefficients
-//        and Y+, Ybar, scale, and writes them as a stream of 4 KB stages (30 pairs x 128 B + 30 descriptors).
+//        block-uniform); orders the kept modes by (m, k, |n|, sign n, l) and cuts them into STEPS: the kept units of one run
+//        whose nu fall into one aligned block of four (4b .. 4b+3), with a descriptor saying how (c, s) is reached.
+//   2. few_sum_pack_kernel  (one block per source and segment): forms the four B matrices of every step from the kept modes'
+//        spline coefficients and Y+, Ybar, scale, in DMMA fragment order, as a stream of stages (4 steps x 1 KB + header).
 //   3. few_sum_kernel       the hot loop.  Stages arrive in shared memory through a ring of TMA bulk copies
-//        (cp.async.bulk + mbarrier) and are read with 128-bit broadcast loads.  Each thread owns R samples in registers;
-//        per sample the two phases are evaluated ONCE in double-double (Horner, reduction by 2 pi, one sincos each).
-//        Output: coalesced 16-byte streaming stores.
-// FP64 pipe only: per-sample elementwise work with a reduction over modes, not a dense contraction.
+//        (cp.async.bulk + mbarrier) and are read with conflict-free 128-bit loads.  Per sample the phases are evaluated ONCE in
+//        double-double (Horner, reduction by 2 pi, one sincos each).  Output: coalesced 16-byte streaming stores.
 #include "few_common.cuh"
 
 namespace {
@@ -29,44 +36,50 @@ namespace {
 constexpr int kPlanThreads = 1024;
 constexpr int kPlanSmemElems = 16384;         // 128 KB of (key, mode) words: the plan kernel's in-shared-memory sort capacity
 constexpr int kSumThreads = 128;
-#ifndef FEW_SUM_R
-#define FEW_SUM_R 4
-#define FEW_SUM_BPS 3
+#ifndef FEW_SUM_G
+#define FEW_SUM_G 4
+#define FEW_SUM_BPS 4
 #endif
-constexpr int kSumR = FEW_SUM_R;              // samples per thread
+constexpr int kSumG = FEW_SUM_G;              // groups of 8 samples per warp
 constexpr int kSumBlocksPerSm = FEW_SUM_BPS;  // resident blocks per SM (register budget 65536 / (128 * blocks))
-constexpr int kTile = kSumThreads * kSumR;    // samples per block
-constexpr int kStagePairs = 30;               // pairs per stage
-constexpr int kStageBytes = 4096;             // 30 * 128 B of coefficients + 64 ints of header
+constexpr int kTile = (kSumThreads / 32) * 8 * kSumG;   // samples per block
+constexpr int kTileQ = kTile / kSumThreads;   // samples per thread in the per-sample prologue / epilogue
+constexpr int kStageSteps = 4;                // steps per stage
+constexpr int kStepD2 = 64;                   // a step's B fragments: [2][32 lanes] double2 = 1 KB
+constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + 128;   // + header: [0] steps in the stage, [1 + i] descriptor of step i
 constexpr int kStageD2 = kStageBytes / 16;    // stage size in double2
 constexpr int kRing = 4;                      // stages in flight per block
 
-// pair descriptor: bit 0 = special (anything but "advance E by one step"); then
-constexpr int kAdvShift = 1, kAdvBits = 12;   // number of E steps before this pair
-constexpr int kNewSub = 1 << 13;              // restart E from Z_phi^m (n changes sign or m changes)
-constexpr int kDirNeg = 1 << 14;              // walk with conj(Z_r)
-constexpr int kDmShift = 15, kDmBits = 7;     // m increment of a new run
-constexpr int kNewRun = 1 << 22;               // new (m, k) run
-constexpr int kKShift = 23, kKBits = 7;       // polar index of the run, offset by 64 (Kerr-shaped lists, |k| <= FEW_MAX_ABS_K)
+// step descriptor
+constexpr int kNewRun = 1;                    // first step of a run (m, k): close the previous run, P <- Z_phi^m Z_theta^k, (c, s) <- rho^col
+constexpr int kAdvShift = 1, kAdvBits = 12;   // multiplications by rho^4 before the step's DMMAs
+constexpr int kDmShift = 13, kDmBits = 7;     // m increment of a new run
+constexpr int kKShift = 20, kKBits = 7;       // polar index of the run, offset by 64 (Kerr-shaped lists, |k| <= FEW_MAX_ABS_K)
 
 struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
     int* tile_start;     // [n_src][n_t + 2]   exclusive prefix of tiles per pseudo-segment; last = total
-    int* n_groups;       // [n_src]            number of (m, n) pairs
+    int* n_steps;        // [n_src]            number of steps
     int* tile_counter;   // [1]                dynamic tile scheduler of the persistent sum kernel
-    int* desc;           // [n_src][n_modes]   pair descriptors
-    int* g_first;        // [n_src][n_modes+1] first sorted mode of each pair
+    int* desc;           // [n_src][cap]       step descriptors
+    int* u_lo;           // [n_src][cap][8]    sorted range [u_lo, u_hi) of the modes of (step, nu & 3, sign of n)
+    int* u_hi;           // [n_src][cap][8]
     int* order_j;        // [n_src][n_modes]   mode index of sorted position r
     double* yfold;       // [n_src][n_modes][4] scale * (Y+ re, Y+ im, Ybar re, Ybar im) of sorted position r
     double* pack;        // [n_src][n_t - 1][max_stages][kStageBytes / 8]
     double* partial;     // [n_src][max_tiles][4]  per-tile sums of conj(d) h (re, im) and |h|^2 (fused inner products)
     unsigned long long* sortbuf;   // [n_src][sort_pow2] plan-kernel sort array when the mode list exceeds shared memory (else empty)
     int sort_pow2;
+    int cap;             // step capacity per source
     int max_stages;
     int max_tiles;
 };
 
-__host__ __device__ inline int stages_for(int n_pairs) { return (n_pairs + kStagePairs - 1) / kStagePairs; }
+// Step capacity: a step holds up to 8 (m, k, n) triples of one run.  Any mode list on a grid (the paper's: 11 m x 8 blocks of
+// nu = 88 steps for 3843 modes) needs far fewer than n_modes / 4 steps; a list with fewer than 4 modes per step on average AND
+// more than 64 steps over that does not fit and is reported (FEW_DEV_SPARSE_LIST -> FEW_ERR_LIMIT).
+__host__ __device__ inline int step_capacity(int n_modes) { int c = n_modes / 4 + 64; return c < n_modes ? c : n_modes; }
+__host__ __device__ inline int stages_for(int n_steps) { return (n_steps + kStageSteps - 1) / kStageSteps; }
 
 __host__ inline long long sum_max_tiles(long long n_samples, int n_t) { return (n_samples + kTile - 1) / kTile + n_t + 1; }
 
@@ -74,13 +87,15 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samp
 {
     few_carver c(ws);
     sum_layout L;
-    L.max_stages = stages_for(n_modes);
+    L.cap = step_capacity(n_modes);
+    L.max_stages = stages_for(L.cap);
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
-    L.n_groups = c.take<int>(n_src);
+    L.n_steps = c.take<int>(n_src);
     L.tile_counter = c.take<int>(1);
-    L.desc = c.take<int>((size_t)n_src * n_modes);
-    L.g_first = c.take<int>((size_t)n_src * (n_modes + 1));
+    L.desc = c.take<int>((size_t)n_src * L.cap);
+    L.u_lo = c.take<int>((size_t)n_src * L.cap * 8);
+    L.u_hi = c.take<int>((size_t)n_src * L.cap * 8);
     L.order_j = c.take<int>((size_t)n_src * n_modes);
     L.yfold = c.take<double>((size_t)n_src * n_modes * 4);
     L.pack = c.take<double>((size_t)n_src * (n_t - 1) * L.max_stages * (kStageBytes / 8));
@@ -131,13 +146,14 @@ __device__ __forceinline__ int plan_block_scan(int v, int* warp_sums, int* total
     return res;
 }
 
-// sort key: m | k + 64 | sign(n) | |n| | l  (ascending): runs of equal (m, k), inside them n = 0, 1, 2, ... then -1, -2, ...
+// sort key: m | k + 64 | |n| | sign(n) | l  (ascending): runs of equal (m, k); inside a run nu = |n| ascending, +nu before -nu
 __device__ __forceinline__ int key_m(unsigned k) { return (int)(k >> 25); }
 __device__ __forceinline__ int key_k(unsigned k) { return (int)((k >> 18) & 0x7f) - 64; }
 __device__ __forceinline__ unsigned key_run(unsigned k) { return k >> 18; }
-__device__ __forceinline__ int key_dir(unsigned k) { return (int)(k >> 17) & 1; }
-__device__ __forceinline__ int key_absn(unsigned k) { return (int)(k >> 5) & 0xfff; }
+__device__ __forceinline__ int key_absn(unsigned k) { return (int)(k >> 6) & 0xfff; }
+__device__ __forceinline__ int key_neg(unsigned k) { return (int)(k >> 5) & 1; }
 __device__ __forceinline__ int key_l(unsigned k) { return (int)(k & 0x1f); }
+__device__ __forceinline__ unsigned key_unit_sign(unsigned k) { return k >> 5; }      // (run, nu, sign): one (m, k, n) triple
 
 // Bitonic compare-exchange steps on buf[0, n) (n a power of two), which holds elements [c0, c0 + n) of the whole array: for
 // size = size_first, 2 size_first, ..., size_last the strides min(size, n)/2 ... 1.  Direction from the GLOBAL index.
@@ -179,6 +195,9 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         if (k <= n_t - 2) B[k + 1] = first_index(t[k], t0, dt, N, false);
         else { B[n_t] = first_index(t[n_t - 1], t0, dt, N, true); B[n_t + 1] = N; B[0] = 0; }
     }
+    int* ulo = L.u_lo + (size_t)src * L.cap * 8;
+    int* uhi = L.u_hi + (size_t)src * L.cap * 8;
+    for (int q = tid; q < L.cap * 8; q += kPlanThreads) { ulo[q] = 0; uhi[q] = 0; }      // empty (step, nu & 3, sign) slots
     __syncthreads();
     if (tid < 32) {           // warp 0: prefix over n_t + 1 pseudo-segments, 32 at a time
         int carry = 0;
@@ -211,7 +230,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
             atomicOr(status, FEW_DEV_BAD_MODE);
             lj = 2; mj = 0; an = 0; nj = 0; kj = 0; j = ok ? j : 0;
         }
-        const unsigned key = ((unsigned)mj << 25) | ((unsigned)(kj + 64) << 18) | ((nj < 0 ? 1u : 0u) << 17) | ((unsigned)an << 5) |
+        const unsigned key = ((unsigned)mj << 25) | ((unsigned)(kj + 64) << 18) | ((unsigned)an << 6) | ((nj < 0 ? 1u : 0u) << 5) |
                              (unsigned)lj;
         plan_sorted[q] = ((unsigned long long)key << 32) | (unsigned)j;
     }
@@ -245,11 +264,10 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
             chunk_pass(size, size);
         }
     }
-    // ---- (d) pairs: chunked scan of "new (m, n)" flags; descriptors; per-mode fold constants
+    // ---- (d) steps: chunked scan of "new (run, nu >> 2)" flags; descriptors; (step, nu & 3, sign) ranges; fold constants
     if (tid == 0) carry_s = 0;
     __syncthreads();
-    int* desc = L.desc + (size_t)src * n_modes;
-    int* gfirst = L.g_first + (size_t)src * (n_modes + 1);
+    int* desc = L.desc + (size_t)src * L.cap;
     int* oj = L.order_j + (size_t)src * n_modes;
     double* yf = L.yfold + (size_t)src * n_modes * 4;
     // every harmonic constant carries the source's prefactor: the real mu/d_L `scale` of Eq. (10) and the complex detector-frame
@@ -258,28 +276,30 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     const double2 fc = factor ? make_double2(sc * factor[src].x, sc * factor[src].y) : make_double2(sc, 0.0);
     for (int base = 0; base < K; base += kPlanThreads) {
         int r = base + tid;
-        bool new_run = false, new_sub = false, new_grp = false;
+        bool new_run = false, new_step = false;
         unsigned key = 0, prev = 0;
         if (r < K) {
             key = (unsigned)(plan_sorted[r] >> 32); prev = r ? (unsigned)(plan_sorted[r - 1] >> 32) : 0u;
             new_run = r == 0 || key_run(key) != key_run(prev);
-            new_sub = new_run || key_dir(key) != key_dir(prev);
-            new_grp = new_sub || key_absn(key) != key_absn(prev);
+            new_step = new_run || (key_absn(key) >> 2) != (key_absn(prev) >> 2);
         }
-        int total, incl = plan_block_scan(new_grp ? 1 : 0, warp_sums, &total);
+        int total, incl = plan_block_scan(new_step ? 1 : 0, warp_sums, &total);
         int carry = carry_s;
         if (r < K) {
-            int j = (int)(unsigned)(plan_sorted[r] & 0xffffffffull);
+            const int j = (int)(unsigned)(plan_sorted[r] & 0xffffffffull);
+            const int s = carry + incl - 1;                 // step of sorted position r
             oj[r] = j;
-            if (new_grp) {
-                int g = carry + incl - 1;
-                int nadv = new_sub ? key_absn(key) : key_absn(key) - key_absn(prev);
-                int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
-                int d = (nadv << kAdvShift) | (new_sub ? kNewSub : 0) | (key_dir(key) ? kDirNeg : 0) | (dm << kDmShift) |
-                        (new_run ? kNewRun : 0) | ((key_k(key) + 64) << kKShift);
-                if (new_sub || nadv != 1) d |= 1;
-                desc[g] = d;
-                gfirst[g] = r;
+            if (s < L.cap) {
+                if (new_step) {
+                    const int blk = key_absn(key) >> 2;
+                    const int adv = new_run ? blk : blk - (key_absn(prev) >> 2);
+                    const int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
+                    desc[s] = (new_run ? kNewRun : 0) | (adv << kAdvShift) | (dm << kDmShift) | ((key_k(key) + 64) << kKShift);
+                }
+                const int slot = s * 8 + (key_absn(key) & 3) * 2 + key_neg(key);
+                if (r == 0 || key_unit_sign(key) != key_unit_sign(prev)) ulo[slot] = r;
+                const unsigned next = r + 1 < K ? (unsigned)(plan_sorted[r + 1] >> 32) : ~0u;
+                if (r + 1 == K || key_unit_sign(key) != key_unit_sign(next)) uhi[slot] = r + 1;
             }
             double2 yp = ylm_plus[(size_t)src * n_modes + j], yb = make_double2(0.0, 0.0);
             if (key_m(key) > 0) {                       // Eq. (9): the (l,-m,-k,-n) mirror, Ybar = (-1)^(l+k) Y_{l,-m}
@@ -294,45 +314,61 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         if (tid == 0) carry_s = carry + total;
         __syncthreads();
     }
-    if (tid == 0) { L.n_groups[src] = carry_s; gfirst[carry_s] = K; if (src == 0) *L.tile_counter = 0; }
+    if (tid == 0) {
+        int S = carry_s;
+        if (S > L.cap) { atomicOr(status, FEW_DEV_SPARSE_LIST); S = L.cap; }
+        L.n_steps[src] = S;
+        if (src == 0) *L.tile_counter = 0;
+    }
 }
 
-// (U_mn, V_mn) per pair and segment, written as the stage stream the sum kernel consumes.
+// The four B matrices of every step, in DMMA.8x8x4 fragment order, written as the stage stream the sum kernel consumes.
+// Lane L of a warp supplies B[k = L & 3][o = L >> 2]: unit k of the step (nu = 4 blk + k), output o = 2 p + part (power p of
+// dx, part 0 = re, 1 = im).  A step is 1 KB: [0][L] = (B1c, B2c), [1][L] = (B1s, B2s) as double2 (conflict-free LDS.128).
 __global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_t, int n_modes, sum_layout L)
 {
-    const int k = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
-    const int G = L.n_groups[src];
-    const int* gfirst = L.g_first + (size_t)src * (n_modes + 1);
+    const int seg = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
+    const int S = L.n_steps[src];
+    const int* ulo = L.u_lo + (size_t)src * L.cap * 8;
+    const int* uhi = L.u_hi + (size_t)src * L.cap * 8;
     const int* oj = L.order_j + (size_t)src * n_modes;
-    const int* desc = L.desc + (size_t)src * n_modes;
+    const int* desc = L.desc + (size_t)src * L.cap;
     const double4* yf = reinterpret_cast<const double4*>(L.yfold) + (size_t)src * n_modes;
-    const double2* in = coef_amp + ((size_t)src * n_seg + k) * 4 * n_modes;
-    double2* out = reinterpret_cast<double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
-    for (int idx = threadIdx.x; idx < 4 * G; idx += blockDim.x) {
-        const int g = idx >> 2, p = idx & 3;
-        double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
-        for (int r = gfirst[g]; r < gfirst[g + 1]; ++r) {
-            const double2 c = in[(size_t)p * n_modes + oj[r]];
-            const double4 y = yf[r];
-            const double ar = y.x * c.x - y.y * c.y, ai = y.x * c.y + y.y * c.x;      // Y+ c
-            const double br = y.z * c.x + y.w * c.y, bi = y.w * c.x - y.z * c.y;      // Ybar conj(c)
-            ur += ar + br; ui += ai + bi;                                             // U  = a + b
-            vr -= ai - bi; vi += ar - br;                                             // V  = i (a - b)
+    const double2* in = coef_amp + ((size_t)src * n_seg + seg) * 4 * n_modes;
+    double2* out = reinterpret_cast<double2*>(L.pack) + ((size_t)src * n_seg + seg) * L.max_stages * kStageD2;
+    for (int idx = threadIdx.x; idx < 32 * S; idx += blockDim.x) {
+        const int s = idx >> 5, lane = idx & 31, k = lane & 3, o = lane >> 2, p = o >> 1, part = o & 1;
+        double ar[2] = {0.0, 0.0}, ai[2] = {0.0, 0.0}, br[2] = {0.0, 0.0}, bi[2] = {0.0, 0.0};   // alpha, beta of +nu [0] and -nu [1]
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg) {
+            const int slot = s * 8 + k * 2 + sg;
+            for (int r = ulo[slot]; r < uhi[slot]; ++r) {
+                const double2 c = in[(size_t)p * n_modes + oj[r]];
+                const double4 y = yf[r];
+                ar[sg] += y.x * c.x - y.y * c.y; ai[sg] += y.x * c.y + y.y * c.x;      // Y+ c
+                br[sg] += y.z * c.x + y.w * c.y; bi[sg] += y.w * c.x - y.z * c.y;      // Ybar conj(c)
+            }
         }
-        double2* slot = out + (size_t)(g / kStagePairs) * kStageD2 + (g % kStagePairs) * 8;
-        slot[p] = make_double2(ur, ui);
-        slot[4 + p] = make_double2(vr, vi);
+        // a = alpha+ + alpha-, b = beta+ + beta-, da = alpha+ - alpha-, db = beta- - beta+ ;  i z = (-z.im, z.re)
+        const double a_r = ar[0] + ar[1], a_i = ai[0] + ai[1], b_r = br[0] + br[1], b_i = bi[0] + bi[1];
+        const double da_r = ar[0] - ar[1], da_i = ai[0] - ai[1], db_r = br[1] - br[0], db_i = bi[1] - bi[0];
+        double b1c, b2c, b1s, b2s;
+        if (part == 0) { b1c = a_r + b_r; b2c = a_r - b_r; b1s = -(da_i + db_i); b2s = -(da_i - db_i); }
+        else           { b1c = a_i + b_i; b2c = a_i - b_i; b1s = da_r + db_r;    b2s = da_r - db_r; }
+        double2* step = out + (size_t)(s / kStageSteps) * kStageD2 + (s % kStageSteps) * kStepD2;
+        step[lane] = make_double2(b1c, b2c);
+        step[32 + lane] = make_double2(b1s, b2s);
     }
-    const int n_stages = stages_for(G);
-    for (int idx = threadIdx.x; idx < n_stages * 64; idx += blockDim.x) {     // header: [0] count, [1] special mask, [2+q] descriptor q
-        const int s = idx >> 6, q = idx & 63;
+    const int n_stages = stages_for(S);
+    for (int idx = threadIdx.x; idx < n_stages * 32; idx += blockDim.x) {     // header: [0] steps in the stage, [1 + i] descriptor i
+        const int st = idx >> 5, q = idx & 31;
         int v = 0;
-        const int cnt = min(kStagePairs, G - s * kStagePairs);
+        const int cnt = min(kStageSteps, S - st * kStageSteps);
         if (q == 0) v = cnt;
-        else if (q == 1) { for (int i = 0; i < cnt; ++i) v |= (desc[s * kStagePairs + i] & 1) << i; }
-        else if (q - 2 < cnt) v = desc[s * kStagePairs + q - 2];
-        reinterpret_cast<int*>(out + (size_t)s * kStageD2 + kStagePairs * 8)[q] = v;
+        else if (q - 1 < cnt) v = desc[st * kStageSteps + q - 1];
+        reinterpret_cast<int*>(out + (size_t)st * kStageD2 + kStageSteps * kStepD2)[q] = v;
     }
+    // steps of the last stage beyond S are never read (the header's count stops the consumer)
 }
 
 // exp(-i Phi) for Phi = c0 + dx (c1 + dx (c2 + dx c3)) with double-double coefficients (R13, R15).
@@ -389,61 +425,36 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
     } while (!ok);
 }
 
-// E <- E * Z_r for the R samples of a thread (Z_r or conj Z_r, whichever zri currently holds)
-template <int R>
-__device__ __forceinline__ void advance_e(double (&er)[R], double (&ei)[R], const double (&zrr)[R], const double (&zri)[R])
+// D(8x8) += A(8x4) B(4x8) in FP64 on the FP64 pipe (SASS DMMA.8x8x4).  Lane L holds A[L >> 2][L & 3], B[L & 3][L >> 2],
+// C[L >> 2][2 (L & 3)], C[L >> 2][2 (L & 3) + 1].
+__device__ __forceinline__ void dmma884(double2& c, double a, double b)
 {
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const double m1 = ei[r] * zri[r], m2 = ei[r] * zrr[r], e0 = er[r];
-        er[r] = fma(e0, zrr[r], -m1);
-        ei[r] = fma(e0, zri[r], m2);
-    }
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c.x), "+d"(c.y) : "d"(a), "d"(b));
 }
 
-// acc_p += e_r U_p + e_i V_p for the four powers p of dx.  Every DFMA has one block-uniform operand (a coefficient, shared by
-// the R samples of the thread) and two per-thread ones.  A DFMA that reads three registers none of which sits in the
-// operand-reuse cache costs the FP64 pipe about one cycle more than the usual two, so the R samples are
-// walked in alternating directions from one coefficient to the next: where the coefficient changes, e stays the same.
-template <int R>
-__device__ __forceinline__ void accumulate_pair(const double2* __restrict__ cp, const double (&er)[R], const double (&ei)[R],
-                                                double (&are)[4][R], double (&aim)[4][R])
-{
-#pragma unroll
-    for (int p = 0; p < 4; ++p) {
-        const double2 u = cp[p];
-#pragma unroll
-        for (int r = 0; r < R; ++r) are[p][r] = fma(er[r], u.x, are[p][r]);
-#pragma unroll
-        for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(er[r], u.y, aim[p][r]);
-    }
-#pragma unroll
-    for (int p = 0; p < 4; ++p) {
-        const double2 v = cp[4 + p];
-#pragma unroll
-        for (int r = 0; r < R; ++r) are[p][r] = fma(ei[r], v.x, are[p][r]);
-#pragma unroll
-        for (int r = R - 1; r >= 0; --r) aim[p][r] = fma(ei[r], v.y, aim[p][r]);
-    }
-}
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
-// kKerr: Kerr-shaped mode lists (Eq. (1), Eq. (19)): a third phase factor Z_theta and runs of equal (m, k) with
-// E restarting from Z_phi^m Z_theta^k; two more per-thread stashes live in dynamic shared memory.  The hot loop is the same.
-template <int R, int kBlocksPerSm, bool kInner, bool kKerr>
+// G: groups of 8 samples per warp (tile = 4 warps x 8 G samples).  kKerr: Kerr-shaped mode lists (Eq. (1),
+// Eq. (19)): a third phase factor Z_theta, runs are (m, k) with P = Z_phi^m Z_theta^k.  The hot loop is the same.
+template <int G, int kBlocksPerSm, bool kInner, bool kKerr>
 __global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
                int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all)
 {
     constexpr bool want_inner = kInner;      // the inner-product epilogue is compiled out of the plain waveform kernel
+    constexpr int T = 32 * G, Q = T / kSumThreads;
     __shared__ __align__(128) double2 ring[kRing][kStageD2];
     __shared__ __align__(8) unsigned long long full[kRing];
-    __shared__ double2 stash_zp[R][kSumThreads], stash_pm[R][kSumThreads];   // per-thread Z_phi and Z_phi^m (touched ~20x per tile)
+    __shared__ __align__(16) double2 zphi_s[T];          // Z_phi = exp(-i Phi_phi) per sample of the tile
+    __shared__ __align__(16) double2 rpow_s[T][4];       // rho, rho^2, rho^3, rho^4 per sample; after the loop: H_p, p = 0..3
+    __shared__ __align__(16) double2 kerr_s[kKerr ? 2 * T : 1];   // kKerr: Z_theta, then the run's Z_phi^m, per sample
     __shared__ int tile_s;
     __shared__ double red_s[3][kSumThreads / 32];
-    extern __shared__ double2 stash_dyn[];      // kKerr: [R][kSumThreads] Z_theta, then [R][kSumThreads] Z_phi^m Z_theta^k
     constexpr int n_ph = kKerr ? 3 : 2;
 
-    const int tid = threadIdx.x, n_seg = n_t - 1;
+    const int tid = threadIdx.x, lane = tid & 31, n_seg = n_t - 1;
+    const int row = lane >> 2, col = lane & 3;
+    const int sbase = (tid >> 5) * (8 * G) + row;         // tile-relative sample of this lane's group 0 (group g: + 8 g)
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kRing; ++s) mbar_init(&full[s], 1);
@@ -452,7 +463,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     }
     unsigned gst = 0;                       // stages consumed by this block so far: ring slot gst % kRing, parity (gst / kRing) & 1
 
-    // Persistent block: tiles (R*128 samples of one sparse segment of one source) are handed out by an atomic counter, so
+    // Persistent block: tiles (T samples of one sparse segment of one source) are handed out by an atomic counter, so
     // SMs never idle on wave boundaries and the blocks of an SM drift apart (one block's phase setup overlaps the others'
     // FP64 loops).
     for (;;) {
@@ -469,7 +480,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (TS[mid] <= tile) lo = mid; else hi = mid; }
     const int p = lo;
     const long long* B = L.bounds + (size_t)src * (n_t + 2);
-    const long long i_begin = B[p] + (long long)(tile - TS[p]) * (R * kSumThreads), i_end = B[p + 1];
+    const long long i_begin = B[p] + (long long)(tile - TS[p]) * T, i_end = B[p + 1];
     double2* h = h_all ? h_all + (size_t)src * N : nullptr;
     const double2* dat = d_all ? d_all + (size_t)src * N : nullptr;
     double* partial = L.partial + ((size_t)src * max_tiles + tile) * 4;
@@ -477,13 +488,14 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (p == 0 || p == n_t) {           // outside [t_0, t_last]: h = 0 (R12)
         if (h) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) { long long i = i_begin + r * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
+            for (int q = 0; q < Q; ++q) { long long i = i_begin + q * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
         }
         if (want_inner && tid < 3) partial[tid] = 0.0;
         continue;
     }
     const int k = p - 1;
-    const int n_stages = stages_for(L.n_groups[src]);
+    const int n_steps = L.n_steps[src];
+    const int n_stages = stages_for(n_steps);
     const double2* gsrc = reinterpret_cast<const double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
 
     // ---- producer prologue: thread 0 arms the ring with the first kRing - 1 stages of this tile
@@ -495,35 +507,41 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         }
     }
 
-    // ---- per-sample setup (overlaps the first copies): dx and the two phase factors
+    // ---- per-sample setup (overlaps the first copies), one thread per sample: dx, the phase factors, rho^1..4
     const double tk = t_all[(size_t)src * n_t + k];
     const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 4 * n_ph;     // [4][n_ph] dd
-    double zrr[R], zri[R], er[R], ei[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        long long i = i_begin + r * kSumThreads + tid;
-        if (i >= i_end) i = i_end - 1;                              // tail lanes recompute the last sample, never store
+    for (int q = 0; q < Q; ++q) {
+        const int sx = q * kSumThreads + tid;
+        long long i = i_begin + sx;
+        if (i >= i_end) i = i_end - 1;                              // tail samples recompute the last one, never stored
         const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
-        double zpr, zpi;
-        phase_factor(cph + 0, n_ph, dx, &zpr, &zpi);
-        phase_factor(cph + n_ph - 1, n_ph, dx, &zrr[r], &zri[r]);
+        double2 zp, r1;
+        phase_factor(cph + 0, n_ph, dx, &zp.x, &zp.y);
+        phase_factor(cph + n_ph - 1, n_ph, dx, &r1.x, &r1.y);
+        zphi_s[sx] = zp;
+        const double2 r2 = cmul(r1, r1);
+        rpow_s[sx][0] = r1; rpow_s[sx][1] = r2; rpow_s[sx][2] = cmul(r2, r1); rpow_s[sx][3] = cmul(r2, r2);
         if (kKerr) {
-            double ztr, zti;
-            phase_factor(cph + 1, n_ph, dx, &ztr, &zti);
-            stash_dyn[r * kSumThreads + tid] = make_double2(ztr, zti);
-            stash_dyn[(R + r) * kSumThreads + tid] = make_double2(1.0, 0.0);
+            double2 zt;
+            phase_factor(cph + 1, n_ph, dx, &zt.x, &zt.y);
+            kerr_s[sx] = zt;
+            kerr_s[T + sx] = make_double2(1.0, 0.0);
         }
-        // Z_phi and the run's Z_phi^m are needed only when m or the sign of n changes: parked in shared memory, not registers
-        stash_zp[r][tid] = make_double2(zpr, zpi);
-        stash_pm[r][tid] = make_double2(1.0, 0.0);
-        er[r] = 1.0; ei[r] = 0.0;
     }
-    double are[4][R], aim[4][R];                                    // sum over pairs of e_r U_p + e_i V_p, p = power of dx
+    __syncthreads();
+
+    // lane state, per group g (sample sbase + 8 g, unit column col): (c, s) = rho^nu of the current step's nu = 4 blk + col;
+    // z4 = rho^4; P of the current run; S, D accumulators of the run (C fragments: power col, (re, im)); H = sum over runs
+    double cs_c[G], cs_s[G], z4r[G], z4i[G], pr[G], pi[G];
+    double2 accS[G], accD[G], H[G];
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-#pragma unroll
-        for (int r = 0; r < R; ++r) are[q][r] = aim[q][r] = 0.0;
-    bool neg = false;                                               // zri currently holds -Im Z_r (walking n downward)
+    for (int g = 0; g < G; ++g) {
+        const double2 z4 = rpow_s[sbase + 8 * g][3];
+        z4r[g] = z4.x; z4i[g] = z4.y;
+        cs_c[g] = 1.0; cs_s[g] = 0.0; pr[g] = 1.0; pi[g] = 0.0;
+        accS[g] = accD[g] = H[g] = make_double2(0.0, 0.0);
+    }
 
     for (int st = 0; st < n_stages; ++st) {
         __syncthreads();                                            // stage st-1 fully consumed (and barriers initialised)
@@ -535,77 +553,76 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         const int b = gst % kRing;
         mbar_wait(&full[b], (gst / kRing) & 1u);
         ++gst;
-        const double2* cp = &ring[b][0];
-        const int* hdr = reinterpret_cast<const int*>(cp + kStagePairs * 8);
-        const int ng = hdr[0];
-        unsigned spec = (unsigned)hdr[1];
-        int gi = 0;
-        while (gi < ng) {
-            if ((spec & 3u) == 0u && gi + 1 < ng) {                 // common: the next two n of the same run, E *= Z_r each
-                advance_e<R>(er, ei, zrr, zri);
-                accumulate_pair<R>(cp, er, ei, are, aim);
-                advance_e<R>(er, ei, zrr, zri);
-                accumulate_pair<R>(cp + 8, er, ei, are, aim);
-                gi += 2; cp += 16; spec >>= 2;
-                continue;
-            }
-            if (spec & 1u) {                                        // rare: new m, sign change of n, or a gap in n
-                const int d = hdr[2 + gi];
-                if (d & kNewRun) {
-                    const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
+        const double2* bp = &ring[b][0] + lane;
+        const int* hdr = reinterpret_cast<const int*>(&ring[b][0] + kStageSteps * kStepD2);
+        const int ns = hdr[0];
+        for (int si = 0; si < ns; ++si, bp += kStepD2) {
+            const int d = hdr[1 + si];
+            int adv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
+            if (d & kNewRun) {      // rare (once per (m, k)): close the previous run, new P, (c, s) restart from rho^col
+                const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        double2 pm = stash_pm[r][tid];
-                        const double2 zp = stash_zp[r][tid];
-                        for (int q = 0; q < dm; ++q) {
-                            double a = pm.x * zp.x - pm.y * zp.y;
-                            pm.y = pm.x * zp.y + pm.y * zp.x;
-                            pm.x = a;
-                        }
-                        stash_pm[r][tid] = pm;
-                        if (kKerr) {                                // base of the run: Z_phi^m Z_theta^k (k < 0: conjugate powers)
-                            const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
-                            double2 zt = stash_dyn[r * kSumThreads + tid];
-                            if (kk < 0) zt.y = -zt.y;
-                            for (int q = 0; q < (kk < 0 ? -kk : kk); ++q) {
-                                double a = pm.x * zt.x - pm.y * zt.y;
-                                pm.y = pm.x * zt.y + pm.y * zt.x;
-                                pm.x = a;
-                            }
-                            stash_dyn[(R + r) * kSumThreads + tid] = pm;
-                        }
+                for (int g = 0; g < G; ++g) {
+                    H[g].x = fma(pr[g], accS[g].x, fma(-pi[g], accD[g].y, H[g].x));      // H += P_r S + i P_i D
+                    H[g].y = fma(pr[g], accS[g].y, fma(pi[g], accD[g].x, H[g].y));
+                    accS[g] = accD[g] = make_double2(0.0, 0.0);
+                    const int sx = sbase + 8 * g;
+                    const double2 zp = zphi_s[sx];
+                    double2 pm = kKerr ? kerr_s[T + sx] : make_double2(pr[g], pi[g]);
+                    for (int q = 0; q < dm; ++q) pm = cmul(pm, zp);
+                    if (kKerr) {                                    // P = Z_phi^m Z_theta^k (k < 0: conjugate powers)
+                        if (col == 0) kerr_s[T + sx] = pm;          // the 4 lanes of a row hold the same value
+                        const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                        double2 zt = kerr_s[sx];
+                        if (kk < 0) zt.y = -zt.y;
+                        for (int q = 0; q < (kk < 0 ? -kk : kk); ++q) pm = cmul(pm, zt);
                     }
+                    pr[g] = pm.x; pi[g] = pm.y;
+                    const double2 r0 = col ? rpow_s[sx][col - 1] : make_double2(1.0, 0.0);
+                    cs_c[g] = r0.x; cs_s[g] = r0.y;
                 }
-                if (d & kNewSub) {
-                    const bool want_neg = (d & kDirNeg) != 0;
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const double2 pm = kKerr ? stash_dyn[(R + r) * kSumThreads + tid] : stash_pm[r][tid];
-                        er[r] = pm.x; ei[r] = pm.y;
-                        if (want_neg != neg) zri[r] = -zri[r];
-                    }
-                    neg = want_neg;
-                }
-                const int nadv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
-                for (int q = 0; q < nadv; ++q) advance_e<R>(er, ei, zrr, zri);
-            } else {
-                advance_e<R>(er, ei, zrr, zri);
+                if (kKerr) __syncwarp();
             }
-            accumulate_pair<R>(cp, er, ei, are, aim);
-            ++gi; cp += 8; spec >>= 1;
+            for (; adv > 0; --adv) {                                // usually once: nu -> nu + 4
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                    const double m1 = cs_s[g] * z4i[g], m2 = cs_s[g] * z4r[g], e0 = cs_c[g];
+                    cs_c[g] = fma(e0, z4r[g], -m1);
+                    cs_s[g] = fma(e0, z4i[g], m2);
+                }
+            }
+            const double2 b12c = bp[0], b12s = bp[32];
+#pragma unroll
+            for (int g = 0; g < G; ++g) dmma884(accS[g], cs_c[g], b12c.x);
+#pragma unroll
+            for (int g = 0; g < G; ++g) dmma884(accD[g], cs_c[g], b12c.y);
+#pragma unroll
+            for (int g = 0; g < G; ++g) dmma884(accS[g], cs_s[g], b12s.x);
+#pragma unroll
+            for (int g = 0; g < G; ++g) dmma884(accD[g], cs_s[g], b12s.y);
         }
     }
+    __syncthreads();                                                // every warp is done with rpow_s: reuse it for H
+#pragma unroll
+    for (int g = 0; g < G; ++g) {                                   // close the last run; H_p of sample sx, power col -> shared
+        H[g].x = fma(pr[g], accS[g].x, fma(-pi[g], accD[g].y, H[g].x));
+        H[g].y = fma(pr[g], accS[g].y, fma(pi[g], accD[g].x, H[g].y));
+        rpow_s[sbase + 8 * g][col] = H[g];
+    }
+    __syncthreads();
 
-    // ---- h = acc_0 + dx (acc_1 + dx (acc_2 + dx acc_3)), once per sample; optionally the tile's share of the PSD = 1 inner
+    // ---- h = H_0 + dx (H_1 + dx (H_2 + dx H_3)), one thread per sample; optionally the tile's share of the PSD = 1 inner
     // products <d|h>, <h|h> so that a likelihood evaluation never writes h to HBM
     double s_re = 0.0, s_im = 0.0, s_hh = 0.0;
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const long long i = i_begin + r * kSumThreads + tid;
+    for (int q = 0; q < Q; ++q) {
+        const int sx = q * kSumThreads + tid;
+        const long long i = i_begin + sx;
         if (i < i_end) {
             const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
-            const double hr = fma(fma(fma(are[3][r], dx, are[2][r]), dx, are[1][r]), dx, are[0][r]);
-            const double hi = fma(fma(fma(aim[3][r], dx, aim[2][r]), dx, aim[1][r]), dx, aim[0][r]);
+            const double2 h0 = rpow_s[sx][0], h1 = rpow_s[sx][1], h2 = rpow_s[sx][2], h3 = rpow_s[sx][3];
+            const double hr = fma(fma(fma(h3.x, dx, h2.x), dx, h1.x), dx, h0.x);
+            const double hi = fma(fma(fma(h3.y, dx, h2.y), dx, h1.y), dx, h0.y);
             if (h) __stcs(&h[i], make_double2(hr, hi));
             if (want_inner) {
                 if (dat) {
@@ -722,18 +739,15 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
     const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
     const unsigned grid = (unsigned)(want < resident ? want : resident);
-    const size_t kerr_smem = 2 * (size_t)kSumR * kSumThreads * sizeof(double2);      // Z_theta and run-base stashes
-#define FEW_SUM_LAUNCH(INNER, KERR, SMEM, DPTR)                                                                                   \
-    few_sum_kernel<kSumR, kSumBlocksPerSm, INNER, KERR><<<grid, kSumThreads, SMEM, st>>>(                                         \
+#define FEW_SUM_LAUNCH(INNER, KERR, DPTR)                                                                                         \
+    few_sum_kernel<kSumG, kSumBlocksPerSm, INNER, KERR><<<grid, kSumThreads, 0, st>>>(                                            \
         t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, DPTR)
-    if (n_phase == 3) {     // static + dynamic shared memory exceeds the 48 KB default: opt in
-        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_kernel<kSumR, kSumBlocksPerSm, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kerr_smem));
-        FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_kernel<kSumR, kSumBlocksPerSm, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kerr_smem));
-        if (inner) FEW_SUM_LAUNCH(true, true, kerr_smem, (const double2*)d);
-        else FEW_SUM_LAUNCH(false, true, kerr_smem, nullptr);
+    if (n_phase == 3) {
+        if (inner) FEW_SUM_LAUNCH(true, true, (const double2*)d);
+        else FEW_SUM_LAUNCH(false, true, nullptr);
     } else {
-        if (inner) FEW_SUM_LAUNCH(true, false, 0, (const double2*)d);
-        else FEW_SUM_LAUNCH(false, false, 0, nullptr);
+        if (inner) FEW_SUM_LAUNCH(true, false, (const double2*)d);
+        else FEW_SUM_LAUNCH(false, false, nullptr);
     }
 #undef FEW_SUM_LAUNCH
     FEW_LAUNCHED(ctx);
