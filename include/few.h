@@ -61,7 +61,7 @@ enum {
 enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_SPARSE_LIST = 4 };
 
 #define FEW_MAX_L 16            /* l <= 16: the explicit Wigner-d sum in FP64 is accurate to 5e-15 for l <= 10 (the paper's range) and 1e-12 at l = 16 */
-#define FEW_MAX_ABS_N 4095      /* |n| <= 4095 */
+#define FEW_MAX_ABS_N 1023      /* |n| <= 1023: rho^n is stepped by a three-term recurrence whose error after b = |n| / 4 steps is <= b^2 ulp */
 #define FEW_MAX_ABS_K 63        /* |k| <= 63 (polar index of Kerr-shaped mode lists, few_sum_waveform_kerr) */
 #define FEW_MAX_NT_SPLINE 736   /* n_t limit of few_spline_fit (one shared-memory column per system) */
 #define FEW_MAX_SELECT_MODES 131072 /* n_modes limit of few_select_modes (owner bitmap of a row in shared memory) */

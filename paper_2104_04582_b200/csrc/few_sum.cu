@@ -41,33 +41,50 @@ constexpr int kSumThreads = 128;
 #define FEW_SUM_BPS 4
 #endif
 constexpr int kSumG = FEW_SUM_G;              // groups of 8 samples per warp
-constexpr int kSumBlocksPerSm = FEW_SUM_BPS;  // resident blocks per SM (register budget 65536 / (128 * blocks))
+constexpr int kSumBlocksPerSm = FEW_SUM_BPS;  // resident blocks per SM, recurrence instantiation (register budget 65536 / (128 * blocks))
+constexpr int kSumTabBlocksPerSm = 4;         // resident blocks per SM, table instantiation (4 x 128 columns = all of tensor memory)
 constexpr int kTile = (kSumThreads / 32) * 8 * kSumG;   // samples per block
-constexpr int kTileQ = kTile / kSumThreads;   // samples per thread in the per-sample prologue / epilogue
-constexpr int kStageSteps = 4;                // steps per stage
+#ifndef FEW_STAGE_STEPS
+#define FEW_STAGE_STEPS 4
+#endif
+constexpr int kStageSteps = FEW_STAGE_STEPS;  // steps per stage (4 or 8)
 constexpr int kStepD2 = 64;                   // a step's B fragments: [2][32 lanes] double2 = 1 KB
-constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + 128;   // + header: [0] steps in the stage, [1 + i] descriptor of step i
+constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + 128;   // + header: [i] descriptor of step i < 4, [4] steps in the stage
 constexpr int kStageD2 = kStageBytes / 16;    // stage size in double2
-constexpr int kRing = 4;                      // stages in flight per block
+#ifndef FEW_RING
+#define FEW_RING 4
+#endif
+constexpr int kRing = FEW_RING;               // stages in flight per block
 
 // step descriptor
 constexpr int kNewRun = 1;                    // first step of a run (m, k): close the previous run, P <- Z_phi^m Z_theta^k, (c, s) <- rho^col
 constexpr int kAdvShift = 1, kAdvBits = 12;   // multiplications by rho^4 before the step's DMMAs
 constexpr int kDmShift = 13, kDmBits = 7;     // m increment of a new run
 constexpr int kKShift = 20, kKBits = 7;       // polar index of the run, offset by 64 (Kerr-shaped lists, |k| <= FEW_MAX_ABS_K)
+constexpr int kSingle = 1 << 27;              // run with m = 0: no mirror, beta = 0, hence D = S and only S is accumulated
+constexpr int kSlotShift = 28, kSlotBits = 3; // table slot of the step's block nu >> 2 (sources in table mode)
+constexpr int kTabSlots = 8;                  // distinct blocks nu >> 2 a source may use in table mode (the paper's grid: nu <= 31 -> 8)
+
+// A tile of the sum kernel as the plan kernel hands it over (one 32-byte record, two 16-byte loads): first sample and sample
+// count, pseudo-segment p (-1: no tile; 0 or n_t: outside the trajectory, h = 0), the source, and the number of coefficient
+// stages the tile consumes (0 for tiles without a summation), and the source's mode (1 table, 0 recurrence: which of the two
+// instantiations of the sum kernel takes the tile).
+struct __align__(16) tile_rec { long long i_begin; int count; int p; int n_stages; int src; int mode; int pad1; };
 
 struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
     int* tile_start;     // [n_src][n_t + 2]   exclusive prefix of tiles per pseudo-segment; last = total
     int* n_steps;        // [n_src]            number of steps
-    int* tile_counter;   // [1]                dynamic tile scheduler of the persistent sum kernel
+    int* blk_list;       // [n_src][8]         table mode: the distinct blocks nu >> 2 of the source, ascending (slot -> block), -1 = unused
+    int* mode_count;     // [2]                sources in recurrence mode [0] / table mode [1] (zeroed before the plan kernel)
+    tile_rec* tiles;     // [n_src][max_tiles] what the plan kernel hands every tile, so that a warp finds its work with one record
     int* desc;           // [n_src][cap]       step descriptors
     int* u_lo;           // [n_src][cap][8]    sorted range [u_lo, u_hi) of the modes of (step, nu & 3, sign of n)
     int* u_hi;           // [n_src][cap][8]
     int* order_j;        // [n_src][n_modes]   mode index of sorted position r
     double* yfold;       // [n_src][n_modes][4] scale * (Y+ re, Y+ im, Ybar re, Ybar im) of sorted position r
     double* pack;        // [n_src][n_t - 1][max_stages][kStageBytes / 8]
-    double* partial;     // [n_src][max_tiles][4]  per-tile sums of conj(d) h (re, im) and |h|^2 (fused inner products)
+    double* partial;     // [n_src][max_tiles][4 warps][4]  per-warp sums of conj(d) h (re, im) and |h|^2 (fused inner products)
     unsigned long long* sortbuf;   // [n_src][sort_pow2] plan-kernel sort array when the mode list exceeds shared memory (else empty)
     int sort_pow2;
     int cap;             // step capacity per source
@@ -92,16 +109,18 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samp
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
     L.n_steps = c.take<int>(n_src);
-    L.tile_counter = c.take<int>(1);
+    L.blk_list = c.take<int>((size_t)n_src * kTabSlots);
+    L.mode_count = c.take<int>(2);
+    const long long mt = sum_max_tiles(n_samples, n_t);
+    L.max_tiles = (int)(mt < 2147483647LL ? mt : 2147483647LL);
+    L.tiles = c.take<tile_rec>((size_t)n_src * (size_t)mt);
     L.desc = c.take<int>((size_t)n_src * L.cap);
     L.u_lo = c.take<int>((size_t)n_src * L.cap * 8);
     L.u_hi = c.take<int>((size_t)n_src * L.cap * 8);
     L.order_j = c.take<int>((size_t)n_src * n_modes);
     L.yfold = c.take<double>((size_t)n_src * n_modes * 4);
     L.pack = c.take<double>((size_t)n_src * (n_t - 1) * L.max_stages * (kStageBytes / 8));
-    const long long mt = sum_max_tiles(n_samples, n_t);
-    L.max_tiles = (int)(mt < 2147483647LL ? mt : 2147483647LL);
-    L.partial = c.take<double>((size_t)n_src * (size_t)mt * 4);
+    L.partial = c.take<double>((size_t)n_src * (size_t)mt * (kSumThreads / 32) * 4);
     int p2 = 1;
     while (p2 < n_modes) p2 <<= 1;
     L.sort_pow2 = p2 > kPlanSmemElems ? p2 : 0;
@@ -264,6 +283,28 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
             chunk_pass(size, size);
         }
     }
+    // ---- (d0) the distinct blocks nu >> 2 of the list: at most kTabSlots of them -> table mode (the sum kernel keeps rho^nu of
+    // every sample in shared memory), else recurrence mode
+    __shared__ unsigned blk_mask[(FEW_MAX_ABS_N + 1) / 4 / 32];
+    __shared__ int mode_s;
+    if (tid < (FEW_MAX_ABS_N + 1) / 4 / 32) blk_mask[tid] = 0u;
+    __syncthreads();
+    for (int r = tid; r < K; r += kPlanThreads) {
+        const int blk = key_absn((unsigned)(plan_sorted[r] >> 32)) >> 2;
+        atomicOr(&blk_mask[blk >> 5], 1u << (blk & 31));
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int cnt = 0;
+        int* bl = L.blk_list + (size_t)src * kTabSlots;
+        for (int q = 0; q < kTabSlots; ++q) bl[q] = -1;
+        for (int wd = 0; wd < (FEW_MAX_ABS_N + 1) / 4 / 32; ++wd) {
+            unsigned mk = blk_mask[wd];
+            while (mk) { const int b = __ffs(mk) - 1; mk &= mk - 1; if (cnt < kTabSlots) bl[cnt] = wd * 32 + b; ++cnt; }
+        }
+        mode_s = cnt <= kTabSlots ? 1 : 0;
+        atomicAdd(&L.mode_count[mode_s], 1);
+    }
     // ---- (d) steps: chunked scan of "new (run, nu >> 2)" flags; descriptors; (step, nu & 3, sign) ranges; fold constants
     if (tid == 0) carry_s = 0;
     __syncthreads();
@@ -294,9 +335,13 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
                     const int blk = key_absn(key) >> 2;
                     const int adv = new_run ? blk : blk - (key_absn(prev) >> 2);
                     const int dm = new_run ? key_m(key) - (r ? key_m(prev) : 0) : 0;
-                    desc[s] = (new_run ? kNewRun : 0) | (adv << kAdvShift) | (dm << kDmShift) | ((key_k(key) + 64) << kKShift);
+                    int slot = 0;                               // rank of blk among the source's distinct blocks
+                    for (int wd = 0; wd < (blk >> 5); ++wd) slot += __popc(blk_mask[wd]);
+                    slot += __popc(blk_mask[blk >> 5] & ((1u << (blk & 31)) - 1u));
+                    desc[s] = (new_run ? kNewRun : 0) | (adv << kAdvShift) | (dm << kDmShift) | ((key_k(key) + 64) << kKShift) |
+                              (key_m(key) == 0 ? kSingle : 0) | ((slot & ((1 << kSlotBits) - 1)) << kSlotShift);
                 }
-                const int slot = s * 8 + (key_absn(key) & 3) * 2 + key_neg(key);
+                const int slot = s * 8 + (key_absn(key) & 3) * 2 + key_neg(key);      // (step, nu & 3, sign) range slot
                 if (r == 0 || key_unit_sign(key) != key_unit_sign(prev)) ulo[slot] = r;
                 const unsigned next = r + 1 < K ? (unsigned)(plan_sorted[r + 1] >> 32) : ~0u;
                 if (r + 1 == K || key_unit_sign(key) != key_unit_sign(next)) uhi[slot] = r + 1;
@@ -318,7 +363,29 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         int S = carry_s;
         if (S > L.cap) { atomicOr(status, FEW_DEV_SPARSE_LIST); S = L.cap; }
         L.n_steps[src] = S;
-        if (src == 0) *L.tile_counter = 0;
+        carry_s = S;
+    }
+    __syncthreads();
+    // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1])
+    {
+        const int n_stages = stages_for(carry_s);
+        tile_rec* rec = L.tiles + (size_t)src * L.max_tiles;
+        for (int p = tid >> 5; p <= n_t; p += kPlanThreads / 32) {           // a warp per pseudo-segment
+            const int q0 = TS[p], q1 = TS[p + 1];
+            const long long b0 = B[p], b1 = B[p + 1];
+            for (int q = q0 + (tid & 31); q < q1; q += 32) {
+                tile_rec r;
+                r.i_begin = b0 + (long long)(q - q0) * kTile;
+                const long long left = b1 - r.i_begin;
+                r.count = (int)(left < kTile ? left : kTile);
+                r.p = p; r.n_stages = (p == 0 || p == n_t) ? 0 : n_stages; r.src = src; r.mode = mode_s; r.pad1 = 0;
+                rec[q] = r;
+            }
+        }
+        for (int q = TS[n_t + 1] + tid; q < L.max_tiles; q += kPlanThreads) {
+            tile_rec r; r.i_begin = 0; r.count = 0; r.p = -1; r.n_stages = 0; r.src = src; r.mode = mode_s; r.pad1 = 0;
+            rec[q] = r;
+        }
     }
 }
 
@@ -360,12 +427,12 @@ __global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_
         step[32 + lane] = make_double2(b1s, b2s);
     }
     const int n_stages = stages_for(S);
-    for (int idx = threadIdx.x; idx < n_stages * 32; idx += blockDim.x) {     // header: [0] steps in the stage, [1 + i] descriptor i
+    for (int idx = threadIdx.x; idx < n_stages * 32; idx += blockDim.x) {     // header: [i] descriptor i, [4] steps in the stage
         const int st = idx >> 5, q = idx & 31;
         int v = 0;
         const int cnt = min(kStageSteps, S - st * kStageSteps);
-        if (q == 0) v = cnt;
-        else if (q - 1 < cnt) v = desc[st * kStageSteps + q - 1];
+        if (q == kStageSteps) v = cnt;
+        else if (q < cnt) v = desc[st * kStageSteps + q];
         reinterpret_cast<int*>(out + (size_t)st * kStageD2 + kStageSteps * kStepD2)[q] = v;
     }
     // steps of the last stage beyond S are never read (the header's count stops the consumer)
@@ -382,7 +449,9 @@ __device__ __forceinline__ dd dd_add_fast(dd a, dd b)            // error O(eps^
     return quick_two_sum(s.hi, s.lo);
 }
 
-__device__ __forceinline__ void phase_factor(const dd* __restrict__ c, int stride, double dx, double* zr, double* zi)
+// (not inlined: called two or three times per sample and tile; the sum kernel's code must stay small enough for the
+// instruction caches -- the kernel ran a fifth slower when its per-tile code was 28 KB)
+__device__ __noinline__ void phase_factor(const dd* __restrict__ c, int stride, double dx, double* zr, double* zi)
 {
     dd r = dd_add_d(c[2 * stride], __dmul_rn(c[3 * stride].hi, dx));
     r = dd_add_fast(dd_mul_d(r, dx), c[stride]);
@@ -434,199 +503,371 @@ __device__ __forceinline__ void dmma884(double2& c, double a, double b)
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
-// G: groups of 8 samples per warp (tile = 4 warps x 8 G samples).  kKerr: Kerr-shaped mode lists (Eq. (1),
-// Eq. (19)): a third phase factor Z_theta, runs are (m, k) with P = Z_phi^m Z_theta^k.  The hot loop is the same.
-template <int G, int kBlocksPerSm, bool kInner, bool kKerr>
+// Tensor memory (TMEM, 256 KB per SM: 128 lanes x 512 columns x 32 bit) used as per-thread scratch: with the 32x32b shape,
+// thread i of warp w reads and writes lane 32 (w % 4) + i, i.e. its own row of the block's allocation.  The table instantiation
+// keeps rho^nu of its 8 G samples there: 16 bytes per (table slot, group) and thread = 128 columns for G = 4, four resident
+// blocks per SM fill the 512 columns.  tcgen05.ld/st are warp-collective and asynchronous (wait::ld / wait::st).
+__device__ __forceinline__ void tmem_alloc(unsigned* smem_dst, unsigned ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(unsigned taddr, unsigned ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_st_x4(unsigned taddr, double2 v)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__double2loint(v.x)),
+                 "r"(__double2hiint(v.x)), "r"(__double2loint(v.y)), "r"(__double2hiint(v.y))
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// four (c, s) pairs = 16 columns of this thread's lane
+__device__ __forceinline__ void tmem_ld_x16(unsigned taddr, double2 (&v)[4])
+{
+    unsigned r[16];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                   "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr)
+                 : "memory");
+    tmem_wait_ld();
+#pragma unroll
+    for (int g = 0; g < 4; ++g) v[g] = make_double2(__hiloint2double(r[4 * g + 1], r[4 * g]), __hiloint2double(r[4 * g + 3], r[4 * g + 2]));
+}
+
+__device__ __forceinline__ tile_rec load_rec(const tile_rec* p)
+{
+    const int4 a = __ldg(reinterpret_cast<const int4*>(p)), b = __ldg(reinterpret_cast<const int4*>(p) + 1);
+    tile_rec r;
+    r.i_begin = ((long long)(unsigned)a.y << 32) | (unsigned)a.x; r.count = a.z; r.p = a.w;
+    r.n_stages = b.x; r.src = b.y; r.mode = b.z; r.pad1 = 0;
+    return r;
+}
+
+// The sum kernel.  A block is 4 warps that share ONE thing: the ring of coefficient stages.  Everything else is per warp:
+// a warp owns 8 G samples of every tile of its block (tile = 4 warps x 8 G samples inside one sparse segment of one source,
+// so the coefficients are block-uniform), evaluates their phases, runs the step loop and stores their h, and never meets
+// another warp at a barrier.  Tiles are assigned statically (block b takes tiles b, b + grid, ...; every tile of a source
+// costs the same), each warp reads the tile records itself, one tile ahead.  Ring protocol: full[slot] is an mbarrier the
+// TMA bulk copy completes; when a warp is done with a slot it bumps done[slot], and the LAST of the 4 warps refills the slot
+// with the stage kRing ahead in the block's stage stream (walking into the next tiles' records where the stream crosses a
+// tile boundary).  So warps drift apart by at most the ring depth and wait only for data.
+// G: groups of 8 samples per warp.  kKerr: Kerr-shaped mode lists (Eq. (1), Eq. (19)): a third phase factor
+// Z_theta, runs are (m, k) with P = Z_phi^m Z_theta^k.  The hot loop is the same.
+// kTab: where the A operands (c, s) = rho^nu come from.  On the FP64 pipe a scalar instruction issued between the DMMAs of
+// other warps costs about 5 cycles, not 2, so the table instantiation computes rho^nu of every sample
+// ONCE per tile -- rho^nu does not depend on the run (m, k) -- into a per-warp shared-memory table in DMMA fragment order
+// and the step loop is loads and DMMAs only; it takes the sources whose lists use at most kTabSlots distinct blocks nu >> 2
+// (the paper's grid: nu <= 31).  The recurrence instantiation steps x_b = rho^(4 b + col) in registers (2 DFMA per group and
+// step) and takes every other source.  Both are launched; each works on the tiles whose record names its mode.
+template <int G, bool kKerr, bool kTab>
+struct sum_smem {
+    static constexpr int W = 8 * G, kWarps = kSumThreads / 32;
+    __align__(128) double2 ring[kRing][kStageD2];
+    __align__(8) unsigned long long full[kRing];
+    int done[kRing];                                            // warps finished with the slot's current stage
+    __align__(16) double2 zphi[kWarps][W];                      // Z_phi = exp(-i Phi_phi) per sample
+    __align__(16) double2 rpow[kWarps][W][4];                   // rho, rho^2, rho^3, rho^4 per sample; after the loop: H_p, p = 0..3
+    __align__(16) double2 pcur[kWarps][W];                      // P = Z_phi^m Z_theta^k of the current run, per sample
+    __align__(16) double2 hacc[kWarps][G][32];                  // per lane and group: H = sum over the closed runs
+    __align__(16) double2 kerr[kKerr ? kWarps : 1][2][kKerr ? W : 1];   // kKerr: Z_theta, the run's Z_phi^m, per sample
+    unsigned tmem_base;                                         // kTab: the block's tensor-memory allocation (rho^nu table)
+};
+template <int G, bool kKerr, bool kTab> constexpr size_t sum_smem_bytes() { return sizeof(sum_smem<G, kKerr, kTab>); }
+
+template <int G, int kBlocksPerSm, bool kInner, bool kKerr, bool kTab>
 __global__ void __launch_bounds__(kSumThreads, kBlocksPerSm)
 few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_phase, double t0, double dt, long long N,
                int n_t, int n_src, int max_tiles, sum_layout L, double2* __restrict__ h_all, const double2* __restrict__ d_all)
 {
     constexpr bool want_inner = kInner;      // the inner-product epilogue is compiled out of the plain waveform kernel
-    constexpr int T = 32 * G, Q = T / kSumThreads;
-    __shared__ __align__(128) double2 ring[kRing][kStageD2];
-    __shared__ __align__(8) unsigned long long full[kRing];
-    __shared__ __align__(16) double2 zphi_s[T];          // Z_phi = exp(-i Phi_phi) per sample of the tile
-    __shared__ __align__(16) double2 rpow_s[T][4];       // rho, rho^2, rho^3, rho^4 per sample; after the loop: H_p, p = 0..3
-    __shared__ __align__(16) double2 kerr_s[kKerr ? 2 * T : 1];   // kKerr: Z_theta, then the run's Z_phi^m, per sample
-    __shared__ int tile_s;
-    __shared__ double red_s[3][kSumThreads / 32];
+    constexpr int W = 8 * G, kWarps = kSumThreads / 32, QW = (W + 31) / 32;     // W: samples per warp and tile
+    using smem_t = sum_smem<G, kKerr, kTab>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    smem_t& sm = *reinterpret_cast<smem_t*>(smem_raw);
+    auto& ring = sm.ring; auto& full = sm.full; auto& done_s = sm.done; auto& zphi_s = sm.zphi; auto& rpow_s = sm.rpow;
+    auto& pcur_s = sm.pcur; auto& hacc_s = sm.hacc; auto& kerr_s = sm.kerr;
     constexpr int n_ph = kKerr ? 3 : 2;
 
-    const int tid = threadIdx.x, lane = tid & 31, n_seg = n_t - 1;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_seg = n_t - 1;
     const int row = lane >> 2, col = lane & 3;
-    const int sbase = (tid >> 5) * (8 * G) + row;         // tile-relative sample of this lane's group 0 (group g: + 8 g)
+    const long long total_tiles = (long long)n_src * max_tiles;
+    const long long stride = gridDim.x;
+    const double2* pack = reinterpret_cast<const double2*>(L.pack);
+
+    // issue the stage `s` stages after the start of tile sequence number `i` of this block (record ri; rn = record of i + 1)
+    // into ring slot `slot`: walks forward through the block's tiles where s runs past a tile's stages
+    auto issue = [&](long long i, int s, tile_rec ri, const tile_rec& rn, unsigned slot) {
+        long long j = i;
+        auto mine = [](const tile_rec& r) { return r.mode == (kTab ? 1 : 0) ? r.n_stages : 0; };
+        while (s >= mine(ri)) {
+            s -= mine(ri);
+            ++j;
+            const long long tg = blockIdx.x + j * stride;
+            if (tg >= total_tiles) return;                          // the stream has ended
+            ri = (j == i + 1) ? rn : load_rec(L.tiles + tg);
+        }
+        const double2* src = pack + ((size_t)ri.src * n_seg + (ri.p - 1)) * L.max_stages * kStageD2 + (size_t)s * kStageD2;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the warps' reads of the slot precede the copy's writes
+        mbar_expect_tx(&full[slot], kStageBytes);
+        bulk_g2s(&ring[slot][0], src, kStageBytes, &full[slot]);
+    };
+
+    if (L.mode_count[kTab ? 1 : 0] == 0) return;       // no source in this instantiation's mode
+    constexpr unsigned kTmemCols = 16 * kTabSlots;     // 128 columns: (c, s) x G = 4 groups x kTabSlots slots per thread
+    if (kTab && warp == 0) tmem_alloc(&sm.tmem_base, kTmemCols);
+    tile_rec cur, nxt;
+    cur.p = -1; cur.n_stages = 0; cur.count = 0; cur.i_begin = 0; cur.src = 0; cur.mode = 0; cur.pad1 = 0;
+    nxt = cur;
+    if ((long long)blockIdx.x < total_tiles) cur = load_rec(L.tiles + blockIdx.x);
+    if (blockIdx.x + stride < total_tiles) nxt = load_rec(L.tiles + blockIdx.x + stride);
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kRing; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < kRing; ++s) { mbar_init(&full[s], 1); done_s[s] = 0; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if ((long long)blockIdx.x < total_tiles) {
+#pragma unroll 1
+            for (int s = 0; s < kRing; ++s) issue(0, s, cur, nxt, s);
+        }
     }
-    unsigned gst = 0;                       // stages consumed by this block so far: ring slot gst % kRing, parity (gst / kRing) & 1
+    if (kTab) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();                        // the only block-wide barrier of the kernel (besides the one before the TMEM release)
+    if (kTab) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const unsigned tmem_row = kTab ? sm.tmem_base + ((unsigned)(warp * 32) << 16) : 0u;   // this warp's lanes of the allocation
+    unsigned gst = 0;                       // stages consumed by this warp so far: ring slot gst % kRing, use number gst / kRing
 
-    // Persistent block: tiles (T samples of one sparse segment of one source) are handed out by an atomic counter, so
-    // SMs never idle on wave boundaries and the blocks of an SM drift apart (one block's phase setup overlaps the others'
-    // FP64 loops).
-    for (;;) {
-    __syncthreads();
-    if (tid == 0) tile_s = atomicAdd(L.tile_counter, 1);
-    __syncthreads();
-    const int tg = tile_s;
-    if (tg >= n_src * max_tiles) break;
-    const int src = tg / max_tiles, tile = tg - src * max_tiles;
-    const int* TS = L.tile_start + (size_t)src * (n_t + 2);
-    if (tile >= TS[n_t + 1]) continue;
-    // pseudo-segment of this tile: largest p with TS[p] <= tile
-    int lo = 0, hi = n_t + 1;
-    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (TS[mid] <= tile) lo = mid; else hi = mid; }
-    const int p = lo;
-    const long long* B = L.bounds + (size_t)src * (n_t + 2);
-    const long long i_begin = B[p] + (long long)(tile - TS[p]) * T, i_end = B[p + 1];
+    for (long long i = 0;; ++i) {
+    const long long tg = blockIdx.x + i * stride;
+    if (tg >= total_tiles) break;
+    tile_rec nn = cur;                      // record of tile i + 2: loaded now, needed at the end of this tile
+    nn.p = -1; nn.n_stages = 0; nn.count = 0;
+    if (tg + 2 * stride < total_tiles) nn = load_rec(L.tiles + tg + 2 * stride);
+    if (cur.p >= 0 && cur.mode == (kTab ? 1 : 0)) {
+    const int src = cur.src, p = cur.p;
+    const long long w_begin = cur.i_begin + warp * W;               // this warp's samples: [w_begin, w_begin + w_count)
+    const int w_count = min(max(cur.count - warp * W, 0), W);
     double2* h = h_all ? h_all + (size_t)src * N : nullptr;
     const double2* dat = d_all ? d_all + (size_t)src * N : nullptr;
-    double* partial = L.partial + ((size_t)src * max_tiles + tile) * 4;
+    double* partial = L.partial + (((size_t)src * max_tiles + (size_t)(tg - (long long)src * max_tiles)) * kWarps + warp) * 4;
 
-    if (p == 0 || p == n_t) {           // outside [t_0, t_last]: h = 0 (R12)
+    if (cur.n_stages == 0) {                // outside [t_0, t_last] (R12), or nothing kept: h = 0
         if (h) {
 #pragma unroll
-            for (int q = 0; q < Q; ++q) { long long i = i_begin + q * kSumThreads + tid; if (i < i_end) h[i] = make_double2(0.0, 0.0); }
+            for (int q = 0; q < QW; ++q) { const int sx = q * 32 + lane; if (sx < w_count) h[w_begin + sx] = make_double2(0.0, 0.0); }
         }
-        if (want_inner && tid < 3) partial[tid] = 0.0;
-        continue;
-    }
+        if (want_inner && lane < 3) partial[lane] = 0.0;
+    } else {
     const int k = p - 1;
-    const int n_steps = L.n_steps[src];
-    const int n_stages = stages_for(n_steps);
-    const double2* gsrc = reinterpret_cast<const double2*>(L.pack) + ((size_t)src * n_seg + k) * L.max_stages * kStageD2;
+    const int n_stages = cur.n_stages;
 
-    // ---- producer prologue: thread 0 arms the ring with the first kRing - 1 stages of this tile
-    if (tid == 0) {
-        for (int s = 0; s < kRing - 1 && s < n_stages; ++s) {
-            const int b = (gst + s) % kRing;
-            mbar_expect_tx(&full[b], kStageBytes);
-            bulk_g2s(&ring[b][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[b]);
-        }
-    }
-
-    // ---- per-sample setup (overlaps the first copies), one thread per sample: dx, the phase factors, rho^1..4
+    // ---- per-sample setup, one lane per sample of the warp: dx, the phase factors, rho^1..4 (and the rho^nu table)
     const double tk = t_all[(size_t)src * n_t + k];
     const dd* cph = coef_phase + ((size_t)src * n_seg + k) * 4 * n_ph;     // [4][n_ph] dd
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        const int sx = q * kSumThreads + tid;
-        long long i = i_begin + sx;
-        if (i >= i_end) i = i_end - 1;                              // tail samples recompute the last one, never stored
-        const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
-        double2 zp, r1;
-        phase_factor(cph + 0, n_ph, dx, &zp.x, &zp.y);
-        phase_factor(cph + n_ph - 1, n_ph, dx, &r1.x, &r1.y);
-        zphi_s[sx] = zp;
-        const double2 r2 = cmul(r1, r1);
-        rpow_s[sx][0] = r1; rpow_s[sx][1] = r2; rpow_s[sx][2] = cmul(r2, r1); rpow_s[sx][3] = cmul(r2, r2);
-        if (kKerr) {
-            double2 zt;
-            phase_factor(cph + 1, n_ph, dx, &zt.x, &zt.y);
-            kerr_s[sx] = zt;
-            kerr_s[T + sx] = make_double2(1.0, 0.0);
+    for (int q = 0; q < QW; ++q) {
+        const int sx = q * 32 + lane;
+        if (sx < W) {
+            long long is = w_begin + sx;
+            const long long i_last = cur.i_begin + cur.count - 1;
+            if (is > i_last) is = i_last;                           // tail samples recompute the last one, never stored
+            const double dx = __dsub_rn(sample_time(t0, dt, is), tk);
+            double2 zp, r1;
+            phase_factor(cph + 0, n_ph, dx, &zp.x, &zp.y);
+            phase_factor(cph + n_ph - 1, n_ph, dx, &r1.x, &r1.y);
+            zphi_s[warp][sx] = zp;
+            pcur_s[warp][sx] = make_double2(1.0, 0.0);
+            const double2 r2 = cmul(r1, r1), r3 = cmul(r2, r1), r4 = cmul(r2, r2);
+            if (kKerr) {
+                double2 zt;
+                phase_factor(cph + 1, n_ph, dx, &zt.x, &zt.y);
+                kerr_s[warp][0][sx] = zt;
+                kerr_s[warp][1][sx] = make_double2(1.0, 0.0);
+            }
+            rpow_s[warp][sx][0] = r1; rpow_s[warp][sx][1] = r2; rpow_s[warp][sx][2] = r3; rpow_s[warp][sx][3] = r4;
         }
     }
-    __syncthreads();
+    __syncwarp();
+    if (kTab) {
+        // table mode: x_b = rho^(4 b + col) of this lane's samples, for the blocks b the source uses (slot -> block, ascending,
+        // in L.blk_list), by the three-term recurrence (below), into the lane's own tensor-memory row: column 16 slot + 4 g
+        // holds (c, s) of group g.  (Rolled loops: nothing here lives in a register array, and the code stays small.)
+        const int* blp = L.blk_list + (size_t)src * kTabSlots;
+        double2 xa[G], xb[G];                                       // x_b, x_{b-1} of the G groups: G independent chains
+        double twg[G];
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int sx = 8 * g + row;
+            const double2 xm = rpow_s[warp][sx][3 - col];
+            xa[g] = col ? rpow_s[warp][sx][col - 1] : make_double2(1.0, 0.0);
+            xb[g] = make_double2(xm.x, -xm.y);
+            twg[g] = 2.0 * rpow_s[warp][sx][3].x;
+        }
+        int slot = 0, target = __ldg(blp);
+#pragma unroll 1
+        for (int b = 0; target >= 0; ++b) {
+            if (b == target) {
+#pragma unroll
+                for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, xa[g]);
+                ++slot;
+                target = slot < kTabSlots ? __ldg(blp + slot) : -1;
+            }
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                const double2 nx = make_double2(fma(twg[g], xa[g].x, -xb[g].x), fma(twg[g], xa[g].y, -xb[g].y));
+                xb[g] = xa[g]; xa[g] = nx;
+            }
+        }
+        tmem_wait_st();
+    }
 
-    // lane state, per group g (sample sbase + 8 g, unit column col): (c, s) = rho^nu of the current step's nu = 4 blk + col;
-    // z4 = rho^4; P of the current run; S, D accumulators of the run (C fragments: power col, (re, im)); H = sum over runs
-    double cs_c[G], cs_s[G], z4r[G], z4i[G], pr[G], pi[G];
-    double2 accS[G], accD[G], H[G];
+    // Lane state, per group g (sample 8 g + row of the warp, unit column col).  S, D: accumulators of the run (C fragments:
+    // power col of dx, (re, im)).  P and H = sum over the closed runs of P_r S + i P_i D are touched once per run and live in
+    // shared memory.  Recurrence mode only: x_b = rho^(4 b + col) = (c, s) of block b obeys the three-term recurrence
+    // x_{b+1} = 2 cos(4 Phi_r) x_b - x_{b-1} (one DFMA per component; its error after b steps is at most b^2 u whatever the
+    // angle: the Green's function sin(j theta) / sin(theta) is bounded by j), started from x_0 = rho^col and
+    // x_{-1} = conj(rho^(4 - col)).  The two most recent blocks live in (xc, xs) and (yc, ys); `odd` says which is current,
+    // so that a step overwrites the older one in place.
+    constexpr int GR = kTab ? 1 : G;
+    double xc[GR], xs[GR], yc[GR], ys[GR], tw[GR];
+    double2 accS[G], accD[G];
 #pragma unroll
     for (int g = 0; g < G; ++g) {
-        const double2 z4 = rpow_s[sbase + 8 * g][3];
-        z4r[g] = z4.x; z4i[g] = z4.y;
-        cs_c[g] = 1.0; cs_s[g] = 0.0; pr[g] = 1.0; pi[g] = 0.0;
-        accS[g] = accD[g] = H[g] = make_double2(0.0, 0.0);
+        if (!kTab) {
+            tw[g % GR] = 2.0 * rpow_s[warp][8 * g + row][3].x;
+            xc[g % GR] = 1.0; xs[g % GR] = 0.0; yc[g % GR] = 1.0; ys[g % GR] = 0.0;
+        }
+        accS[g] = accD[g] = make_double2(0.0, 0.0);
+        hacc_s[warp][g][lane] = make_double2(0.0, 0.0);
     }
+    bool single = false;                    // the current run has m = 0: D = S
+    bool odd = false;                       // (recurrence mode) the current block is in (yc, ys)
 
     for (int st = 0; st < n_stages; ++st) {
-        __syncthreads();                                            // stage st-1 fully consumed (and barriers initialised)
-        if (tid == 0 && st + kRing - 1 < n_stages) {
-            const int s = st + kRing - 1, b = (gst + kRing - 1) % kRing;
-            mbar_expect_tx(&full[b], kStageBytes);
-            bulk_g2s(&ring[b][0], gsrc + (size_t)s * kStageD2, kStageBytes, &full[b]);
-        }
-        const int b = gst % kRing;
-        mbar_wait(&full[b], (gst / kRing) & 1u);
+        const unsigned slot = gst % kRing;
+        mbar_wait(&full[slot], (gst / kRing) & 1u);
         ++gst;
-        const double2* bp = &ring[b][0] + lane;
-        const int* hdr = reinterpret_cast<const int*>(&ring[b][0] + kStageSteps * kStepD2);
-        const int ns = hdr[0];
+        const double2* bp = &ring[slot][0] + lane;
+        const int* hdr = reinterpret_cast<const int*>(&ring[slot][0] + kStageSteps * kStepD2);
+        int4 d4 = *reinterpret_cast<const int4*>(hdr), d8 = kStageSteps > 4 ? *(reinterpret_cast<const int4*>(hdr) + 1) : make_int4(0, 0, 0, 0);
+        static_assert(kStageSteps == 4 || kStageSteps == 8, "descriptor registers hold 4 or 8 steps");
+        const int ns = hdr[kStageSteps];
         for (int si = 0; si < ns; ++si, bp += kStepD2) {
-            const int d = hdr[1 + si];
-            int adv = (d >> kAdvShift) & ((1 << kAdvBits) - 1);
-            if (d & kNewRun) {      // rare (once per (m, k)): close the previous run, new P, (c, s) restart from rho^col
+            const int d = d4.x;
+            d4.x = d4.y; d4.y = d4.z; d4.z = d4.w;
+            if (kStageSteps > 4) { d4.w = d8.x; d8.x = d8.y; d8.y = d8.z; d8.z = d8.w; }
+            const double2 b12c = bp[0], b12s = bp[32];              // issued first: in flight during the scalar work below
+            double2 av[G];                                          // table mode: (c, s) of this lane's unit, per group
+            if (kTab) {
+                const int ts = (d >> kSlotShift) & ((1 << kSlotBits) - 1);
+                static_assert(!kTab || G == 4, "the table instantiation is written for G = 4 (16 columns per slot)");
+                tmem_ld_x16(tmem_row + 16 * ts, av);
+            }
+            if (d & kNewRun) {      // rare (once per (m, k)): close the previous run, new P, (recurrence) x restarts from rho^col
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                    const int sx = 8 * g + row;
+                    const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
+                    double2 Hg = hacc_s[warp][g][lane];
+                    Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));              // H += P_r S + i P_i D
+                    Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
+                    hacc_s[warp][g][lane] = Hg;
+                    accS[g] = accD[g] = make_double2(0.0, 0.0);
+                    if (!kTab) {
+                        const double2 x0 = col ? rpow_s[warp][sx][col - 1] : make_double2(1.0, 0.0), xm = rpow_s[warp][sx][3 - col];
+                        xc[g % GR] = x0.x; xs[g % GR] = x0.y; yc[g % GR] = xm.x; ys[g % GR] = -xm.y;
+                    }
+                }
+                __syncwarp();                                       // every lane has read the old P
+                // new P = Z_phi^m Z_theta^k, ONE lane per sample: a scalar FP64 instruction costs the shared pipe ~5 cycles, so
+                // 4 instructions and an exchange through shared memory beat 16 instructions without one (measured)
                 const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                    H[g].x = fma(pr[g], accS[g].x, fma(-pi[g], accD[g].y, H[g].x));      // H += P_r S + i P_i D
-                    H[g].y = fma(pr[g], accS[g].y, fma(pi[g], accD[g].x, H[g].y));
-                    accS[g] = accD[g] = make_double2(0.0, 0.0);
-                    const int sx = sbase + 8 * g;
-                    const double2 zp = zphi_s[sx];
-                    double2 pm = kKerr ? kerr_s[T + sx] : make_double2(pr[g], pi[g]);
-                    for (int q = 0; q < dm; ++q) pm = cmul(pm, zp);
-                    if (kKerr) {                                    // P = Z_phi^m Z_theta^k (k < 0: conjugate powers)
-                        if (col == 0) kerr_s[T + sx] = pm;          // the 4 lanes of a row hold the same value
-                        const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
-                        double2 zt = kerr_s[sx];
-                        if (kk < 0) zt.y = -zt.y;
-                        for (int q = 0; q < (kk < 0 ? -kk : kk); ++q) pm = cmul(pm, zt);
+                for (int q = 0; q < QW; ++q) {
+                    const int sx = q * 32 + lane;
+                    if (sx < W) {
+                        const double2 zp = zphi_s[warp][sx];
+                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
+                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
+                        if (kKerr) {                                // k < 0: conjugate powers
+                            kerr_s[warp][1][sx] = pm;
+                            const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                            double2 zt = kerr_s[warp][0][sx];
+                            if (kk < 0) zt.y = -zt.y;
+                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
+                        }
+                        pcur_s[warp][sx] = pm;
                     }
-                    pr[g] = pm.x; pi[g] = pm.y;
-                    const double2 r0 = col ? rpow_s[sx][col - 1] : make_double2(1.0, 0.0);
-                    cs_c[g] = r0.x; cs_s[g] = r0.y;
                 }
-                if (kKerr) __syncwarp();
+                __syncwarp();
+                single = (d & kSingle) != 0;
+                odd = false;
             }
-            for (; adv > 0; --adv) {                                // usually once: nu -> nu + 4
+            if (!kTab) {
+                for (int adv = (d >> kAdvShift) & ((1 << kAdvBits) - 1); adv > 0; --adv) {   // usually once: block b -> b + 1, over block b - 1
+                    if (!odd) {
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                    const double m1 = cs_s[g] * z4i[g], m2 = cs_s[g] * z4r[g], e0 = cs_c[g];
-                    cs_c[g] = fma(e0, z4r[g], -m1);
-                    cs_s[g] = fma(e0, z4i[g], m2);
+                        for (int g = 0; g < GR; ++g) { yc[g] = fma(tw[g], xc[g], -yc[g]); ys[g] = fma(tw[g], xs[g], -ys[g]); }
+                    } else {
+#pragma unroll
+                        for (int g = 0; g < GR; ++g) { xc[g] = fma(tw[g], yc[g], -xc[g]); xs[g] = fma(tw[g], ys[g], -xs[g]); }
+                    }
+                    odd = !odd;
                 }
+#pragma unroll
+                for (int g = 0; g < G; ++g) av[g] = odd ? make_double2(yc[g % GR], ys[g % GR]) : make_double2(xc[g % GR], xs[g % GR]);
             }
-            const double2 b12c = bp[0], b12s = bp[32];
 #pragma unroll
-            for (int g = 0; g < G; ++g) dmma884(accS[g], cs_c[g], b12c.x);
+            for (int g = 0; g < G; ++g) dmma884(accS[g], av[g].x, b12c.x);
+            if (!single) {
 #pragma unroll
-            for (int g = 0; g < G; ++g) dmma884(accD[g], cs_c[g], b12c.y);
+                for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].x, b12c.y);
+            }
 #pragma unroll
-            for (int g = 0; g < G; ++g) dmma884(accS[g], cs_s[g], b12s.x);
+            for (int g = 0; g < G; ++g) dmma884(accS[g], av[g].y, b12s.x);
+            if (!single) {
 #pragma unroll
-            for (int g = 0; g < G; ++g) dmma884(accD[g], cs_s[g], b12s.y);
+                for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].y, b12s.y);
+            }
+        }
+        __syncwarp();                                               // every lane has read the slot
+        if (lane == 0) {                                            // (the slot's data has been consumed: the loads fed DMMAs)
+            if (atomicAdd(&done_s[slot], 1) == kWarps - 1) {        // the last of the 4 warps refills the slot
+                done_s[slot] = 0;
+                issue(i, st + kRing, cur, nxt, slot);
+            }
         }
     }
-    __syncthreads();                                                // every warp is done with rpow_s: reuse it for H
 #pragma unroll
     for (int g = 0; g < G; ++g) {                                   // close the last run; H_p of sample sx, power col -> shared
-        H[g].x = fma(pr[g], accS[g].x, fma(-pi[g], accD[g].y, H[g].x));
-        H[g].y = fma(pr[g], accS[g].y, fma(pi[g], accD[g].x, H[g].y));
-        rpow_s[sbase + 8 * g][col] = H[g];
+        const int sx = 8 * g + row;
+        const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
+        double2 Hg = hacc_s[warp][g][lane];
+        Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));
+        Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
+        rpow_s[warp][sx][col] = Hg;                                 // (rho^1..4 of this sample are not needed any more)
     }
-    __syncthreads();
+    __syncwarp();
 
-    // ---- h = H_0 + dx (H_1 + dx (H_2 + dx H_3)), one thread per sample; optionally the tile's share of the PSD = 1 inner
+    // ---- h = H_0 + dx (H_1 + dx (H_2 + dx H_3)), one lane per sample; optionally the warp's share of the PSD = 1 inner
     // products <d|h>, <h|h> so that a likelihood evaluation never writes h to HBM
     double s_re = 0.0, s_im = 0.0, s_hh = 0.0;
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        const int sx = q * kSumThreads + tid;
-        const long long i = i_begin + sx;
-        if (i < i_end) {
-            const double dx = __dsub_rn(sample_time(t0, dt, i), tk);
-            const double2 h0 = rpow_s[sx][0], h1 = rpow_s[sx][1], h2 = rpow_s[sx][2], h3 = rpow_s[sx][3];
+    for (int q = 0; q < QW; ++q) {
+        const int sx = q * 32 + lane;
+        if (sx < w_count) {
+            const long long is = w_begin + sx;
+            const double dx = __dsub_rn(sample_time(t0, dt, is), tk);
+            const double2 h0 = rpow_s[warp][sx][0], h1 = rpow_s[warp][sx][1], h2 = rpow_s[warp][sx][2], h3 = rpow_s[warp][sx][3];
             const double hr = fma(fma(fma(h3.x, dx, h2.x), dx, h1.x), dx, h0.x);
             const double hi = fma(fma(fma(h3.y, dx, h2.y), dx, h1.y), dx, h0.y);
-            if (h) __stcs(&h[i], make_double2(hr, hi));
+            if (h) __stcs(&h[is], make_double2(hr, hi));
             if (want_inner) {
                 if (dat) {
-                    const double2 dv = __ldcs(&dat[i]);
+                    const double2 dv = __ldcs(&dat[is]);
                     s_re = fma(dv.x, hr, fma(dv.y, hi, s_re));      // Re conj(d) h
                     s_im = fma(dv.x, hi, fma(-dv.y, hr, s_im));     // Im conj(d) h
                 }
@@ -634,26 +875,28 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             }
         }
     }
-    if (want_inner) {                   // fixed tree: lanes by butterfly, then the warps in order -> the same bits every run
+    if (want_inner) {                   // fixed butterfly over the lanes -> the same bits every run
 #pragma unroll
         for (int o = 16; o; o >>= 1) {
             s_re += __shfl_xor_sync(0xffffffffu, s_re, o);
             s_im += __shfl_xor_sync(0xffffffffu, s_im, o);
             s_hh += __shfl_xor_sync(0xffffffffu, s_hh, o);
         }
-        if ((tid & 31) == 0) { red_s[0][tid >> 5] = s_re; red_s[1][tid >> 5] = s_im; red_s[2][tid >> 5] = s_hh; }
-        __syncthreads();
-        if (tid < 3) {
-            double v = 0.0;
-#pragma unroll
-            for (int w = 0; w < kSumThreads / 32; ++w) v += red_s[tid][w];
-            partial[tid] = v;
-        }
+        if (lane == 0) { partial[0] = s_re; partial[1] = s_im; partial[2] = s_hh; }
     }
-    }   // persistent tile loop
+    __syncwarp();                       // the warp's shared arrays are rewritten by the next tile's setup
+    }   // tile with a summation
+    }   // tile exists
+    cur = nxt; nxt = nn;
+    }   // this block's tiles
+    if (kTab) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0) tmem_dealloc(sm.tmem_base, kTmemCols);
+    }
 }
 
-// inner[src] = 2 dt * (sum over the source's tiles of the per-tile partials): Eq. (16) with S_n = 1 by Parseval.  One block per
+// inner[src] = 2 dt * (sum over the source's tiles and their warps of the partials): Eq. (16) with S_n = 1 by Parseval.  One block per
 // source; thread q adds tiles q, q + 256, ... in order, then a fixed tree: deterministic.
 constexpr int kInnerThreads = 256;
 __global__ void __launch_bounds__(kInnerThreads)
@@ -662,9 +905,9 @@ few_sum_inner_kernel(sum_layout L, int n_t, int max_tiles, double dt, double* __
     __shared__ double red[3][kInnerThreads / 32];
     const int src = blockIdx.x, tid = threadIdx.x;
     const int n_tiles = L.tile_start[(size_t)src * (n_t + 2) + n_t + 1];
-    const double* P = L.partial + (size_t)src * max_tiles * 4;
+    const double* P = L.partial + (size_t)src * max_tiles * (kSumThreads / 32) * 4;
     double a = 0.0, b = 0.0, c = 0.0;
-    for (int q = tid; q < n_tiles; q += kInnerThreads) { a += P[4 * (size_t)q]; b += P[4 * (size_t)q + 1]; c += P[4 * (size_t)q + 2]; }
+    for (int q = tid; q < n_tiles * (kSumThreads / 32); q += kInnerThreads) { a += P[4 * (size_t)q]; b += P[4 * (size_t)q + 1]; c += P[4 * (size_t)q + 2]; }
     for (int o = 16; o; o >>= 1) {
         a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); c += __shfl_xor_sync(0xffffffffu, c, o);
     }
@@ -725,6 +968,7 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
     sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
 
+    FEW_CUDA_CHECK(cudaMemsetAsync(L.mode_count, 0, 2 * sizeof(int), st));
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
     few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
@@ -737,11 +981,24 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     FEW_LAUNCHED(ctx);
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
-    const long long want = max_tiles * n_src, resident = (long long)ctx->sm_count * kSumBlocksPerSm;
-    const unsigned grid = (unsigned)(want < resident ? want : resident);
+    // both instantiations are launched: the table one (2 blocks per SM, ~101 KB of shared memory each) takes the sources whose
+    // lists fit its table, the recurrence one (4 blocks per SM) the others; an instantiation with no source returns at once
+    const long long want = max_tiles * n_src;
 #define FEW_SUM_LAUNCH(INNER, KERR, DPTR)                                                                                         \
-    few_sum_kernel<kSumG, kSumBlocksPerSm, INNER, KERR><<<grid, kSumThreads, 0, st>>>(                                            \
-        t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, DPTR)
+    do {                                                                                                                          \
+        auto ktab = few_sum_kernel<kSumG, kSumTabBlocksPerSm, INNER, KERR, true>;                                                 \
+        auto krec = few_sum_kernel<kSumG, kSumBlocksPerSm, INNER, KERR, false>;                                                   \
+        const size_t smem_tab = sum_smem_bytes<kSumG, KERR, true>(), smem_rec = sum_smem_bytes<kSumG, KERR, false>();             \
+        FEW_REQUIRE(smem_tab <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "sum kernel's shared memory exceeds the device limit");   \
+        FEW_CUDA_CHECK(cudaFuncSetAttribute(ktab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tab));                   \
+        FEW_CUDA_CHECK(cudaFuncSetAttribute(krec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rec));                   \
+        const long long res_tab = (long long)ctx->sm_count * kSumTabBlocksPerSm, res_rec = (long long)ctx->sm_count * kSumBlocksPerSm; \
+        ktab<<<(unsigned)(want < res_tab ? want : res_tab), kSumThreads, smem_tab, st>>>(                                         \
+            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, DPTR);                    \
+        FEW_LAUNCHED(ctx);                                                                                                        \
+        krec<<<(unsigned)(want < res_rec ? want : res_rec), kSumThreads, smem_rec, st>>>(                                         \
+            t, (const dd*)coef_phase_dd, t0, dt, n_samples, n_t, n_src, (int)max_tiles, L, (double2*)h, DPTR);                    \
+    } while (0)
     if (n_phase == 3) {
         if (inner) FEW_SUM_LAUNCH(true, true, (const double2*)d);
         else FEW_SUM_LAUNCH(false, true, nullptr);
