@@ -69,12 +69,13 @@ constexpr int kTabSlots = 8;                  // distinct blocks nu >> 2 a sourc
 // count, pseudo-segment p (-1: no tile; 0 or n_t: outside the trajectory, h = 0), the source, and the number of coefficient
 // stages the tile consumes (0 for tiles without a summation), and the source's mode (1 table, 0 recurrence: which of the two
 // instantiations of the sum kernel takes the tile).
-struct __align__(16) tile_rec { long long i_begin; int count; int p; int n_stages; int src; int mode; int pad1; };
+struct __align__(16) tile_rec { long long i_begin; int count; int p; int n_stages; int src; int mode; int pad1; };   // n_stages, mode: filled by load_rec from src_info
 
 struct sum_layout {
     long long* bounds;   // [n_src][n_t + 2]   pseudo-segment p covers samples [bounds[p], bounds[p+1])
     int* tile_start;     // [n_src][n_t + 2]   exclusive prefix of tiles per pseudo-segment; last = total
     int* n_steps;        // [n_src]            number of steps
+    int2* src_info;      // [n_src]            (coefficient stages per tile, mode: 1 table / 0 recurrence) of the source
     int* blk_list;       // [n_src][8]         table mode: the distinct blocks nu >> 2 of the source, ascending (slot -> block), -1 = unused
     int* mode_count;     // [2]                sources in recurrence mode [0] / table mode [1] (zeroed before the plan kernel)
     tile_rec* tiles;     // [n_src][max_tiles] what the plan kernel hands every tile, so that a warp finds its work with one record
@@ -109,6 +110,7 @@ sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samp
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
     L.n_steps = c.take<int>(n_src);
+    L.src_info = c.take<int2>(n_src);
     L.blk_list = c.take<int>((size_t)n_src * kTabSlots);
     L.mode_count = c.take<int>(2);
     const long long mt = sum_max_tiles(n_samples, n_t);
@@ -205,7 +207,9 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
 
     const int src = blockIdx.x, tid = threadIdx.x;
     const double* t = t_all + (size_t)src * n_t;
-
+    // Two blocks per source work side by side: blockIdx.y == 1 lays out the tiles (a), (e) -- that needs the time grids only --
+    // and blockIdx.y == 0 orders the kept modes and cuts them into steps (b)-(d).
+    if (blockIdx.y == 1) {
     // ---- (a) sample ranges of the pseudo-segments and their tile prefix
     long long* B = L.bounds + (size_t)src * (n_t + 2);
     int* TS = L.tile_start + (size_t)src * (n_t + 2);
@@ -214,9 +218,6 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         if (k <= n_t - 2) B[k + 1] = first_index(t[k], t0, dt, N, false);
         else { B[n_t] = first_index(t[n_t - 1], t0, dt, N, true); B[n_t + 1] = N; B[0] = 0; }
     }
-    int* ulo = L.u_lo + (size_t)src * L.cap * 8;
-    int* uhi = L.u_hi + (size_t)src * L.cap * 8;
-    for (int q = tid; q < L.cap * 8; q += kPlanThreads) { ulo[q] = 0; uhi[q] = 0; }      // empty (step, nu & 3, sign) slots
     __syncthreads();
     if (tid < 32) {           // warp 0: prefix over n_t + 1 pseudo-segments, 32 at a time
         int carry = 0;
@@ -231,7 +232,33 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         }
         if (tid == 0) TS[n_t + 1] = carry;
     }
+    __syncthreads();
+    // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1])
+    {
+        tile_rec* rec = L.tiles + (size_t)src * L.max_tiles;
+        for (int p = tid >> 5; p <= n_t; p += kPlanThreads / 32) {           // a warp per pseudo-segment
+            const int q0 = TS[p], q1 = TS[p + 1];
+            const long long b0 = B[p], b1 = B[p + 1];
+            for (int q = q0 + (tid & 31); q < q1; q += 32) {
+                tile_rec r;
+                r.i_begin = b0 + (long long)(q - q0) * kTile;
+                const long long left = b1 - r.i_begin;
+                r.count = (int)(left < kTile ? left : kTile);
+                r.p = p; r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
+                rec[q] = r;
+            }
+        }
+        for (int q = TS[n_t + 1] + tid; q < L.max_tiles; q += kPlanThreads) {
+            tile_rec r; r.i_begin = 0; r.count = 0; r.p = -1; r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
+            rec[q] = r;
+        }
+    }
+    return;
+    }   // blockIdx.y == 1
 
+    int* ulo = L.u_lo + (size_t)src * L.cap * 8;
+    int* uhi = L.u_hi + (size_t)src * L.cap * 8;
+    for (int q = tid; q < L.cap * 8; q += kPlanThreads) { ulo[q] = 0; uhi[q] = 0; }      // empty (step, nu & 3, sign) slots
     // ---- (b) kept modes -> keys
     const int K = n_keep ? min(max(n_keep[src], 0), n_modes) : n_modes;
     int n_pow2 = 1;
@@ -363,36 +390,14 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         int S = carry_s;
         if (S > L.cap) { atomicOr(status, FEW_DEV_SPARSE_LIST); S = L.cap; }
         L.n_steps[src] = S;
-        carry_s = S;
-    }
-    __syncthreads();
-    // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1])
-    {
-        const int n_stages = stages_for(carry_s);
-        tile_rec* rec = L.tiles + (size_t)src * L.max_tiles;
-        for (int p = tid >> 5; p <= n_t; p += kPlanThreads / 32) {           // a warp per pseudo-segment
-            const int q0 = TS[p], q1 = TS[p + 1];
-            const long long b0 = B[p], b1 = B[p + 1];
-            for (int q = q0 + (tid & 31); q < q1; q += 32) {
-                tile_rec r;
-                r.i_begin = b0 + (long long)(q - q0) * kTile;
-                const long long left = b1 - r.i_begin;
-                r.count = (int)(left < kTile ? left : kTile);
-                r.p = p; r.n_stages = (p == 0 || p == n_t) ? 0 : n_stages; r.src = src; r.mode = mode_s; r.pad1 = 0;
-                rec[q] = r;
-            }
-        }
-        for (int q = TS[n_t + 1] + tid; q < L.max_tiles; q += kPlanThreads) {
-            tile_rec r; r.i_begin = 0; r.count = 0; r.p = -1; r.n_stages = 0; r.src = src; r.mode = mode_s; r.pad1 = 0;
-            rec[q] = r;
-        }
+        L.src_info[src] = make_int2(stages_for(S), mode_s);
     }
 }
 
 // The four B matrices of every step, in DMMA.8x8x4 fragment order, written as the stage stream the sum kernel consumes.
 // Lane L of a warp supplies B[k = L & 3][o = L >> 2]: unit k of the step (nu = 4 blk + k), output o = 2 p + part (power p of
 // dx, part 0 = re, 1 = im).  A step is 1 KB: [0][L] = (B1c, B2c), [1][L] = (B1s, B2s) as double2 (conflict-free LDS.128).
-__global__ void few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_t, int n_modes, sum_layout L)
+__global__ void __launch_bounds__(1024) few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_t, int n_modes, sum_layout L)
 {
     const int seg = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
     const int S = L.n_steps[src];
@@ -538,12 +543,15 @@ __device__ __forceinline__ void tmem_ld_x16(unsigned taddr, double2 (&v)[4])
     for (int g = 0; g < 4; ++g) v[g] = make_double2(__hiloint2double(r[4 * g + 1], r[4 * g]), __hiloint2double(r[4 * g + 3], r[4 * g + 2]));
 }
 
-__device__ __forceinline__ tile_rec load_rec(const tile_rec* p)
+__device__ __forceinline__ tile_rec load_rec(const tile_rec* p, const int2* __restrict__ src_info, int n_t)
 {
     const int4 a = __ldg(reinterpret_cast<const int4*>(p)), b = __ldg(reinterpret_cast<const int4*>(p) + 1);
     tile_rec r;
     r.i_begin = ((long long)(unsigned)a.y << 32) | (unsigned)a.x; r.count = a.z; r.p = a.w;
-    r.n_stages = b.x; r.src = b.y; r.mode = b.z; r.pad1 = 0;
+    r.src = b.y; r.pad1 = 0;
+    const int2 info = __ldg(src_info + r.src);          // per source: stages per tile, mode (a cached load)
+    r.n_stages = (r.p <= 0 || r.p == n_t) ? 0 : info.x;
+    r.mode = info.y;
     return r;
 }
 
@@ -608,7 +616,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             ++j;
             const long long tg = blockIdx.x + j * stride;
             if (tg >= total_tiles) return;                          // the stream has ended
-            ri = (j == i + 1) ? rn : load_rec(L.tiles + tg);
+            ri = (j == i + 1) ? rn : load_rec(L.tiles + tg, L.src_info, n_t);
         }
         const double2* src = pack + ((size_t)ri.src * n_seg + (ri.p - 1)) * L.max_stages * kStageD2 + (size_t)s * kStageD2;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the warps' reads of the slot precede the copy's writes
@@ -622,8 +630,8 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     tile_rec cur, nxt;
     cur.p = -1; cur.n_stages = 0; cur.count = 0; cur.i_begin = 0; cur.src = 0; cur.mode = 0; cur.pad1 = 0;
     nxt = cur;
-    if ((long long)blockIdx.x < total_tiles) cur = load_rec(L.tiles + blockIdx.x);
-    if (blockIdx.x + stride < total_tiles) nxt = load_rec(L.tiles + blockIdx.x + stride);
+    if ((long long)blockIdx.x < total_tiles) cur = load_rec(L.tiles + blockIdx.x, L.src_info, n_t);
+    if (blockIdx.x + stride < total_tiles) nxt = load_rec(L.tiles + blockIdx.x + stride, L.src_info, n_t);
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kRing; ++s) { mbar_init(&full[s], 1); done_s[s] = 0; }
@@ -645,7 +653,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (tg >= total_tiles) break;
     tile_rec nn = cur;                      // record of tile i + 2: loaded now, needed at the end of this tile
     nn.p = -1; nn.n_stages = 0; nn.count = 0;
-    if (tg + 2 * stride < total_tiles) nn = load_rec(L.tiles + tg + 2 * stride);
+    if (tg + 2 * stride < total_tiles) nn = load_rec(L.tiles + tg + 2 * stride, L.src_info, n_t);
     if (cur.p >= 0 && cur.mode == (kTab ? 1 : 0)) {
     const int src = cur.src, p = cur.p;
     const long long w_begin = cur.i_begin + warp * W;               // this warp's samples: [w_begin, w_begin + w_count)
@@ -970,7 +978,7 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
 
     FEW_CUDA_CHECK(cudaMemsetAsync(L.mode_count, 0, 2 * sizeof(int), st));
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-    few_sum_plan_kernel<<<n_src, kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
+    few_sum_plan_kernel<<<dim3(n_src, 2), kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
                                                           n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_LAUNCHED(ctx);
