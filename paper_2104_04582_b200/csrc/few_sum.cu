@@ -769,7 +769,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             if (kStageSteps > 4) { d4.w = d8.x; d8.x = d8.y; d8.y = d8.z; d8.z = d8.w; }
             const double2 b12c = bp[0], b12s = bp[32];              // issued first: in flight during the scalar work below
             double2 av[G];                                          // table mode: (c, s) of this lane's unit, per group
-            if (kTab) {
+            if constexpr (kTab) {
                 const int ts = (d >> kSlotShift) & ((1 << kSlotBits) - 1);
                 static_assert(!kTab || G == 4, "the table instantiation is written for G = 4 (16 columns per slot)");
                 tmem_ld_x16(tmem_row + 16 * ts, av);

@@ -361,6 +361,73 @@ def test_many_l_per_pair_and_n_gaps(api):
     assert nk[0] == len(l) and rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
 
 
+def wide_n_problem(seed, n_values, n_src=1, n_samples=900):
+    """A mode list whose radial indices spread over many blocks of four: l = 2..4, m = 0..2, n in n_values."""
+    rng = np.random.default_rng(seed)
+    modes = [(l, m, n) for l in (2, 3, 4) for m in range(0, 3) for n in n_values]
+    l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
+    n_t = 12
+    t = np.stack([np.sort(rng.uniform(0, 700.0, n_t)) for _ in range(n_src)]); t[:, 0] = 0.0
+    amp = (rng.normal(size=(n_src, n_t, len(l))) + 1j * rng.normal(size=(n_src, n_t, len(l)))) * 10.0 ** rng.uniform(-2, 0, (n_src, 1, len(l)))
+    phase = np.stack([0.31 * t + 2e-4 * t ** 2, 0.17 * t + 1e-4 * t ** 2], axis=2)
+    return synth.Workload("wide_n", t, phase, amp, l, m, n, rng.uniform(0.3, 2.8, n_src), rng.uniform(0, 6.28, n_src), 1.5, 0.71, n_samples, 0.0)
+
+
+def test_sum_recurrence_instantiation_more_than_8_nu_blocks(api):
+    """Lists with more than 8 distinct blocks |n| >> 2 do not fit the tensor-memory table of the summation kernel and take its
+    recurrence instantiation (rho^nu stepped in registers); 11 blocks here, with gaps, both signs and |n| up to 43."""
+    w = wide_n_problem(11, [-43, -40, -33, -21, -12, -9, -2, 0, 1, 6, 14, 19, 25, 30, 36])
+    assert len({abs(int(x)) // 4 for x in w.n}) > 8
+    h, keep, nk = run_gpu_chain(api, w)
+    ref = oracle.waveform(w)
+    assert nk[0] == w.n_modes and rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
+    assert np.max(np.abs(h[0] - ref[0])) <= 1e-10 * np.max(np.abs(ref[0]))
+
+
+def test_sum_batch_mixing_table_and_recurrence_sources(api):
+    """One call, two kinds of kept lists: sources whose selection leaves <= 8 nu-blocks (table instantiation) and sources
+    that keep a list with 12 (recurrence instantiation); each kernel takes its own tiles of the shared tile list."""
+    w = wide_n_problem(12, list(range(-46, 47, 4)) + [1, 2, 3], n_src=4, n_samples=700)
+    g = gpu_inputs(w)
+    yp, ym = api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"])
+    ca = api.few_spline_fit(g["t"], g["amp"]); cp = api.few_spline_fit_dd(g["t"], g["phase"])
+    narrow = np.flatnonzero(np.abs(w.n) <= 14).astype(np.int32)          # 4 blocks -> table mode
+    keep = np.full((w.n_src, w.n_modes), -1, np.int32); nk = np.zeros(w.n_src, np.int32)
+    for s in range(w.n_src):
+        sel = narrow if s % 2 == 0 else np.arange(w.n_modes, dtype=np.int32)
+        keep[s, : len(sel)] = sel; nk[s] = len(sel)
+    h = api.few_sum_waveform(g["t"], ca, cp, g["l"], g["m"], g["n"], dev(keep), dev(nk), yp, ym, w.t0, w.dt, w.n_samples).cpu().numpy()
+    api.few_device_status()
+    for s in range(w.n_src):
+        ref = oracle_with_gpu_keep(w, s, keep[s][: nk[s]], [(0, w.n_samples)])[0]
+        assert rel_l2(h[s], ref) <= REL_L2_TOL and mismatch(h[s], ref) <= MISMATCH_TOL, s
+
+
+def test_sum_large_n_and_sparse_list_limit(api):
+    """|n| up to FEW_MAX_ABS_N = 1023 (256 steps of the three-term recurrence: error <= 256^2 ulp) is summed; a list with
+    fewer than 4 modes per step and more than 64 steps over n_modes / 4 does not fit the step capacity and is reported."""
+    rng = np.random.default_rng(5)
+    modes = [(2, 2, n) for n in (0, 1, 250, -640, 1023, -1023)] + [(3, 1, 512)]
+    l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
+    n_t = 8
+    t = np.linspace(0.0, 64.0, n_t)
+    amp = rng.normal(size=(1, n_t, len(l))) + 1j * rng.normal(size=(1, n_t, len(l)))
+    phase = np.stack([0.05 * t + 1e-4 * t ** 2, 0.011 * t + 3e-5 * t ** 2], axis=1)[None]
+    w = synth.Workload("large_n", t[None], phase, amp, l, m, n, np.array([0.9]), np.array([2.0]), 0.0, 0.05, 1200, 0.0)
+    h, keep, nk = run_gpu_chain(api, w)
+    ref = oracle.waveform(w)
+    assert rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
+    # 400 modes, every one alone in its step (n = 4 j): 400 steps > 400 / 4 + 64
+    modes = [(2, 0, 4 * j) for j in range(200)] + [(2, 1, 4 * j) for j in range(200)]
+    l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
+    amp = rng.normal(size=(1, n_t, len(l))) + 1j * rng.normal(size=(1, n_t, len(l)))
+    w2 = synth.Workload("sparse", t[None], phase, amp, l, m, n, np.array([0.9]), np.array([2.0]), 0.0, 0.05, 64, 0.0)
+    g = gpu_inputs(w2)
+    api.few_waveform(g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], 0.0, w2.t0, w2.dt, w2.n_samples)
+    assert api.few_device_status(raise_on_error=False) == -7            # FEW_ERR_LIMIT (FEW_DEV_SPARSE_LIST)
+    assert api.few_device_status(raise_on_error=False) == 0
+
+
 @pytest.mark.parametrize("pinned_out", [True, False])
 def test_whole_path_host_buffers(api, pinned_out):
     """few_waveform_host: pinned h is written by the summation kernel itself (mapped stores), pageable h by a copy."""
