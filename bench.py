@@ -143,11 +143,18 @@ def oracle_sample(w, target_s: float, threads: int | None = None, max_samples: i
 
 
 def kept_structure(w, keep_h, nk_h):
-    """(kept modes, (m, n) pairs) summed over the sources: bookkeeping for the roofline (the kernel sums all l of an (m, n) pair
-    into one pair of splines before the sample loop)."""
+    """Bookkeeping for the roofline, summed over the sources: kept modes; (m, n) pairs (all l of a pair are summed into one
+    pair of splines before the sample loop); STEPS of the summation kernel = kept (m, |n| >> 2) blocks (one step = 4 DMMA.8x8x4
+    per 8 samples, 2 when m = 0: DESIGN.md section 5) as (steps, steps with m = 0)."""
     K = int(nk_h.sum())
-    pairs = sum(len({(int(w.m[j]), int(w.n[j])) for j in keep_h[s, : nk_h[s]]}) for s in range(w.n_src))
-    return K, pairs
+    pairs = steps = single = 0
+    for s in range(w.n_src):
+        kept = keep_h[s, : nk_h[s]]
+        pairs += len({(int(w.m[j]), int(w.n[j])) for j in kept})
+        blocks = {(int(w.m[j]), abs(int(w.n[j])) >> 2) for j in kept}
+        steps += len(blocks)
+        single += sum(1 for (mm, _) in blocks if mm == 0)
+    return K, pairs, steps, single
 
 
 class Bench:
@@ -172,7 +179,7 @@ class Bench:
         for _ in range(n):
             flush.fill_(1); self.step()
         self.api.few_device_status()
-        self.K, self.pairs = kept_structure(self.w, self.keep.cpu().numpy(), self.nk.cpu().numpy())
+        self.K, self.pairs, self.steps, self.single = kept_structure(self.w, self.keep.cpu().numpy(), self.nk.cpu().numpy())
 
     def timed(self, steps, flush, barrier=None):
         """steps timed steps, L2 flushed before each (outside the event pair), CUDA events on the launch stream; the library's
@@ -210,11 +217,17 @@ class Bench:
         return sec, int(h2d), int(h_host.numel() * 16)
 
 
-def sum_kernel_roofline(w, pairs, kernel_ms, sm_max_mhz):
-    """FP64 ALU roofline of few_sum_kernel: executed flops of the formulation / time, against the nominal pipe."""
+def sum_kernel_roofline(w, pairs, kernel_ms, sm_max_mhz, steps=None, single=0):
+    """FP64 ALU roofline of the summation kernel.  achieved = ALGORITHMIC flops / time: 38 flop per sample and kept (m, n) pair
+    (the work of the pair formulation, a property of the kept list, not of the kernel: DESIGN.md section 5), against the nominal
+    FP64 pipe.  With `steps` also what the kernel's DMMAs execute, padding included: a step is 4 DMMA.8x8x4 per 8 samples (2 when
+    m = 0), 512 flop each, i.e. 256 (128) flop per sample and step."""
     peak = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     achieved = float(w.n_samples) * pairs * FLOP_PER_PAIR / (kernel_ms * 1e-3) / 1e12
-    return achieved, peak
+    if steps is None:
+        return achieved, peak
+    dmma = float(w.n_samples) * (256.0 * (steps - single) + 128.0 * single) / (kernel_ms * 1e-3) / 1e12
+    return achieved, peak, dmma
 
 
 def time_stages(api, torch, w, g, flush, reps: int = 10):
@@ -428,9 +441,10 @@ def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
         b.warm(warm, flush)
         step_ms, sum_ms, launches = b.timed(steps, flush)
         kms = float(np.mean(sum_ms))
-        ach, peak = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz)
-        r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "steps": steps,
+        ach, peak, dmma = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz, b.steps, b.single)
+        r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "kernel_steps": b.steps, "steps": steps,
              "ms_per_step": float(np.mean(step_ms)), "kernel_ms": kms, "tflops": ach, "frac": ach / peak,
+             "dmma_tflops_executed": dmma, "dmma_share_of_pipe": dmma / peak,
              "evals_per_s": float(w.n_samples) * b.K / (float(np.mean(step_ms)) * 1e-3), "gpu_launches_per_step": launches / steps}
         return b, r
 
@@ -502,7 +516,7 @@ def main():
         torch.cuda.synchronize()
 
     bench.warm(args.warmup, flush)
-    K_kept, pairs = bench.K, bench.pairs
+    K_kept, pairs, bench_steps, bench_single = bench.K, bench.pairs, bench.steps, bench.single
     evals_per_step = float(w.n_samples) * K_kept
 
     # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
@@ -564,16 +578,20 @@ def main():
         return 0
 
     sum_ms_avg = float(np.mean(sum_ms))
-    achieved_tflops, peak_tflops = sum_kernel_roofline(w, pairs, sum_ms_avg, sm_max_mhz)
+    achieved_tflops, peak_tflops, dmma_tflops = sum_kernel_roofline(w, pairs, sum_ms_avg, sm_max_mhz, bench_steps, bench_single)
     nominal_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
     traffic = SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if (args.eps is None and world == 1) else None
-    roofline = {"bound": "alu", "kernel": "few_sum_kernel", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "few_sum_kernel (table instantiation; the recurrence instantiation is launched too and returns at once unless a source needs it)", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops, "traffic": traffic,
                 "traffic_source": SUM_KERNEL_DRAM_TRAFFIC_SOURCE if traffic is not None else None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / float(np.mean(step_ms)),
-                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (18 DFMA + 2 DMUL) per sample*(m,n)-pair x {float(w.n_samples) * pairs:.4g} "
+                "executed_dmma": {"tflops": dmma_tflops, "share_of_pipe": dmma_tflops / peak_tflops, "kernel_steps": bench_steps,
+                                  "steps_m0": bench_single,
+                                  "note": "what the kernel's DMMA.8x8x4 execute, zero padding included: 256 flop per sample and step "
+                                          "(128 for m = 0); the rest of the pipe's time goes to scalar FP64 (phases, rho^nu table, run closes)"},
+                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (the (m,n)-pair formulation: 2 complex cubic Horners + complex rotation + 4 FMA) per sample*(m,n)-pair x {float(w.n_samples) * pairs:.4g} "
                                f"pair evaluations per launch on this rank ({pairs} pairs from {K_kept} kept modes)",
                 "nominal_per_mode": {"achieved": nominal_tflops, "frac": nominal_tflops / peak_tflops,
                                      "note": "20 flop per sample*mode evaluation (per-mode formulation); exceeds the executed "

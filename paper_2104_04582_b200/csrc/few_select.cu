@@ -87,44 +87,65 @@ __device__ __forceinline__ int block_scan_int(int v, int* warp_sums, int* total)
     return res;
 }
 
-// Mirror list (modes with m > 0 in ascending j), |Y|^2 per entry, bitmap cleared.  One block per source.
+// Mirror list (modes with m > 0 in ascending j), |Y|^2 per entry, bitmap cleared.  One block per source.  The mirror index of a
+// mode is the number of m > 0 modes before it: warp ballots per 1024-mode chunk, ONE scan of the (chunk, warp) counts, then
+// popc of the lanes below -- two block barriers in all, whatever n_modes (the 42 273-mode grid took 42 block scans before).
+constexpr int kPrepChunks = FEW_MAX_SELECT_MODES / kPrepThreads;
 __global__ void __launch_bounds__(kPrepThreads)
 few_select_prepare_kernel(const int* __restrict__ m, const double2* __restrict__ ylm_plus, const double2* __restrict__ ylm_minus,
                           int n_modes, sel_layout L, int* status)
 {
-    __shared__ int warp_sums[32];
-    __shared__ int carry_s;
-    const int src = blockIdx.x, tid = threadIdx.x;
-    if (tid == 0) carry_s = 0;
-    __syncthreads();
+    __shared__ int wcnt[kPrepChunks * 32];       // m > 0 modes per (chunk, warp), then their exclusive prefix
+    __shared__ int total_s;
+    const int src = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const bool with_y = ylm_plus != nullptr;
-    double* y2 = L.y2 + (size_t)src * 2 * n_modes;
-    for (int base = 0; base < n_modes; base += kPrepThreads) {
-        int j = base + tid;
-        int mj = j < n_modes ? m[j] : 0;
+    const int n_chunks = (n_modes + kPrepThreads - 1) / kPrepThreads;
+#pragma unroll 4
+    for (int c = 0; c < n_chunks; ++c) {                 // (unrolled: the loads of several chunks in flight)
+        const int j = c * kPrepThreads + tid;
+        const int mj = j < n_modes ? m[j] : 0;
         if (j < n_modes && mj < 0) atomicOr(status, FEW_DEV_BAD_MODE);
-        int flag = (with_y && j < n_modes && mj > 0) ? 1 : 0, total;
-        int incl = block_scan_int<kPrepThreads>(flag, warp_sums, &total);
-        int carry = carry_s;
+        const unsigned b = __ballot_sync(0xffffffffu, with_y && j < n_modes && mj > 0);
+        if (lane == 0) wcnt[c * 32 + wid] = __popc(b);
+    }
+    __syncthreads();
+    if (wid == 0) {                              // warp 0: exclusive scan of the n_chunks * 32 counts, 32 at a time
+        int carry = 0;
+        for (int base = 0; base < n_chunks * 32; base += 32) {
+            const int v = wcnt[base + lane];
+            int incl = v;
+            for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += u; }
+            wcnt[base + lane] = carry + incl - v;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        if (lane == 0) total_s = carry;
+    }
+    __syncthreads();
+    double* y2 = L.y2 + (size_t)src * 2 * n_modes;
+#pragma unroll 4
+    for (int c = 0; c < n_chunks; ++c) {
+        const int j = c * kPrepThreads + tid;
+        const int mj = j < n_modes ? m[j] : 0;
+        const bool flag = with_y && j < n_modes && mj > 0;
+        const unsigned b = __ballot_sync(0xffffffffu, flag);
         if (j < n_modes) {
-            double2 yp = with_y ? ylm_plus[(size_t)src * n_modes + j] : make_double2(1.0, 0.0);
+            const double2 yp = with_y ? ylm_plus[(size_t)src * n_modes + j] : make_double2(1.0, 0.0);
             y2[j] = __dadd_rn(__dmul_rn(yp.x, yp.x), __dmul_rn(yp.y, yp.y));
             double w_m = 0.0;
+            int me = -1;
             if (flag) {
-                int e = carry + incl - 1;
+                const int e = wcnt[c * 32 + wid] + __popc(b & ((1u << lane) - 1u));
+                me = n_modes + e;
                 if (src == 0) L.owner[e] = j;
-                double2 ym = ylm_minus[(size_t)src * n_modes + j];
+                const double2 ym = ylm_minus[(size_t)src * n_modes + j];
                 w_m = __dadd_rn(__dmul_rn(ym.x, ym.x), __dmul_rn(ym.y, ym.y));
                 y2[n_modes + e] = w_m;
             }
-            if (src == 0) L.mirror_e[j] = flag ? n_modes + carry + incl - 1 : -1;
+            if (src == 0) L.mirror_e[j] = me;
             L.y2m[(size_t)src * n_modes + j] = w_m;
         }
-        __syncthreads();
-        if (tid == 0) carry_s = carry + total;
-        __syncthreads();
     }
-    if (src == 0 && tid == 0) { *L.n_entries = n_modes + carry_s; *L.fb_count = 0; }
+    if (src == 0 && tid == 0) { *L.n_entries = n_modes + total_s; *L.fb_count = 0; }
     for (int w = tid; w < sel_words(n_modes); w += kPrepThreads) L.bitmap[(size_t)src * sel_words(n_modes) + w] = 0u;
 }
 
@@ -325,9 +346,24 @@ __device__ __forceinline__ void select_core(const Entries& E, double thr, int b_
 // row: ~10 passes of 676 KB) and the rows the fast kernel leaves in fb_list (flat spectra, degenerate thresholds); with
 // fb_list == NULL the grid is (n_t, n_src) and every row is done here.
 constexpr int kStreamThreads = 1024;
-constexpr int kStreamBucket = 2048;
+constexpr int kStreamBucket = 1024;
 constexpr int kStreamWords = FEW_MAX_SELECT_MODES / 32;
-using stream_shared = sel_shared<kStreamThreads, kStreamBucket, kStreamWords>;
+constexpr int kStreamCand = 14336;     // candidates (power >= tau) of a long row that the kernel keeps in shared memory (168 KB)
+struct stream_shared : sel_shared<kStreamThreads, kStreamBucket, kStreamWords> {
+    long long cand_k[kStreamCand];
+    int cand_e[kStreamCand];
+    int warp_sums[32];
+};
+
+// Entries policy 3: the candidates of a long row, compacted into shared memory (keys and entry indices).
+template <int T>
+struct smem_entries {
+    const long long* k; const int* e; int n;
+    template <class F> __device__ __forceinline__ void for_each(F f) const
+    {
+        for (int q = threadIdx.x; q < n; q += T) f(k[q], e[q], (q / T) & 3);
+    }
+};
 
 __global__ void __launch_bounds__(kStreamThreads)
 few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L,
@@ -342,8 +378,10 @@ few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_mod
     for (int q = fb_list ? blockIdx.x : 0; q < n_rows; q += gridDim.x) {
         const int row = fb_list ? fb_list[q] : blockIdx.y * n_t + blockIdx.x;
         const int src = row / n_t, k = row - src * n_t;
-        stream_entries<kStreamThreads> E{amp + ((size_t)src * n_t + k) * n_modes, L.y2 + (size_t)src * 2 * n_modes,
-                                         L.y2m + (size_t)src * n_modes, L.mirror_e, n_modes};
+        const double2* a = amp + ((size_t)src * n_t + k) * n_modes;
+        const double* y2p = L.y2 + (size_t)src * 2 * n_modes;
+        const double* y2m = L.y2m + (size_t)src * n_modes;
+        stream_entries<kStreamThreads> E{a, y2p, y2m, L.mirror_e, n_modes};
         __syncthreads();                                 // the previous row's shared state is no longer read
         for (int w = tid; w < words; w += kStreamThreads) S.bitmap[w] = 0u;
         if (tid == 0) S.bkt_count = 0;
@@ -351,10 +389,51 @@ few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_mod
         double t2[2] = {0.0, 0.0};
         E.for_each([&](long long key, int, int c) { t2[c] += __longlong_as_double(key); });
         const double total = block_sum((t2[0] + t2[1]) + (0.0 + 0.0), S.red, slot);      // the same tree as the core's g(0)
+        const double thr = (1.0 - eps) * total;
         // buckets below that of tau = eps total / (4 n) hold less than eps total / 4 altogether: the search starts there
         const long long tau_key = __double_as_longlong(0.25 * eps * total / (double)n_ent);
         const int b_lo = (eps > 1e-10 && tau_key > 0) ? (int)(tau_key >> kBucketShift) : 0;
-        select_core(E, (1.0 - eps) * total, b_lo, (int)(__double_as_longlong(total) >> kBucketShift), n_modes, L.owner, S, slot);
+        const int b_hi = (int)(__double_as_longlong(total) >> kBucketShift);
+        // Second (and normally last) pass over the row: the entries below tau are certainly dropped (the fast kernel's argument),
+        // the others -- a few thousand of a Kerr-shaped row's 78 507 -- are compacted, in a fixed order, into shared memory and
+        // selected there; before, every step of the search streamed the whole row from L2 again (~13 passes).
+        bool done = false;
+        if (thr > 0.0 && tau_key > 0 && eps > 1e-10) {
+            int n_cand = 0;
+            for (int base = 0; base < n_modes; base += kStreamThreads) {
+                const int j = base + tid;
+                long long kp = -1, km = -1;
+                int me = -1;
+                if (j < n_modes) {
+                    const double2 v = a[j];
+                    const double a2 = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
+                    kp = __double_as_longlong(__dmul_rn(a2, y2p[j]));
+                    me = L.mirror_e[j];
+                    if (me >= 0) km = __double_as_longlong(__dmul_rn(a2, y2m[j]));
+                }
+                const int cnt = (kp >= tau_key ? 1 : 0) + (km >= tau_key ? 1 : 0);
+                int tot;
+                const int incl = block_scan_int<kStreamThreads>(cnt, S.warp_sums, &tot);
+                int pos = n_cand + incl - cnt;
+                if (kp >= tau_key) { if (pos < kStreamCand) { S.cand_k[pos] = kp; S.cand_e[pos] = j; } ++pos; }
+                if (km >= tau_key) { if (pos < kStreamCand) { S.cand_k[pos] = km; S.cand_e[pos] = me; } }
+                n_cand += tot;                           // block-uniform
+            }
+            __syncthreads();
+            if (n_cand <= kStreamCand) {
+                smem_entries<kStreamThreads> C{S.cand_k, S.cand_e, n_cand};
+                double tc = 0.0;
+                C.for_each([&](long long key, int, int) { tc += __longlong_as_double(key); });
+                const double total_cand = block_sum(tc, S.red, slot);
+                if (total_cand < thr) {                  // every candidate has C_{r-1} < thr: all kept
+                    C.for_each([&](long long, int e, int) { const int j = e < n_modes ? e : L.owner[e - n_modes]; atomicOr(&S.bitmap[j >> 5], 1u << (j & 31)); });
+                } else {
+                    select_core(C, thr, b_lo, b_hi, n_modes, L.owner, S, slot);
+                }
+                done = true;
+            }
+        }
+        if (!done) select_core(E, thr, b_lo, b_hi, n_modes, L.owner, S, slot);
         __syncthreads();
         unsigned* gb = L.bitmap + (size_t)src * words;
         for (int w = tid; w < words; w += kStreamThreads)
@@ -460,12 +539,12 @@ few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes
         if (S.bitmap[w]) atomicOr(&gb[w], S.bitmap[w]);
 }
 
-// bitmap -> ascending keep_idx (padded with -1) and n_keep.  One block per source.  keep_all: identity list.
+// bitmap -> ascending keep_idx (padded with -1) and n_keep.  One block per source.  keep_all: identity list.  A thread takes
+// whole bitmap words (popc), one block scan per 1024 words (32 768 modes), then writes its word's set bits in order.
 __global__ void __launch_bounds__(kPrepThreads)
 few_select_compact_kernel(sel_layout L, int n_modes, int keep_all, int* __restrict__ keep_idx, int* __restrict__ n_keep)
 {
     __shared__ int warp_sums[32];
-    __shared__ int carry_s;
     const int src = blockIdx.x, tid = threadIdx.x;
     int* out = keep_idx + (size_t)src * n_modes;
     if (keep_all) {
@@ -473,22 +552,21 @@ few_select_compact_kernel(sel_layout L, int n_modes, int keep_all, int* __restri
         if (tid == 0) n_keep[src] = n_modes;
         return;
     }
-    const unsigned* gb = L.bitmap + (size_t)src * sel_words(n_modes);
-    if (tid == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < n_modes; base += kPrepThreads) {
-        int j = base + tid;
-        int flag = (j < n_modes && ((gb[j >> 5] >> (j & 31)) & 1u)) ? 1 : 0, total;
-        int incl = block_scan_int<kPrepThreads>(flag, warp_sums, &total);
-        int carry = carry_s;
-        if (flag) out[carry + incl - 1] = j;
-        __syncthreads();
-        if (tid == 0) carry_s = carry + total;
-        __syncthreads();
+    const int words = sel_words(n_modes);
+    const unsigned* gb = L.bitmap + (size_t)src * words;
+    int carry = 0;                               // block-uniform
+    for (int base = 0; base < words; base += kPrepThreads) {
+        const int w = base + tid;
+        unsigned bits = w < words ? gb[w] : 0u;
+        if (w == words - 1 && (n_modes & 31)) bits &= (1u << (n_modes & 31)) - 1u;
+        int total;
+        const int cnt = __popc(bits);
+        int pos = carry + block_scan_int<kPrepThreads>(cnt, warp_sums, &total) - cnt;
+        while (bits) { const int b = __ffs(bits) - 1; bits &= bits - 1; out[pos++] = w * 32 + b; }
+        carry += total;
     }
-    const int cnt = carry_s;
-    for (int j = cnt + tid; j < n_modes; j += kPrepThreads) out[j] = -1;
-    if (tid == 0) n_keep[src] = cnt;
+    for (int j = carry + tid; j < n_modes; j += kPrepThreads) out[j] = -1;
+    if (tid == 0) n_keep[src] = carry;
 }
 
 }  // namespace

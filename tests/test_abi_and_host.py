@@ -115,6 +115,22 @@ s0, sc = shard_sources(wb.n_src, rank, world)
 mine = synth.Workload(wb.name, wb.t[s0:s0+sc], wb.phase[s0:s0+sc], wb.amp[s0:s0+sc], wb.l, wb.m, wb.n, wb.theta[s0:s0+sc], wb.phi[s0:s0+sc], wb.t0, wb.dt, wb.n_samples, wb.eps)
 hb = oracle.waveform(mine)
 assert np.array_equal(hb, oracle.waveform(wb)[s0:s0+sc])
+# (d) the split bench.py --gpus N runs on the GPU path (bench.shard_workload: config 3 by source, config 4 by time range), with
+# the oracle standing in for few_waveform: the ranks' pieces reassemble to the unsharded result bit for bit
+import bench
+w3 = synth.random_problem(9, n_src=7, n_modes=5, n_samples=96)
+mine = bench.shard_workload(w3, 3, rank, world)
+s0, sc = shard_sources(w3.n_src, rank, world)
+assert mine.n_src == sc and np.array_equal(mine.t, w3.t[s0:s0+sc]) and mine.n_samples == w3.n_samples
+assert np.array_equal(oracle.waveform(mine), oracle.waveform(w3)[s0:s0+sc])
+w4 = synth.make_config(0)
+mine = bench.shard_workload(w4, 4, rank, world)
+i0, cnt = shard_samples(w4.n_samples, rank, world)
+assert mine.n_samples == cnt and mine.t0 == w4.t0 + i0 * w4.dt and mine.n_src == 1
+assert np.array_equal(oracle.waveform(mine)[0], oracle.waveform(w4)[0][i0:i0+cnt])
+assert bench.shard_workload(w4, 1, rank, world) is w4                     # configs 1, 2: replicas
+lab3, sc3 = bench.parallelism_label(w3, 3, world); lab4, sc4 = bench.parallelism_label(w4, 4, world)
+assert sc3 == sc4 == "strong" and "by source" in lab3 and "time range" in lab4
 # (c) bench-style timing reduction: max over ranks
 tmax = torch.tensor([float(rank + 1)]); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
 assert tmax.item() == 2.0

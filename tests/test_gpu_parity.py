@@ -478,6 +478,35 @@ def test_full_size_sampled_parity(api, cfg):
     assert rel_l2(h[0][idx], one) <= REL_L2_TOL
 
 
+def test_sharded_calls_reassemble_bit_equal(api):
+    """The property the multi-GPU split relies on: a waveform computed as two contiguous sample ranges
+    (each call repeating S0-S2-S1 and passing t0 + i0 dt), and a batch computed as two source ranges, concatenate BIT-EQUAL to
+    the unsharded call -- every sample's arithmetic depends on its own t_i only, whatever tile, warp or lane it lands in."""
+    from paper_2104_04582_b200.shard import shard_samples, shard_sources, shard_t0
+    w = synth.make_config(1)
+    h, keep, nk = run_gpu_chain(api, w)
+    parts = []
+    for rank in range(2):
+        i0, cnt = shard_samples(w.n_samples, rank, 2)
+        ws = synth.Workload(w.name, w.t, w.phase, w.amp, w.l, w.m, w.n, w.theta, w.phi, shard_t0(w.t0, w.dt, i0), w.dt, cnt, w.eps)
+        hs, ks, ns = run_gpu_chain(api, ws)
+        assert np.array_equal(ks, keep) and np.array_equal(ns, nk)
+        parts.append(hs[0])
+    assert np.array_equal(np.concatenate(parts), h[0])
+    # an odd split point (not a multiple of the tile) gives the same bits too
+    i0 = 1_234_567
+    wa = synth.Workload(w.name, w.t, w.phase, w.amp, w.l, w.m, w.n, w.theta, w.phi, w.t0, w.dt, i0, w.eps)
+    wb = synth.Workload(w.name, w.t, w.phase, w.amp, w.l, w.m, w.n, w.theta, w.phi, shard_t0(w.t0, w.dt, i0), w.dt, w.n_samples - i0, w.eps)
+    assert np.array_equal(np.concatenate([run_gpu_chain(api, wa)[0][0], run_gpu_chain(api, wb)[0][0]]), h[0])
+    wb3 = synth.make_config(3, n_src=9, n_samples=5_000, t0=3_000_000.0)
+    h3, _, _ = run_gpu_chain(api, wb3)
+    for rank in range(2):
+        s0, sc = shard_sources(wb3.n_src, rank, 2)
+        wr = synth.Workload(wb3.name, wb3.t[s0:s0 + sc], wb3.phase[s0:s0 + sc], wb3.amp[s0:s0 + sc], wb3.l, wb3.m, wb3.n, wb3.theta[s0:s0 + sc],
+                            wb3.phi[s0:s0 + sc], wb3.t0, wb3.dt, wb3.n_samples, wb3.eps)
+        assert np.array_equal(run_gpu_chain(api, wr)[0], h3[s0:s0 + sc])
+
+
 def knot_windows(w, s, knots, n_win):
     """Sample windows of n_win samples centred on the first dense sample at or after the given sparse knots of source s."""
     out = []
