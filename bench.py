@@ -417,6 +417,43 @@ def parallelism_label(w, config: int, world: int):
     return f"{world} independent replicas (one waveform per GPU, an MCMC's walkers), no collective", "weak"
 
 
+PROBES_SRC = os.path.join(ROOT, "bench_probes.cu")
+PROBES_SO = os.path.join(ROOT, "bench_probes.so")
+
+
+def build_probes(force: bool = False) -> str:
+    """nvcc -> bench_probes.so next to bench.py (measurement aids only; libfew_b200 does not contain them)."""
+    if force or not os.path.exists(PROBES_SO) or os.path.getmtime(PROBES_SO) < os.path.getmtime(PROBES_SRC):
+        tmp = PROBES_SO + f".tmp{os.getpid()}"
+        subprocess.check_call(["nvcc", "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+                               "-shared", PROBES_SRC, "-o", tmp])
+        os.replace(tmp, PROBES_SO)
+    return PROBES_SO
+
+
+def run_probes():
+    """`--probes`: the FP64-pipe facts the summation kernel is designed around, one JSON line.
+    DMMA.8x8x4 holds the pipe of a sub-partition 16 cycles; `share` = 256 * warps cycles / measured cycles per iteration."""
+    import ctypes
+    lib = ctypes.CDLL(build_probes())
+    lib.probe_dmma_mix.argtypes = [ctypes.c_int] * 5 + [ctypes.POINTER(ctypes.c_float)]
+    _, sm_max_mhz, _ = load_peaks()
+    iters, out = 4000, []
+    cases = [(1, 0, 0), (2, 0, 0), (4, 0, 0), (3, 0, 1), (3, 0, 2), (1, 0, 2)] + [(4, c, 0) for c in (2, 4, 8, 16, 32)]
+    for warps, chain, mode in cases:
+        ms = ctypes.c_float(0.0)
+        rc = lib.probe_dmma_mix(148, warps, iters, chain, mode, ctypes.byref(ms))
+        assert rc == 0, rc
+        cyc = ms.value * 1e-3 * sm_max_mhz * 1e6 / iters
+        out.append({"dmma_warps_per_scheduler": warps, "dependent_dfma_between_batches": chain,
+                    "other_warps": ["idle", "one dependent DFMA chain", "8 independent DFMA chains"][mode],
+                    "cycles_per_iteration": cyc, "dmma_share_of_pipe": 256.0 * warps / cyc,
+                    "extra_cycles_per_scalar_instruction": (cyc - 256.0 * warps) / (warps * chain) if chain else None})
+    print(json.dumps({"probes": "DMMA.8x8x4 batches of 16 per warp (256 pipe cycles), 4 warps per scheduler = 512-thread blocks, 148 blocks",
+                      "sm_mhz_assumed": sm_max_mhz, "results": out}), flush=True)
+    return 0
+
+
 def shard_workload(w, config: int, rank: int, world: int):
     """The rank's share of the workload.  No data-path collective."""
     from paper_2104_04582_b200 import synth
@@ -481,12 +518,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the short runs of configs 2, 3, 4 that the default run appends")
+    ap.add_argument("--probes", action="store_true", help="run the FP64-pipe probes of bench_probes.cu and print their JSON line")
     ap.add_argument("--eps", type=float, default=None)
     ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows: detector frame, fused inner products, direct sum")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
+    if args.probes:
+        return run_probes()
     args.warmup = max(args.warmup, 3)
 
     import torch

@@ -454,22 +454,34 @@ __device__ __forceinline__ dd dd_add_fast(dd a, dd b)            // error O(eps^
     return quick_two_sum(s.hi, s.lo);
 }
 
-// (not inlined: called two or three times per sample and tile; the sum kernel's code must stay small enough for the
-// instruction caches -- the kernel ran a fifth slower when its per-tile code was 28 KB)
-__device__ __noinline__ void phase_factor(const dd* __restrict__ c, int stride, double dx, double* zr, double* zi)
+// All NP phase factors of a sample at once, z[p] = exp(-i Phi_p(dx)), c = [4][NP] dd coefficients: the NP evaluations are
+// independent dependent-chains, written side by side so that they overlap (a lone chain of ~70 scalar FP64 instructions
+// between other warps' DMMAs costs the pipe 4-9 cycles per instruction, profiles/r02_fp64_pipe_probes.md).  Not inlined: the
+// sum kernel's code must stay small enough for the instruction caches (it ran a fifth slower with 28 KB of per-tile code).
+template <int NP>
+__device__ __noinline__ void phase_factors(const dd* __restrict__ c, double dx, double2* __restrict__ z)
 {
-    dd r = dd_add_d(c[2 * stride], __dmul_rn(c[3 * stride].hi, dx));
-    r = dd_add_fast(dd_mul_d(r, dx), c[stride]);
-    r = dd_add_fast(dd_mul_d(r, dx), c[0]);
+    dd r[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r[p] = dd_add_d(c[2 * NP + p], __dmul_rn(c[3 * NP + p].hi, dx));
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r[p] = dd_add_fast(dd_mul_d(r[p], dx), c[NP + p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r[p] = dd_add_fast(dd_mul_d(r[p], dx), c[p]);
     const double p1 = 0x1.921fb54000000p+2, p2 = 0x1.10b4611800000p-28, p3 = 0x1.313198a2e0370p-59;   // 2 pi = p1 + p2 + p3
-    const double kk = rint(r.hi * 1.591549430918953456e-01);
-    double q = fma(-kk, p1, r.hi);            // exact
-    q = fma(-kk, p2, q);
-    const double ql = fma(-kk, p3, r.lo);
-    double s, co;
-    sincos(q, &s, &co);
-    *zr = fma(-ql, s, co);                    // cos(q + ql)
-    *zi = -fma(ql, co, s);                    // -sin(q + ql)
+    double q[NP], ql[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const double kk = rint(r[p].hi * 1.591549430918953456e-01);
+        q[p] = fma(-kk, p2, fma(-kk, p1, r[p].hi));       // the inner fma is exact
+        ql[p] = fma(-kk, p3, r[p].lo);
+    }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        double s, co;
+        sincos(q[p], &s, &co);
+        z[p] = make_double2(fma(-ql[p], s, co), -fma(ql[p], co, s));     // cos(q + ql), -sin(q + ql)
+    }
 }
 
 // ---- mbarrier / TMA bulk copy (1-D cp.async.bulk global -> shared, completion counted in bytes on an mbarrier)
@@ -683,15 +695,14 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             const long long i_last = cur.i_begin + cur.count - 1;
             if (is > i_last) is = i_last;                           // tail samples recompute the last one, never stored
             const double dx = __dsub_rn(sample_time(t0, dt, is), tk);
-            double2 zp, r1;
-            phase_factor(cph + 0, n_ph, dx, &zp.x, &zp.y);
-            phase_factor(cph + n_ph - 1, n_ph, dx, &r1.x, &r1.y);
+            double2 zf[n_ph];
+            phase_factors<n_ph>(cph, dx, zf);
+            const double2 zp = zf[0], r1 = zf[n_ph - 1];
             zphi_s[warp][sx] = zp;
             pcur_s[warp][sx] = make_double2(1.0, 0.0);
             const double2 r2 = cmul(r1, r1), r3 = cmul(r2, r1), r4 = cmul(r2, r2);
             if (kKerr) {
-                double2 zt;
-                phase_factor(cph + 1, n_ph, dx, &zt.x, &zt.y);
+                const double2 zt = zf[n_ph > 2 ? 1 : 0];
                 kerr_s[warp][0][sx] = zt;
                 kerr_s[warp][1][sx] = make_double2(1.0, 0.0);
             }
