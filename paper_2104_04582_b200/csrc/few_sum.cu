@@ -763,6 +763,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         hacc_s[warp][g][lane] = make_double2(0.0, 0.0);
     }
     bool single = false;                    // the current run has m = 0: D = S
+    int new_run_d = 0;                      // descriptor of a run whose P is still to be computed (0: none)
     bool odd = false;                       // (recurrence mode) the current block is in (yc, ys)
 
     for (int st = 0; st < n_stages; ++st) {
@@ -800,28 +801,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                         xc[g % GR] = x0.x; xs[g % GR] = x0.y; yc[g % GR] = xm.x; ys[g % GR] = -xm.y;
                     }
                 }
-                __syncwarp();                                       // every lane has read the old P
-                // new P = Z_phi^m Z_theta^k, ONE lane per sample: a scalar FP64 instruction costs the shared pipe ~5 cycles, so
-                // 4 instructions and an exchange through shared memory beat 16 instructions without one (measured)
-                const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
-#pragma unroll
-                for (int q = 0; q < QW; ++q) {
-                    const int sx = q * 32 + lane;
-                    if (sx < W) {
-                        const double2 zp = zphi_s[warp][sx];
-                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
-                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
-                        if (kKerr) {                                // k < 0: conjugate powers
-                            kerr_s[warp][1][sx] = pm;
-                            const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
-                            double2 zt = kerr_s[warp][0][sx];
-                            if (kk < 0) zt.y = -zt.y;
-                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
-                        }
-                        pcur_s[warp][sx] = pm;
-                    }
-                }
-                __syncwarp();
+                new_run_d = d;                                      // the new P is computed after this step's DMMAs are issued
                 single = (d & kSingle) != 0;
                 odd = false;
             }
@@ -850,6 +830,34 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             if (!single) {
 #pragma unroll
                 for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].y, b12s.y);
+            }
+            if (new_run_d) {
+                // new P = Z_phi^m Z_theta^k of the run that has just started (its close, one run later, is the first reader): after
+                // the step's DMMAs, so that the exchange through shared memory runs beside them instead of in front of them.
+                // ONE lane per sample: scalar FP64 instructions are dear next to DMMAs, and 4 of them plus two warp barriers
+                // beat 16 without (measured).
+                const int dn = new_run_d;
+                new_run_d = 0;
+                const int dm = (dn >> kDmShift) & ((1 << kDmBits) - 1);
+                __syncwarp();                                       // every lane has read the old P (the close above)
+#pragma unroll
+                for (int q = 0; q < QW; ++q) {
+                    const int sx = q * 32 + lane;
+                    if (sx < W) {
+                        const double2 zp = zphi_s[warp][sx];
+                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
+                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
+                        if (kKerr) {                                // k < 0: conjugate powers
+                            kerr_s[warp][1][sx] = pm;
+                            const int kk = ((dn >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                            double2 zt = kerr_s[warp][0][sx];
+                            if (kk < 0) zt.y = -zt.y;
+                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
+                        }
+                        pcur_s[warp][sx] = pm;
+                    }
+                }
+                __syncwarp();
             }
         }
         __syncwarp();                                               // every lane has read the slot
