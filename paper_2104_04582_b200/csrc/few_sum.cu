@@ -207,9 +207,9 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
 
     const int src = blockIdx.x, tid = threadIdx.x;
     const double* t = t_all + (size_t)src * n_t;
-    // Two blocks per source work side by side: blockIdx.y == 1 lays out the tiles (a), (e) -- that needs the time grids only --
+    // Blocks of a source work side by side: blockIdx.y >= 1 lay out the tiles (a), (e) -- that needs the time grids only --
     // and blockIdx.y == 0 orders the kept modes and cuts them into steps (b)-(d).
-    if (blockIdx.y == 1) {
+    if (blockIdx.y >= 1) {
     // ---- (a) sample ranges of the pseudo-segments and their tile prefix
     long long* B = L.bounds + (size_t)src * (n_t + 2);
     int* TS = L.tile_start + (size_t)src * (n_t + 2);
@@ -233,28 +233,32 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
         if (tid == 0) TS[n_t + 1] = carry;
     }
     __syncthreads();
-    // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1])
+    // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1]).
+    // The gridDim.y - 1 tile blocks of a source each recompute (a) (cheap; they write the same B, TS) and share the records:
+    // a thread takes tiles q, q + stride, ... and finds p by binary search (24.6 k records from one block took 36 us)
     {
         tile_rec* rec = L.tiles + (size_t)src * L.max_tiles;
-        for (int p = tid >> 5; p <= n_t; p += kPlanThreads / 32) {           // a warp per pseudo-segment
-            const int q0 = TS[p], q1 = TS[p + 1];
-            const long long b0 = B[p], b1 = B[p + 1];
-            for (int q = q0 + (tid & 31); q < q1; q += 32) {
-                tile_rec r;
-                r.i_begin = b0 + (long long)(q - q0) * kTile;
+        const int n_tiles = TS[n_t + 1];
+        const int tb = gridDim.y - 1, ry = blockIdx.y - 1;
+        for (int q = ry * kPlanThreads + tid; q < L.max_tiles; q += tb * kPlanThreads) {
+            tile_rec r;
+            r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
+            if (q < n_tiles) {
+                int lo = 0, hi = n_t + 1;                        // largest p with TS[p] <= q
+                while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (TS[mid] <= q) lo = mid; else hi = mid; }
+                const long long b0 = B[lo], b1 = B[lo + 1];
+                r.i_begin = b0 + (long long)(q - TS[lo]) * kTile;
                 const long long left = b1 - r.i_begin;
                 r.count = (int)(left < kTile ? left : kTile);
-                r.p = p; r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
-                rec[q] = r;
+                r.p = lo;
+            } else {
+                r.i_begin = 0; r.count = 0; r.p = -1;
             }
-        }
-        for (int q = TS[n_t + 1] + tid; q < L.max_tiles; q += kPlanThreads) {
-            tile_rec r; r.i_begin = 0; r.count = 0; r.p = -1; r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
             rec[q] = r;
         }
     }
     return;
-    }   // blockIdx.y == 1
+    }   // blockIdx.y >= 1
 
     int* ulo = L.u_lo + (size_t)src * L.cap * 8;
     int* uhi = L.u_hi + (size_t)src * L.cap * 8;
@@ -283,7 +287,34 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     for (int q = K + tid; q < n_pow2; q += kPlanThreads) plan_sorted[q] = ~0ull;      // padding sorts to the end
     __syncthreads();
     // ---- (c) bitonic sort (keys are unique for a valid mode list; duplicates order by mode index)
-    if (in_smem) {
+    if (n_pow2 <= kPlanThreads && smem_elems >= 2 * kPlanThreads) {
+        // up to 1024 keys (every list of the Schwarzschild grid after selection): one element per thread; compare-exchange
+        // partners less than a warp apart are reached by shuffles, the others through shared memory, double-buffered: 15 block
+        // barriers instead of 55
+        unsigned long long v = tid < n_pow2 ? plan_sorted[tid] : ~0ull;
+        __syncthreads();
+        unsigned long long* xbuf = plan_smem;                      // [2][kPlanThreads]
+        int pp = 0;
+        for (int size = 2; size <= kPlanThreads; size <<= 1) {
+            for (int stride = size >> 1; stride > 0; stride >>= 1) {
+                unsigned long long o;
+                if (stride >= 32) {
+                    xbuf[pp * kPlanThreads + tid] = v;
+                    __syncthreads();
+                    o = xbuf[pp * kPlanThreads + (tid ^ stride)];
+                    pp ^= 1;
+                } else {
+                    o = __shfl_xor_sync(0xffffffffu, v, stride);
+                }
+                const bool up = (tid & size) == 0, lower = (tid & stride) == 0;
+                const bool take_min = lower == up;
+                v = (take_min == (o < v)) ? o : v;
+            }
+        }
+        __syncthreads();
+        if (tid < n_pow2) plan_sorted[tid] = v;
+        __syncthreads();
+    } else if (in_smem) {
         plan_bitonic_steps(plan_sorted, 0, n_pow2, 2, n_pow2);
     } else {
         const int CH = smem_elems;
@@ -995,9 +1026,10 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
     sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
 
+    const int plan_tile_blocks = n_src >= 64 ? 1 : (64 / n_src < 8 ? 64 / n_src : 8);     // tile blocks per source: 8 for one waveform
     FEW_CUDA_CHECK(cudaMemsetAsync(L.mode_count, 0, 2 * sizeof(int), st));
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-    few_sum_plan_kernel<<<dim3(n_src, 2), kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
+    few_sum_plan_kernel<<<dim3(n_src, 1 + plan_tile_blocks), kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
                                                           n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_LAUNCHED(ctx);
