@@ -31,8 +31,9 @@
  *     lives on the device (t increasing, (l,m,n) validity) is checked by the kernels, which OR a FEW_DEV_* bit into a
  *     device status word read back by few_device_status().  Outputs are unspecified when a bit is set.
  *   - Layouts are C-contiguous with the LAST index fastest.  Complex numbers are (re, im) pairs of doubles.
- *   - n_t, n_samples, t0, dt are uniform across a batch (true for every workload of the paper); sources differ in
- *     t, amplitudes, phases, angles and kept modes.
+ *   - n_samples, t0, dt are uniform across a batch; sources differ in t, amplitudes, phases, angles and kept modes.  n_t is
+ *     uniform in the plain entry points (true for every benchmark workload of the paper); the *_ragged entry points take each
+ *     source's own knot count in padded arrays (adaptive trajectories), see "Ragged batches" below.
  *   - There is no CPU fallback: without a CUDA device few_create fails with FEW_ERR_CUDA.
  */
 #ifndef FEW_H
@@ -49,7 +50,7 @@ extern "C" {
 enum {
     FEW_OK = 0,
     FEW_ERR_INVALID_ARG = -1,     /* NULL pointer, non-positive size, bad flag */
-    FEW_ERR_TOO_FEW_POINTS = -2,  /* n_t < 4: a not-a-knot cubic spline needs 4 knots */
+    FEW_ERR_TOO_FEW_POINTS = -2,  /* n_t < 4: a not-a-knot cubic spline needs 4 knots; ragged: n_t_src[s] outside [4, n_t] (few_device_status) */
     FEW_ERR_NOT_INCREASING = -3,  /* t not strictly increasing (reported by few_device_status) */
     FEW_ERR_BAD_MODE = -4,        /* l < 2, |m| > l, m < 0, |n| > FEW_MAX_ABS_N, |k| > FEW_MAX_ABS_K, l > FEW_MAX_L (few_device_status / few_ylm) */
     FEW_ERR_WORKSPACE = -5,       /* workspace NULL, misaligned or smaller than the query says */
@@ -58,7 +59,7 @@ enum {
 };
 
 /* bits of the device status word */
-enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_SPARSE_LIST = 4 };
+enum { FEW_DEV_NOT_INCREASING = 1, FEW_DEV_BAD_MODE = 2, FEW_DEV_SPARSE_LIST = 4, FEW_DEV_BAD_COUNT = 8 };
 
 #define FEW_MAX_L 16            /* l <= 16: the explicit Wigner-d sum in FP64 is accurate to 5e-15 for l <= 10 (the paper's range) and 1e-12 at l = 16 */
 #define FEW_MAX_ABS_N 1023      /* |n| <= 1023: rho^n is stepped by a three-term recurrence whose error after b = |n| / 4 steps is <= b^2 ulp */
@@ -76,7 +77,7 @@ const char* few_last_error(void);
 int few_version(void);
 
 /* Synchronises `stream`, returns FEW_OK or the FEW_ERR_* of the lowest FEW_DEV_* bit set by kernels since the last
- * call, and clears the word.  Optional `bits_out` (host) receives the raw bits. */
+ * call (FEW_DEV_BAD_COUNT first: a wrong knot count makes the kernels read padding, which sets other bits too), and clears the word.  Optional `bits_out` (host) receives the raw bits. */
 int few_device_status(few_ctx* ctx, int* bits_out, void* stream);
 
 /* ---- S0: spin-weighted spherical harmonics, s = -2 (Goldberg et al. convention, R11).
@@ -219,6 +220,39 @@ int few_waveform_ssb(few_ctx* ctx, const double* t, const double* phase, const d
                      double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
                      double* h, const double* d, double* inner, int* keep_idx, int* n_keep,
                      void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- Ragged batches: every source with its own number of sparse points.  The trajectory module steps adaptively ("~100"
+ * points) and stops where the inspiral ends, so the sources of a batch of parameter draws differ in
+ * length and end time.  All arrays keep the PADDED layouts documented above, with n_t = the largest count of the batch (the row
+ * stride); n_t_src[n_src] int32 (device; host for few_waveform_host_ragged) is source s's count, 4 <= n_t_src[s] <= n_t -- a
+ * count outside that range sets FEW_DEV_BAD_COUNT (few_device_status: FEW_ERR_TOO_FEW_POINTS), outputs then unspecified but
+ * in bounds.  For source s only rows k < n_t_src[s] of t, y, amp, phase are read (the padding may hold anything, NaN included);
+ * the fits write coefficient rows k < n_t_src[s] - 1 and leave the others untouched; selection takes the union over the steps
+ * k < n_t_src[s]; the summation gives h = 0 after t[s][n_t_src[s] - 1], which is how sources end at different samples inside the
+ * uniform n_samples.  n_t_src == NULL is the uniform call.  Workspace queries are the uniform ones with the padded n_t.
+ * Otherwise each function is its namesake: few_spline_fit, few_spline_fit_dd, few_select_modes, few_sum_waveform_kerr (the most
+ * general summation: n_phase = 2, k = NULL, factor = d = inner = NULL give few_sum_waveform), few_waveform, few_waveform_host. */
+int few_spline_fit_ragged(few_ctx* ctx, const double* t, const double* y, const int* n_t_src, int n_src, int n_t, int n_sys,
+                          double* coef, void* workspace, size_t workspace_bytes, void* stream);
+int few_spline_fit_dd_ragged(few_ctx* ctx, const double* t, const double* y, const int* n_t_src, int n_src, int n_t, int n_sys,
+                             double* coef_dd, void* stream);
+int few_select_modes_ragged(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
+                            const int* n_t_src, double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,
+                            void* workspace, size_t workspace_bytes, void* stream);
+int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int* n_t_src, const double* coef_amp, const double* coef_phase_dd,
+                            int n_phase, const int* l, const int* m, const int* k, const int* n, const int* keep_idx,
+                            const int* n_keep, const double* ylm_plus, const double* ylm_minus, const double* scale,
+                            const double* factor, double t0, double dt, long long n_samples, double* h, const double* d,
+                            double* inner, int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
+int few_waveform_ragged(few_ctx* ctx, const double* t, const int* n_t_src, const double* phase, const double* amp,
+                        const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
+                        double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                        double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream);
+int few_waveform_host_ragged(few_ctx* ctx, const double* t_host, const int* n_t_src_host, const double* phase_host,
+                             const double* amp_host, const int* l_host, const int* m_host, const int* n_host,
+                             const double* theta_host, const double* phi_host, const double* scale_host, double eps, double t0,
+                             double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                             double* h_host, int* keep_idx_host, int* n_keep_host);
 
 /* ---- Whole path on HOST buffers (same shapes, all pointers host; pinned memory recommended): copies inputs host->device
  * into a device arena the context keeps between calls (grow-only, released by few_destroy), runs few_waveform and delivers h

@@ -22,7 +22,8 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_launch_count", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
            "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
-           "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr"]
+           "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr", "few_spline_fit_ragged", "few_spline_fit_dd_ragged",
+           "few_select_modes_ragged", "few_sum_waveform_ragged", "few_waveform_ragged", "few_waveform_host_ragged"]
 
 
 class FewError(RuntimeError):
@@ -60,6 +61,12 @@ def _load() -> C.CDLL:
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
         "few_sum_waveform_ex": (i, [vp] * 13 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
         "few_sum_waveform_kerr": (i, [vp, vp, vp, vp, i] + [vp] * 10 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
+        "few_spline_fit_ragged": (i, [vp, vp, vp, vp, i, i, i, vp, vp, sz, vp]),
+        "few_spline_fit_dd_ragged": (i, [vp, vp, vp, vp, i, i, i, vp, vp]),
+        "few_select_modes_ragged": (i, [vp, vp, vp, vp, vp, vp, d, i, i, i, vp, vp, vp, sz, vp]),
+        "few_sum_waveform_ragged": (i, [vp, vp, vp, vp, vp, i] + [vp] * 10 + [d, d, ll, vp, vp, vp, i, i, i, vp, sz, vp]),
+        "few_waveform_ragged": (i, [vp] * 11 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
+        "few_waveform_host_ragged": (i, [vp] * 11 + [d, d, d, ll, i, i, i, vp, vp, vp]),
         "few_frame_constants": (i, [vp, vp, vp, i, vp, vp, vp, vp]),
         "few_frame_rotate": (i, [vp, vp, vp, i, ll, vp, vp]),
         "few_inner_products_workspace": (sz, [i, ll]),
@@ -346,6 +353,87 @@ def few_waveform_host(t, phase, amp, l, m, n, theta, phi, eps: float, t0: float,
                                 _hp(phi, torch.float64), _hp(scale, torch.float64), float(eps), float(t0), float(dt), int(n_samples),
                                 n_src, n_t, n_modes, _hp(h, torch.complex128), _hp(keep_idx, torch.int32), _hp(n_keep, torch.int32)),
          "few_waveform_host")
+    return h
+
+
+# ---- ragged batches (few.h "Ragged batches"): padded arrays with n_t = the largest knot count, n_t_src [n_src] i32 per source
+
+def few_spline_fit_ragged(t, y, n_t_src, out=None, workspace=None):
+    """few_spline_fit on padded t [n_src, n_t], y [n_src, n_t, n_sys]; rows k >= n_t_src[s] - 1 of coef are left untouched."""
+    if y.dtype == torch.complex128:
+        y = torch.view_as_real(y).reshape(y.shape[0], y.shape[1], -1)
+    n_src, n_t, n_sys = y.shape
+    coef = out if out is not None else torch.zeros((n_src, max(n_t - 1, 0), 4, n_sys), dtype=torch.float64, device=y.device)
+    ws = workspace if workspace is not None else _ws(_lib.few_spline_fit_workspace(n_src, n_t), y.device)
+    _chk(_lib.few_spline_fit_ragged(context(), _p(t, torch.float64), _p(y, torch.float64), _p(n_t_src, torch.int32), n_src, n_t, n_sys,
+                                    _p(coef, torch.float64), _p(ws), ws.numel(), _stream()), "few_spline_fit_ragged")
+    return coef
+
+
+def few_spline_fit_dd_ragged(t, y, n_t_src, out=None):
+    n_src, n_t, n_sys = y.shape
+    coef = out if out is not None else torch.zeros((n_src, max(n_t - 1, 0), 4, n_sys, 2), dtype=torch.float64, device=y.device)
+    _chk(_lib.few_spline_fit_dd_ragged(context(), _p(t, torch.float64), _p(y, torch.float64), _p(n_t_src, torch.int32), n_src, n_t, n_sys,
+                                       _p(coef, torch.float64), _stream()), "few_spline_fit_dd_ragged")
+    return coef
+
+
+def few_select_modes_ragged(amp, m, ylm_plus, ylm_minus, n_t_src, eps: float, workspace=None, keep_idx=None, n_keep=None):
+    n_src, n_t, n_modes = amp.shape
+    keep = keep_idx if keep_idx is not None else torch.empty((n_src, n_modes), dtype=torch.int32, device=amp.device)
+    nk = n_keep if n_keep is not None else torch.empty((n_src,), dtype=torch.int32, device=amp.device)
+    ws = workspace if workspace is not None else _ws(_lib.few_select_modes_workspace(n_src, n_t, n_modes), amp.device)
+    _chk(_lib.few_select_modes_ragged(context(), _p(amp, torch.complex128), _p(m, torch.int32), _p(ylm_plus), _p(ylm_minus),
+                                      _p(n_t_src, torch.int32), float(eps), n_src, n_t, n_modes, _p(keep), _p(nk), _p(ws), ws.numel(),
+                                      _stream()), "few_select_modes_ragged")
+    return keep, nk
+
+
+def few_sum_waveform_ragged(t, n_t_src, coef_amp, coef_phase_dd, l, m, k, n, keep_idx, n_keep, ylm_plus, ylm_minus, t0: float,
+                            dt: float, n_samples: int, scale=None, factor=None, d=None, want_inner: bool = False,
+                            want_h: bool = True, out=None, workspace=None):
+    """few_sum_waveform_kerr with per-source knot counts.  -> (h or None, inner or None)."""
+    n_src, n_t = t.shape
+    n_modes = l.shape[0]
+    n_phase = int(coef_phase_dd.shape[3])
+    h = None
+    if want_h:
+        h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
+    ws = workspace if workspace is not None else _ws(_lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples)), t.device)
+    _chk(_lib.few_sum_waveform_ragged(context(), _p(t, torch.float64), _p(n_t_src, torch.int32), _p(coef_amp, torch.float64),
+                                      _p(coef_phase_dd, torch.float64), n_phase, _p(l, torch.int32), _p(m, torch.int32), _p(k),
+                                      _p(n, torch.int32), _p(keep_idx), _p(n_keep), _p(ylm_plus, torch.complex128),
+                                      _p(ylm_minus, torch.complex128), _p(scale), _p(factor), float(t0), float(dt), int(n_samples),
+                                      _p(h), _p(d), _p(inner), n_src, n_t, n_modes, _p(ws), ws.numel(), _stream()),
+         "few_sum_waveform_ragged")
+    return h, inner
+
+
+def few_waveform_ragged(t, n_t_src, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int, scale=None,
+                        out=None, keep_idx=None, n_keep=None, workspace=None):
+    """Whole path on device tensors, sources with their own knot counts.  -> h [n_src, n_samples] complex128."""
+    n_src, n_t, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
+    ws = workspace if workspace is not None else _ws(few_waveform_workspace(n_src, n_t, n_modes, n_samples), t.device)
+    _chk(_lib.few_waveform_ragged(context(), _p(t, torch.float64), _p(n_t_src, torch.int32), _p(phase, torch.float64),
+                                  _p(amp, torch.complex128), _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32),
+                                  _p(theta, torch.float64), _p(phi, torch.float64), _p(scale), float(eps), float(t0), float(dt),
+                                  int(n_samples), n_src, n_t, n_modes, _p(h), _p(keep_idx), _p(n_keep), _p(ws), ws.numel(), _stream()),
+         "few_waveform_ragged")
+    return h
+
+
+def few_waveform_host_ragged(t, n_t_src, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int,
+                             scale=None, out=None, keep_idx=None, n_keep=None, device: int | None = None):
+    """Whole path on HOST tensors, sources with their own knot counts (n_t_src: CPU i32).  -> h (CPU) [n_src, n_samples]."""
+    n_src, n_t, n_modes = amp.shape
+    h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, pin_memory=True)
+    _chk(_lib.few_waveform_host_ragged(context(device), _hp(t, torch.float64), _hp(n_t_src, torch.int32), _hp(phase, torch.float64),
+                                       _hp(amp, torch.complex128), _hp(l, torch.int32), _hp(m, torch.int32), _hp(n, torch.int32),
+                                       _hp(theta, torch.float64), _hp(phi, torch.float64), _hp(scale, torch.float64), float(eps),
+                                       float(t0), float(dt), int(n_samples), n_src, n_t, n_modes, _hp(h, torch.complex128),
+                                       _hp(keep_idx, torch.int32), _hp(n_keep, torch.int32)), "few_waveform_host_ragged")
     return h
 
 

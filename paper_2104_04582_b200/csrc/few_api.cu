@@ -120,6 +120,7 @@ extern "C" int few_device_status(few_ctx* ctx, int* bits_out, void* stream)
     FEW_CUDA_CHECK(cudaMemsetAsync(ctx->d_status, 0, sizeof(int), st));
     FEW_CUDA_CHECK(cudaStreamSynchronize(st));
     if (bits_out) *bits_out = bits;
+    if (bits & FEW_DEV_BAD_COUNT) { few_set_error("device check: a source's knot count n_t_src[s] is outside [4, n_t]"); return FEW_ERR_TOO_FEW_POINTS; }
     if (bits & FEW_DEV_NOT_INCREASING) { few_set_error("device check: sparse times not strictly increasing"); return FEW_ERR_NOT_INCREASING; }
     if (bits & FEW_DEV_BAD_MODE) { few_set_error("device check: invalid (l, m, n) or kept-mode index"); return FEW_ERR_BAD_MODE; }
     if (bits & FEW_DEV_SPARSE_LIST) { few_set_error("device check: kept-mode list too sparse in (m, k, |n|) for the summation's step capacity"); return FEW_ERR_LIMIT; }
@@ -173,7 +174,7 @@ extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long l
 
 namespace {
 // theta/phi: source-frame viewing angles, or (sky != NULL) computed from the detector-frame angles by few_frame_constants.
-int waveform_impl(few_ctx* ctx, const double* t, const double* phase, int n_phase, const double* amp, const int* l, const int* m,
+int waveform_impl(few_ctx* ctx, const double* t, const int* n_t_src, const double* phase, int n_phase, const double* amp, const int* l, const int* m,
                   const int* k, const int* n, const double* theta, const double* phi, const double* sky, const double* scale, double eps, double t0, double dt,
                   long long n_samples, int n_src, int n_t, int n_modes, double* h, const double* d, double* inner, int* keep_idx,
                   int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
@@ -202,23 +203,23 @@ int waveform_impl(few_ctx* ctx, const double* t, const double* phase, int n_phas
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[0], ctx->ev_fork, 0));
     FEW_CUDA_CHECK(cudaStreamWaitEvent(ctx->side[1], ctx->ev_fork, 0));
     // from here on every path, failing or not, joins the side streams back into the caller's stream before returning
-    int rc = few_spline_fit(ctx, t, amp, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]);
-    if (rc == FEW_OK) rc = few_spline_fit_dd(ctx, t, phase, n_src, n_t, n_phase, L.coef_phase, ctx->side[1]);
+    int rc = few_spline_fit_ragged(ctx, t, amp, n_t_src, n_src, n_t, 2 * n_modes, L.coef_amp, L.spl_ws, L.spl_bytes, ctx->side[0]);
+    if (rc == FEW_OK) rc = few_spline_fit_dd_ragged(ctx, t, phase, n_t_src, n_src, n_t, n_phase, L.coef_phase, ctx->side[1]);
     const double* factor = nullptr;
     if (rc == FEW_OK && sky) {      // Eq. (4)-(8): viewing angles for the harmonics, one complex constant per source for the summation
         rc = few_frame_constants(ctx, sky, scale, n_src, L.theta_src, L.phi_src, L.factor, stream);
         theta = L.theta_src; phi = L.phi_src; factor = L.factor; scale = nullptr;
     }
     if (rc == FEW_OK) rc = few_ylm_modes(ctx, theta, phi, l, m, n_src, n_modes, L.ylm_plus, L.ylm_minus, stream);
-    if (rc == FEW_OK) rc = few_select_modes(ctx, amp, m, L.ylm_plus, L.ylm_minus, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream);
+    if (rc == FEW_OK) rc = few_select_modes_ragged(ctx, amp, m, L.ylm_plus, L.ylm_minus, n_t_src, eps, n_src, n_t, n_modes, kidx, nk, L.sel_ws, L.sel_bytes, stream);
     cudaError_t je = cudaEventRecord(ctx->ev_join[0], ctx->side[0]);
     if (je == cudaSuccess) je = cudaEventRecord(ctx->ev_join[1], ctx->side[1]);
     if (je == cudaSuccess) je = cudaStreamWaitEvent(st, ctx->ev_join[0], 0);
     if (je == cudaSuccess) je = cudaStreamWaitEvent(st, ctx->ev_join[1], 0);
     if (rc != FEW_OK) return rc;
     if (je != cudaSuccess) { few_set_error("few_waveform: joining the spline-fit streams failed: %s", cudaGetErrorString(je)); return FEW_ERR_CUDA; }
-    return few_sum_waveform_kerr(ctx, t, L.coef_amp, L.coef_phase, n_phase, l, m, k, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale, factor,
-                                 t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
+    return few_sum_waveform_ragged(ctx, t, n_t_src, L.coef_amp, L.coef_phase, n_phase, l, m, k, n, kidx, nk, L.ylm_plus, L.ylm_minus, scale,
+                                   factor, t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, L.sum_ws, L.sum_bytes, stream);
 }
 }  // namespace
 
@@ -229,8 +230,19 @@ extern "C" int few_waveform(few_ctx* ctx, const double* t, const double* phase, 
 {
     FEW_REQUIRE(theta && phi, FEW_ERR_INVALID_ARG, "theta or phi is NULL");
     FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
-    return waveform_impl(ctx, t, phase, 2, amp, l, m, nullptr, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
+    return waveform_impl(ctx, t, nullptr, phase, 2, amp, l, m, nullptr, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
                          nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
+}
+
+extern "C" int few_waveform_ragged(few_ctx* ctx, const double* t, const int* n_t_src, const double* phase, const double* amp,
+                                   const int* l, const int* m, const int* n, const double* theta, const double* phi, const double* scale,
+                                   double eps, double t0, double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                                   double* h, int* keep_idx, int* n_keep, void* workspace, size_t workspace_bytes, void* stream)
+{
+    FEW_REQUIRE(theta && phi, FEW_ERR_INVALID_ARG, "theta or phi is NULL");
+    FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
+    return waveform_impl(ctx, t, n_t_src, phase, 2, amp, l, m, nullptr, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes,
+                         h, nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 
 extern "C" int few_waveform_kerr(few_ctx* ctx, const double* t, const double* phase, const double* amp,
@@ -240,7 +252,7 @@ extern "C" int few_waveform_kerr(few_ctx* ctx, const double* t, const double* ph
 {
     FEW_REQUIRE(theta && phi && k, FEW_ERR_INVALID_ARG, "theta, phi or k is NULL");
     FEW_REQUIRE(n_samples == 0 || h, FEW_ERR_INVALID_ARG, "h is NULL");
-    return waveform_impl(ctx, t, phase, 3, amp, l, m, k, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
+    return waveform_impl(ctx, t, nullptr, phase, 3, amp, l, m, k, n, theta, phi, nullptr, scale, eps, t0, dt, n_samples, n_src, n_t, n_modes, h,
                          nullptr, nullptr, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 
@@ -252,15 +264,15 @@ extern "C" int few_waveform_ssb(few_ctx* ctx, const double* t, const double* pha
 {
     FEW_REQUIRE(sky != nullptr, FEW_ERR_INVALID_ARG, "sky is NULL");
     FEW_REQUIRE(n_samples == 0 || h || inner, FEW_ERR_INVALID_ARG, "h and inner are both NULL");
-    return waveform_impl(ctx, t, phase, 2, amp, l, m, nullptr, n, nullptr, nullptr, sky, mu_over_dl, eps, t0, dt, n_samples, n_src, n_t, n_modes,
+    return waveform_impl(ctx, t, nullptr, phase, 2, amp, l, m, nullptr, n, nullptr, nullptr, sky, mu_over_dl, eps, t0, dt, n_samples, n_src, n_t, n_modes,
                          h, d, inner, keep_idx, n_keep, workspace, workspace_bytes, stream);
 }
 
-extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
-                                 const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
-                                 const double* phi_host, const double* scale_host, double eps, double t0, double dt,
-                                 long long n_samples, int n_src, int n_t, int n_modes,
-                                 double* h_host, int* keep_idx_host, int* n_keep_host)
+extern "C" int few_waveform_host_ragged(few_ctx* ctx, const double* t_host, const int* n_t_src_host, const double* phase_host,
+                                        const double* amp_host, const int* l_host, const int* m_host, const int* n_host,
+                                        const double* theta_host, const double* phi_host, const double* scale_host, double eps, double t0,
+                                        double dt, long long n_samples, int n_src, int n_t, int n_modes,
+                                        double* h_host, int* keep_idx_host, int* n_keep_host)
 {
     FEW_REQUIRE(ctx && t_host && phase_host && amp_host && l_host && m_host && n_host && theta_host && phi_host,
                 FEW_ERR_INVALID_ARG, "NULL argument");
@@ -294,7 +306,7 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     size_t total = 0;
     few_carver sz(nullptr);
     sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_lmn); sz.take<char>(b_t); sz.take<char>(b_ph);
-    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang);
+    sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_ang); sz.take<char>(b_nk);
     const size_t small_bytes = sz.off;
     sz.take<char>(b_amp); sz.take<char>(b_h_dev); sz.take<char>(b_keep); sz.take<char>(b_nk);
     sz.take<char>(ws_bytes);
@@ -323,6 +335,7 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     int* d_l = (int*)c.take<char>(b_lmn); int* d_m = (int*)c.take<char>(b_lmn); int* d_n = (int*)c.take<char>(b_lmn);
     double* d_t = (double*)c.take<char>(b_t); double* d_ph = (double*)c.take<char>(b_ph);
     double* d_th = (double*)c.take<char>(b_ang); double* d_phi = (double*)c.take<char>(b_ang); double* d_sc = (double*)c.take<char>(b_ang);
+    int* d_nts = (int*)c.take<char>(b_nk);      // per-source knot counts of a ragged batch
     double* d_amp = (double*)c.take<char>(b_amp);
     double* d_h = (double*)c.take<char>(b_h_dev); int* d_keep = (int*)c.take<char>(b_keep); int* d_nk = (int*)c.take<char>(b_nk);
     void* d_ws = c.take<char>(ws_bytes);
@@ -338,6 +351,8 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
         memcpy(hc.take<char>(b_ang), theta_host, b_ang); memcpy(hc.take<char>(b_ang), phi_host, b_ang);
         char* sc = hc.take<char>(b_ang);
         if (scale_host) memcpy(sc, scale_host, b_ang);
+        char* nts = hc.take<char>(b_nk);
+        if (n_t_src_host) memcpy(nts, n_t_src_host, b_nk);
     }
     const int n_groups = n_src < kHostGroups ? n_src : kHostGroups;
     cudaStream_t cs = ctx->copy_stream;
@@ -355,9 +370,9 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
         const size_t s0 = (size_t)n_src * g / n_groups, s1 = (size_t)n_src * (g + 1) / n_groups, ns = s1 - s0;
         e = cudaStreamWaitEvent(st, ctx->ev_group[g], 0);
         if (e != cudaSuccess) break;
-        rc = few_waveform(ctx, d_t + s0 * n_t, d_ph + s0 * n_t * 2, d_amp + s0 * n_t * n_modes * 2, d_l, d_m, d_n, d_th + s0, d_phi + s0,
-                          scale_host ? d_sc + s0 : nullptr, eps, t0, dt, n_samples, (int)ns, n_t, n_modes,
-                          h_out + s0 * (size_t)n_samples * 2, d_keep + s0 * n_modes, d_nk + s0, d_ws, ws_bytes, st);
+        rc = few_waveform_ragged(ctx, d_t + s0 * n_t, n_t_src_host ? d_nts + s0 : nullptr, d_ph + s0 * n_t * 2, d_amp + s0 * n_t * n_modes * 2,
+                                 d_l, d_m, d_n, d_th + s0, d_phi + s0, scale_host ? d_sc + s0 : nullptr, eps, t0, dt, n_samples, (int)ns,
+                                 n_t, n_modes, h_out + s0 * (size_t)n_samples * 2, d_keep + s0 * n_modes, d_nk + s0, d_ws, ws_bytes, st);
         if (rc == FEW_OK && n_samples && !h_mapped)
             e = cudaMemcpyAsync(h_host + s0 * (size_t)n_samples * 2, d_h + s0 * (size_t)n_samples * 2, ns * (size_t)n_samples * 16,
                                 cudaMemcpyDeviceToHost, st);
@@ -370,6 +385,16 @@ extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const doubl
     if (e != cudaSuccess) { few_set_error("few_waveform_host: %s", cudaGetErrorString(e)); rc = FEW_ERR_CUDA; }
     cudaStreamSynchronize(st);
     return rc;
+}
+
+extern "C" int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_host, const double* amp_host,
+                                 const int* l_host, const int* m_host, const int* n_host, const double* theta_host,
+                                 const double* phi_host, const double* scale_host, double eps, double t0, double dt,
+                                 long long n_samples, int n_src, int n_t, int n_modes,
+                                 double* h_host, int* keep_idx_host, int* n_keep_host)
+{
+    return few_waveform_host_ragged(ctx, t_host, nullptr, phase_host, amp_host, l_host, m_host, n_host, theta_host, phi_host, scale_host, eps,
+                                    t0, dt, n_samples, n_src, n_t, n_modes, h_host, keep_idx_host, n_keep_host);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -51,6 +51,18 @@ void few_set_error(const char* fmt, ...);
 
 static inline size_t few_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+// Knot count of a source.  Uniform batches pass n_t_src == NULL: every source has n_t knots.  Ragged batches (the *_ragged
+// entry points) keep the padded [n_src][n_t] layouts and give each source's own count; one outside [4, n_t] is reported
+// (FEW_DEV_BAD_COUNT) and replaced by 4 (the first four rows exist for every source), so that no kernel reads the padding or
+// anything outside the arrays.
+__device__ __forceinline__ int few_knots(const int* __restrict__ n_t_src, int src, int n_t, int* status)
+{
+    if (!n_t_src) return n_t;
+    int v = n_t_src[src];
+    if (v < 4 || v > n_t) { atomicOr(status, FEW_DEV_BAD_COUNT); v = n_t < 4 ? n_t : 4; }
+    return v;
+}
+
 // Carves consecutive 256-byte-aligned sub-buffers out of a caller-owned workspace.
 struct few_carver {
     char* base; size_t off;

@@ -366,9 +366,11 @@ struct smem_entries {
 };
 
 __global__ void __launch_bounds__(kStreamThreads)
-few_select_row_stream_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L,
-                             const int* __restrict__ fb_list, const int* __restrict__ fb_count)
+few_select_row_stream_kernel(const double2* __restrict__ amp, const int* __restrict__ n_t_src, int n_t, int n_modes, double eps, sel_layout L,
+                             const int* __restrict__ fb_list, const int* __restrict__ fb_count, int* status)
 {
+    // ragged batch: the steps past the source's last knot are padding (block-uniform; listed rows were checked by the fast kernel)
+    if (!fb_list && (int)blockIdx.x >= few_knots(n_t_src, blockIdx.y, n_t, status)) return;
     extern __shared__ __align__(16) unsigned char stream_smem[];
     stream_shared& S = *reinterpret_cast<stream_shared*>(stream_smem);
     const int tid = threadIdx.x;
@@ -456,8 +458,10 @@ constexpr int kFastWords = kFastModes / 32;
 
 template <int NPT>
 __global__ void __launch_bounds__(kSelThreads, 3)
-few_select_row_fast_kernel(const double2* __restrict__ amp, int n_t, int n_modes, double eps, sel_layout L)
+few_select_row_fast_kernel(const double2* __restrict__ amp, const int* __restrict__ n_t_src, int n_t, int n_modes, double eps, sel_layout L,
+                           int* status)
 {
+    if ((int)blockIdx.x >= few_knots(n_t_src, blockIdx.y, n_t, status)) return;     // ragged batch: padding step (block-uniform)
     __shared__ sel_shared<kSelThreads, kBucketMax, kFastWords> S;
     __shared__ long long cand_k[kCandMax];
     __shared__ int cand_e[kCandMax];
@@ -579,9 +583,9 @@ extern "C" size_t few_select_modes_workspace(int n_src, int n_t, int n_modes)
     return bytes;
 }
 
-extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
-                                double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,
-                                void* workspace, size_t workspace_bytes, void* stream)
+extern "C" int few_select_modes_ragged(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
+                                       const int* n_t_src, double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,
+                                       void* workspace, size_t workspace_bytes, void* stream)
 {
     FEW_REQUIRE(ctx && amp && m && keep_idx && n_keep, FEW_ERR_INVALID_ARG, "NULL argument");
     FEW_REQUIRE(n_src > 0 && n_t > 0 && n_modes > 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
@@ -606,19 +610,27 @@ extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, c
     FEW_REQUIRE(sizeof(stream_shared) <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "stream kernel's shared memory exceeds the device limit");
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_select_row_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(stream_shared)));
     if (n_modes <= kFastModes) {
-        few_select_row_fast_kernel<16><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t, n_modes, eps, L);
+        few_select_row_fast_kernel<16><<<grid, kSelThreads, 0, st>>>((const double2*)amp, n_t_src, n_t, n_modes, eps, L, ctx->d_status);
         FEW_LAUNCHED(ctx);
         // the rows the fast kernel left (usually none): a small persistent grid walks the list
         const long long n_rows = (long long)n_t * n_src;
         const unsigned fb_grid = (unsigned)(n_rows < ctx->sm_count ? n_rows : ctx->sm_count);
-        few_select_row_stream_kernel<<<fb_grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t, n_modes, eps, L,
-                                                                                             L.fb_list, L.fb_count);
+        few_select_row_stream_kernel<<<fb_grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t_src, n_t, n_modes, eps, L,
+                                                                                             L.fb_list, L.fb_count, ctx->d_status);
     } else {
-        few_select_row_stream_kernel<<<grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t, n_modes, eps, L, nullptr,
-                                                                                          nullptr);
+        few_select_row_stream_kernel<<<grid, kStreamThreads, sizeof(stream_shared), st>>>((const double2*)amp, n_t_src, n_t, n_modes, eps, L, nullptr,
+                                                                                          nullptr, ctx->d_status);
     }
     FEW_LAUNCHED(ctx);
     few_select_compact_kernel<<<n_src, kPrepThreads, 0, st>>>(L, n_modes, 0, keep_idx, n_keep);
     FEW_LAUNCHED(ctx);
     return FEW_OK;
+}
+
+extern "C" int few_select_modes(few_ctx* ctx, const double* amp, const int* m, const double* ylm_plus, const double* ylm_minus,
+                                double eps, int n_src, int n_t, int n_modes, int* keep_idx, int* n_keep,
+                                void* workspace, size_t workspace_bytes, void* stream)
+{
+    return few_select_modes_ragged(ctx, amp, m, ylm_plus, ylm_minus, nullptr, eps, n_src, n_t, n_modes, keep_idx, n_keep, workspace,
+                                   workspace_bytes, stream);
 }

@@ -66,13 +66,13 @@ __device__ void factor_grid(const double* __restrict__ t, int n, double* inv_h, 
 
 // Factorisation of every source's grid into the workspace: fac[src][6][n_t] = inv_h, w, inv_d, u, rA, rB.
 __global__ void __launch_bounds__(128)
-few_spline_factor_kernel(const double* __restrict__ t_all, int n_t, double* __restrict__ fac_all, int* status)
+few_spline_factor_kernel(const double* __restrict__ t_all, const int* __restrict__ n_t_src, int n_t, double* __restrict__ fac_all, int* status)
 {
     extern __shared__ double smem[];
-    const int n = n_t;
-    factor_grid(t_all + (size_t)blockIdx.x * n, n, smem, smem + n, smem + 2 * n, smem + 3 * n, smem + 4 * n, smem + 5 * n, status);
+    const int n = few_knots(n_t_src, blockIdx.x, n_t, status);      // the source's knots; n_t is the stride of the padded arrays
+    factor_grid(t_all + (size_t)blockIdx.x * n_t, n, smem, smem + n, smem + 2 * n, smem + 3 * n, smem + 4 * n, smem + 5 * n, status);
     __syncthreads();
-    double* fac = fac_all + (size_t)blockIdx.x * 6 * n;
+    double* fac = fac_all + (size_t)blockIdx.x * 6 * n_t;
     for (int i = threadIdx.x; i < 6 * n; i += blockDim.x) fac[i] = smem[i];
 }
 
@@ -95,22 +95,22 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <bool kLatency>
 __global__ void __launch_bounds__(128)
 few_spline_fit_kernel(const double* __restrict__ t_all, const double* __restrict__ fac_all, const double* __restrict__ y_all,
-                      int n_t, int n_sys, double* __restrict__ coef_all, int* status)
+                      const int* __restrict__ n_t_src, int n_t, int n_sys, double* __restrict__ coef_all, int* status)
 {
     extern __shared__ double4 smem4[];
-    const int W = blockDim.x, tid = threadIdx.x, n = n_t;
+    const int W = blockDim.x, tid = threadIdx.x, n = few_knots(n_t_src, blockIdx.y, n_t, status);
     double4* F = smem4;                                   // [n] {w_i, rA_i, rB_i, 1/h_i}
     double2* Bk = reinterpret_cast<double2*>(F + n);      // [n] {u_i, 1/d'_i}
     double* D = reinterpret_cast<double*>(Bk + n);        // [n][W]
     double* Y = D + (size_t)n * W;                        // kLatency: [n][W] knot values, then [6][n] raw factorisation
     const int src = blockIdx.y;
     const int q = blockIdx.x * W + tid;
-    const double* y = y_all + (size_t)src * n * n_sys + q;
+    const double* y = y_all + (size_t)src * n_t * n_sys + q;
     if (kLatency) {
         if (q < n_sys)
             for (int i = 0; i < n; ++i) cp_async_8(&Y[i * W + tid], y + (size_t)i * n_sys);
         double* raw = Y + (size_t)n * W;
-        factor_grid(t_all + (size_t)src * n, n, raw, raw + n, raw + 2 * n, raw + 3 * n, raw + 4 * n, raw + 5 * n, status);
+        factor_grid(t_all + (size_t)src * n_t, n, raw, raw + n, raw + 2 * n, raw + 3 * n, raw + 4 * n, raw + 5 * n, status);
         __syncthreads();
         for (int i = tid; i < n; i += W) {
             F[i] = make_double4(raw[n + i], raw[4 * n + i], raw[5 * n + i], raw[i]);
@@ -118,7 +118,7 @@ few_spline_fit_kernel(const double* __restrict__ t_all, const double* __restrict
         }
         cp_async_wait_all();
     } else {
-        const double* fac = fac_all + (size_t)src * 6 * n;   // inv_h, w, inv_d, u, rA, rB
+        const double* fac = fac_all + (size_t)src * 6 * n_t; // inv_h, w, inv_d, u, rA, rB
         for (int i = tid; i < n; i += W) {
             F[i] = make_double4(fac[n + i], fac[4 * n + i], fac[5 * n + i], fac[i]);
             Bk[i] = make_double2(fac[3 * n + i], fac[2 * n + i]);
@@ -126,7 +126,7 @@ few_spline_fit_kernel(const double* __restrict__ t_all, const double* __restrict
     }
     __syncthreads();
     if (q >= n_sys) return;
-    double* coef = coef_all + (size_t)src * (n - 1) * 4 * n_sys + q;
+    double* coef = coef_all + (size_t)src * (n_t - 1) * 4 * n_sys + q;
     auto ld = [&](int i) {
         if (!(i >= 0 && i < n)) return 0.0;
         return kLatency ? Y[i * W + tid] : __ldg(y + (size_t)i * n_sys);
@@ -209,11 +209,11 @@ constexpr int kDdThreads = 128;
 constexpr int kDdRefine = 2;
 
 __global__ void __launch_bounds__(kDdThreads)
-few_spline_fit_dd_kernel(const double* __restrict__ t_all, const double* __restrict__ y_all,
+few_spline_fit_dd_kernel(const double* __restrict__ t_all, const double* __restrict__ y_all, const int* __restrict__ n_t_src,
                          int n_t, int n_sys, double* __restrict__ coef_all, int* status)
 {
     extern __shared__ double smem[];
-    const int n = n_t, tid = threadIdx.x;
+    const int n = few_knots(n_t_src, blockIdx.y, n_t, status), tid = threadIdx.x;
     double* inv_h = smem;                 // FP64 preconditioner (factor_grid)
     double* wm = inv_h + n;
     double* inv_d = wm + n;
@@ -228,9 +228,9 @@ few_spline_fit_dd_kernel(const double* __restrict__ t_all, const double* __restr
 
     const int src = blockIdx.y, q0 = blockIdx.x * kDdSys;
     const int ns = min(kDdSys, n_sys - q0);
-    const double* t = t_all + (size_t)src * n;
-    const double* y = y_all + (size_t)src * n * n_sys + q0;
-    dd* coef = reinterpret_cast<dd*>(coef_all) + (size_t)src * (n - 1) * 4 * n_sys + q0;
+    const double* t = t_all + (size_t)src * n_t;
+    const double* y = y_all + (size_t)src * n_t * n_sys + q0;
+    dd* coef = reinterpret_cast<dd*>(coef_all) + (size_t)src * (n_t - 1) * 4 * n_sys + q0;
 
     factor_grid(t, n, inv_h, wm, inv_d, um, rA, rB, status);
     for (int i = tid; i < n - 1; i += kDdThreads) {
@@ -323,8 +323,8 @@ extern "C" size_t few_spline_fit_workspace(int n_src, int n_t)
     return few_align_up((size_t)n_src * 6 * n_t * sizeof(double));
 }
 
-extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
-                              double* coef, void* workspace, size_t workspace_bytes, void* stream)
+extern "C" int few_spline_fit_ragged(few_ctx* ctx, const double* t, const double* y, const int* n_t_src, int n_src, int n_t, int n_sys,
+                                     double* coef, void* workspace, size_t workspace_bytes, void* stream)
 {
     int rc = few_spline_check(ctx, t, y, coef, n_src, n_t, n_sys);
     if (rc) return rc;
@@ -341,13 +341,13 @@ extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, in
         const int W = 32;
         dim3 grid((n_sys + W - 1) / W, n_src);
         FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes_lat(W)));
-        few_spline_fit_kernel<true><<<grid, W, bytes_lat(W), st>>>(t, nullptr, y, n_t, n_sys, coef, ctx->d_status);
+        few_spline_fit_kernel<true><<<grid, W, bytes_lat(W), st>>>(t, nullptr, y, n_t_src, n_t, n_sys, coef, ctx->d_status);
         FEW_LAUNCHED(ctx);
         return FEW_OK;
     }
     // Throughput regime.  Block width W (systems per block): as wide as possible (longer contiguous rows per store) while at
     // least two blocks fit an SM and the grid still covers every SM twice.
-    few_spline_factor_kernel<<<n_src, 128, (size_t)6 * n_t * sizeof(double), st>>>(t, n_t, fac, ctx->d_status);
+    few_spline_factor_kernel<<<n_src, 128, (size_t)6 * n_t * sizeof(double), st>>>(t, n_t_src, n_t, fac, ctx->d_status);
     FEW_LAUNCHED(ctx);
     auto bytes = [&](int w) { return (size_t)n_t * (48 + 8 * (size_t)w); };
     int W = 128;
@@ -355,13 +355,19 @@ extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, in
     FEW_REQUIRE(bytes(W) <= cap, FEW_ERR_LIMIT, "n_t too large for shared memory");
     dim3 grid((n_sys + W - 1) / W, n_src);
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes(W)));
-    few_spline_fit_kernel<false><<<grid, W, bytes(W), st>>>(t, fac, y, n_t, n_sys, coef, ctx->d_status);
+    few_spline_fit_kernel<false><<<grid, W, bytes(W), st>>>(t, fac, y, n_t_src, n_t, n_sys, coef, ctx->d_status);
     FEW_LAUNCHED(ctx);
     return FEW_OK;
 }
 
-extern "C" int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
-                                 double* coef_dd, void* stream)
+extern "C" int few_spline_fit(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
+                              double* coef, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return few_spline_fit_ragged(ctx, t, y, nullptr, n_src, n_t, n_sys, coef, workspace, workspace_bytes, stream);
+}
+
+extern "C" int few_spline_fit_dd_ragged(few_ctx* ctx, const double* t, const double* y, const int* n_t_src, int n_src, int n_t, int n_sys,
+                                        double* coef_dd, void* stream)
 {
     int rc = few_spline_check(ctx, t, y, coef_dd, n_src, n_t, n_sys);
     if (rc) return rc;
@@ -369,7 +375,13 @@ extern "C" int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y,
     FEW_REQUIRE(bytes <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "n_t too large for shared memory");
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_spline_fit_dd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     dim3 grid((n_sys + kDdSys - 1) / kDdSys, n_src);
-    few_spline_fit_dd_kernel<<<grid, kDdThreads, bytes, (cudaStream_t)stream>>>(t, y, n_t, n_sys, coef_dd, ctx->d_status);
+    few_spline_fit_dd_kernel<<<grid, kDdThreads, bytes, (cudaStream_t)stream>>>(t, y, n_t_src, n_t, n_sys, coef_dd, ctx->d_status);
     FEW_LAUNCHED(ctx);
     return FEW_OK;
+}
+
+extern "C" int few_spline_fit_dd(few_ctx* ctx, const double* t, const double* y, int n_src, int n_t, int n_sys,
+                                 double* coef_dd, void* stream)
+{
+    return few_spline_fit_dd_ragged(ctx, t, y, nullptr, n_src, n_t, n_sys, coef_dd, stream);
 }

@@ -66,7 +66,7 @@ constexpr int kSlotShift = 28, kSlotBits = 3; // table slot of the step's block 
 constexpr int kTabSlots = 8;                  // distinct blocks nu >> 2 a source may use in table mode (the paper's grid: nu <= 31 -> 8)
 
 // A tile of the sum kernel as the plan kernel hands it over (one 32-byte record, two 16-byte loads): first sample and sample
-// count, pseudo-segment p (-1: no tile; 0 or n_t: outside the trajectory, h = 0), the source, and the number of coefficient
+// count, pseudo-segment p (-1: no tile; 0: outside the trajectory, h = 0), the source, and the number of coefficient
 // stages the tile consumes (0 for tiles without a summation), and the source's mode (1 table, 0 recurrence: which of the two
 // instantiations of the sum kernel takes the tile).
 struct __align__(16) tile_rec { long long i_begin; int count; int p; int n_stages; int src; int mode; int pad1; };   // n_stages, mode: filled by load_rec from src_info
@@ -137,6 +137,7 @@ __device__ __forceinline__ double sample_time(double t0, double dt, long long i)
 __device__ long long first_index(double tk, double t0, double dt, long long N, bool strict)
 {
     // smallest i in [0, N] with t_i >= tk (strict: t_i > tk); t_i is non-decreasing in i for dt > 0
+    if (!(tk == tk)) return 0;       // NaN knot (reported elsewhere as not increasing): any in-range value, without the searches
     double x = (tk - t0) / dt;
     long long i = !(x > 0.0) ? 0 : (x >= (double)N ? N : (long long)ceil(x));
     if (strict) {
@@ -198,7 +199,7 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
                     const int* __restrict__ kpol, const int* __restrict__ n, const int* __restrict__ keep_idx, const int* __restrict__ n_keep,
                     const double2* __restrict__ ylm_plus, const double2* __restrict__ ylm_minus,
                     const double* __restrict__ scale, const double2* __restrict__ factor, double t0, double dt, long long N,
-                    int n_t, int n_modes, int smem_elems, sum_layout L, int* status)
+                    const int* __restrict__ n_t_src, int n_t, int n_modes, int smem_elems, sum_layout L, int* status)
 {
     extern __shared__ unsigned long long plan_smem[];             // [smem_elems]
     unsigned long long* plan_sorted;                              // [n_pow2] (key << 32 | mode index), sorted ascending
@@ -210,27 +211,29 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     // Blocks of a source work side by side: blockIdx.y >= 1 lay out the tiles (a), (e) -- that needs the time grids only --
     // and blockIdx.y == 0 orders the kept modes and cuts them into steps (b)-(d).
     if (blockIdx.y >= 1) {
-    // ---- (a) sample ranges of the pseudo-segments and their tile prefix
+    // ---- (a) sample ranges of the pseudo-segments and their tile prefix.  ns = the source's own knot count (ragged batches;
+    // = n_t otherwise): pseudo-segments 0 .. ns, the arrays keep the stride n_t + 2 and the tile total also goes to TS[n_t + 1]
+    const int ns = few_knots(n_t_src, src, n_t, status);
     long long* B = L.bounds + (size_t)src * (n_t + 2);
     int* TS = L.tile_start + (size_t)src * (n_t + 2);
-    for (int k = tid; k < n_t; k += kPlanThreads) {
-        if (k + 1 < n_t && !(t[k + 1] > t[k])) atomicOr(status, FEW_DEV_NOT_INCREASING);
-        if (k <= n_t - 2) B[k + 1] = first_index(t[k], t0, dt, N, false);
-        else { B[n_t] = first_index(t[n_t - 1], t0, dt, N, true); B[n_t + 1] = N; B[0] = 0; }
+    for (int k = tid; k < ns; k += kPlanThreads) {
+        if (k + 1 < ns && !(t[k + 1] > t[k])) atomicOr(status, FEW_DEV_NOT_INCREASING);
+        if (k <= ns - 2) B[k + 1] = first_index(t[k], t0, dt, N, false);
+        else { B[ns] = first_index(t[ns - 1], t0, dt, N, true); B[ns + 1] = N; B[0] = 0; }
     }
     __syncthreads();
-    if (tid < 32) {           // warp 0: prefix over n_t + 1 pseudo-segments, 32 at a time
+    if (tid < 32) {           // warp 0: prefix over ns + 1 pseudo-segments, 32 at a time
         int carry = 0;
-        for (int base = 0; base <= n_t; base += 32) {
+        for (int base = 0; base <= ns; base += 32) {
             int p = base + tid;
             int cnt = 0;
-            if (p <= n_t) { long long c = B[p + 1] - B[p]; if (c < 0) c = 0; cnt = (int)((c + kTile - 1) / kTile); }
+            if (p <= ns) { long long c = B[p + 1] - B[p]; if (c < 0) c = 0; cnt = (int)((c + kTile - 1) / kTile); }
             int v = cnt;
             for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, v, o); if (tid >= o) v += u; }
-            if (p <= n_t) TS[p] = carry + v - cnt;
+            if (p <= ns) TS[p] = carry + v - cnt;
             carry += __shfl_sync(0xffffffffu, v, 31);
         }
-        if (tid == 0) TS[n_t + 1] = carry;
+        if (tid == 0) { TS[ns + 1] = carry; TS[n_t + 1] = carry; }
     }
     __syncthreads();
     // ---- (e) tile records: tile q of pseudo-segment p covers samples [B[p] + (q - TS[p]) kTile, ...) inside [B[p], B[p+1]).
@@ -238,19 +241,19 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
     // a thread takes tiles q, q + stride, ... and finds p by binary search (24.6 k records from one block took 36 us)
     {
         tile_rec* rec = L.tiles + (size_t)src * L.max_tiles;
-        const int n_tiles = TS[n_t + 1];
+        const int n_tiles = TS[ns + 1];
         const int tb = gridDim.y - 1, ry = blockIdx.y - 1;
         for (int q = ry * kPlanThreads + tid; q < L.max_tiles; q += tb * kPlanThreads) {
             tile_rec r;
             r.n_stages = 0; r.src = src; r.mode = 0; r.pad1 = 0;
             if (q < n_tiles) {
-                int lo = 0, hi = n_t + 1;                        // largest p with TS[p] <= q
+                int lo = 0, hi = ns + 1;                         // largest p with TS[p] <= q
                 while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (TS[mid] <= q) lo = mid; else hi = mid; }
                 const long long b0 = B[lo], b1 = B[lo + 1];
                 r.i_begin = b0 + (long long)(q - TS[lo]) * kTile;
                 const long long left = b1 - r.i_begin;
                 r.count = (int)(left < kTile ? left : kTile);
-                r.p = lo;
+                r.p = lo == ns ? 0 : lo;                         // after the last knot = before the first: outside, h = 0
             } else {
                 r.i_begin = 0; r.count = 0; r.p = -1;
             }
@@ -428,9 +431,11 @@ few_sum_plan_kernel(const double* __restrict__ t_all, const int* __restrict__ l,
 // The four B matrices of every step, in DMMA.8x8x4 fragment order, written as the stage stream the sum kernel consumes.
 // Lane L of a warp supplies B[k = L & 3][o = L >> 2]: unit k of the step (nu = 4 blk + k), output o = 2 p + part (power p of
 // dx, part 0 = re, 1 = im).  A step is 1 KB: [0][L] = (B1c, B2c), [1][L] = (B1s, B2s) as double2 (conflict-free LDS.128).
-__global__ void __launch_bounds__(1024) few_sum_pack_kernel(const double2* __restrict__ coef_amp, int n_t, int n_modes, sum_layout L)
+__global__ void __launch_bounds__(1024) few_sum_pack_kernel(const double2* __restrict__ coef_amp, const int* __restrict__ n_t_src, int n_t,
+                                                            int n_modes, sum_layout L)
 {
     const int seg = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
+    if (n_t_src && seg >= n_t_src[src] - 1) return;      // ragged batch: no such segment (its coefficients were never written)
     const int S = L.n_steps[src];
     const int* ulo = L.u_lo + (size_t)src * L.cap * 8;
     const int* uhi = L.u_hi + (size_t)src * L.cap * 8;
@@ -586,14 +591,14 @@ __device__ __forceinline__ void tmem_ld_x16(unsigned taddr, double2 (&v)[4])
     for (int g = 0; g < 4; ++g) v[g] = make_double2(__hiloint2double(r[4 * g + 1], r[4 * g]), __hiloint2double(r[4 * g + 3], r[4 * g + 2]));
 }
 
-__device__ __forceinline__ tile_rec load_rec(const tile_rec* p, const int2* __restrict__ src_info, int n_t)
+__device__ __forceinline__ tile_rec load_rec(const tile_rec* p, const int2* __restrict__ src_info)
 {
     const int4 a = __ldg(reinterpret_cast<const int4*>(p)), b = __ldg(reinterpret_cast<const int4*>(p) + 1);
     tile_rec r;
     r.i_begin = ((long long)(unsigned)a.y << 32) | (unsigned)a.x; r.count = a.z; r.p = a.w;
     r.src = b.y; r.pad1 = 0;
     const int2 info = __ldg(src_info + r.src);          // per source: stages per tile, mode (a cached load)
-    r.n_stages = (r.p <= 0 || r.p == n_t) ? 0 : info.x;
+    r.n_stages = r.p <= 0 ? 0 : info.x;
     r.mode = info.y;
     return r;
 }
@@ -659,7 +664,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             ++j;
             const long long tg = blockIdx.x + j * stride;
             if (tg >= total_tiles) return;                          // the stream has ended
-            ri = (j == i + 1) ? rn : load_rec(L.tiles + tg, L.src_info, n_t);
+            ri = (j == i + 1) ? rn : load_rec(L.tiles + tg, L.src_info);
         }
         const double2* src = pack + ((size_t)ri.src * n_seg + (ri.p - 1)) * L.max_stages * kStageD2 + (size_t)s * kStageD2;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the warps' reads of the slot precede the copy's writes
@@ -673,8 +678,8 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     tile_rec cur, nxt;
     cur.p = -1; cur.n_stages = 0; cur.count = 0; cur.i_begin = 0; cur.src = 0; cur.mode = 0; cur.pad1 = 0;
     nxt = cur;
-    if ((long long)blockIdx.x < total_tiles) cur = load_rec(L.tiles + blockIdx.x, L.src_info, n_t);
-    if (blockIdx.x + stride < total_tiles) nxt = load_rec(L.tiles + blockIdx.x + stride, L.src_info, n_t);
+    if ((long long)blockIdx.x < total_tiles) cur = load_rec(L.tiles + blockIdx.x, L.src_info);
+    if (blockIdx.x + stride < total_tiles) nxt = load_rec(L.tiles + blockIdx.x + stride, L.src_info);
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kRing; ++s) { mbar_init(&full[s], 1); done_s[s] = 0; }
@@ -696,7 +701,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (tg >= total_tiles) break;
     tile_rec nn = cur;                      // record of tile i + 2: loaded now, needed at the end of this tile
     nn.p = -1; nn.n_stages = 0; nn.count = 0;
-    if (tg + 2 * stride < total_tiles) nn = load_rec(L.tiles + tg + 2 * stride, L.src_info, n_t);
+    if (tg + 2 * stride < total_tiles) nn = load_rec(L.tiles + tg + 2 * stride, L.src_info);
     if (cur.p >= 0 && cur.mode == (kTab ? 1 : 0)) {
     const int src = cur.src, p = cur.p;
     const long long w_begin = cur.i_begin + warp * W;               // this warp's samples: [w_begin, w_begin + w_count)
@@ -995,11 +1000,11 @@ extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, lo
     return bytes;
 }
 
-extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd, int n_phase,
-                                     const int* l, const int* m, const int* k, const int* n, const int* keep_idx, const int* n_keep,
-                                     const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
-                                     double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
-                                     int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
+extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int* n_t_src, const double* coef_amp, const double* coef_phase_dd,
+                                       int n_phase, const int* l, const int* m, const int* k, const int* n, const int* keep_idx,
+                                       const int* n_keep, const double* ylm_plus, const double* ylm_minus, const double* scale,
+                                       const double* factor, double t0, double dt, long long n_samples, double* h, const double* d,
+                                       double* inner, int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
 {
     FEW_REQUIRE(n_phase == 2 || n_phase == 3, FEW_ERR_INVALID_ARG, "n_phase must be 2 (Phi_phi, Phi_r) or 3 (Phi_phi, Phi_theta, Phi_r)");
     FEW_REQUIRE(n_phase == 3 || k == nullptr, FEW_ERR_INVALID_ARG, "a polar index k needs the third phase (n_phase = 3)");
@@ -1031,17 +1036,17 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
     FEW_CUDA_CHECK(cudaFuncSetAttribute(few_sum_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
     few_sum_plan_kernel<<<dim3(n_src, 1 + plan_tile_blocks), kPlanThreads, psm, st>>>(t, l, m, k, n, keep_idx, n_keep, (const double2*)ylm_plus,
                                                           (const double2*)ylm_minus, scale, (const double2*)factor, t0, dt, n_samples,
-                                                          n_t, n_modes, plan_elems, L, ctx->d_status);
+                                                          n_t_src, n_t, n_modes, plan_elems, L, ctx->d_status);
     FEW_LAUNCHED(ctx);
     // few blocks (one waveform): 1024 threads finish a segment's 4 x pairs items in one sweep; a batch fills the SMs with
     // several 256-thread blocks each, which hides the dependent index -> coefficient loads better
     const int pack_threads = (long long)(n_t - 1) * n_src < 2LL * ctx->sm_count ? 1024 : 256;
-    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), pack_threads, 0, st>>>((const double2*)coef_amp, n_t, n_modes, L);
+    few_sum_pack_kernel<<<dim3(n_t - 1, n_src), pack_threads, 0, st>>>((const double2*)coef_amp, n_t_src, n_t, n_modes, L);
     FEW_LAUNCHED(ctx);
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
     FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
-    // both instantiations are launched: the table one (2 blocks per SM, ~101 KB of shared memory each) takes the sources whose
-    // lists fit its table, the recurrence one (4 blocks per SM) the others; an instantiation with no source returns at once
+    // both instantiations are launched: the table one (rho^nu of the 8 nu-blocks in use kept in tensor memory) takes the sources
+    // whose lists fit its table, the recurrence one the others; an instantiation with no source returns at once
     const long long want = max_tiles * n_src;
 #define FEW_SUM_LAUNCH(INNER, KERR, DPTR)                                                                                         \
     do {                                                                                                                          \
@@ -1073,6 +1078,16 @@ extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double
         FEW_LAUNCHED(ctx);
     }
     return FEW_OK;
+}
+
+extern "C" int few_sum_waveform_kerr(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd, int n_phase,
+                                     const int* l, const int* m, const int* k, const int* n, const int* keep_idx, const int* n_keep,
+                                     const double* ylm_plus, const double* ylm_minus, const double* scale, const double* factor,
+                                     double t0, double dt, long long n_samples, double* h, const double* d, double* inner,
+                                     int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return few_sum_waveform_ragged(ctx, t, nullptr, coef_amp, coef_phase_dd, n_phase, l, m, k, n, keep_idx, n_keep, ylm_plus, ylm_minus,
+                                   scale, factor, t0, dt, n_samples, h, d, inner, n_src, n_t, n_modes, workspace, workspace_bytes, stream);
 }
 
 extern "C" int few_sum_waveform_ex(few_ctx* ctx, const double* t, const double* coef_amp, const double* coef_phase_dd,

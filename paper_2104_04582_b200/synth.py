@@ -53,6 +53,7 @@ class Workload:
     n_samples: int
     eps: float
     k: np.ndarray | None = None     # polar index per mode (Kerr-shaped workloads: phase then has 3 columns, Phi_phi, Phi_theta, Phi_r)
+    n_t_src: np.ndarray | None = None   # ragged batches: knots per source, int32 [n_src]; rows beyond a source's count are padding (NaN)
 
     @property
     def n_src(self): return self.t.shape[0]
@@ -176,6 +177,38 @@ def make_config(config: int, *, n_samples: int | None = None, n_src: int | None 
     if t0 is not None: w.t0 = float(t0)
     if eps is not None: w.eps = float(eps)
     return w
+
+
+def make_ragged(counts=(40, 80, 137, 80, 40, 137), *, n_samples: int = 40_000, dt: float = 15.0, eps: float = 1e-5,
+                seed: int = 0) -> Workload:
+    """A ragged batch: sources drawn like config 3's (parameters uniform in the same ranges) but each with its own number of
+    trajectory points and its own end time, as an adaptive integrator that stops at the separatrix hands them over
+    ("~100" points).  Arrays are padded to the largest count; the padding is NaN so that any
+    read of it shows up in the output.  Source s ends at T_s in [0.45, 1.05] x n_samples x dt: some end inside the output window
+    (h = 0 from there on), some after it."""
+    l, m, n = mode_grid()
+    counts = np.asarray(counts, np.int32)
+    n_src, n_max = len(counts), int(counts.max())
+    t = np.full((n_src, n_max), np.nan)
+    phase = np.full((n_src, n_max, 2), np.nan)
+    amp = np.full((n_src, n_max, len(l)), np.nan + 1j * np.nan, dtype=np.complex128)
+    th, ph_ = np.empty(n_src), np.empty(n_src)
+    for s in range(n_src):
+        rng = np.random.Generator(np.random.PCG64(SEED_BASE + 7000 + 100 * seed + s))
+        p0 = rng.uniform(10.0, 16.0); e0 = rng.uniform(0.1, 0.6); M = 10.0 ** rng.uniform(5.0, 7.0)
+        th[s] = rng.uniform(0.0, np.pi); ph_[s] = rng.uniform(0.0, 2.0 * np.pi)
+        T = rng.uniform(0.45, 1.05) * n_samples * dt
+        e1 = 0.5 * e0
+        ts, p, a = _one_source(rng, T=T, n_t=int(counts[s]), uniform=False, p0=p0, p1=6.0 + 2 * e1 + 0.1, e0=e0, e1=e1, M=M, l=l, n=n)
+        t[s, :counts[s]] = ts; phase[s, :counts[s]] = p; amp[s, :counts[s]] = a
+    return Workload(f"ragged{n_src}", t, phase, amp, l, m, n, th, ph_, 0.0, dt, int(n_samples), eps, n_t_src=counts)
+
+
+def source_of(w: Workload, s: int) -> Workload:
+    """Source s of a batch as a one-source uniform workload with its own knot count (the padding cut off)."""
+    c = int(w.n_t_src[s]) if w.n_t_src is not None else w.n_t
+    return Workload(f"{w.name}[{s}]", w.t[s:s + 1, :c].copy(), w.phase[s:s + 1, :c].copy(), w.amp[s:s + 1, :c].copy(), w.l, w.m, w.n,
+                    w.theta[s:s + 1].copy(), w.phi[s:s + 1].copy(), w.t0, w.dt, w.n_samples, w.eps, k=w.k)
 
 
 def random_problem(seed: int, *, n_src=1, n_t=12, n_modes=10, l_max=5, n_max=3, T=1000.0, n_samples=257,
