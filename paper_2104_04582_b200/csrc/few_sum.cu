@@ -25,7 +25,7 @@
 //        block-uniform); orders the kept modes by (m, k, |n|, sign n, l) and cuts them into STEPS: the kept units of one run
 //        whose nu fall into one aligned block of four (4b .. 4b+3), with a descriptor saying how (c, s) is reached.
 //   2. few_sum_pack_kernel  (one block per source and segment): forms the four B matrices of every step from the kept modes'
-//        spline coefficients and Y+, Ybar, scale, in DMMA fragment order, as a stream of stages (4 steps x 1 KB + header).
+//        spline coefficients and Y+, Ybar, scale, in DMMA fragment order, as a stream of stages (16 steps x 1 KB + header).
 //   3. few_sum_kernel       the hot loop.  Stages arrive in shared memory through a ring of TMA bulk copies
 //        (cp.async.bulk + mbarrier) and are read with conflict-free 128-bit loads.  Per sample the phases are evaluated ONCE in
 //        double-double (Horner, reduction by 2 pi, one sincos each).  Output: coalesced 16-byte streaming stores.
@@ -35,24 +35,26 @@ namespace {
 
 constexpr int kPlanThreads = 1024;
 constexpr int kPlanSmemElems = 16384;         // 128 KB of (key, mode) words: the plan kernel's in-shared-memory sort capacity
-constexpr int kSumThreads = 128;
-#ifndef FEW_SUM_G
-#define FEW_SUM_G 4
-#define FEW_SUM_BPS 4
+#ifndef FEW_SUM_WARPS
+#define FEW_SUM_WARPS 4
 #endif
-constexpr int kSumG = FEW_SUM_G;              // groups of 8 samples per warp
-constexpr int kSumBlocksPerSm = FEW_SUM_BPS;  // resident blocks per SM, recurrence instantiation (register budget 65536 / (128 * blocks))
-constexpr int kSumTabBlocksPerSm = 4;         // resident blocks per SM, table instantiation (4 x 128 columns = all of tensor memory)
+constexpr int kSumThreads = 32 * FEW_SUM_WARPS;   // warps per block: 4, 8 or 16 (16 warps are resident per SM either way)
+constexpr int kSumG = 4;                      // groups of 8 samples per warp
+constexpr int kSumBlocksPerSm = 16 / FEW_SUM_WARPS;      // resident blocks per SM, recurrence instantiation (register budget 65536 / (32 * 16))
+constexpr int kSumTabBlocksPerSm = 16 / FEW_SUM_WARPS;   // resident blocks per SM, table instantiation (16 x 32 lanes x 128 columns = all of tensor memory)
 constexpr int kTile = (kSumThreads / 32) * 8 * kSumG;   // samples per block
 #ifndef FEW_STAGE_STEPS
-#define FEW_STAGE_STEPS 4
+#define FEW_STAGE_STEPS 16
 #endif
-constexpr int kStageSteps = FEW_STAGE_STEPS;  // steps per stage (4 or 8)
+constexpr int kStageSteps = FEW_STAGE_STEPS;  // steps per stage.  Measured (config 1 kernel, B200): 4 steps x ring 4 1.128 ms, 8 x 3 1.110,
+                                              // 16 x 2 1.069, 20 x 2 1.063: what a stage boundary costs (warp barrier, done counter, mbarrier
+                                              // wait) is paid per stage, and the ring's depth does not matter (8 x 2, 8 x 3, 8 x 4 alike)
 constexpr int kStepD2 = 64;                   // a step's B fragments: [2][32 lanes] double2 = 1 KB
-constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + 128;   // + header: [i] descriptor of step i < 4, [4] steps in the stage
+constexpr int kHdrInts = kStageSteps < 32 ? 32 : 128;           // header: [i] descriptor of step i, [kStageSteps] steps in the stage
+constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + kHdrInts * 4;
 constexpr int kStageD2 = kStageBytes / 16;    // stage size in double2
 #ifndef FEW_RING
-#define FEW_RING 4
+#define FEW_RING 2
 #endif
 constexpr int kRing = FEW_RING;               // stages in flight per block
 
@@ -468,8 +470,8 @@ __global__ void __launch_bounds__(1024) few_sum_pack_kernel(const double2* __res
         step[32 + lane] = make_double2(b1s, b2s);
     }
     const int n_stages = stages_for(S);
-    for (int idx = threadIdx.x; idx < n_stages * 32; idx += blockDim.x) {     // header: [i] descriptor i, [4] steps in the stage
-        const int st = idx >> 5, q = idx & 31;
+    for (int idx = threadIdx.x; idx < n_stages * kHdrInts; idx += blockDim.x) {     // header: [i] descriptor i, [kStageSteps] steps in the stage
+        const int st = idx / kHdrInts, q = idx % kHdrInts;
         int v = 0;
         const int cnt = min(kStageSteps, S - st * kStageSteps);
         if (q == kStageSteps) v = cnt;
@@ -628,7 +630,8 @@ struct sum_smem {
     __align__(16) double2 zphi[kWarps][W];                      // Z_phi = exp(-i Phi_phi) per sample
     __align__(16) double2 rpow[kWarps][W][4];                   // rho, rho^2, rho^3, rho^4 per sample; after the loop: H_p, p = 0..3
     __align__(16) double2 pcur[kWarps][W];                      // P = Z_phi^m Z_theta^k of the current run, per sample
-    __align__(16) double2 hacc[kWarps][G][32];                  // per lane and group: H = sum over the closed runs
+    __align__(16) double2 hacc[kTab ? 1 : kWarps][G][32];       // per lane and group: H = sum over the closed runs (table mode: in rpow,
+                                                                // whose rho^1..4 are dead once the table is built; same index map)
     __align__(16) double2 kerr[kKerr ? kWarps : 1][2][kKerr ? W : 1];   // kKerr: Z_theta, the run's Z_phi^m, per sample
     unsigned tmem_base;                                         // kTab: the block's tensor-memory allocation (rho^nu table)
 };
@@ -645,7 +648,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     extern __shared__ __align__(128) unsigned char smem_raw[];
     smem_t& sm = *reinterpret_cast<smem_t*>(smem_raw);
     auto& ring = sm.ring; auto& full = sm.full; auto& done_s = sm.done; auto& zphi_s = sm.zphi; auto& rpow_s = sm.rpow;
-    auto& pcur_s = sm.pcur; auto& hacc_s = sm.hacc; auto& kerr_s = sm.kerr;
+    auto& pcur_s = sm.pcur; auto& kerr_s = sm.kerr;
     constexpr int n_ph = kKerr ? 3 : 2;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_seg = n_t - 1;
@@ -673,7 +676,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     };
 
     if (L.mode_count[kTab ? 1 : 0] == 0) return;       // no source in this instantiation's mode
-    constexpr unsigned kTmemCols = 16 * kTabSlots;     // 128 columns: (c, s) x G = 4 groups x kTabSlots slots per thread
+    constexpr unsigned kTmemCols = 16 * kTabSlots * ((kWarps + 3) / 4);     // 128 columns per warp: (c, s) x G = 4 groups x kTabSlots slots per thread
     if (kTab && warp == 0) tmem_alloc(&sm.tmem_base, kTmemCols);
     tile_rec cur, nxt;
     cur.p = -1; cur.n_stages = 0; cur.count = 0; cur.i_begin = 0; cur.src = 0; cur.mode = 0; cur.pad1 = 0;
@@ -693,7 +696,10 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (kTab) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();                        // the only block-wide barrier of the kernel (besides the one before the TMEM release)
     if (kTab) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const unsigned tmem_row = kTab ? sm.tmem_base + ((unsigned)(warp * 32) << 16) : 0u;   // this warp's lanes of the allocation
+    // this warp's lanes (32 (warp % 4) ...) and columns of the allocation
+    const unsigned tmem_row = kTab ? sm.tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(warp >> 2) * (16 * kTabSlots) : 0u;
+    // H of lane (row, col), group g: [g][lane] of the warp = [sample 8 g + row][col] of rpow (32 g + lane either way)
+    double2* const hacc_w = kTab ? &rpow_s[warp][0][0] : &sm.hacc[kTab ? 0 : warp][0][0];
     unsigned gst = 0;                       // stages consumed by this warp so far: ring slot gst % kRing, use number gst / kRing
 
     for (long long i = 0;; ++i) {
@@ -750,9 +756,18 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         // table mode: x_b = rho^(4 b + col) of this lane's samples, for the blocks b the source uses (slot -> block, ascending,
         // in L.blk_list), by the three-term recurrence (below), into the lane's own tensor-memory row: column 16 slot + 4 g
         // holds (c, s) of group g.  (Rolled loops: nothing here lives in a register array, and the code stays small.)
-        const int* blp = L.blk_list + (size_t)src * kTabSlots;
-        double2 xa[G], xb[G];                                       // x_b, x_{b-1} of the G groups: G independent chains
-        double twg[G];
+        const int4* blp = reinterpret_cast<const int4*>(L.blk_list + (size_t)src * kTabSlots);
+        const int4 bl0 = __ldg(blp), bl1 = __ldg(blp + 1);          // slot -> block, ascending, -1 = unused (blocks <= 255)
+        static_assert(kTabSlots == 8 && FEW_MAX_ABS_N / 4 < 256, "the block list is packed into 8 bytes");
+        unsigned long long bls = 0ull;                              // byte q = block of slot q; the byte after the last slot = 0xff..
+        int n_slots = 0;
+        {
+            const int bl[8] = {bl0.x, bl0.y, bl0.z, bl0.w, bl1.x, bl1.y, bl1.z, bl1.w};
+#pragma unroll
+            for (int q = 0; q < 8; ++q) if (bl[q] >= 0) { bls |= (unsigned long long)(unsigned)bl[q] << (8 * q); n_slots = q + 1; }
+        }
+        double2 xa[G], xb[G];                                       // x_b, x_{b-1} of the G groups: G independent chains,
+        double twg[G];                                              // stepped in place (ping-pong: no register moves)
 #pragma unroll
         for (int g = 0; g < G; ++g) {
             const int sx = 8 * g + row;
@@ -761,22 +776,28 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             xb[g] = make_double2(xm.x, -xm.y);
             twg[g] = 2.0 * rpow_s[warp][sx][3].x;
         }
-        int slot = 0, target = __ldg(blp);
+        int slot = 0, target = n_slots ? (int)(bls & 0xffu) : -1;
 #pragma unroll 1
-        for (int b = 0; target >= 0; ++b) {
-            if (b == target) {
+        for (int b = 0; target >= 0; b += 2) {
+            if (b == target) {                                      // x_b is in xa
 #pragma unroll
                 for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, xa[g]);
-                ++slot;
-                target = slot < kTabSlots ? __ldg(blp + slot) : -1;
+                ++slot; bls >>= 8;
+                target = slot < n_slots ? (int)(bls & 0xffu) : -1;
             }
 #pragma unroll
-            for (int g = 0; g < G; ++g) {
-                const double2 nx = make_double2(fma(twg[g], xa[g].x, -xb[g].x), fma(twg[g], xa[g].y, -xb[g].y));
-                xb[g] = xa[g]; xa[g] = nx;
+            for (int g = 0; g < G; ++g) { xb[g].x = fma(twg[g], xa[g].x, -xb[g].x); xb[g].y = fma(twg[g], xa[g].y, -xb[g].y); }
+            if (b + 1 == target) {                                  // x_{b+1} is in xb
+#pragma unroll
+                for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, xb[g]);
+                ++slot; bls >>= 8;
+                target = slot < n_slots ? (int)(bls & 0xffu) : -1;
             }
+#pragma unroll
+            for (int g = 0; g < G; ++g) { xa[g].x = fma(twg[g], xb[g].x, -xa[g].x); xa[g].y = fma(twg[g], xb[g].y, -xa[g].y); }
         }
         tmem_wait_st();
+        __syncwarp();                       // rho^1..4 have been read: their storage becomes H (below)
     }
 
     // Lane state, per group g (sample 8 g + row of the warp, unit column col).  S, D: accumulators of the run (C fragments:
@@ -796,7 +817,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             xc[g % GR] = 1.0; xs[g % GR] = 0.0; yc[g % GR] = 1.0; ys[g % GR] = 0.0;
         }
         accS[g] = accD[g] = make_double2(0.0, 0.0);
-        hacc_s[warp][g][lane] = make_double2(0.0, 0.0);
+        hacc_w[32 * g + lane] = make_double2(0.0, 0.0);
     }
     bool single = false;                    // the current run has m = 0: D = S
     int new_run_d = 0;                      // descriptor of a run whose P is still to be computed (0: none)
@@ -809,12 +830,17 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         const double2* bp = &ring[slot][0] + lane;
         const int* hdr = reinterpret_cast<const int*>(&ring[slot][0] + kStageSteps * kStepD2);
         int4 d4 = *reinterpret_cast<const int4*>(hdr), d8 = kStageSteps > 4 ? *(reinterpret_cast<const int4*>(hdr) + 1) : make_int4(0, 0, 0, 0);
-        static_assert(kStageSteps == 4 || kStageSteps == 8, "descriptor registers hold 4 or 8 steps");
+        static_assert(kStageSteps == 4 || kStageSteps == 8 || (kStageSteps > 8 && kStageSteps < 128), "descriptors: 4 or 8 in registers, more from the header");
         const int ns = hdr[kStageSteps];
         for (int si = 0; si < ns; ++si, bp += kStepD2) {
-            const int d = d4.x;
-            d4.x = d4.y; d4.y = d4.z; d4.z = d4.w;
-            if (kStageSteps > 4) { d4.w = d8.x; d8.x = d8.y; d8.y = d8.z; d8.z = d8.w; }
+            int d;
+            if (kStageSteps <= 8) {
+                d = d4.x;
+                d4.x = d4.y; d4.y = d4.z; d4.z = d4.w;
+                if (kStageSteps > 4) { d4.w = d8.x; d8.x = d8.y; d8.y = d8.z; d8.z = d8.w; }
+            } else {
+                d = hdr[si];
+            }
             const double2 b12c = bp[0], b12s = bp[32];              // issued first: in flight during the scalar work below
             double2 av[G];                                          // table mode: (c, s) of this lane's unit, per group
             if constexpr (kTab) {
@@ -827,10 +853,10 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                 for (int g = 0; g < G; ++g) {
                     const int sx = 8 * g + row;
                     const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
-                    double2 Hg = hacc_s[warp][g][lane];
+                    double2 Hg = hacc_w[32 * g + lane];
                     Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));              // H += P_r S + i P_i D
                     Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
-                    hacc_s[warp][g][lane] = Hg;
+                    hacc_w[32 * g + lane] = Hg;
                     accS[g] = accD[g] = make_double2(0.0, 0.0);
                     if (!kTab) {
                         const double2 x0 = col ? rpow_s[warp][sx][col - 1] : make_double2(1.0, 0.0), xm = rpow_s[warp][sx][3 - col];
@@ -908,7 +934,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     for (int g = 0; g < G; ++g) {                                   // close the last run; H_p of sample sx, power col -> shared
         const int sx = 8 * g + row;
         const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
-        double2 Hg = hacc_s[warp][g][lane];
+        double2 Hg = hacc_w[32 * g + lane];
         Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));
         Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
         rpow_s[warp][sx][col] = Hg;                                 // (rho^1..4 of this sample are not needed any more)
