@@ -63,7 +63,7 @@ constexpr int kNewRun = 1;                    // first step of a run (m, k): clo
 constexpr int kAdvShift = 1, kAdvBits = 12;   // multiplications by rho^4 before the step's DMMAs
 constexpr int kDmShift = 13, kDmBits = 7;     // m increment of a new run
 constexpr int kKShift = 20, kKBits = 7;       // polar index of the run, offset by 64 (Kerr-shaped lists, |k| <= FEW_MAX_ABS_K)
-constexpr int kSingle = 1 << 27;              // run with m = 0: no mirror, beta = 0, hence D = S and only S is accumulated
+constexpr int kSingle = 1 << 27;              // run with m = 0: no mirror, beta = 0, hence D = S: the c half is accumulated in S, the s half in D
 constexpr int kSlotShift = 28, kSlotBits = 3; // table slot of the step's block nu >> 2 (sources in table mode)
 constexpr int kTabSlots = 8;                  // distinct blocks nu >> 2 a source may use in table mode (the paper's grid: nu <= 31 -> 8)
 
@@ -819,10 +819,31 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         accS[g] = accD[g] = make_double2(0.0, 0.0);
         hacc_w[32 * g + lane] = make_double2(0.0, 0.0);
     }
-    bool single = false;                    // the current run has m = 0: D = S
+    bool single = false;                    // the current run has m = 0: D = S, and both accumulators gather S (c half, s half)
     int new_run_d = 0;                      // descriptor of a run whose P is still to be computed (0: none)
     bool odd = false;                       // (recurrence mode) the current block is in (yc, ys)
 
+    auto update_P = [&](const int dn) {      // P <- P Z_phi^dm (Z_theta^k): one lane per sample, exchanged through shared memory
+                const int dm = (dn >> kDmShift) & ((1 << kDmBits) - 1);
+                __syncwarp();                                       // every lane has read the old P (the close above)
+#pragma unroll
+                for (int q = 0; q < QW; ++q) {
+                    const int sx = q * 32 + lane;
+                    if (sx < W) {
+                        const double2 zp = zphi_s[warp][sx];
+                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
+                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
+                        if (kKerr) {                                // k < 0: conjugate powers
+                            kerr_s[warp][1][sx] = pm;
+                            const int kk = ((dn >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                            double2 zt = kerr_s[warp][0][sx];
+                            if (kk < 0) zt.y = -zt.y;
+                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
+                        }
+                        pcur_s[warp][sx] = pm;
+                    }
+                }
+    };
     for (int st = 0; st < n_stages; ++st) {
         const unsigned slot = gst % kRing;
         mbar_wait(&full[slot], (gst / kRing) & 1u);
@@ -852,7 +873,9 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
 #pragma unroll
                 for (int g = 0; g < G; ++g) {
                     const int sx = 8 * g + row;
-                    const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
+                    const double2 P = pcur_s[warp][sx];
+                    if (single) { accS[g].x += accD[g].x; accS[g].y += accD[g].y; accD[g] = accS[g]; }
+                    const double2 dd_ = accD[g];
                     double2 Hg = hacc_w[32 * g + lane];
                     Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));              // H += P_r S + i P_i D
                     Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
@@ -887,9 +910,14 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
 #pragma unroll
                 for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].x, b12c.y);
             }
+            // m = 0: the s half goes to the idle D accumulators (S = accS + accD at the close), so that two DMMAs on one
+            // accumulator are 8 instructions apart, as in the other runs, instead of 4 (a dependent DMMA waits ~200 cycles)
+            if (single) {
 #pragma unroll
-            for (int g = 0; g < G; ++g) dmma884(accS[g], av[g].y, b12s.x);
-            if (!single) {
+                for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].y, b12s.x);
+            } else {
+#pragma unroll
+                for (int g = 0; g < G; ++g) dmma884(accS[g], av[g].y, b12s.x);
 #pragma unroll
                 for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].y, b12s.y);
             }
@@ -900,25 +928,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                 // beat 16 without (measured).
                 const int dn = new_run_d;
                 new_run_d = 0;
-                const int dm = (dn >> kDmShift) & ((1 << kDmBits) - 1);
-                __syncwarp();                                       // every lane has read the old P (the close above)
-#pragma unroll
-                for (int q = 0; q < QW; ++q) {
-                    const int sx = q * 32 + lane;
-                    if (sx < W) {
-                        const double2 zp = zphi_s[warp][sx];
-                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
-                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
-                        if (kKerr) {                                // k < 0: conjugate powers
-                            kerr_s[warp][1][sx] = pm;
-                            const int kk = ((dn >> kKShift) & ((1 << kKBits) - 1)) - 64;
-                            double2 zt = kerr_s[warp][0][sx];
-                            if (kk < 0) zt.y = -zt.y;
-                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
-                        }
-                        pcur_s[warp][sx] = pm;
-                    }
-                }
+                update_P(dn);
                 __syncwarp();
             }
         }
@@ -933,7 +943,9 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
 #pragma unroll
     for (int g = 0; g < G; ++g) {                                   // close the last run; H_p of sample sx, power col -> shared
         const int sx = 8 * g + row;
-        const double2 P = pcur_s[warp][sx], dd_ = single ? accS[g] : accD[g];
+        const double2 P = pcur_s[warp][sx];
+        if (single) { accS[g].x += accD[g].x; accS[g].y += accD[g].y; accD[g] = accS[g]; }
+        const double2 dd_ = accD[g];
         double2 Hg = hacc_w[32 * g + lane];
         Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));
         Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
