@@ -820,30 +820,8 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         hacc_w[32 * g + lane] = make_double2(0.0, 0.0);
     }
     bool single = false;                    // the current run has m = 0: D = S, and both accumulators gather S (c half, s half)
-    int new_run_d = 0;                      // descriptor of a run whose P is still to be computed (0: none)
     bool odd = false;                       // (recurrence mode) the current block is in (yc, ys)
 
-    auto update_P = [&](const int dn) {      // P <- P Z_phi^dm (Z_theta^k): one lane per sample, exchanged through shared memory
-                const int dm = (dn >> kDmShift) & ((1 << kDmBits) - 1);
-                __syncwarp();                                       // every lane has read the old P (the close above)
-#pragma unroll
-                for (int q = 0; q < QW; ++q) {
-                    const int sx = q * 32 + lane;
-                    if (sx < W) {
-                        const double2 zp = zphi_s[warp][sx];
-                        double2 pm = kKerr ? kerr_s[warp][1][sx] : pcur_s[warp][sx];
-                        for (int e = 0; e < dm; ++e) pm = cmul(pm, zp);
-                        if (kKerr) {                                // k < 0: conjugate powers
-                            kerr_s[warp][1][sx] = pm;
-                            const int kk = ((dn >> kKShift) & ((1 << kKBits) - 1)) - 64;
-                            double2 zt = kerr_s[warp][0][sx];
-                            if (kk < 0) zt.y = -zt.y;
-                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm = cmul(pm, zt);
-                        }
-                        pcur_s[warp][sx] = pm;
-                    }
-                }
-    };
     for (int st = 0; st < n_stages; ++st) {
         const unsigned slot = gst % kRing;
         mbar_wait(&full[slot], (gst / kRing) & 1u);
@@ -862,34 +840,74 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             } else {
                 d = hdr[si];
             }
-            const double2 b12c = bp[0], b12s = bp[32];              // issued first: in flight during the scalar work below
+            double2 b12c, b12s;
             double2 av[G];                                          // table mode: (c, s) of this lane's unit, per group
-            if constexpr (kTab) {
-                const int ts = (d >> kSlotShift) & ((1 << kSlotBits) - 1);
-                static_assert(!kTab || G == 4, "the table instantiation is written for G = 4 (16 columns per slot)");
-                tmem_ld_x16(tmem_row + 16 * ts, av);
-            }
+            auto load_step = [&]() {
+                b12c = bp[0]; b12s = bp[32];
+                if constexpr (kTab) {
+                    const int ts = (d >> kSlotShift) & ((1 << kSlotBits) - 1);
+                    static_assert(!kTab || G == 4, "the table instantiation is written for G = 4 (16 columns per slot)");
+                    tmem_ld_x16(tmem_row + 16 * ts, av);
+                }
+            };
             if (d & kNewRun) {      // rare (once per (m, k)): close the previous run, new P, (recurrence) x restarts from rho^col
+                // One burst: every shared-memory operand first (P and H of the 4 groups; Z_phi and P of the lane's own sample),
+                // then the scalar FP64 instructions in waves of independent ones (the new P's complex product, the 2 G inner
+                // and the 2 G outer FMAs of H += P_r S + i P_i D), then the stores.  A warp that stalls between two FP64
+                // instructions waits ~200 cycles behind the other warps' DMMAs before the pipe takes its next one
+                // (profiles/r02_sum_kernel.md), so the close costs one such wait instead of one per group; and it runs BEFORE
+                // this step's operand loads, while their 24 registers are free (with them live ptxas copied the 16 table
+                // registers of every step: slower than no burst at all).
+                {
+                    double2 Pg[G], Hg[G];
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                    const int sx = 8 * g + row;
-                    const double2 P = pcur_s[warp][sx];
-                    if (single) { accS[g].x += accD[g].x; accS[g].y += accD[g].y; accD[g] = accS[g]; }
-                    const double2 dd_ = accD[g];
-                    double2 Hg = hacc_w[32 * g + lane];
-                    Hg.x = fma(P.x, accS[g].x, fma(-P.y, dd_.y, Hg.x));              // H += P_r S + i P_i D
-                    Hg.y = fma(P.x, accS[g].y, fma(P.y, dd_.x, Hg.y));
-                    hacc_w[32 * g + lane] = Hg;
-                    accS[g] = accD[g] = make_double2(0.0, 0.0);
-                    if (!kTab) {
-                        const double2 x0 = col ? rpow_s[warp][sx][col - 1] : make_double2(1.0, 0.0), xm = rpow_s[warp][sx][3 - col];
-                        xc[g % GR] = x0.x; xs[g % GR] = x0.y; yc[g % GR] = xm.x; ys[g % GR] = -xm.y;
+                    for (int g = 0; g < G; ++g) { Pg[g] = pcur_s[warp][8 * g + row]; Hg[g] = hacc_w[32 * g + lane]; }
+                    // the new run's P = P Z_phi^dm (Z_theta^k), one lane per sample, in the same burst: operands first
+                    static_assert(W == 32, "one lane per sample");
+                    const double2 zp1 = zphi_s[warp][lane];
+                    double2 pm1 = kKerr ? kerr_s[warp][1][lane] : pcur_s[warp][lane];
+                    double2 zt1 = kKerr ? kerr_s[warp][0][lane] : make_double2(1.0, 0.0);
+                    __syncwarp();                                   // every lane has read the old P
+                    {
+                        const int dm = (d >> kDmShift) & ((1 << kDmBits) - 1);
+                        for (int e = 0; e < dm; ++e) pm1 = cmul(pm1, zp1);
+                        if (kKerr) {
+                            kerr_s[warp][1][lane] = pm1;
+                            const int kk = ((d >> kKShift) & ((1 << kKBits) - 1)) - 64;
+                            if (kk < 0) zt1.y = -zt1.y;
+                            for (int e = 0; e < (kk < 0 ? -kk : kk); ++e) pm1 = cmul(pm1, zt1);
+                        }
+                        pcur_s[warp][lane] = pm1;
+                    }
+                    if (single) {
+#pragma unroll
+                        for (int g = 0; g < G; ++g) { accS[g].x += accD[g].x; accS[g].y += accD[g].y; accD[g] = accS[g]; }
+                    }
+#pragma unroll
+                    for (int g = 0; g < G; ++g) {
+                        Hg[g].x = fma(-Pg[g].y, accD[g].y, Hg[g].x);
+                        Hg[g].y = fma(Pg[g].y, accD[g].x, Hg[g].y);
+                    }
+#pragma unroll
+                    for (int g = 0; g < G; ++g) {
+                        Hg[g].x = fma(Pg[g].x, accS[g].x, Hg[g].x);
+                        Hg[g].y = fma(Pg[g].x, accS[g].y, Hg[g].y);
+                    }
+#pragma unroll
+                    for (int g = 0; g < G; ++g) {
+                        hacc_w[32 * g + lane] = Hg[g]; accS[g] = accD[g] = make_double2(0.0, 0.0);
+                        if (!kTab) {
+                            const int sx = 8 * g + row;
+                            const double2 x0 = col ? rpow_s[warp][sx][col - 1] : make_double2(1.0, 0.0), xm = rpow_s[warp][sx][3 - col];
+                            xc[g % GR] = x0.x; xs[g % GR] = x0.y; yc[g % GR] = xm.x; ys[g % GR] = -xm.y;
+                        }
                     }
                 }
-                new_run_d = d;                                      // the new P is computed after this step's DMMAs are issued
+                __syncwarp();                                       // the new P is visible to the next close
                 single = (d & kSingle) != 0;
                 odd = false;
             }
+            load_step();
             if (!kTab) {
                 for (int adv = (d >> kAdvShift) & ((1 << kAdvBits) - 1); adv > 0; --adv) {   // usually once: block b -> b + 1, over block b - 1
                     if (!odd) {
@@ -920,16 +938,6 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
                 for (int g = 0; g < G; ++g) dmma884(accS[g], av[g].y, b12s.x);
 #pragma unroll
                 for (int g = 0; g < G; ++g) dmma884(accD[g], av[g].y, b12s.y);
-            }
-            if (new_run_d) {
-                // new P = Z_phi^m Z_theta^k of the run that has just started (its close, one run later, is the first reader): after
-                // the step's DMMAs, so that the exchange through shared memory runs beside them instead of in front of them.
-                // ONE lane per sample: scalar FP64 instructions are dear next to DMMAs, and 4 of them plus two warp barriers
-                // beat 16 without (measured).
-                const int dn = new_run_d;
-                new_run_d = 0;
-                update_P(dn);
-                __syncwarp();
             }
         }
         __syncwarp();                                               // every lane has read the slot
