@@ -403,6 +403,25 @@ def test_sum_batch_mixing_table_and_recurrence_sources(api):
         assert rel_l2(h[s], ref) <= REL_L2_TOL and mismatch(h[s], ref) <= MISMATCH_TOL, s
 
 
+@pytest.mark.parametrize("ms", [(0,), (2, 5), (0, 4)])
+def test_sum_lists_of_m0_runs_only_and_without_m0(api, ms):
+    """Runs with m = 0 accumulate the c half of a step in S and the s half in D (summed at the close); other runs keep S and D
+    apart.  Lists made of m = 0 runs only, without any, and with an m increment above 1, long enough (8 nu-blocks per run) to
+    cross the 16-step stages of the coefficient ring."""
+    rng = np.random.default_rng(21 + sum(ms))
+    modes = [(l, m, n) for m in ms for l in (max(2, m), max(2, m) + 1, max(2, m) + 3) for n in range(-31, 32, 3)]
+    l, m, n = (np.asarray(x, np.int32) for x in zip(*modes))
+    n_t = 10
+    t = np.sort(rng.uniform(0, 900.0, n_t)); t[0] = 0.0
+    amp = (rng.normal(size=(1, n_t, len(l))) + 1j * rng.normal(size=(1, n_t, len(l)))) * 10.0 ** rng.uniform(-2, 0, (1, 1, len(l)))
+    phase = np.stack([0.23 * t + 1.5e-4 * t ** 2, 0.19 * t + 0.7e-4 * t ** 2], axis=1)[None]
+    w = synth.Workload("m_runs", t[None], phase, amp, l, m, n, np.array([1.1]), np.array([5.0]), 2.0, 0.53, 1700, 0.0)
+    h, keep, nk = run_gpu_chain(api, w)
+    ref = oracle.waveform(w)
+    assert nk[0] == w.n_modes and rel_l2(h[0], ref[0]) <= REL_L2_TOL and mismatch(h[0], ref[0]) <= MISMATCH_TOL
+    assert np.max(np.abs(h[0] - ref[0])) <= 1e-10 * np.max(np.abs(ref[0]))
+
+
 def test_sum_large_n_and_sparse_list_limit(api):
     """|n| up to FEW_MAX_ABS_N = 1023 (256 steps of the three-term recurrence: error <= 256^2 ulp) is summed; a list with
     fewer than 4 modes per step and more than 64 steps over n_modes / 4 does not fit the step capacity and is reported."""
