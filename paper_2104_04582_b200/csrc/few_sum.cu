@@ -14,10 +14,11 @@
 //   B2c = (alpha+ + alpha-) - (beta+ + beta-),   B2s = i(alpha+ - alpha-) - i(beta- - beta+).
 // S and D are [samples] x [4 powers of dx x (re, im)] = sum over units of [samples x units] . [units x 8]: a small dense FP64
 // contraction per sample tile, executed as DMMA.8x8x4 (mma.sync.m8n8k4.f64) on the FP64 pipe -- 8 samples x 4 consecutive nu
-// per instruction; a lane carries (c_nu, s_nu) of ONE sample and ONE of the four nu and steps it by rho^4 (2 DMUL + 2 DFMA)
-// between the 4 DMMAs of a step.  Per sample and unit: 32 FMA in DMMAs + 4 scalar FP64 operations (40 scalar operations in
-// the per-(m,n)-pair DFMA form this replaces).  The same IEEE FMA arithmetic on the same pipe; what changes is that a DMMA
-// reads 4 registers per 8 FMA where a DFMA reads 3 per FMA, which is what held the DFMA form at 0.75 of the pipe.
+// per instruction; a lane carries (c_nu, s_nu) of ONE sample and ONE of the four nu, read from a per-tile table of rho^nu in
+// tensor memory (or, for lists with more than 8 nu-blocks, stepped by a three-term recurrence in registers).  Per sample and
+// unit: 32 FMA in DMMAs (40 scalar operations in the per-(m,n)-pair DFMA form this replaces).  The same IEEE FMA arithmetic on
+// the same pipe; what changes is that a DMMA reads 4 registers per 8 FMA where a DFMA reads 3 per FMA, which is what held the
+// DFMA form at 0.75 of the pipe.
 //
 // Three launches per call, all on the caller's stream, nothing read back to the host:
 //   1. few_sum_plan_kernel  (one block per source): clips the dense sample grid to the sparse segments and prefix-sums
@@ -609,16 +610,17 @@ __device__ __forceinline__ tile_rec load_rec(const tile_rec* p, const int2* __re
 // a warp owns 8 G samples of every tile of its block (tile = 4 warps x 8 G samples inside one sparse segment of one source,
 // so the coefficients are block-uniform), evaluates their phases, runs the step loop and stores their h, and never meets
 // another warp at a barrier.  Tiles are assigned statically (block b takes tiles b, b + grid, ...; every tile of a source
-// costs the same), each warp reads the tile records itself, one tile ahead.  Ring protocol: full[slot] is an mbarrier the
+// costs the same), each warp reads the tile records itself, two tiles ahead.  Ring protocol: full[slot] is an mbarrier the
 // TMA bulk copy completes; when a warp is done with a slot it bumps done[slot], and the LAST of the 4 warps refills the slot
 // with the stage kRing ahead in the block's stage stream (walking into the next tiles' records where the stream crosses a
-// tile boundary).  So warps drift apart by at most the ring depth and wait only for data.
+// tile boundary).  So warps drift apart by at most the ring depth and wait only for data.  (Blocks of 8 or 16 warps --
+// FEW_SUM_WARPS, one ring for more warps and longer stages -- are parity-green and 1-4 % slower on short kept lists.)
 // G: groups of 8 samples per warp.  kKerr: Kerr-shaped mode lists (Eq. (1), Eq. (19)): a third phase factor
 // Z_theta, runs are (m, k) with P = Z_phi^m Z_theta^k.  The hot loop is the same.
 // kTab: where the A operands (c, s) = rho^nu come from.  On the FP64 pipe a scalar instruction issued between the DMMAs of
-// other warps costs about 5 cycles, not 2, so the table instantiation computes rho^nu of every sample
-// ONCE per tile -- rho^nu does not depend on the run (m, k) -- into a per-warp shared-memory table in DMMA fragment order
-// and the step loop is loads and DMMAs only; it takes the sources whose lists use at most kTabSlots distinct blocks nu >> 2
+// other warps costs far more than its two cycles, so the table instantiation computes rho^nu of every
+// sample ONCE per tile -- rho^nu does not depend on the run (m, k) -- into the warp's rows of the block's tensor-memory
+// allocation, in DMMA fragment order, and the step loop is loads and DMMAs only; it takes the sources whose lists use at most kTabSlots distinct blocks nu >> 2
 // (the paper's grid: nu <= 31).  The recurrence instantiation steps x_b = rho^(4 b + col) in registers (2 DFMA per group and
 // step) and takes every other source.  Both are launched; each works on the tiles whose record names its mode.
 template <int G, bool kKerr, bool kTab>
