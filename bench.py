@@ -201,6 +201,28 @@ class Bench:
             torch.cuda.synchronize()
         return [a.elapsed_time(b) for a, b in ev], sum_ms, launches
 
+    def graph_replay(self, steps, flush):
+        """The same step captured once into a CUDA graph (few_waveform is capturable: one stream, two forked and joined side
+        streams, no host synchronisation, no allocation) and replayed: what is left of the CPU's share of the 12 launches."""
+        torch, api = self.torch, self.api
+        api.few_profile_enable(False)                   # the profiling events are not part of the captured work
+        try:
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                self.step()
+            for _ in range(3):
+                flush.fill_(1); graph.replay()
+            torch.cuda.synchronize()
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for a, b in ev:
+                flush.fill_(1)
+                a.record(); graph.replay(); b.record()
+            torch.cuda.synchronize()
+            del graph
+            return float(np.mean([a.elapsed_time(b) for a, b in ev]))
+        finally:
+            api.few_profile_enable(True)
+
     def e2e(self, reps, device_index):
         """The same step through few_waveform_host (C ABI, HOST pointers): H2D + kernels + D2H inside the call."""
         torch, api, w, p = self.torch, self.api, self.w, self.pinned
@@ -598,6 +620,13 @@ def main():
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "note": "few_waveform_host (C ABI, host pointers): H2D of the sparse inputs + kernels + D2H of h, pinned host buffers"}
 
+    graph_ms = None
+    if world == 1 and not args.no_e2e:
+        try:
+            graph_ms = bench.graph_replay(args.steps, flush)
+        except Exception as exc:                      # a measurement aid: the line stays valid without it
+            graph_ms = f"unavailable: {exc}"
+
     hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
     stages = None
     if args.stages and rank == 0:
@@ -651,6 +680,10 @@ def main():
            "ms_per_waveform": ms_per_step / w_full.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
            "gpu_launches": int(launches), "gpu_launches_note": "counted by the library at its launch sites (few_launch_count) over the timed steps of this rank",
            "clocks": clocks, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
+    if graph_ms is not None:
+        out["graph_replay"] = {"ms_per_step": graph_ms,
+                               "note": "the same few_waveform call captured once into a CUDA graph and replayed (L2 flushed, CUDA events): "
+                                       "the step without the host's share of its launches; `value` and `ms_per_step` are the plain call"}
     if stages is not None:
         for v in stages.values():
             if "gbs" in v:

@@ -605,6 +605,34 @@ def test_config4_full_size_sampled_parity_eps_sweep(api, eps):
     print(f"config 4 eps={eps:g}: kept {int(nk[0])}, windowed rel-L2 {rel_l2(got, refs):.3e}")
 
 
+def test_whole_path_under_cuda_graph_capture(api):
+    """few_waveform enqueues everything on the caller's stream and two internal side streams forked and joined by events, never
+    synchronises the host and allocates nothing: the call can be captured into a CUDA graph.  A replay on new input values gives
+    the bits of the eager call."""
+    w = synth.make_config(1)
+    n = 40_000
+    g = gpu_inputs(w)
+    args = lambda amp: (g["t"], g["phase"], amp, g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0 + 3.0e6, w.dt, n)
+    ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, n), dtype=torch.uint8, device=g["t"].device)
+    h_g = torch.zeros((w.n_src, n), dtype=torch.complex128, device=g["t"].device)
+    amp_g = g["amp"].clone()
+    api.few_profile_enable(False)
+    api.few_waveform(*args(amp_g), out=h_g, workspace=ws)                 # warm-up outside the capture (attributes, lazy loading)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        api.few_waveform(*args(amp_g), out=h_g, workspace=ws)
+    for scale in (1.0, 0.5):
+        amp_g.copy_(g["amp"] * scale)
+        h_g.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        h_e = api.few_waveform(*args(g["amp"] * scale))
+        api.few_device_status()
+        assert torch.equal(h_g, h_e), scale
+    assert float(h_g.abs().max()) > 0.0
+
+
 def test_fp64_peak_probe_runs(api):
     """The one measurement aid left in the ABI (the roofline denominator bench.py prints beside the nominal peak) launches,
     writes finite values and sustains a plausible FP64 rate; no throughput ordering is asserted."""
