@@ -768,8 +768,8 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
 #pragma unroll
             for (int q = 0; q < 8; ++q) if (bl[q] >= 0) { bls |= (unsigned long long)(unsigned)bl[q] << (8 * q); n_slots = q + 1; }
         }
-        double2 xa[G], xb[G];                                       // x_b, x_{b-1} of the G groups: G independent chains,
-        double twg[G];                                              // stepped in place (ping-pong: no register moves)
+        double2 xa[G], xb[G];                                       // x_b, x_{b-1} of the G groups: G independent chains
+        double twg[G];
 #pragma unroll
         for (int g = 0; g < G; ++g) {
             const int sx = 8 * g + row;
@@ -779,24 +779,30 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
             twg[g] = 2.0 * rpow_s[warp][sx][3].x;
         }
         int slot = 0, target = n_slots ? (int)(bls & 0xffu) : -1;
+        // four levels of the recurrence at a time, their 32 DFMA back to back, then the stores of those of the four blocks that
+        // the list uses: a warp that leaves the FP64 pipe between two levels (the stores, a branch) waits for it again
 #pragma unroll 1
-        for (int b = 0; target >= 0; b += 2) {
-            if (b == target) {                                      // x_b is in xa
+        for (int b = 0; target >= 0; b += 4) {
+            double2 l1[G], l2[G], l3[G], l4[G];
 #pragma unroll
-                for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, xa[g]);
-                ++slot; bls >>= 8;
-                target = slot < n_slots ? (int)(bls & 0xffu) : -1;
+            for (int g = 0; g < G; ++g) { l1[g].x = fma(twg[g], xa[g].x, -xb[g].x); l1[g].y = fma(twg[g], xa[g].y, -xb[g].y); }
+#pragma unroll
+            for (int g = 0; g < G; ++g) { l2[g].x = fma(twg[g], l1[g].x, -xa[g].x); l2[g].y = fma(twg[g], l1[g].y, -xa[g].y); }
+#pragma unroll
+            for (int g = 0; g < G; ++g) { l3[g].x = fma(twg[g], l2[g].x, -l1[g].x); l3[g].y = fma(twg[g], l2[g].y, -l1[g].y); }
+#pragma unroll
+            for (int g = 0; g < G; ++g) { l4[g].x = fma(twg[g], l3[g].x, -l2[g].x); l4[g].y = fma(twg[g], l3[g].y, -l2[g].y); }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (b + q == target) {
+#pragma unroll
+                    for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, q == 0 ? xa[g] : q == 1 ? l1[g] : q == 2 ? l2[g] : l3[g]);
+                    ++slot; bls >>= 8;
+                    target = slot < n_slots ? (int)(bls & 0xffu) : -1;
+                }
             }
 #pragma unroll
-            for (int g = 0; g < G; ++g) { xb[g].x = fma(twg[g], xa[g].x, -xb[g].x); xb[g].y = fma(twg[g], xa[g].y, -xb[g].y); }
-            if (b + 1 == target) {                                  // x_{b+1} is in xb
-#pragma unroll
-                for (int g = 0; g < G; ++g) tmem_st_x4(tmem_row + 16 * slot + 4 * g, xb[g]);
-                ++slot; bls >>= 8;
-                target = slot < n_slots ? (int)(bls & 0xffu) : -1;
-            }
-#pragma unroll
-            for (int g = 0; g < G; ++g) { xa[g].x = fma(twg[g], xb[g].x, -xa[g].x); xa[g].y = fma(twg[g], xb[g].y, -xa[g].y); }
+            for (int g = 0; g < G; ++g) { xb[g] = l3[g]; xa[g] = l4[g]; }
         }
         tmem_wait_st();
         __syncwarp();                       // rho^1..4 have been read: their storage becomes H (below)
