@@ -40,7 +40,7 @@ FLOP_PER_PAIR = 38.0          # executed algorithm: per sa
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch: static figures from `ncu --set full` captures (the
 # run itself does not measure them); the coefficient stream and h stay in the 126 MB L2 while the kernel runs
-SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 8.15e6, "config2_1yr_allmodes": 13.72e6}
+SUM_KERNEL_DRAM_TRAFFIC = {"config1_1yr_eps1e-5": 8.14e6, "config2_1yr_allmodes": 13.46e6}
 SUM_KERNEL_DRAM_TRAFFIC_SOURCE = "profiles/r02_sum_kernel.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum; static, not measured by this run)"
 
 
