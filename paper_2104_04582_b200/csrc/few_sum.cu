@@ -757,11 +757,11 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
     if (kTab) {
         // table mode: x_b = rho^(4 b + col) of this lane's samples, for the blocks b the source uses (slot -> block, ascending,
         // in L.blk_list), by the three-term recurrence (below), into the lane's own tensor-memory row: column 16 slot + 4 g
-        // holds (c, s) of group g.  (Rolled loops: nothing here lives in a register array, and the code stays small.)
+        // holds (c, s) of group g.  (A rolled loop of four levels: the per-tile code must stay small for the instruction caches.)
         const int4* blp = reinterpret_cast<const int4*>(L.blk_list + (size_t)src * kTabSlots);
         const int4 bl0 = __ldg(blp), bl1 = __ldg(blp + 1);          // slot -> block, ascending, -1 = unused (blocks <= 255)
         static_assert(kTabSlots == 8 && FEW_MAX_ABS_N / 4 < 256, "the block list is packed into 8 bytes");
-        unsigned long long bls = 0ull;                              // byte q = block of slot q; the byte after the last slot = 0xff..
+        unsigned long long bls = 0ull;                              // byte q = block of slot q, n_slots of them
         int n_slots = 0;
         {
             const int bl[8] = {bl0.x, bl0.y, bl0.z, bl0.w, bl1.x, bl1.y, bl1.z, bl1.w};
