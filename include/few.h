@@ -182,6 +182,30 @@ size_t few_inner_products_workspace(int n_src, long long n_samples);
 int few_inner_products(few_ctx* ctx, const double* d, const double* h, int n_src, long long n_samples, double dt,
                        double* inner, void* workspace, size_t workspace_bytes, void* stream);
 
+/* few_inner_products for callers that cannot allocate device memory.  few_inner_products wants a workspace, so somebody has to
+ * call an allocator first.  Not every caller may: host code running where the CUDA runtime rejects allocation calls, a sampler
+ * whose whole device-memory budget sits in a pool it must not grow, a plug-in that is handed device pointers by its host
+ * application and has no allocator of its own.  This variant takes inputs and outputs only and keeps its per-chunk partial sums
+ * in an array that is part of the library's device image.  It calls no cudaMalloc, cudaFree or allocating library routine.
+ *   - Result: inner[n_src][3], bit-identical to few_inner_products on the same d, h, dt (same kernels, same reduction order).
+ *   - Limit: n_src * ceil(n_samples / 2048) <= FEW_INNER_STATIC_MAX_CHUNKS (one source of up to 33 554 432 samples -- 10 years at
+ *     10 s -- or e.g. 16 sources of 2 097 152); beyond it the call fails with FEW_ERR_LIMIT before touching the GPU, and
+ *     few_last_error() says so.  The array costs FEW_INNER_STATIC_MAX_CHUNKS * 32 B = 512 KB of device memory on every GPU that
+ *     loads the library, from load to process exit, whether this function is called or not.
+ *   - ctx may be NULL (few_create allocates, so a caller that cannot allocate may have no context); if given it must belong to
+ *     the current device and only counts the two launches.  d, h, inner and stream must belong to the calling thread's CURRENT
+ *     device: the scratch array used is the current device's copy.
+ *   - Set-up: the first call made on each device asks the CUDA runtime for the device address of the array (cudaGetSymbolAddress,
+ *     return code checked, cached per device under a lock).  Make that first call outside any stream capture.
+ *   - The array is shared by every call in the process and keeps the previous call's contents.  Nothing in it needs clearing:
+ *     each call overwrites every slot it later reads.  For the same reason two calls whose kernels can overlap on one GPU
+ *     (different streams, or different host threads) race on it and give garbage: keep calls on one device ordered, on one stream
+ *     or with events.  Calls on different GPUs are independent.
+ *   - n_samples = 0 zeroes inner (cudaMemsetAsync) as few_inner_products does.  Other errors as few_inner_products. */
+#define FEW_INNER_STATIC_MAX_CHUNKS 16384
+int few_inner_products_static(few_ctx* ctx, const double* d, const double* h, int n_src, long long n_samples, double dt,
+                              double* inner, void* stream);
+
 /* ---- NEXT-3: direct (non-interpolated) summation: amplitudes and phases given at every output sample.
  *   h_i = scale * factor * sum_j [ Y+_j W_ij + (m_j > 0) (-1)^{l_j} Y-_j conj(W_ij) ],  W_ij = A_ij exp(-i(m_j Phi_phi,i + n_j Phi_r,i)).
  * amp[n_src][n_samples][n_modes][2] (modes fastest: the amplitude module's layout); phase[n_src][n_samples][2] =

@@ -21,7 +21,7 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_ylm_modes", "few_spline_fit_workspace", "few_spline_fit", "few_spline_fit_dd", "few_select_modes_workspace", "few_select_modes",
            "few_sum_waveform_workspace", "few_sum_waveform", "few_waveform_workspace", "few_waveform", "few_waveform_host",
            "few_fp64_peak_probe", "few_launch_count", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
-           "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_waveform_ssb", "few_sum_direct_workspace",
+           "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_inner_products_static", "few_waveform_ssb", "few_sum_direct_workspace",
            "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr", "few_spline_fit_ragged", "few_spline_fit_dd_ragged",
            "few_select_modes_ragged", "few_sum_waveform_ragged", "few_waveform_ragged", "few_waveform_host_ragged"]
 
@@ -71,6 +71,7 @@ def _load() -> C.CDLL:
         "few_frame_rotate": (i, [vp, vp, vp, i, ll, vp, vp]),
         "few_inner_products_workspace": (sz, [i, ll]),
         "few_inner_products": (i, [vp, vp, vp, i, ll, d, vp, vp, sz, vp]),
+        "few_inner_products_static": (i, [vp, vp, vp, i, ll, d, vp, vp]),
         "few_waveform_ssb": (i, [vp] * 9 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, vp, vp, sz, vp]),
         "few_sum_direct_workspace": (sz, [i, i]),
         "few_sum_direct": (i, [vp] * 10 + [ll, i, i, vp, vp, sz, vp]),
@@ -275,6 +276,28 @@ def few_inner_products(d, h, dt: float, workspace=None):
     _chk(_lib.few_inner_products(context(), _p(d, torch.complex128), _p(h, torch.complex128), n_src, int(n_samples), float(dt),
                                  _p(inner), _p(ws), ws.numel(), _stream()), "few_inner_products")
     return inner
+
+
+INNER_STATIC_MAX_CHUNKS = 16384     # FEW_INNER_STATIC_MAX_CHUNKS of include/few.h
+
+
+def few_inner_products_static(d, h, dt: float, out, use_context: bool = True):
+    """few_inner_products without a workspace, for callers that may not allocate device memory (code running where the CUDA
+    runtime refuses allocations, a sampler whose memory pool must not grow, a plug-in without an allocator of its own).
+
+    d, h [n_src, n_samples] c128 and the result buffer `out` [n_src, 3] f64 are the caller's; this binding allocates nothing
+    either, which is why `out` is required.  The partial sums go to a 512 KB array built into the library, so the call is
+    limited to n_src * ceil(n_samples / 2048) <= INNER_STATIC_MAX_CHUNKS (FewError with FEW_ERR_LIMIT beyond) and two calls
+    that could run at the same time on one GPU (two streams, two threads) would corrupt each other: keep them on one stream.
+    The first call on a device looks up the array's device address; make it before any stream capture.
+    use_context=False passes ctx = NULL, as a caller that never ran few_create (which allocates) would.  Returns `out`."""
+    n_src, n_samples = h.shape
+    if tuple(out.shape) != (n_src, 3):
+        raise ValueError("out must be [n_src, 3]")
+    ctx = context() if use_context else None
+    _chk(_lib.few_inner_products_static(ctx, _p(d, torch.complex128), _p(h, torch.complex128), n_src, int(n_samples), float(dt),
+                                        _p(out, torch.float64), _stream()), "few_inner_products_static")
+    return out
 
 
 def few_waveform_ssb(t, phase, amp, l, m, n, sky, eps: float, t0: float, dt: float, n_samples: int, mu_over_dl=None, d=None,

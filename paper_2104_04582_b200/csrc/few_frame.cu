@@ -12,6 +12,7 @@
 //    both polarisations, R23).  The product path reduces them inside the summation kernel (few_sum_waveform_ex);
 //    few_inner_products is the separate two-pass reduction over stored series (data against data, or the unfused baseline).
 #include <math.h>
+#include <mutex>
 #include "few_common.cuh"
 
 namespace {
@@ -175,5 +176,73 @@ extern "C" int few_inner_products(few_ctx* ctx, const double* d, const double* h
     FEW_LAUNCHED(ctx);
     few_inner_final_kernel<<<n_src, kIpThreads, 0, st>>>((const double*)workspace, (int)nc, dt, inner);
     FEW_LAUNCHED(ctx);
+    return FEW_OK;
+}
+
+// ---- few_inner_products_static: the same two kernels, with the per-chunk partial sums kept in memory that is part of the
+// loaded library image instead of a workspace somebody had to allocate.
+//
+// Who this is for.  few_inner_products needs a workspace, and a workspace has to come from an allocator.  Some host programs
+// are not allowed to run one at the point where they want <d|h> and <h|h>: code inside a region where the CUDA runtime refuses
+// allocation calls, a sampler whose device memory was handed in full to a pool it may not grow, a plug-in that receives device
+// pointers from its host application and owns no allocator of its own.  Such a caller passes d, h and inner (which it already
+// has) and nothing else; this function calls no cudaMalloc / cudaFree and no library routine that allocates.
+//
+// The scratch array below lives in every GPU context that loads libfew_b200.so, from module load until the process exits,
+// whether or not this entry point is ever called: kIpStaticMaxChunks x 4 doubles = 512 KB per GPU.  That is the price, and the
+// reason the limit is modest.
+//
+// In HOST code the identifier few_ip_static_scratch is only a handle for the runtime (its host address means nothing to the
+// GPU), so the address the kernels get is looked up with cudaGetSymbolAddress -- once per device, with that device current, on
+// the first call made on that device -- and kept in g_ip_static_ptr.
+constexpr int kIpStaticMaxChunks = FEW_INNER_STATIC_MAX_CHUNKS;
+constexpr int kIpStaticMaxDevices = 64;
+
+static __device__ __align__(256) double few_ip_static_scratch[(size_t)kIpStaticMaxChunks * 4];
+
+namespace {
+std::mutex g_ip_static_lock;
+double* g_ip_static_ptr[kIpStaticMaxDevices];   // device address of few_ip_static_scratch on device i; NULL = not looked up yet
+}  // namespace
+
+extern "C" int few_inner_products_static(few_ctx* ctx, const double* d, const double* h, int n_src, long long n_samples, double dt,
+                                         double* inner, void* stream)
+{
+    FEW_REQUIRE(inner, FEW_ERR_INVALID_ARG, "inner is NULL");
+    FEW_REQUIRE(n_src > 0 && n_src <= 65535 && n_samples >= 0, FEW_ERR_INVALID_ARG, "bad sizes");
+    FEW_REQUIRE(dt > 0.0 && isfinite(dt), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
+    const long long nc = ip_chunks(n_samples);
+    FEW_REQUIRE(nc <= kIpStaticMaxChunks && (long long)n_src * nc <= kIpStaticMaxChunks, FEW_ERR_LIMIT,
+                "n_src * ceil(n_samples / 2048) exceeds FEW_INNER_STATIC_MAX_CHUNKS: the built-in scratch array is too small for "
+                "this call; use few_inner_products with a caller-owned workspace");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_samples == 0) { FEW_CUDA_CHECK(cudaMemsetAsync(inner, 0, (size_t)n_src * 3 * sizeof(double), st)); return FEW_OK; }
+    FEW_REQUIRE(d && h, FEW_ERR_INVALID_ARG, "d or h is NULL");
+
+    int dev = -1;
+    FEW_CUDA_CHECK(cudaGetDevice(&dev));
+    FEW_REQUIRE(dev >= 0 && dev < kIpStaticMaxDevices, FEW_ERR_LIMIT, "device ordinal beyond the 64 this entry point keeps an address for");
+    FEW_REQUIRE(!ctx || ctx->device == dev, FEW_ERR_INVALID_ARG, "ctx belongs to another device than the current one");
+    double* scratch;
+    {
+        std::lock_guard<std::mutex> guard(g_ip_static_lock);
+        if (!g_ip_static_ptr[dev]) {   // first call on this device: ask the runtime where this device's copy of the array is
+            void* p = nullptr;
+            FEW_CUDA_CHECK(cudaGetSymbolAddress(&p, few_ip_static_scratch));
+            FEW_REQUIRE(p, FEW_ERR_CUDA, "cudaGetSymbolAddress returned a NULL address");
+            g_ip_static_ptr[dev] = static_cast<double*>(p);
+        }
+        scratch = g_ip_static_ptr[dev];
+    }
+    // Nothing in the array has to start at zero: the first kernel stores (never accumulates into) the slots [src][chunk][0..2] for
+    // every chunk of this call, and the second kernel reads exactly those slots, behind it on the same stream.  Whatever an
+    // earlier call left in the array is either overwritten or never looked at.
+    few_inner_partial_kernel<<<dim3((unsigned)nc, n_src), kIpThreads, 0, st>>>((const double2*)d, (const double2*)h, n_samples, (int)nc,
+                                                                             scratch);
+    if (ctx) ++ctx->launches;
+    FEW_CUDA_CHECK(cudaGetLastError());
+    few_inner_final_kernel<<<n_src, kIpThreads, 0, st>>>(scratch, (int)nc, dt, inner);
+    if (ctx) ++ctx->launches;
+    FEW_CUDA_CHECK(cudaGetLastError());
     return FEW_OK;
 }
