@@ -35,8 +35,18 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-FLOP_PER_EVAL = 20.0          # nominal per-mode figure of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA)
-FLOP_PER_PAIR = 38.0          # executed algorithm: per sample and (m,n) pair 18 DFMA + 2 DMUL = 20 FP64 slots
+FLOP_PER_EVAL = 20.0          # WORK-EQUIVALENT, per-mode form of SURVEY 8(d): complex cubic Horner (6 DFMA) + complex MAC (4 DFMA) per sample*mode
+FLOP_PER_PAIR = 38.0          # WORK-EQUIVALENT, round 1's scalar (m,n)-pair form: 18 DFMA + 2 DMUL per sample*pair.  Neither is what the DMMA
+                              # kernel executes (the l-merge and the +-n sharing remove work), so fractions built on them may exceed 1.
+# What few_sum_kernel EXECUTES on the FP64 pipe, per sample:
+#   DMMA.8x8x4: 4 per step and 8 samples (2 when m = 0), 256 FMA each -> 256 (128) flop per sample and step, zero padding included;
+#   scalar DFMA/DMUL/DADD (phases, rho^nu table, run closes, output): 258 + 20 per (m, k) run thread-instructions per sample, each
+#   holding one FMA slot of the pipe (counted as 2 flop).  From smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on of the two
+#   captures in profiles/r02_sum_kernel.md: 358.0 per sample at 5 runs (config 1), 477.9 at 11 runs (config 2); the SASS count of the
+#   source page gives the same slope (16 per close + 4 per new P) and 267 for the constant (lanes predicated off make up the rest).
+DMMA_FLOP_PER_SAMPLE_STEP = 256.0
+SCALAR_FP64_PER_SAMPLE = 258.0
+SCALAR_FP64_PER_SAMPLE_RUN = 20.0
 DFMA_PER_CLK_PER_SM = 64      # B200 FP64 pipe: 16 lanes x 4 sub-partitions (public 37 TFLOP/s at 148 SM, 1.965 GHz)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE few_sum_kernel launch: static figures from `ncu --set full` captures (the
 # run itself does not measure them); the coefficient stream and h stay in the 126 MB L2 while the kernel runs
@@ -145,16 +155,17 @@ def oracle_sample(w, target_s: float, threads: int | None = None, max_samples: i
 def kept_structure(w, keep_h, nk_h):
     """Bookkeeping for the roofline, summed over the sources: kept modes; (m, n) pairs (all l of a pair are summed into one
     pair of splines before the sample loop); STEPS of the summation kernel = kept (m, |n| >> 2) blocks (one step = 4 DMMA.8x8x4
-    per 8 samples, 2 when m = 0: DESIGN.md section 5) as (steps, steps with m = 0)."""
+    per 8 samples, 2 when m = 0: DESIGN.md section 5) as (steps, steps with m = 0), and the number of (m) RUNS (the scalar close + new P per run)."""
     K = int(nk_h.sum())
-    pairs = steps = single = 0
+    pairs = steps = single = runs = 0
     for s in range(w.n_src):
         kept = keep_h[s, : nk_h[s]]
         pairs += len({(int(w.m[j]), int(w.n[j])) for j in kept})
         blocks = {(int(w.m[j]), abs(int(w.n[j])) >> 2) for j in kept}
         steps += len(blocks)
         single += sum(1 for (mm, _) in blocks if mm == 0)
-    return K, pairs, steps, single
+        runs += len({mm for (mm, _) in blocks})          # a run = the kept modes of one m (Schwarzschild lists: k = 0)
+    return K, pairs, steps, single, runs
 
 
 class Bench:
@@ -179,7 +190,7 @@ class Bench:
         for _ in range(n):
             flush.fill_(1); self.step()
         self.api.few_device_status()
-        self.K, self.pairs, self.steps, self.single = kept_structure(self.w, self.keep.cpu().numpy(), self.nk.cpu().numpy())
+        self.K, self.pairs, self.steps, self.single, self.runs = kept_structure(self.w, self.keep.cpu().numpy(), self.nk.cpu().numpy())
 
     def timed(self, steps, flush, barrier=None):
         """steps timed steps, L2 flushed before each (outside the event pair), CUDA events on the launch stream; the library's
@@ -239,17 +250,18 @@ class Bench:
         return sec, int(h2d), int(h_host.numel() * 16)
 
 
-def sum_kernel_roofline(w, pairs, kernel_ms, sm_max_mhz, steps=None, single=0):
-    """FP64 ALU roofline of the summation kernel.  achieved = ALGORITHMIC flops / time: 38 flop per sample and kept (m, n) pair
-    (the work of the pair formulation, a property of the kept list, not of the kernel: DESIGN.md section 5), against the nominal
-    FP64 pipe.  With `steps` also what the kernel's DMMAs execute, padding included: a step is 4 DMMA.8x8x4 per 8 samples (2 when
-    m = 0), 512 flop each, i.e. 256 (128) flop per sample and step."""
+def sum_kernel_roofline(w, pairs, kernel_ms, sm_max_mhz, steps, single, runs, n_src=1):
+    """FP64 ALU roofline of the summation kernel (table instantiation) from what it EXECUTES on the FP64 pipe (SURVEY 8(d)(i),
+    H6): DMMA flop, zero padding included (256 per sample and step, 128 when m = 0) + 2 flop per scalar FP64 thread-instruction
+    ((258 + 20 per run) per sample, measured: see the constants), divided by the kernel's event time and by the nominal pipe
+    (148 SM x 64 FMA/clk x 2 x sm_max_mhz).  `steps`, `single`, `runs` are summed over the `n_src` sources of the launch.
+    The two work-equivalents (38 flop per sample*(m,n) pair, 20 per sample*mode) are returned beside it; they count work the
+    kernel no longer does and may exceed the peak."""
     peak = 148 * DFMA_PER_CLK_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    achieved = float(w.n_samples) * pairs * FLOP_PER_PAIR / (kernel_ms * 1e-3) / 1e12
-    if steps is None:
-        return achieved, peak
-    dmma = float(w.n_samples) * (256.0 * (steps - single) + 128.0 * single) / (kernel_ms * 1e-3) / 1e12
-    return achieved, peak, dmma
+    per_s = float(w.n_samples) / (kernel_ms * 1e-3) / 1e12
+    dmma = per_s * (DMMA_FLOP_PER_SAMPLE_STEP * (steps - single) + 0.5 * DMMA_FLOP_PER_SAMPLE_STEP * single)
+    scalar = per_s * 2.0 * (SCALAR_FP64_PER_SAMPLE * n_src + SCALAR_FP64_PER_SAMPLE_RUN * runs)
+    return {"peak": peak, "executed": dmma + scalar, "dmma": dmma, "scalar": scalar, "pair_equivalent": per_s * pairs * FLOP_PER_PAIR}
 
 
 def time_stages(api, torch, w, g, flush, reps: int = 10):
@@ -374,7 +386,7 @@ def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: i
         K = wk.n_modes if n_keep is None else n_keep
         fl = FLOP_PER_PAIR * wk.n_samples * triples
         out["kerr_shaped_sum"][label] = {"ms": ms, "sum_kernel_ms": kern_ms, "kept_modes": K, "mkn_triples": triples,
-                                         "evals_per_s": wk.n_samples * K / (ms * 1e-3), "tflops_executed": fl / (kern_ms * 1e-3) / 1e12}
+                                         "evals_per_s": wk.n_samples * K / (ms * 1e-3), "tflops_pair_equivalent": fl / (kern_ms * 1e-3) / 1e12}
     # the Kerr-shaped chain on the device: S2 on 100 rows of 78 507 entries (streamed keys), S1 on 84 546 systems, S3 on the kept list
     amp_k = torch.as_tensor(wk.amp).to(dev)
     ph_k = torch.as_tensor(wk.phase).to(dev)
@@ -500,10 +512,13 @@ def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
         b.warm(warm, flush)
         step_ms, sum_ms, launches = b.timed(steps, flush)
         kms = float(np.mean(sum_ms))
-        ach, peak, dmma = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz, b.steps, b.single)
-        r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "kernel_steps": b.steps, "steps": steps,
-             "ms_per_step": float(np.mean(step_ms)), "kernel_ms": kms, "tflops": ach, "frac": ach / peak,
-             "dmma_tflops_executed": dmma, "dmma_share_of_pipe": dmma / peak,
+        rf = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz, b.steps, b.single, b.runs, w.n_src)
+        r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "kernel_steps": b.steps,
+             "steps_m0": b.single, "runs": b.runs, "steps": steps,
+             "ms_per_step": float(np.mean(step_ms)), "kernel_ms": kms, "tflops": rf["executed"], "frac": rf["executed"] / rf["peak"],
+             "dmma_tflops_executed": rf["dmma"], "dmma_share_of_pipe": rf["dmma"] / rf["peak"],
+             "scalar_fp64_share_of_pipe": rf["scalar"] / rf["peak"],
+             "pair_equivalent_frac": rf["pair_equivalent"] / rf["peak"],
              "evals_per_s": float(w.n_samples) * b.K / (float(np.mean(step_ms)) * 1e-3), "gpu_launches_per_step": launches / steps}
         return b, r
 
@@ -578,7 +593,7 @@ def main():
         torch.cuda.synchronize()
 
     bench.warm(args.warmup, flush)
-    K_kept, pairs, bench_steps, bench_single = bench.K, bench.pairs, bench.steps, bench.single
+    K_kept, pairs, bench_steps, bench_single, bench_runs = bench.K, bench.pairs, bench.steps, bench.single, bench.runs
     evals_per_step = float(w.n_samples) * K_kept
 
     # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
@@ -647,24 +662,30 @@ def main():
         return 0
 
     sum_ms_avg = float(np.mean(sum_ms))
-    achieved_tflops, peak_tflops, dmma_tflops = sum_kernel_roofline(w, pairs, sum_ms_avg, sm_max_mhz, bench_steps, bench_single)
+    rf = sum_kernel_roofline(w, pairs, sum_ms_avg, sm_max_mhz, bench_steps, bench_single, bench_runs, w.n_src)
+    achieved_tflops, peak_tflops = rf["executed"], rf["peak"]
     nominal_tflops = evals_per_step * FLOP_PER_EVAL / (sum_ms_avg * 1e-3) / 1e12
     traffic = SUM_KERNEL_DRAM_TRAFFIC.get(w.name) if (args.eps is None and world == 1) else None
     roofline = {"bound": "alu", "kernel": "few_sum_kernel (table instantiation; the recurrence instantiation is launched too and returns at once unless a source needs it)", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops, "traffic": traffic,
                 "traffic_source": SUM_KERNEL_DRAM_TRAFFIC_SOURCE if traffic is not None else None,
                 "peak_kind": f"nominal FP64 pipe: 148 SM x 64 DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (sm_max_mhz {peak_kind})",
+                "achieved_kind": "EXECUTED FP64 flop per launch on this rank / kernel event time: n_samples x [256 x (kernel_steps - steps_m0) + 128 x steps_m0 "
+                                 f"(DMMA.8x8x4, zero padding included) + 2 x ({SCALAR_FP64_PER_SAMPLE:.0f} x n_src + {SCALAR_FP64_PER_SAMPLE_RUN:.0f} x runs) (scalar DFMA/DMUL/DADD "
+                                 "thread-instructions, one FMA slot each; counts from profiles/r02_sum_kernel.md)]",
                 "peak_measured_dfma_probe": fp64_measured_tflops, "frac_of_measured_probe": achieved_tflops / fp64_measured_tflops,
                 "kernel_ms": sum_ms_avg, "kernel_share_of_step": sum_ms_avg / float(np.mean(step_ms)),
-                "executed_dmma": {"tflops": dmma_tflops, "share_of_pipe": dmma_tflops / peak_tflops, "kernel_steps": bench_steps,
-                                  "steps_m0": bench_single,
-                                  "note": "what the kernel's DMMA.8x8x4 execute, zero padding included: 256 flop per sample and step "
-                                          "(128 for m = 0); the rest of the pipe's time goes to scalar FP64 (phases, rho^nu table, run closes)"},
-                "algorithmic": f"{FLOP_PER_PAIR:.0f} flop (the (m,n)-pair formulation: 2 complex cubic Horners + complex rotation + 4 FMA) per sample*(m,n)-pair x {float(w.n_samples) * pairs:.4g} "
-                               f"pair evaluations per launch on this rank ({pairs} pairs from {K_kept} kept modes)",
+                "kernel_steps": bench_steps, "steps_m0": bench_single, "runs": bench_runs,
+                "executed_dmma": {"tflops": rf["dmma"], "share_of_pipe": rf["dmma"] / peak_tflops},
+                "executed_scalar_fp64": {"tflops": rf["scalar"], "share_of_pipe": rf["scalar"] / peak_tflops,
+                                         "thread_instructions_per_sample": SCALAR_FP64_PER_SAMPLE + SCALAR_FP64_PER_SAMPLE_RUN * bench_runs / max(w.n_src, 1)},
+                "pair_equivalent": {"achieved": rf["pair_equivalent"], "frac": rf["pair_equivalent"] / peak_tflops,
+                                    "note": f"WORK-EQUIVALENT, may exceed 1: {FLOP_PER_PAIR:.0f} flop (round 1's scalar (m,n)-pair form) per sample*(m,n)-pair x "
+                                            f"{float(w.n_samples) * pairs:.4g} pair evaluations per launch on this rank ({pairs} pairs from {K_kept} kept modes); the DMMA form "
+                                            "executes 32 FMA per unit where two pairs were counted as 2 x 19"},
                 "nominal_per_mode": {"achieved": nominal_tflops, "frac": nominal_tflops / peak_tflops,
-                                     "note": "20 flop per sample*mode evaluation (per-mode formulation); exceeds the executed "
-                                             "figure because all l of an (m,n) pair are summed into one spline before the sample loop"}}
+                                     "note": "WORK-EQUIVALENT, may exceed 1: 20 flop per sample*mode evaluation (per-mode form, SURVEY 8(d)); all l of an "
+                                             "(m,n) pair are summed into one spline before the sample loop, so the kernel does less"}}
     cpu = None
     if not args.no_cpu_baseline:
         v, desc, cores, t_run, n, K = oracle_sample(w, 12.0)

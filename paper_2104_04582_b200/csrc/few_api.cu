@@ -192,6 +192,10 @@ int waveform_impl(few_ctx* ctx, const double* t, const int* n_t_src, const doubl
     FEW_REQUIRE(n_modes <= FEW_MAX_SELECT_MODES, FEW_ERR_LIMIT, "n_modes > FEW_MAX_SELECT_MODES");
     FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
     FEW_REQUIRE(d == nullptr || inner != nullptr, FEW_ERR_INVALID_ARG, "d given but inner is NULL");
+    if (n_samples > 0) {
+        const int lim = few_sum_check_limits(ctx, n_src, n_t, n_modes, n_samples, n_phase);
+        if (lim != FEW_OK) return lim;
+    }
     wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, nullptr);
     int* kidx = keep_idx ? keep_idx : L.keep_idx;
     int* nk = n_keep ? n_keep : L.n_keep;
@@ -279,6 +283,22 @@ extern "C" int few_waveform_host_ragged(few_ctx* ctx, const double* t_host, cons
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
     FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
     FEW_REQUIRE(n_samples == 0 || h_host, FEW_ERR_INVALID_ARG, "h_host is NULL");
+    // Everything that can be refused from the arguments alone is refused here, before a copy is enqueued: a host->device copy
+    // still in flight when the call returns would read buffers the caller is free to release.
+    FEW_REQUIRE(dt > 0.0 && isfinite(dt) && isfinite(t0), FEW_ERR_INVALID_ARG, "dt must be positive and finite");
+    FEW_REQUIRE(n_t <= FEW_MAX_NT_SPLINE, FEW_ERR_LIMIT, "n_t > FEW_MAX_NT_SPLINE");
+    FEW_REQUIRE(n_modes <= FEW_MAX_SELECT_MODES, FEW_ERR_LIMIT, "n_modes > FEW_MAX_SELECT_MODES");
+    if (n_t_src_host)      // the counts are on the host: validated here (device-pointer calls report them through few_device_status)
+        for (int s = 0; s < n_src; ++s)
+            FEW_REQUIRE(n_t_src_host[s] >= 4 && n_t_src_host[s] <= n_t, FEW_ERR_TOO_FEW_POINTS, "a source's knot count n_t_src_host[s] is outside [4, n_t]");
+    {
+        const int per_call = n_src < kHostGroups ? 1 : (n_src + kHostGroups - 1) / kHostGroups;       // sources per few_waveform call below
+        FEW_REQUIRE(per_call <= 65535, FEW_ERR_LIMIT, "n_src > 8 * 65535");
+        if (n_samples > 0) {
+            const int lim = few_sum_check_limits(ctx, per_call, n_t, n_modes, n_samples, 2);
+            if (lim != FEW_OK) return lim;
+        }
+    }
     struct device_guard {           // the context's device is current inside the call; the caller's is restored on every return
         int prev = -1;
         ~device_guard() { if (prev >= 0) cudaSetDevice(prev); }
@@ -383,7 +403,10 @@ extern "C" int few_waveform_host_ragged(few_ctx* ctx, const double* t_host, cons
         if (e == cudaSuccess) rc = few_device_status(ctx, nullptr, st);   // synchronises
     }
     if (e != cudaSuccess) { few_set_error("few_waveform_host: %s", cudaGetErrorString(e)); rc = FEW_ERR_CUDA; }
+    // On every path, failing or not, nothing of this call is in flight when it returns: the kernels' stream and the copy stream
+    // (whose host->device copies read the caller's amp_host and the staging block the next call overwrites) are both drained.
     cudaStreamSynchronize(st);
+    cudaStreamSynchronize(cs);
     return rc;
 }
 

@@ -28,6 +28,10 @@ struct few_ctx {
 
 void few_set_error(const char* fmt, ...);
 
+// few_sum.cu: every size limit of the summation (tile count, shared memory of its kernels) in one place, so that the summation,
+// few_waveform and few_waveform_host can all check them BEFORE they enqueue anything.  FEW_OK or FEW_ERR_LIMIT.
+int few_sum_check_limits(const few_ctx* ctx, int n_src, int n_t, int n_modes, long long n_samples, int n_phase);
+
 #define FEW_CUDA_CHECK(expr)                                                                     \
     do {                                                                                         \
         cudaError_t _e = (expr);                                                                 \

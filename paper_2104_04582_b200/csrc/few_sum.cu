@@ -438,7 +438,11 @@ __global__ void __launch_bounds__(1024) few_sum_pack_kernel(const double2* __res
                                                             int n_modes, sum_layout L)
 {
     const int seg = blockIdx.x, src = blockIdx.y, n_seg = n_t - 1;
-    if (n_t_src && seg >= n_t_src[src] - 1) return;      // ragged batch: no such segment (its coefficients were never written)
+    if (n_t_src) {      // ragged batch: segments beyond the source's own count do not exist (their coefficients were never written).
+        int v = n_t_src[src];                              // A bad count is replaced by 4 exactly as few_knots() does in the plan, fit and
+        if (v < 4 || v > n_t) v = n_t < 4 ? n_t : 4;       // selection kernels (which also report it), so that every stage the plan's tiles
+        if (seg >= v - 1) return;                          // point at is written in this call and the sum kernel never reads stale memory
+    }
     const int S = L.n_steps[src];
     const int* ulo = L.u_lo + (size_t)src * L.cap * 8;
     const int* uhi = L.u_hi + (size_t)src * L.cap * 8;
@@ -838,7 +842,7 @@ few_sum_kernel(const double* __restrict__ t_all, const dd* __restrict__ coef_pha
         const int* hdr = reinterpret_cast<const int*>(&ring[slot][0] + kStageSteps * kStepD2);
         int4 d4 = *reinterpret_cast<const int4*>(hdr), d8 = kStageSteps > 4 ? *(reinterpret_cast<const int4*>(hdr) + 1) : make_int4(0, 0, 0, 0);
         static_assert(kStageSteps == 4 || kStageSteps == 8 || (kStageSteps > 8 && kStageSteps < 128), "descriptors: 4 or 8 in registers, more from the header");
-        const int ns = hdr[kStageSteps];
+        const int ns = min(hdr[kStageSteps], kStageSteps);   // the clamp keeps the walk inside the ring slot whatever the header holds
         for (int si = 0; si < ns; ++si, bp += kStepD2) {
             int d;
             if (kStageSteps <= 8) {
@@ -1046,6 +1050,20 @@ int plan_smem_elems(int n_modes)
 
 }  // namespace
 
+int few_sum_check_limits(const few_ctx* ctx, int n_src, int n_t, int n_modes, long long n_samples, int n_phase)
+{
+    FEW_REQUIRE(n_src <= 65535 && n_t <= 65535, FEW_ERR_LIMIT, "n_src or n_t > 65535");
+    FEW_REQUIRE((size_t)plan_smem_elems(n_modes) * 8 <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "plan kernel's shared memory exceeds the device limit");
+    const size_t smem_tab = n_phase == 3 ? sum_smem_bytes<kSumG, true, true>() : sum_smem_bytes<kSumG, false, true>();
+    const size_t smem_rec = n_phase == 3 ? sum_smem_bytes<kSumG, true, false>() : sum_smem_bytes<kSumG, false, false>();
+    FEW_REQUIRE(smem_tab <= (size_t)ctx->smem_optin && smem_rec <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT,
+                "sum kernel's shared memory exceeds the device limit");
+    const long long max_tiles = sum_max_tiles(n_samples, n_t);
+    FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
+    FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
+    return FEW_OK;
+}
+
 extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
 {
     if (n_src <= 0 || n_t < 2 || n_modes <= 0 || n_samples < 0) return 0;
@@ -1078,11 +1096,13 @@ extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int*
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
                     workspace_bytes >= few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
+    {   // every size limit, before the first launch
+        const int lim = few_sum_check_limits(ctx, n_src, n_t, n_modes, n_samples, n_phase);
+        if (lim != FEW_OK) return lim;
+    }
     const int plan_elems = plan_smem_elems(n_modes);
     const size_t psm = (size_t)plan_elems * 8;
-    FEW_REQUIRE(psm <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "plan kernel's shared memory exceeds the device limit");
-    long long max_tiles = sum_max_tiles(n_samples, n_t);
-    FEW_REQUIRE(max_tiles < 2147483647LL, FEW_ERR_LIMIT, "n_samples too large");
+    const long long max_tiles = sum_max_tiles(n_samples, n_t);
     sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
 
     const int plan_tile_blocks = n_src >= 64 ? 1 : (64 / n_src < 8 ? 64 / n_src : 8);     // tile blocks per source: 8 for one waveform
@@ -1098,7 +1118,6 @@ extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int*
     few_sum_pack_kernel<<<dim3(n_t - 1, n_src), pack_threads, 0, st>>>((const double2*)coef_amp, n_t_src, n_t, n_modes, L);
     FEW_LAUNCHED(ctx);
     if (ctx->profile) FEW_CUDA_CHECK(cudaEventRecord(ctx->ev_sum[0], st));
-    FEW_REQUIRE(max_tiles * n_src < 2147483647LL - 65536, FEW_ERR_LIMIT, "n_src * n_samples too large");
     // both instantiations are launched: the table one (rho^nu of the 8 nu-blocks in use kept in tensor memory) takes the sources
     // whose lists fit its table, the recurrence one the others; an instantiation with no source returns at once
     const long long want = max_tiles * n_src;
@@ -1107,7 +1126,6 @@ extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int*
         auto ktab = few_sum_kernel<kSumG, kSumTabBlocksPerSm, INNER, KERR, true>;                                                 \
         auto krec = few_sum_kernel<kSumG, kSumBlocksPerSm, INNER, KERR, false>;                                                   \
         const size_t smem_tab = sum_smem_bytes<kSumG, KERR, true>(), smem_rec = sum_smem_bytes<kSumG, KERR, false>();             \
-        FEW_REQUIRE(smem_tab <= (size_t)ctx->smem_optin, FEW_ERR_LIMIT, "sum kernel's shared memory exceeds the device limit");   \
         FEW_CUDA_CHECK(cudaFuncSetAttribute(ktab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tab));                   \
         FEW_CUDA_CHECK(cudaFuncSetAttribute(krec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rec));                   \
         const long long res_tab = (long long)ctx->sm_count * kSumTabBlocksPerSm, res_rec = (long long)ctx->sm_count * kSumBlocksPerSm; \

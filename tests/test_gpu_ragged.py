@@ -168,7 +168,46 @@ def test_ragged_bad_count_is_reported(api, batch, bad):
     g = gpu_inputs(w)
     cnt = w.n_t_src.copy()
     cnt[1] = bad
-    api.few_waveform_ragged(g["t"], dev(cnt), g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
-                            2_000)
+    # The workspace starts as 0xFF bytes (NaN as doubles, -1 / huge as counts): whatever the kernels read must have been written
+    # in this call.  few.h promises "outputs unspecified but in bounds" for a bad count: no fault, and here no NaN either, since
+    # the bad source is treated as a 4-knot source by every kernel alike.
+    n_src, n_t, n_modes = g["amp"].shape
+    ws = torch.full((max(api.few_waveform_workspace(n_src, n_t, n_modes, 2_000), 256),), 0xFF, dtype=torch.uint8, device="cuda:0")
+    h = api.few_waveform_ragged(g["t"], dev(cnt), g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt,
+                                2_000, workspace=ws)
+    torch.cuda.synchronize()                                                 # raises if a kernel faulted
+    assert bool(torch.isfinite(torch.view_as_real(h)).all())
     assert api.few_device_status(raise_on_error=False) == -2                 # FEW_ERR_TOO_FEW_POINTS (FEW_DEV_BAD_COUNT)
     assert api.few_device_status(raise_on_error=False) == 0
+
+
+def test_host_path_refuses_bad_arguments_before_copying(api, batch):
+    """few_waveform_host(_ragged) checks what it can from the arguments alone -- the size limits and, since they are on the host,
+    the per-source knot counts -- before it enqueues a single copy, so that a refused call leaves nothing in flight that still
+    reads the caller's buffers.  The context stays usable afterwards."""
+    w = batch
+    cpu = lambda a, dt=None: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).pin_memory()      # noqa: E731
+    args = [cpu(w.t), None, cpu(w.phase), cpu(w.amp), cpu(w.l), cpu(w.m), cpu(w.n), cpu(w.theta), cpu(w.phi), w.eps, w.t0, w.dt, 2_000]
+    for bad in (3, 138, -1):
+        cnt = w.n_t_src.copy()
+        cnt[1] = bad
+        args[1] = cpu(cnt)
+        with pytest.raises(api.FewError) as e:
+            api.few_waveform_host_ragged(*args)
+        assert e.value.code == -2                                            # FEW_ERR_TOO_FEW_POINTS
+    n_t = 737                                                                # FEW_MAX_NT_SPLINE + 1
+    z = lambda *shape, dt=torch.float64: torch.zeros(shape, dtype=dt).pin_memory()                # noqa: E731
+    with pytest.raises(api.FewError) as e:
+        api.few_waveform_host(z(1, n_t), z(1, n_t, 2), z(1, n_t, 3, dt=torch.complex128), cpu(w.l[:3]), cpu(w.m[:3]), cpu(w.n[:3]),
+                              z(1), z(1), 0.0, 0.0, 10.0, 100)
+    assert e.value.code == -7                                                # FEW_ERR_LIMIT
+    with pytest.raises(api.FewError) as e:                                   # dt = 0
+        api.few_waveform_host_ragged(*(args[:1] + [cpu(w.n_t_src)] + args[2:11] + [0.0, 2_000]))
+    assert e.value.code == -1
+    assert api.few_device_status(raise_on_error=False) == 0                  # nothing ran, nothing was flagged
+    args[1] = cpu(w.n_t_src)
+    hh = api.few_waveform_host_ragged(*args)                                 # and the next good call is unaffected
+    g = gpu_inputs(w)
+    h = api.few_waveform_ragged(g["t"], g["cnt"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0,
+                                w.dt, 2_000)
+    assert np.array_equal(hh.numpy().view(np.float64), h.cpu().numpy().view(np.float64))
