@@ -179,6 +179,11 @@ class Bench:
         self.h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=dev)
         self.keep = torch.empty((w.n_src, w.n_modes), dtype=torch.int32, device=dev)
         self.nk = torch.empty((w.n_src,), dtype=torch.int32, device=dev)
+        # the summation's workspace is laid out for the steps this mode list can produce at most (88 on the paper's grid) instead of
+        # the default capacity (few.h, few_set_max_steps): same kernels, same bits, a fraction of the device memory
+        self.step_bound = api.few_max_steps_for_modes(self.pinned["m"], self.pinned["n"])
+        api.few_set_max_steps(self.step_bound)
+        self.ws_default_bytes = api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples, max_steps=0)
         self.ws = torch.empty(api.few_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=dev)
 
     def step(self):
@@ -274,7 +279,7 @@ def time_stages(api, torch, w, g, flush, reps: int = 10):
     cdd = api.few_spline_fit_dd(g["t"], g["phase"])
     spl_ws = torch.empty(max(api._lib.few_spline_fit_workspace(w.n_src, w.n_t), 256), dtype=torch.uint8, device=coef.device)
     sel_ws = torch.empty(api._lib.few_select_modes_workspace(w.n_src, w.n_t, w.n_modes), dtype=torch.uint8, device=coef.device)
-    sum_ws = torch.empty(api._lib.few_sum_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=coef.device)
+    sum_ws = torch.empty(api.few_sum_waveform_workspace(w.n_src, w.n_t, w.n_modes, w.n_samples), dtype=torch.uint8, device=coef.device)
     h = torch.empty((w.n_src, w.n_samples), dtype=torch.complex128, device=coef.device)
     calls = {
         "S0_ylm_modes": lambda: api.few_ylm_modes(g["theta"], g["phi"], g["l"], g["m"]),
@@ -363,13 +368,15 @@ def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: i
     # Kerr-shaped list (NEXT-4, summation part): 42 273 modes = 7381 (m, k, n) triples, third phase, one year at dt = 10 s;
     # all modes, then the 4000 strongest at mid-trajectory (a kept list of the size selection would hand over)
     wk = synth.make_kerr()
+    main_bound = api.few_max_steps_for_modes(torch.as_tensor(w.m), torch.as_tensor(w.n))
+    api.few_set_max_steps(api.few_max_steps_for_modes(torch.as_tensor(wk.m), torch.as_tensor(wk.n), torch.as_tensor(wk.k)))   # 11 m x 11 k x 8 blocks
     tk = torch.as_tensor(wk.t).to(dev)
     coef = api.few_spline_fit(tk, torch.as_tensor(wk.amp).to(dev))
     cdd = api.few_spline_fit_dd(tk, torch.as_tensor(wk.phase).to(dev))
     lk, mk, kk, nk_ = (torch.as_tensor(x).to(dev) for x in (wk.l, wk.m, wk.k, wk.n))
     ypk, ymk = api.few_ylm_modes(g["theta"][:1], g["phi"][:1], lk, mk)
     hk = torch.empty((1, wk.n_samples), dtype=torch.complex128, device=dev)
-    kws = torch.empty(api._lib.few_sum_waveform_workspace(1, wk.n_t, wk.n_modes, wk.n_samples), dtype=torch.uint8, device=dev)
+    kws = torch.empty(api.few_sum_waveform_workspace(1, wk.n_t, wk.n_modes, wk.n_samples), dtype=torch.uint8, device=dev)
     out["kerr_shaped_sum"] = {}
     for label, n_keep in (("all_modes", None), ("kept_4000", 4000)):
         keep = nkeep = None
@@ -409,6 +416,7 @@ def time_next(api, torch, w, g, flush, hbm_gbs, reps: int = 5, direct_samples: i
                                            "algorithmic_bytes": nb_sel, "gbs": nb_sel / ms_sel / 1e6},
                                 "spline_fit": {"ms": ms_fit, "algorithmic_bytes": nb_fit, "gbs": nb_fit / ms_fit / 1e6,
                                                "hbm_frac": nb_fit / ms_fit / 1e6 / hbm_gbs}}
+    api.few_set_max_steps(main_bound)
     return out
 
 
@@ -514,7 +522,7 @@ def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
         kms = float(np.mean(sum_ms))
         rf = sum_kernel_roofline(w, b.pairs, kms, sm_max_mhz, b.steps, b.single, b.runs, w.n_src)
         r = {"workload": w.name, "eps": float(w.eps), "kept_modes": b.K, "mn_pairs": b.pairs, "kernel_steps": b.steps,
-             "steps_m0": b.single, "runs": b.runs, "steps": steps,
+             "steps_m0": b.single, "runs": b.runs, "steps": steps, "workspace_bytes": int(b.ws.numel()), "workspace_default_bytes": int(b.ws_default_bytes),
              "ms_per_step": float(np.mean(step_ms)), "kernel_ms": kms, "tflops": rf["executed"], "frac": rf["executed"] / rf["peak"],
              "dmma_tflops_executed": rf["dmma"], "dmma_share_of_pipe": rf["dmma"] / rf["peak"],
              "scalar_fp64_share_of_pipe": rf["scalar"] / rf["peak"],
@@ -594,6 +602,7 @@ def main():
 
     bench.warm(args.warmup, flush)
     K_kept, pairs, bench_steps, bench_single, bench_runs = bench.K, bench.pairs, bench.steps, bench.single, bench.runs
+    bench_ws = (bench.ws.numel(), bench.ws_default_bytes, bench.step_bound)
     evals_per_step = float(w.n_samples) * K_kept
 
     # FP64 peak probe (register-resident DFMA chains), timed alone: the measured denominator beside the nominal one
@@ -699,6 +708,9 @@ def main():
            "config": config_dict(w_full, parallelism=parallelism),
            "kept_modes": K_kept, "mn_pairs": pairs, "timing": "L2 flushed between timed steps (256 MiB write); CUDA events on the launch stream; max over ranks",
            "ms_per_waveform": ms_per_step / w_full.n_src, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+           "workspace": {"bytes": int(bench_ws[0]), "default_bytes": int(bench_ws[1]), "max_steps": int(bench_ws[2]),
+                         "note": "few_waveform workspace of this rank with the step bound few_max_steps_for_modes gives for the mode list "
+                                 "(few_set_max_steps), against the default capacity"},
            "gpu_launches": int(launches), "gpu_launches_note": "counted by the library at its launch sites (few_launch_count) over the timed steps of this rank",
            "clocks": clocks, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms)}
     if graph_ms is not None:

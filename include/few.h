@@ -134,6 +134,24 @@ int few_sum_waveform(few_ctx* ctx, const double* t, const double* coef_amp, cons
                      double t0, double dt, long long n_samples, double* h,
                      int n_src, int n_t, int n_modes, void* workspace, size_t workspace_bytes, void* stream);
 
+/* A caller's bound on the summation's STEPS per source, to shrink its workspace.  The summation consumes the kept modes as steps:
+ * one step = the kept modes of one (m, k) whose |n| lie in one aligned block of four (4b .. 4b+3).  By default the workspace is laid
+ * out for min(n_modes, n_modes / 4 + 64) steps per source, which no kept list of the call can exceed but which is far more than a
+ * list on a grid needs: the paper's 3843-mode grid (m = 0..10, |n| <= 30) gives at most 11 x 8 = 88 steps where
+ * the default reserves 1024 -- 105 MB of coefficient stages per source at n_t = 100 instead of 9 MB.
+ *   few_max_steps_for_modes  HOST helper: the number of distinct (m, k, |n| >> 2) in a mode list (k_host may be NULL = 0), i.e. the
+ *                            most steps ANY kept subset of that list can produce.  Returns the count (>= 1) or a negative FEW_ERR_*.
+ *   few_set_max_steps        stores the bound in the context (0 = back to the default).  From then on every summation through this
+ *                            context (few_sum_waveform*, few_waveform*) lays its workspace out for min(default, max_steps) steps per
+ *                            source and expects at least few_*_workspace_ex(..., max_steps) bytes.  A kept list that needs more steps is
+ *                            cut at the bound and reported: FEW_DEV_SPARSE_LIST -> few_device_status returns FEW_ERR_LIMIT.
+ *   few_*_workspace_ex       the workspace queries for a given bound (max_steps = 0: the plain queries).
+ * few_waveform_host(_ragged) has the mode list on the host and applies few_max_steps_for_modes itself for the duration of the call. */
+int few_max_steps_for_modes(const int* m_host, const int* k_host, const int* n_host, int n_modes);
+int few_set_max_steps(few_ctx* ctx, int max_steps);
+size_t few_sum_waveform_workspace_ex(int n_src, int n_t, int n_modes, long long n_samples, int max_steps);
+size_t few_waveform_workspace_ex(int n_src, int n_t, int n_modes, long long n_samples, int max_steps);
+
 /* Extended form of S3.  Adds
  *   factor[n_src][2] or NULL: a complex per-source prefactor (few_frame_constants: the detector-frame transformation of
  *     Eq. (4)-(8) and mu/d_L).  h is linear in the harmonic constants, so the factor is folded into them before the sample

@@ -23,7 +23,8 @@ SYMBOLS = ["few_create", "few_destroy", "few_strerror", "few_last_error", "few_v
            "few_fp64_peak_probe", "few_launch_count", "few_profile_enable", "few_profile_sum_ms", "few_sum_waveform_ex", "few_frame_constants",
            "few_frame_rotate", "few_inner_products_workspace", "few_inner_products", "few_inner_products_static", "few_waveform_ssb", "few_sum_direct_workspace",
            "few_sum_direct", "few_sum_waveform_kerr", "few_waveform_kerr", "few_spline_fit_ragged", "few_spline_fit_dd_ragged",
-           "few_select_modes_ragged", "few_sum_waveform_ragged", "few_waveform_ragged", "few_waveform_host_ragged"]
+           "few_select_modes_ragged", "few_sum_waveform_ragged", "few_waveform_ragged", "few_waveform_host_ragged",
+           "few_max_steps_for_modes", "few_set_max_steps", "few_sum_waveform_workspace_ex", "few_waveform_workspace_ex"]
 
 
 class FewError(RuntimeError):
@@ -56,6 +57,10 @@ def _load() -> C.CDLL:
         "few_sum_waveform_workspace": (sz, [i, i, i, ll]),
         "few_sum_waveform": (i, [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, d, d, ll, vp, i, i, i, vp, sz, vp]),
         "few_waveform_workspace": (sz, [i, i, i, ll]),
+        "few_waveform_workspace_ex": (sz, [i, i, i, ll, i]),
+        "few_sum_waveform_workspace_ex": (sz, [i, i, i, ll, i]),
+        "few_set_max_steps": (i, [vp, i]),
+        "few_max_steps_for_modes": (i, [vp, vp, vp, i]),
         "few_waveform": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_kerr": (i, [vp] * 11 + [d, d, d, ll, i, i, i, vp, vp, vp, vp, sz, vp]),
         "few_waveform_host": (i, [vp] * 10 + [d, d, d, ll, i, i, i, vp, vp, vp]),
@@ -196,7 +201,7 @@ def few_sum_waveform(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, ylm_
     n_src, n_t = t.shape
     n_modes = l.shape[0]
     h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
-    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    need = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples)
     ws = workspace if workspace is not None else _ws(need, t.device)
     _chk(_lib.few_sum_waveform(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
                                _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32), _p(keep_idx), _p(n_keep),
@@ -216,7 +221,7 @@ def few_sum_waveform_ex(t, coef_amp, coef_phase_dd, l, m, n, keep_idx, n_keep, y
     if want_h:
         h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
     inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
-    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    need = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples)
     ws = workspace if workspace is not None else _ws(need, t.device)
     _chk(_lib.few_sum_waveform_ex(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
                                   _p(l, torch.int32), _p(m, torch.int32), _p(n, torch.int32), _p(keep_idx), _p(n_keep),
@@ -238,7 +243,7 @@ def few_sum_waveform_kerr(t, coef_amp, coef_phase_dd, l, m, k, n, keep_idx, n_ke
     if want_h:
         h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
     inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
-    need = _lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples))
+    need = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples)
     ws = workspace if workspace is not None else _ws(need, t.device)
     _chk(_lib.few_sum_waveform_kerr(context(), _p(t, torch.float64), _p(coef_amp, torch.float64), _p(coef_phase_dd, torch.float64),
                                     n_phase, _p(l, torch.int32), _p(m, torch.int32), _p(k), _p(n, torch.int32), _p(keep_idx),
@@ -327,8 +332,35 @@ def few_sum_direct(amp, phase, l, m, n, ylm_plus, ylm_minus, scale=None, factor=
     return h
 
 
-def few_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int) -> int:
-    return int(_lib.few_waveform_workspace(n_src, n_t, n_modes, int(n_samples)))
+_max_steps: dict[int, int] = {}     # the bound set per device through few_set_max_steps (the binding's own workspace sizes follow it)
+
+
+def few_max_steps_for_modes(m, n, k=None) -> int:
+    """Most summation steps any kept subset of the mode list (m, k, n: CPU i32 tensors, k optional) can produce (HOST helper)."""
+    rc = int(_lib.few_max_steps_for_modes(_hp(m, torch.int32), _hp(k, torch.int32), _hp(n, torch.int32), int(m.numel())))
+    if rc < 0:
+        raise FewError(rc, "few_max_steps_for_modes")
+    return rc
+
+
+def few_set_max_steps(max_steps: int) -> None:
+    """Bound the summation's steps per source on the current device's context (0 = default): smaller workspaces, see few.h."""
+    _chk(_lib.few_set_max_steps(context(), int(max_steps)), "few_set_max_steps")
+    _max_steps[torch.cuda.current_device()] = int(max_steps)
+
+
+def _cap() -> int:
+    return _max_steps.get(torch.cuda.current_device(), 0) if torch.cuda.is_available() else 0
+
+
+def few_sum_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int, max_steps: int | None = None) -> int:
+    """Bytes few_sum_waveform* needs; max_steps None = the bound currently set on this device's context."""
+    return int(_lib.few_sum_waveform_workspace_ex(n_src, n_t, n_modes, int(n_samples), _cap() if max_steps is None else int(max_steps)))
+
+
+def few_waveform_workspace(n_src: int, n_t: int, n_modes: int, n_samples: int, max_steps: int | None = None) -> int:
+    """Bytes few_waveform* needs; max_steps None = the bound currently set on this device's context."""
+    return int(_lib.few_waveform_workspace_ex(n_src, n_t, n_modes, int(n_samples), _cap() if max_steps is None else int(max_steps)))
 
 
 def few_waveform(t, phase, amp, l, m, n, theta, phi, eps: float, t0: float, dt: float, n_samples: int, scale=None,
@@ -423,7 +455,7 @@ def few_sum_waveform_ragged(t, n_t_src, coef_amp, coef_phase_dd, l, m, k, n, kee
     if want_h:
         h = out if out is not None else torch.empty((n_src, int(n_samples)), dtype=torch.complex128, device=t.device)
     inner = torch.empty((n_src, 3), dtype=torch.float64, device=t.device) if (want_inner or d is not None) else None
-    ws = workspace if workspace is not None else _ws(_lib.few_sum_waveform_workspace(n_src, n_t, n_modes, int(n_samples)), t.device)
+    ws = workspace if workspace is not None else _ws(few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples), t.device)
     _chk(_lib.few_sum_waveform_ragged(context(), _p(t, torch.float64), _p(n_t_src, torch.int32), _p(coef_amp, torch.float64),
                                       _p(coef_phase_dd, torch.float64), n_phase, _p(l, torch.int32), _p(m, torch.int32), _p(k),
                                       _p(n, torch.int32), _p(keep_idx), _p(n_keep), _p(ylm_plus, torch.complex128),

@@ -140,7 +140,7 @@ struct wf_layout {
     size_t sel_bytes, sum_bytes, spl_bytes;
 };
 
-wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, size_t* bytes)
+wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, int max_steps, size_t* bytes)
 {
     few_carver c(ws);
     wf_layout L;
@@ -154,7 +154,7 @@ wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_sample
     L.phi_src = c.take<double>(n_src);
     L.factor = c.take<double>((size_t)n_src * 2);
     L.sel_bytes = few_select_modes_workspace(n_src, n_t, n_modes);
-    L.sum_bytes = few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples);
+    L.sum_bytes = few_sum_waveform_workspace_ex(n_src, n_t, n_modes, n_samples, max_steps);
     L.spl_bytes = few_spline_fit_workspace(n_src, n_t);
     L.spl_ws = c.take<char>(L.spl_bytes);
     L.sel_ws = c.take<char>(L.sel_bytes);
@@ -164,12 +164,17 @@ wf_layout wf_carve(void* ws, int n_src, int n_t, int n_modes, long long n_sample
 }
 }  // namespace
 
-extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
+extern "C" size_t few_waveform_workspace_ex(int n_src, int n_t, int n_modes, long long n_samples, int max_steps)
 {
     if (n_src <= 0 || n_t < 4 || n_modes <= 0) return 0;
     size_t bytes = 0;
-    wf_carve(nullptr, n_src, n_t, n_modes, n_samples, &bytes);
+    wf_carve(nullptr, n_src, n_t, n_modes, n_samples, max_steps, &bytes);
     return bytes;
+}
+
+extern "C" size_t few_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
+{
+    return few_waveform_workspace_ex(n_src, n_t, n_modes, n_samples, 0);
 }
 
 namespace {
@@ -183,7 +188,7 @@ int waveform_impl(few_ctx* ctx, const double* t, const int* n_t_src, const doubl
     FEW_REQUIRE(n_src > 0 && n_modes > 0 && n_samples >= 0, FEW_ERR_INVALID_ARG, "sizes must be positive");
     FEW_REQUIRE(n_t >= 4, FEW_ERR_TOO_FEW_POINTS, "n_t < 4");
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
-                    workspace_bytes >= few_waveform_workspace(n_src, n_t, n_modes, n_samples),
+                    workspace_bytes >= few_waveform_workspace_ex(n_src, n_t, n_modes, n_samples, ctx->max_steps),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
     // every limit a sub-call checks is checked HERE, before anything is enqueued: once the side streams are forked, an early
     // return would leave them running into a workspace the caller is free to release
@@ -196,7 +201,7 @@ int waveform_impl(few_ctx* ctx, const double* t, const int* n_t_src, const doubl
         const int lim = few_sum_check_limits(ctx, n_src, n_t, n_modes, n_samples, n_phase);
         if (lim != FEW_OK) return lim;
     }
-    wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, nullptr);
+    wf_layout L = wf_carve(workspace, n_src, n_t, n_modes, n_samples, ctx->max_steps, nullptr);
     int* kidx = keep_idx ? keep_idx : L.keep_idx;
     int* nk = n_keep ? n_keep : L.n_keep;
     // The spline fits depend on the inputs only, so they run on two side streams beside harmonics + mode selection and
@@ -309,7 +314,18 @@ extern "C" int few_waveform_host_ragged(few_ctx* ctx, const double* t_host, cons
     const size_t b_lmn = (size_t)n_modes * 4, b_ang = (size_t)n_src * 8, b_h = (size_t)n_src * n_samples * 16;
     const size_t b_keep = (size_t)n_src * n_modes * 4, b_nk = (size_t)n_src * 4;
     const int group_max = (n_src + kHostGroups - 1) / kHostGroups > 1 ? (n_src + kHostGroups - 1) / kHostGroups : 1;
-    const size_t ws_bytes = few_waveform_workspace(n_src < kHostGroups ? 1 : group_max, n_t, n_modes, n_samples);
+    // The mode list is on the host here, so the summation's workspace is sized for the steps this list can produce at most (the
+    // distinct (m, |n| >> 2): 88 on the paper's grid) instead of the default capacity (1024 there): 12 x less device memory per
+    // source.  A bound the caller set with few_set_max_steps is kept if it is lower; the context's setting is restored on return.
+    struct cap_guard {
+        few_ctx* c; int saved;
+        ~cap_guard() { c->max_steps = saved; }
+    } cap{ctx, ctx->max_steps};
+    {
+        const int bound = few_max_steps_for_modes(m_host, nullptr, n_host, n_modes);
+        if (bound > 0 && (ctx->max_steps == 0 || bound < ctx->max_steps)) ctx->max_steps = bound;
+    }
+    const size_t ws_bytes = few_waveform_workspace_ex(n_src < kHostGroups ? 1 : group_max, n_t, n_modes, n_samples, ctx->max_steps);
     // If h_host is pinned (page-locked, hence device-accessible under unified addressing) the summation kernel stores the
     // waveform straight into it: the device->host transfer then rides on the kernel's own coalesced streaming stores and
     // overlaps the FP64 work, instead of following it as a separate copy.  Pageable memory takes the staged path.

@@ -15,6 +15,7 @@ struct few_ctx {
     int profile;         // few_profile_enable
     int profile_valid;   // a sum kernel was bracketed since profiling was switched on
     long long launches;  // kernels launched through this context so far (few_launch_count)
+    int max_steps;       // few_set_max_steps: caller's bound on the summation's steps per source (0 = the default capacity)
     cudaEvent_t ev_sum[2];
     cudaStream_t side[2];  // few_waveform: the two spline fits run beside harmonics + mode selection
     cudaEvent_t ev_fork, ev_join[2];

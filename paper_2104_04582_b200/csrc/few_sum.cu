@@ -30,6 +30,8 @@
 //   3. few_sum_kernel       the hot loop.  Stages arrive in shared memory through a ring of TMA bulk copies
 //        (cp.async.bulk + mbarrier) and are read with conflict-free 128-bit loads.  Per sample the phases are evaluated ONCE in
 //        double-double (Horner, reduction by 2 pi, one sincos each).  Output: coalesced 16-byte streaming stores.
+#include <algorithm>
+#include <vector>
 #include "few_common.cuh"
 
 namespace {
@@ -104,11 +106,19 @@ __host__ __device__ inline int stages_for(int n_steps) { return (n_steps + kStag
 
 __host__ inline long long sum_max_tiles(long long n_samples, int n_t) { return (n_samples + kTile - 1) / kTile + n_t + 1; }
 
-sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, size_t* bytes = nullptr)
+// Steps per source the workspace is laid out for: the default covers any kept list of the call (step_capacity), a caller's
+// bound (few_set_max_steps) can only lower it.  A list that needs more sets FEW_DEV_SPARSE_LIST in the plan kernel either way.
+__host__ inline int effective_cap(int n_modes, int max_steps)
+{
+    const int def = step_capacity(n_modes);
+    return (max_steps > 0 && max_steps < def) ? max_steps : def;
+}
+
+sum_layout sum_carve(void* ws, int n_src, int n_t, int n_modes, long long n_samples, int max_steps, size_t* bytes = nullptr)
 {
     few_carver c(ws);
     sum_layout L;
-    L.cap = step_capacity(n_modes);
+    L.cap = effective_cap(n_modes, max_steps);
     L.max_stages = stages_for(L.cap);
     L.bounds = c.take<long long>((size_t)n_src * (n_t + 2));
     L.tile_start = c.take<int>((size_t)n_src * (n_t + 2));
@@ -1064,12 +1074,54 @@ int few_sum_check_limits(const few_ctx* ctx, int n_src, int n_t, int n_modes, lo
     return FEW_OK;
 }
 
-extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
+extern "C" size_t few_sum_waveform_workspace_ex(int n_src, int n_t, int n_modes, long long n_samples, int max_steps)
 {
     if (n_src <= 0 || n_t < 2 || n_modes <= 0 || n_samples < 0) return 0;
     size_t bytes = 0;
-    sum_carve(nullptr, n_src, n_t, n_modes, n_samples, &bytes);
+    sum_carve(nullptr, n_src, n_t, n_modes, n_samples, max_steps, &bytes);
     return bytes;
+}
+
+extern "C" size_t few_sum_waveform_workspace(int n_src, int n_t, int n_modes, long long n_samples)
+{
+    return few_sum_waveform_workspace_ex(n_src, n_t, n_modes, n_samples, 0);
+}
+
+extern "C" int few_set_max_steps(few_ctx* ctx, int max_steps)
+{
+    FEW_REQUIRE(ctx != nullptr, FEW_ERR_INVALID_ARG, "ctx is NULL");
+    FEW_REQUIRE(max_steps >= 0, FEW_ERR_INVALID_ARG, "max_steps must be >= 0 (0 = the default capacity)");
+    ctx->max_steps = max_steps;
+    return FEW_OK;
+}
+
+extern "C" int few_max_steps_for_modes(const int* m_host, const int* k_host, const int* n_host, int n_modes)
+{
+    FEW_REQUIRE(m_host && n_host && n_modes > 0, FEW_ERR_INVALID_ARG, "NULL argument or n_modes <= 0");
+    // Valid lists (0 <= m <= FEW_MAX_L, |k| <= FEW_MAX_ABS_K, |n| <= FEW_MAX_ABS_N) are counted in a bitmap, a few microseconds for
+    // the paper's grid (few_waveform_host does this on every call); anything else goes through a sort, so that the count is
+    // right for any input and the kernels are the ones to report a bad mode.
+    constexpr int kNuBlocks = FEW_MAX_ABS_N / 4 + 1, kKSpan = 2 * FEW_MAX_ABS_K + 1;
+    const int k_span = k_host ? kKSpan : 1;
+    std::vector<unsigned long long> bits(((size_t)(FEW_MAX_L + 1) * k_span * kNuBlocks + 63) / 64, 0ull);
+    bool in_range = true;
+    int count = 0;
+    for (int j = 0; j < n_modes && in_range; ++j) {      // a step = one (m, k) run x one aligned block of four |n|: count the distinct (m, k, |n| >> 2)
+        const int mm = m_host[j], kk = k_host ? k_host[j] : 0;
+        const long long nu = n_host[j] < 0 ? -(long long)n_host[j] : (long long)n_host[j];
+        if (mm < 0 || mm > FEW_MAX_L || kk < -FEW_MAX_ABS_K || kk > FEW_MAX_ABS_K || nu > FEW_MAX_ABS_N) { in_range = false; break; }
+        const size_t bit = ((size_t)mm * k_span + (size_t)(k_host ? kk + FEW_MAX_ABS_K : 0)) * kNuBlocks + (size_t)(nu >> 2);
+        const unsigned long long mask = 1ull << (bit & 63);
+        if (!(bits[bit >> 6] & mask)) { bits[bit >> 6] |= mask; ++count; }
+    }
+    if (in_range) return count;
+    std::vector<long long> keys((size_t)n_modes);
+    for (int j = 0; j < n_modes; ++j) {
+        const long long nu = n_host[j] < 0 ? -(long long)n_host[j] : (long long)n_host[j];
+        keys[j] = ((long long)m_host[j] << 40) ^ (((long long)(k_host ? k_host[j] : 0) + 1024) << 24) ^ (nu >> 2);
+    }
+    std::sort(keys.begin(), keys.end());
+    return (int)(std::unique(keys.begin(), keys.end()) - keys.begin());
 }
 
 extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int* n_t_src, const double* coef_amp, const double* coef_phase_dd,
@@ -1094,7 +1146,7 @@ extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int*
     }
     FEW_REQUIRE(h != nullptr || inner != nullptr, FEW_ERR_INVALID_ARG, "h and inner are both NULL");
     FEW_REQUIRE(workspace && ((uintptr_t)workspace % 256) == 0 &&
-                    workspace_bytes >= few_sum_waveform_workspace(n_src, n_t, n_modes, n_samples),
+                    workspace_bytes >= few_sum_waveform_workspace_ex(n_src, n_t, n_modes, n_samples, ctx->max_steps),
                 FEW_ERR_WORKSPACE, "workspace NULL, misaligned or too small");
     {   // every size limit, before the first launch
         const int lim = few_sum_check_limits(ctx, n_src, n_t, n_modes, n_samples, n_phase);
@@ -1103,7 +1155,7 @@ extern "C" int few_sum_waveform_ragged(few_ctx* ctx, const double* t, const int*
     const int plan_elems = plan_smem_elems(n_modes);
     const size_t psm = (size_t)plan_elems * 8;
     const long long max_tiles = sum_max_tiles(n_samples, n_t);
-    sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples);
+    sum_layout L = sum_carve(workspace, n_src, n_t, n_modes, n_samples, ctx->max_steps);
 
     const int plan_tile_blocks = n_src >= 64 ? 1 : (64 / n_src < 8 ? 64 / n_src : 8);     // tile blocks per source: 8 for one waveform
     FEW_CUDA_CHECK(cudaMemsetAsync(L.mode_count, 0, 2 * sizeof(int), st));

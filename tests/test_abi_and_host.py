@@ -58,6 +58,32 @@ def test_host_entry_points(lib):
     assert lib.few_sum_waveform_workspace(1, 100, 3843, 1000) >= 99 * 3843 * 64
 
 
+def test_step_bound_helper_and_workspace_queries(lib):
+    """few_max_steps_for_modes counts the distinct (m, k, |n| >> 2) of a mode list; the *_workspace_ex queries shrink with the
+    bound and fall back to the default for 0 or for a bound above it (host-only: no GPU needed)."""
+    from paper_2104_04582_b200 import synth
+    l, m, n = synth.mode_grid()
+    i32p = ctypes.POINTER(ctypes.c_int)
+    lib.few_max_steps_for_modes.argtypes = [i32p, i32p, i32p, ctypes.c_int]
+    ptr = lambda a: np.ascontiguousarray(a, np.int32).ctypes.data_as(i32p)      # noqa: E731
+    mm, nn = np.ascontiguousarray(m, np.int32), np.ascontiguousarray(n, np.int32)
+    assert lib.few_max_steps_for_modes(ptr(mm), None, ptr(nn), len(mm)) == 88          # 11 m x 8 blocks of four |n|, PAPER.md:141, 225
+    brute = len({(int(a), abs(int(b)) >> 2) for a, b in zip(mm, nn)})
+    assert brute == 88
+    k = np.arange(len(mm), dtype=np.int32) % 3 - 1                                     # a polar index multiplies the runs
+    assert lib.few_max_steps_for_modes(ptr(mm), ptr(k), ptr(nn), len(mm)) == len({(int(a), int(c), abs(int(b)) >> 2) for a, b, c in zip(mm, nn, k)})
+    assert lib.few_max_steps_for_modes(None, None, ptr(nn), len(mm)) == -1
+    for name in ("few_sum_waveform_workspace_ex", "few_waveform_workspace_ex"):
+        f = getattr(lib, name)
+        f.restype, f.argtypes = ctypes.c_size_t, [ctypes.c_int] * 3 + [ctypes.c_longlong, ctypes.c_int]
+        plain = getattr(lib, name[:-3])
+        plain.restype, plain.argtypes = ctypes.c_size_t, [ctypes.c_int] * 3 + [ctypes.c_longlong]
+        full = plain(64, 80, 3843, 1_051_920)
+        assert f(64, 80, 3843, 1_051_920, 0) == full == f(64, 80, 3843, 1_051_920, 100_000)
+        assert f(64, 80, 3843, 1_051_920, 88) < 0.35 * full
+        assert f(64, 80, 3843, 1_051_920, 40) < f(64, 80, 3843, 1_051_920, 88)
+
+
 def test_no_cpu_fallback_without_gpu(lib):
     import torch
     if torch.cuda.is_available():

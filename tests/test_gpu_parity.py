@@ -447,6 +447,56 @@ def test_sum_large_n_and_sparse_list_limit(api):
     assert api.few_device_status(raise_on_error=False) == 0
 
 
+def test_step_bound_shrinks_the_workspace_and_keeps_the_bits(api):
+    """few_set_max_steps (few.h): with the bound few_max_steps_for_modes gives for the grid (88) the workspace is a fraction of
+    the default one and the waveform has the same bits; a bound the kept list exceeds is reported as FEW_ERR_LIMIT with every
+    access still in bounds; a workspace sized for a smaller bound than the context's is refused; few_waveform_host bounds its own
+    workspace from the host mode list and leaves the context's setting alone."""
+    w = synth.make_config(3, n_src=3, n_samples=20_000)
+    g = gpu_inputs(w)
+    n_src, n_t, n_modes = w.amp.shape
+    args = (g["t"], g["phase"], g["amp"], g["l"], g["m"], g["n"], g["theta"], g["phi"], w.eps, w.t0, w.dt, w.n_samples)
+    ref = api.few_waveform(*args)
+    api.few_device_status()
+    bound = api.few_max_steps_for_modes(torch.as_tensor(w.m), torch.as_tensor(w.n))
+    assert bound == 88                                                    # 11 values of m x 8 blocks of four |n| (|n| <= 30)
+    full = api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples)
+    try:
+        api.few_set_max_steps(bound)
+        small = api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples)
+        assert small == api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples, max_steps=bound) and small < 0.4 * full
+        ws = torch.full((small,), 0xFF, dtype=torch.uint8, device="cuda")
+        h = api.few_waveform(*args, workspace=ws)
+        api.few_device_status()
+        assert torch.equal(torch.view_as_real(h), torch.view_as_real(ref))
+        cpu = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()      # noqa: E731
+        hh = api.few_waveform_host(cpu(w.t), cpu(w.phase), cpu(w.amp), cpu(w.l), cpu(w.m), cpu(w.n), cpu(w.theta), cpu(w.phi),
+                                   w.eps, w.t0, w.dt, w.n_samples)
+        assert np.array_equal(hh.numpy().view(np.float64), ref.cpu().numpy().view(np.float64))
+        # a workspace laid out for a smaller bound than the context holds is too small
+        tiny = torch.empty(api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples, max_steps=8), dtype=torch.uint8, device="cuda")
+        with pytest.raises(api.FewError) as e:
+            api.few_waveform(*args, workspace=tiny)
+        assert e.value.code == -5                                         # FEW_ERR_WORKSPACE
+        # a bound below what the kept lists need (tens of steps per source): reported, nothing out of bounds
+        api.few_set_max_steps(8)
+        ws8 = torch.full((api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples),), 0xFF, dtype=torch.uint8, device="cuda")
+        api.few_waveform(*args, workspace=ws8)
+        torch.cuda.synchronize()
+        assert api.few_device_status(raise_on_error=False) == -7          # FEW_ERR_LIMIT (FEW_DEV_SPARSE_LIST)
+        # the host path computes its own bound (88 > 8 is not lower, so the caller's 8 stands and is reported the same way)
+        with pytest.raises(api.FewError) as e:
+            api.few_waveform_host(cpu(w.t), cpu(w.phase), cpu(w.amp), cpu(w.l), cpu(w.m), cpu(w.n), cpu(w.theta), cpu(w.phi),
+                                  w.eps, w.t0, w.dt, w.n_samples)
+        assert e.value.code == -7
+    finally:
+        api.few_set_max_steps(0)
+    assert api.few_waveform_workspace(n_src, n_t, n_modes, w.n_samples) == full
+    h = api.few_waveform(*args)
+    api.few_device_status()
+    assert torch.equal(torch.view_as_real(h), torch.view_as_real(ref))
+
+
 @pytest.mark.parametrize("pinned_out", [True, False])
 def test_whole_path_host_buffers(api, pinned_out):
     """few_waveform_host: pinned h is written by the summation kernel itself (mapped stores), pageable h by a copy."""
