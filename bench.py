@@ -553,6 +553,62 @@ def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
     return out
 
 
+def self_launch(args) -> int:
+    """`python bench.py --gpus N` without torchrun: start N copies of this command, one rank per GPU (RANK, LOCAL_RANK, WORLD_SIZE,
+    MASTER_ADDR = 127.0.0.1, a free MASTER_PORT), exactly what `python -m torch.distributed.run --nproc-per-node N` would set up.
+    Rank 0 prints the one JSON line.  Fails loudly when the node has fewer than N GPUs: never a silent 1-GPU run labelled N."""
+    import socket
+    n = args.gpus
+    if not args.dry_shard:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < n:
+            sys.exit(f"bench.py: --gpus {n} needs {n} CUDA devices on this node, found {have}")
+    sock = socket.socket(); sock.bind(("127.0.0.1", 0)); port = sock.getsockname()[1]; sock.close()
+    procs = []
+    for r in range(n):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), LOCAL_WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__), *sys.argv[1:]], env=env))
+    rcs = [p.wait() for p in procs]
+    bad = [(r, rc) for r, rc in enumerate(rcs) if rc != 0]
+    if bad:
+        print(f"bench.py: ranks failed (rank, exit code): {bad}", file=sys.stderr)
+        return 1
+    return 0
+
+
+def dry_shard(args) -> int:
+    """--dry-shard: the host side of a --gpus N run with no GPU in it (gloo): rendezvous from the environment, the rank's share of
+    the workload (shard_workload), barrier, max-over-ranks and sum-over-ranks reductions as the timed run does them; rank 0 prints
+    one line.  Workload shapes only: nothing is computed."""
+    import torch
+    import torch.distributed as dist
+    from paper_2104_04582_b200 import synth
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    w_full = synth.make_config(0) if args.config == 4 else synth.random_problem(9, n_src=7, n_modes=5, n_samples=96)
+    w = shard_workload(w_full, args.config, rank, world)
+    parallelism, scaling = parallelism_label(w_full, args.config, world)
+    share = torch.tensor([float(w.n_src) * float(w.n_samples)], dtype=torch.float64)
+    t = torch.tensor([float(rank + 1)], dtype=torch.float64)
+    if world > 1:
+        dist.barrier()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        allsh = [torch.zeros(1, dtype=torch.float64) for _ in range(world)]
+        dist.all_gather(allsh, share)
+    else:
+        allsh = [share]
+    if rank == 0:
+        print(json.dumps({"dry_shard": True, "n_gpus": world, "ranks_seen": len(allsh), "max_over_ranks": float(t.item()),
+                          "scaling": scaling, "parallelism": parallelism, "source_samples_per_rank": [float(x.item()) for x in allsh],
+                          "source_samples_total": float(w_full.n_src) * float(w_full.n_samples)}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -567,9 +623,21 @@ def main():
     ap.add_argument("--eps", type=float, default=None)
     ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows: detector frame, fused inner products, direct sum")
+    ap.add_argument("--dry-shard", action="store_true",
+                    help="no GPU work: go through the launch, rendezvous (gloo), sharding and max-over-ranks reduction of a --gpus N run and "
+                         "print one line with each rank's share (what the CPU test of the multi-GPU entry point runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        return self_launch(args)                  # plain `python bench.py --gpus N`: start the N ranks ourselves
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE')}: launch with --nproc-per-node {args.gpus} "
+                 f"(or without torchrun: bench.py starts its own ranks)")
+    if args.dry_shard:
+        return dry_shard(args)
     if args.probes:
         return run_probes()
     args.warmup = max(args.warmup, 3)

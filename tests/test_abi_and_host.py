@@ -174,3 +174,29 @@ def test_gloo_world2_sharded_paths(tmp_path):
     outs = [p.communicate(timeout=240)[0] for p in procs]
     for r, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0 and f"ok {r}" in o, o
+
+
+def test_bench_gpus_n_launches_its_own_ranks():
+    """`python bench.py --gpus N` without torchrun starts N ranks itself (bench.self_launch): here through --dry-shard, the same
+    launch, rendezvous, sharding and reductions with gloo and no GPU.  Two ranks are seen, one line is printed, the shares add up;
+    a mismatch between --gpus and an existing WORLD_SIZE, or too few GPUs for a real run, is an error and not a silent 1-GPU run."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    bench = os.path.join(ROOT, "bench.py")
+    for cfg, scaling in ((3, "strong"), (4, "strong"), (1, "weak")):
+        p = subprocess.run([sys.executable, bench, "--gpus", "2", "--dry-shard", "--config", str(cfg)], capture_output=True, text=True,
+                           env=env, timeout=240)
+        assert p.returncode == 0, p.stderr
+        lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
+        assert len(lines) == 1, p.stdout
+        d = json.loads(lines[0])
+        assert d["n_gpus"] == 2 and d["ranks_seen"] == 2 and d["max_over_ranks"] == 2.0 and d["scaling"] == scaling
+        total = sum(d["source_samples_per_rank"])
+        assert total == (d["source_samples_total"] if scaling == "strong" else 2 * d["source_samples_total"])
+    p = subprocess.run([sys.executable, bench, "--gpus", "4", "--dry-shard"], capture_output=True, text=True,
+                       env=dict(env, WORLD_SIZE="2", RANK="0"), timeout=120)
+    assert p.returncode != 0 and "WORLD_SIZE" in p.stderr
+    import torch
+    if torch.cuda.device_count() < 2:
+        p = subprocess.run([sys.executable, bench, "--gpus", "2"], capture_output=True, text=True, env=env, timeout=240)
+        assert p.returncode != 0 and "needs 2 CUDA devices" in p.stderr and p.stdout.strip() == ""
