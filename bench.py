@@ -129,13 +129,22 @@ def oracle_sample(w, target_s: float, threads: int | None = None, max_samples: i
         oracle.set_threads(threads)
     cores = oracle.num_threads()
     mid = (w.n_samples // 2) // 256 * 256
+    per_step = {}
 
     def run(n):
         ws = synth.Workload(w.name, w.t[:1], w.phase[:1], w.amp[:1], w.l, w.m, w.n, w.theta[:1], w.phi[:1],
                             w.t0 + mid * w.dt, w.dt, n, w.eps)
-        t0 = time.perf_counter()
-        _, parts = oracle.waveform(ws, return_parts=True)
-        return time.perf_counter() - t0, len(parts[0]["keep_idx"])
+        # oracle.waveform's own chain (same calls, same order: PAPER.md:192), with a clock between the steps
+        c = [time.perf_counter()]
+        yp, ym = oracle.ylm_modes(ws.l, ws.m, float(ws.theta[0]), float(ws.phi[0])); c.append(time.perf_counter())
+        keep, _ = oracle.select_modes(ws.amp[0], ws.m, yp, ym, ws.eps); c.append(time.perf_counter())
+        ca = oracle.spline_fit(ws.t[0], np.ascontiguousarray(ws.amp[0]).view(np.float64))
+        cp = oracle.spline_fit_ext(ws.t[0], ws.phase[0]); c.append(time.perf_counter())
+        oracle.sum_waveform(ws.t[0], ca, cp, ws.l, ws.m, ws.n, keep, yp, ym, ws.t0, ws.dt, n); c.append(time.perf_counter())
+        per_step.clear()
+        per_step.update({"O2_harmonics_s": c[1] - c[0], "O3_selection_s": c[2] - c[1], "O1_spline_fits_s": c[3] - c[2],
+                         "O4_summation_s": c[4] - c[3], "O4_samples": int(n), "O3_rows": int(ws.n_t), "O1_systems": int(2 * ws.n_modes + 2)})
+        return c[4] - c[0], len(keep)
 
     try:
         # two calibration sizes separate the fixed cost (harmonics, selection, fits) from the per-sample cost
@@ -149,6 +158,7 @@ def oracle_sample(w, target_s: float, threads: int | None = None, max_samples: i
     finally:
         if threads is not None:
             oracle.set_threads(all_cores)
+    oracle_sample.per_step = dict(per_step)          # seconds of each oracle step in the last (timed) run
     return n * K / t_run, f"{n} contiguous samples of source 0 from sample {mid}, whole path, K={K}", cores, t_run, n, K
 
 
@@ -459,43 +469,6 @@ def parallelism_label(w, config: int, world: int):
     return f"{world} independent replicas (one waveform per GPU, an MCMC's walkers), no collective", "weak"
 
 
-PROBES_SRC = os.path.join(ROOT, "bench_probes.cu")
-PROBES_SO = os.path.join(ROOT, "bench_probes.so")
-
-
-def build_probes(force: bool = False) -> str:
-    """nvcc -> bench_probes.so next to bench.py (measurement aids only; libfew_b200 does not contain them)."""
-    if force or not os.path.exists(PROBES_SO) or os.path.getmtime(PROBES_SO) < os.path.getmtime(PROBES_SRC):
-        tmp = PROBES_SO + f".tmp{os.getpid()}"
-        subprocess.check_call(["nvcc", "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
-                               "-shared", PROBES_SRC, "-o", tmp])
-        os.replace(tmp, PROBES_SO)
-    return PROBES_SO
-
-
-def run_probes():
-    """`--probes`: the FP64-pipe facts the summation kernel is designed around, one JSON line.
-    DMMA.8x8x4 holds the pipe of a sub-partition 16 cycles; `share` = 256 * warps cycles / measured cycles per iteration."""
-    import ctypes
-    lib = ctypes.CDLL(build_probes())
-    lib.probe_dmma_mix.argtypes = [ctypes.c_int] * 5 + [ctypes.POINTER(ctypes.c_float)]
-    _, sm_max_mhz, _ = load_peaks()
-    iters, out = 4000, []
-    cases = [(1, 0, 0), (2, 0, 0), (4, 0, 0), (3, 0, 1), (3, 0, 2), (1, 0, 2)] + [(4, c, 0) for c in (2, 4, 8, 16, 32)]
-    for warps, chain, mode in cases:
-        ms = ctypes.c_float(0.0)
-        rc = lib.probe_dmma_mix(148, warps, iters, chain, mode, ctypes.byref(ms))
-        assert rc == 0, rc
-        cyc = ms.value * 1e-3 * sm_max_mhz * 1e6 / iters
-        out.append({"dmma_warps_per_scheduler": warps, "dependent_dfma_between_batches": chain,
-                    "other_warps": ["idle", "one dependent DFMA chain", "8 independent DFMA chains"][mode],
-                    "cycles_per_iteration": cyc, "dmma_share_of_pipe": 256.0 * warps / cyc,
-                    "extra_cycles_per_scalar_instruction": (cyc - 256.0 * warps) / (warps * chain) if chain else None})
-    print(json.dumps({"probes": "DMMA.8x8x4 batches of 16 per warp (256 pipe cycles), 4 warps per scheduler = 512-thread blocks, 148 blocks",
-                      "sm_mhz_assumed": sm_max_mhz, "results": out}), flush=True)
-    return 0
-
-
 def shard_workload(w, config: int, rank: int, world: int):
     """The rank's share of the workload.  No data-path collective."""
     from paper_2104_04582_b200 import synth
@@ -619,7 +592,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the short runs of configs 2, 3, 4 that the default run appends")
-    ap.add_argument("--probes", action="store_true", help="run the FP64-pipe probes of bench_probes.cu and print their JSON line")
     ap.add_argument("--eps", type=float, default=None)
     ap.add_argument("--stages", action="store_true", help="also time every C-ABI stage on its own (S0, S1, S2, S3) and report GB/s")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows: detector frame, fused inner products, direct sum")
@@ -638,8 +610,6 @@ def main():
                  f"(or without torchrun: bench.py starts its own ranks)")
     if args.dry_shard:
         return dry_shard(args)
-    if args.probes:
-        return run_probes()
     args.warmup = max(args.warmup, 3)
 
     import torch
@@ -766,7 +736,9 @@ def main():
     cpu = None
     if not args.no_cpu_baseline:
         v, desc, cores, t_run, n, K = oracle_sample(w, 12.0)
-        cpu = {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": t_run, "cpu_model": cpu_model()}
+        cpu = {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": t_run, "cpu_model": cpu_model(),
+               "per_step": dict(oracle_sample.per_step, note="seconds of the oracle's steps inside the timed sample (PAPER.md:342, 350 quote "
+                                "CPU/GPU ratios per step): O3 selection on every sparse row, O1 fits of all systems, O4 summation of the slice")}
         v1, desc1, cores1, t1, n1, K1 = oracle_sample(w, 8.0, threads=1, max_samples=1 << 18)
         cpu["one_core"] = {"value": v1, "unit": "evals/s", "cores": cores1, "sample": desc1, "seconds": t1,
                            "note": "the paper's CPU convention is one core (PAPER.md:332, 378)"}

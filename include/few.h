@@ -308,6 +308,8 @@ int few_waveform_host(few_ctx* ctx, const double* t_host, const double* phase_ho
                       long long n_samples, int n_src, int n_t, int n_modes,
                       double* h_host, int* keep_idx_host, int* n_keep_host);
 
+/* ==== The four entry points below are MEASUREMENT AIDS for bench.py, not part of the method: nothing on the hot path calls them. ==== */
+
 /* ---- Measurement aid: register-resident DFMA chains on every SM (the FP64 roofline denominator).
  * Launches `blocks` x `threads` threads, each doing `iters` x 16 dependent-chain-free DFMAs; writes one double per thread
  * to sink[blocks*threads].  FLOPs = 2 * 16 * iters * blocks * threads. */

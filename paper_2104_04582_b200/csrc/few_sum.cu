@@ -38,28 +38,21 @@ namespace {
 
 constexpr int kPlanThreads = 1024;
 constexpr int kPlanSmemElems = 16384;         // 128 KB of (key, mode) words: the plan kernel's in-shared-memory sort capacity
-#ifndef FEW_SUM_WARPS
-#define FEW_SUM_WARPS 4
-#endif
-constexpr int kSumThreads = 32 * FEW_SUM_WARPS;   // warps per block: 4, 8 or 16 (16 warps are resident per SM either way)
+// The block shape below (4 warps, 16-step stages, ring of 2) is the only one that is built and tested; the others that were
+// measured (8 and 16 warps per block, 4- to 64-step stages, rings of 3 to 6) are in profiles/r02_variants.md.
+constexpr int kSumWarps = 4;                  // warps per block (16 warps are resident per SM)
+constexpr int kSumThreads = 32 * kSumWarps;
 constexpr int kSumG = 4;                      // groups of 8 samples per warp
-constexpr int kSumBlocksPerSm = 16 / FEW_SUM_WARPS;      // resident blocks per SM, recurrence instantiation (register budget 65536 / (32 * 16))
-constexpr int kSumTabBlocksPerSm = 16 / FEW_SUM_WARPS;   // resident blocks per SM, table instantiation (16 x 32 lanes x 128 columns = all of tensor memory)
+constexpr int kSumBlocksPerSm = 16 / kSumWarps;      // resident blocks per SM, recurrence instantiation (register budget 65536 / (32 * 16))
+constexpr int kSumTabBlocksPerSm = 16 / kSumWarps;   // resident blocks per SM, table instantiation (16 x 32 lanes x 128 columns = all of tensor memory)
 constexpr int kTile = (kSumThreads / 32) * 8 * kSumG;   // samples per block
-#ifndef FEW_STAGE_STEPS
-#define FEW_STAGE_STEPS 16
-#endif
-constexpr int kStageSteps = FEW_STAGE_STEPS;  // steps per stage.  Measured (config 1 kernel, B200): 4 steps x ring 4 1.128 ms, 8 x 3 1.110,
-                                              // 16 x 2 1.069, 20 x 2 1.063: what a stage boundary costs (warp barrier, done counter, mbarrier
-                                              // wait) is paid per stage, and the ring's depth does not matter (8 x 2, 8 x 3, 8 x 4 alike)
+constexpr int kStageSteps = 16;               // steps per stage: what a stage boundary costs (warp barrier, done counter, mbarrier wait) is
+                                              // paid per stage, and the ring's depth does not matter
 constexpr int kStepD2 = 64;                   // a step's B fragments: [2][32 lanes] double2 = 1 KB
 constexpr int kHdrInts = kStageSteps < 32 ? 32 : 128;           // header: [i] descriptor of step i, [kStageSteps] steps in the stage
 constexpr int kStageBytes = kStageSteps * kStepD2 * 16 + kHdrInts * 4;
 constexpr int kStageD2 = kStageBytes / 16;    // stage size in double2
-#ifndef FEW_RING
-#define FEW_RING 2
-#endif
-constexpr int kRing = FEW_RING;               // stages in flight per block
+constexpr int kRing = 2;                      // stages in flight per block
 
 // step descriptor
 constexpr int kNewRun = 1;                    // first step of a run (m, k): close the previous run, P <- Z_phi^m Z_theta^k, (c, s) <- rho^col
@@ -627,8 +620,8 @@ __device__ __forceinline__ tile_rec load_rec(const tile_rec* p, const int2* __re
 // costs the same), each warp reads the tile records itself, two tiles ahead.  Ring protocol: full[slot] is an mbarrier the
 // TMA bulk copy completes; when a warp is done with a slot it bumps done[slot], and the LAST of the 4 warps refills the slot
 // with the stage kRing ahead in the block's stage stream (walking into the next tiles' records where the stream crosses a
-// tile boundary).  So warps drift apart by at most the ring depth and wait only for data.  (Blocks of 8 or 16 warps --
-// FEW_SUM_WARPS, one ring for more warps and longer stages -- are parity-green and 1-4 % slower on short kept lists.)
+// tile boundary).  So warps drift apart by at most the ring depth and wait only for data.  (Blocks of 8 or 16 warps measured
+// 1-4 % slower on short kept lists, profiles/r02_variants.md; they are not built.)
 // G: groups of 8 samples per warp.  kKerr: Kerr-shaped mode lists (Eq. (1), Eq. (19)): a third phase factor
 // Z_theta, runs are (m, k) with P = Z_phi^m Z_theta^k.  The hot loop is the same.
 // kTab: where the A operands (c, s) = rho^nu come from.  On the FP64 pipe a scalar instruction issued between the DMMAs of

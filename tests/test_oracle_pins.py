@@ -549,3 +549,57 @@ def test_o4_outside_range_and_knot_samples():
     W = A * np.exp(-1j * th)
     ref = np.sum(yp * W + np.where(w.m > 0, (-1.0) ** w.l * ym * np.conj(W), 0))
     assert abs(hl[0] - ref) <= 1e-12 * abs(ref)
+
+
+_SAN_WORKER = r"""
+import sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np
+import oracle
+oracle._SO = sys.argv[2]            # the sanitised build; oracle.build() finds it up to date and loads it
+from paper_2104_04582_b200 import synth
+oracle.set_threads(2)
+w0 = synth.make_config(0)
+h0 = oracle.waveform(w0)
+assert np.all(np.isfinite(h0.view(np.float64)))
+w1 = synth.make_config(1, n_samples=1500, t0=12_000_000.0)       # 3843 modes, selection at eps = 1e-5, 100 knots
+h1, parts = oracle.waveform(w1, return_parts=True)
+assert np.all(np.isfinite(h1.view(np.float64)))
+yp, ym = oracle.ylm_modes(w1.l, w1.m, float(w1.theta[0]), float(w1.phi[0]))
+for eps in (1e-2, 0.0, 1.0):
+    keep, margin = oracle.select_modes(w1.amp[0], w1.m, yp, ym, eps)
+    assert len(keep) >= 1
+wk = synth.make_kerr(n_samples=200, n_t=12, l_max=3, k_max=2, n_max=2, t0=2_000_000.0)
+ca = oracle.spline_fit(wk.t[0], np.ascontiguousarray(wk.amp[0]).view(np.float64))
+cp = oracle.spline_fit_ext(wk.t[0], wk.phase[0])
+ypk, ymk = oracle.ylm_modes(wk.l, wk.m, 0.8, 1.3)
+hk = oracle.sum_waveform_kerr(wk.t[0], ca, cp, wk.l, wk.m, wk.k, wk.n, None, ypk, ymk, wk.t0, wk.dt, wk.n_samples)
+assert np.all(np.isfinite(hk.view(np.float64)))
+d = np.ones(64, np.complex128)
+oracle.inner(d, d, 10.0); oracle.frame(0.3, 1.0, 1.2, 2.0)
+print("sanitised oracle ok")
+"""
+
+
+def test_oracle_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the oracle built with -fsanitize=address,undefined and run on config 0, a config-1 slice with
+    selection, the selection alone at three thresholds and a Kerr-shaped slice.  Any out-of-bounds access, use after free,
+    signed overflow or misaligned access aborts the worker (halt_on_error, -fno-sanitize-recover)."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    so = str(tmp_path / "libfew_oracle_san.so")
+    subprocess.check_call(["gcc", "-O1", "-g", "-fopenmp", "-ffp-contract=off", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+                           "-fno-omit-frame-pointer", "-shared", "-fPIC", "-std=c11", os.path.join(root, "oracle", "few_oracle.c"),
+                           "-o", so, "-lm"])
+    asan = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("libasan.so not found next to gcc")
+    script = tmp_path / "san_worker.py"
+    script.write_text(_SAN_WORKER)
+    env = dict(os.environ, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:halt_on_error=1:abort_on_error=0",
+               UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1")
+    p = subprocess.run([sys.executable, str(script), root, so], capture_output=True, text=True, env=env, timeout=600)
+    assert p.returncode == 0 and "sanitised oracle ok" in p.stdout, p.stdout[-2000:] + p.stderr[-4000:]
+    assert "runtime error" not in p.stderr and "AddressSanitizer" not in p.stderr, p.stderr[-4000:]
