@@ -511,7 +511,7 @@ def also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local):
     torch.cuda.empty_cache()
     w3 = synth.make_config(3)
     b, r = short(w3, steps=3)
-    st = time_stages(api, torch, w3, b.g, flush, reps=5)
+    st = time_stages(api, torch, w3, b.g, flush, reps=20)
     for name, key in (("S1_spline_fit", "S1"), ("S2_select_modes", "S2")):
         r[key] = {"ms": st[name]["ms_avg"], "gbs": st[name]["gbs"], "hbm_frac": st[name]["gbs"] / hbm_gbs,
                   "algorithmic_bytes": st[name]["algorithmic_bytes"]}
@@ -694,11 +694,20 @@ def main():
     if args.stages and rank == 0:
         stages = time_stages(api, torch, w, bench.g, flush)
     nxt = None
-    if args.next and rank == 0:
+    default_run = world == 1 and args.config == 1 and args.eps is None and not args.no_also
+    if (args.next or default_run) and rank == 0:
+        # in full with --next; the default N = 1 line carries a compact block (3 timed calls per row)
         del bench.h
-        nxt = time_next(api, torch, w, bench.g, flush, hbm_gbs)
+        nxt = time_next(api, torch, w, bench.g, flush, hbm_gbs, reps=5 if args.next else 3)
+        if not args.next:
+            nxt = {"source_frame_step_ms": nxt["source_frame_step_ms"], "ssb_step_ms_fused": nxt["ssb_step_ms_fused"],
+                   "likelihood_step_ms_fused_no_h": nxt["likelihood_step_ms_fused_no_h"],
+                   "inner_products_pass_ms": nxt["inner_products_pass"]["ms"],
+                   "direct_sum": {k: nxt["direct_sum"][k] for k in ("ms", "gbs", "hbm_frac")},
+                   "kerr_shaped_chain": {k: nxt["kerr_shaped_chain"][k] for k in ("step_ms", "kept_modes", "evals_per_s")},
+                   "note": "SURVEY 8(f) rows on this workload, 3 timed calls each after an L2 flush; `--next` prints the full block"}
     also = None
-    if world == 1 and args.config == 1 and args.eps is None and not args.no_also:
+    if default_run:
         del bench
         torch.cuda.empty_cache()
         also = also_configs(api, torch, dev, flush, hbm_gbs, sm_max_mhz, local)
